@@ -1,0 +1,197 @@
+"""CPU fp64 oracle of the Mixture Graph TF-propagation path -- TEST INFRASTRUCTURE ONLY.
+
+Thin ctypes/numpy wrapper around ``mg_oracle.c`` (see its header for citations and pins).
+Only ``tests/``, ``__graft_entry__.smoke()`` and ``bench.py``'s ``cpu_baseline`` /
+``--impl reference`` legs may import this package.  It imports nothing from the CUDA library,
+the host builder or the input generators; inputs are passed in as numpy arrays.
+
+Function -> passage (PAPER.md line):
+  mip_dims             O-1  L80
+  leaf_index           Q14  L76, L130 (sources = the segment IDs present)
+  histogram_mipmap     O-2  Eq. 4 L78-L80 (integer counts scaled to 8^l)
+  direct_colour        O-2  L66 (<m, x>)
+  brute_force_histogram O-3 Eq. 4 unrolled
+  graph_eval           O-4  L259, L269, L371, Eq. 8
+  topo_levels          L211
+  graph_eval_levels    L213, L373 (the paper's OpenMP CPU baseline shape)
+  symbolic_eval        O-5  L321, L375
+  lookup               L221, L267
+  to_rgba8 / to_rgba16f  Q13 (defined by this repo; not in the paper)
+All functions are pinned by tests/test_oracle_pins.py; none is "parity unpinned".
+"""
+from __future__ import annotations
+
+import ctypes as C
+
+import numpy as np
+
+from .build import build as _build
+
+_lib = C.CDLL(_build())
+
+_u32p = np.ctypeslib.ndpointer(np.uint32, flags="C_CONTIGUOUS")
+_u64p = np.ctypeslib.ndpointer(np.uint64, flags="C_CONTIGUOUS")
+_f64p = np.ctypeslib.ndpointer(np.float64, flags="C_CONTIGUOUS")
+_u8p = np.ctypeslib.ndpointer(np.uint8, flags="C_CONTIGUOUS")
+_u64 = C.c_uint64
+_u32 = C.c_uint32
+
+_lib.mgo_mip_dims.argtypes = [_u64, _u64, _u64, _u64p, C.c_int]
+_lib.mgo_mip_dims.restype = C.c_int
+_lib.mgo_hist_level0.argtypes = [_u32p, _u64, _u32, _u64p]
+_lib.mgo_hist_level0.restype = None
+_lib.mgo_hist_next_level.argtypes = [_u64p, _u64, _u64, _u64, _u32, _u64p]
+_lib.mgo_hist_next_level.restype = None
+_lib.mgo_direct_colour.argtypes = [_u64p, _u64, _u32, _u32, _f64p, _f64p]
+_lib.mgo_direct_colour.restype = None
+_lib.mgo_brute_force_histogram.argtypes = [_u32p, _u64, _u64, _u64, _u32, _u32, _u64, _u64, _u64, _f64p]
+_lib.mgo_brute_force_histogram.restype = None
+_lib.mgo_graph_eval.argtypes = [_u32p, _u32p, _f64p, _u64, _u64, _f64p, _f64p]
+_lib.mgo_graph_eval.restype = None
+_lib.mgo_topo_levels.argtypes = [_u32p, _u32p, _u64, _u64, _u32p]
+_lib.mgo_topo_levels.restype = C.c_int64
+_lib.mgo_graph_eval_levels.argtypes = [_u32p, _u32p, _f64p, _u64, _u64p, _u64p, _u32, _f64p, _f64p, C.c_int]
+_lib.mgo_graph_eval_levels.restype = C.c_int
+_lib.mgo_symbolic_eval.argtypes = [_u32p, _u32p, _f64p, _u64, _u64, _f64p]
+_lib.mgo_symbolic_eval.restype = None
+_lib.mgo_lookup.argtypes = [_u32p, _u64, _f64p, _f64p, C.c_int]
+_lib.mgo_lookup.restype = C.c_int
+_lib.mgo_to_rgba8.argtypes = [_f64p, _u64, _u8p]
+_lib.mgo_to_rgba8.restype = None
+_lib.mgo_colourise_rgba8.argtypes = [_u32p, _u64, _f64p, _u8p, C.c_int]
+_lib.mgo_colourise_rgba8.restype = C.c_int
+
+
+def _c(a, dt):
+    return np.ascontiguousarray(a, dtype=dt)
+
+
+def mip_dims(dims_xyz):
+    """[(X_l, Y_l, Z_l)] for l = 0..l_max (ceil-halving to 1^3, L80)."""
+    buf = np.zeros(3 * 64, dtype=np.uint64)
+    n = _lib.mgo_mip_dims(int(dims_xyz[0]), int(dims_xyz[1]), int(dims_xyz[2]), buf, 64)
+    return [tuple(int(v) for v in buf[3 * l:3 * l + 3]) for l in range(n)]
+
+
+def leaf_index(S):
+    """Sorted distinct segment IDs present in S (they are the sources, L130; background 0 is an
+    ordinary segment, Q14) and the per-voxel leaf number.  Returns (ids, seg_index like S)."""
+    ids, inv = np.unique(np.asarray(S), return_inverse=True)
+    return ids.astype(np.uint32), inv.reshape(np.shape(S)).astype(np.uint32)
+
+
+def histogram_mipmap(seg_index, n_seg):
+    """Dense integer histogram mipmap: list over levels of uint64 [Z_l, Y_l, X_l, n_seg] with
+    every voxel's counts summing to 8^l (O-2).  Small volumes only (dense)."""
+    seg_index = _c(seg_index, np.uint32)
+    Z, Y, X = seg_index.shape
+    dims = mip_dims((X, Y, Z))
+    lv = np.zeros((Z, Y, X, n_seg), dtype=np.uint64)
+    _lib.mgo_hist_level0(seg_index.reshape(-1), seg_index.size, n_seg, lv.reshape(-1))
+    out = [lv]
+    for l in range(1, len(dims)):
+        cx, cy, cz = dims[l - 1]
+        px, py, pz = dims[l]
+        nxt = np.zeros((pz, py, px, n_seg), dtype=np.uint64)
+        _lib.mgo_hist_next_level(out[-1].reshape(-1), cx, cy, cz, n_seg, nxt.reshape(-1))
+        out.append(nxt)
+    return out
+
+
+def direct_colour(counts, level, tf):
+    """C_dir = (sum_s c_s TF[s]) / 8^l, fp64 [Z_l, Y_l, X_l, 4]."""
+    counts = _c(counts, np.uint64)
+    n_seg = counts.shape[-1]
+    tf = _c(tf, np.float64)
+    assert tf.shape == (n_seg, 4)
+    out = np.zeros(counts.shape[:-1] + (4,), dtype=np.float64)
+    _lib.mgo_direct_colour(counts.reshape(-1), counts.size // n_seg, n_seg, level, tf.reshape(-1),
+                           out.reshape(-1))
+    return out
+
+
+def brute_force_histogram(seg_index, n_seg, level, i, j, k):
+    """Normalised histogram (sums to 1) of voxel (i,j,k) of ``level`` by the unrolled Eq. 4."""
+    seg_index = _c(seg_index, np.uint32)
+    Z, Y, X = seg_index.shape
+    h = np.zeros(n_seg, dtype=np.float64)
+    _lib.mgo_brute_force_histogram(seg_index.reshape(-1), X, Y, Z, n_seg, level, i, j, k, h)
+    return h
+
+
+def graph_eval(child_a, child_b, weight, n_leaves, tf):
+    """c[n] fp64 [n_nodes, 4]: leaves = tf, then (1-w) c[a] + w c[b] in index order (O-4).
+    ``weight`` may be fp32 (converted exactly) or fp64."""
+    a, b = _c(child_a, np.uint32), _c(child_b, np.uint32)
+    w = _c(weight, np.float64)
+    tf = _c(tf, np.float64)
+    n = a.size
+    assert b.size == n and w.size == n and tf.shape == (n_leaves, 4)
+    c = np.zeros((n, 4), dtype=np.float64)
+    _lib.mgo_graph_eval(a, b, w, n, n_leaves, tf.reshape(-1), c.reshape(-1))
+    return c
+
+
+def topo_levels(child_a, child_b, n_leaves):
+    """(level u32 [n_nodes], depth): sources 0, otherwise max(v1, v2) + 1 (L211)."""
+    a, b = _c(child_a, np.uint32), _c(child_b, np.uint32)
+    lev = np.zeros(a.size, dtype=np.uint32)
+    depth = _lib.mgo_topo_levels(a, b, a.size, n_leaves, lev)
+    if depth < 0:
+        raise ValueError("child index does not precede its parent (Eq. 8)")
+    return lev, int(depth)
+
+
+def graph_eval_levels(child_a, child_b, weight, n_leaves, tf, n_threads=0):
+    """Level-synchronous OpenMP evaluation (the paper's CPU baseline, L213/L373).
+    Returns (c fp64 [n_nodes, 4], threads used)."""
+    a, b = _c(child_a, np.uint32), _c(child_b, np.uint32)
+    w = _c(weight, np.float64)
+    tf = _c(tf, np.float64)
+    lev, depth = topo_levels(a, b, n_leaves)
+    order = np.argsort(lev, kind="stable").astype(np.uint64)
+    start = np.searchsorted(lev[order.astype(np.int64)], np.arange(depth + 2)).astype(np.uint64)
+    c = np.zeros((a.size, 4), dtype=np.float64)
+    used = _lib.mgo_graph_eval_levels(a, b, w, n_leaves, order, start, depth, tf.reshape(-1),
+                                      c.reshape(-1), n_threads)
+    return c, used
+
+
+def symbolic_eval(child_a, child_b, weight, n_leaves):
+    """mu fp64 [n_nodes, n_leaves]: unit vectors on the leaves, propagated (O-5)."""
+    a, b = _c(child_a, np.uint32), _c(child_b, np.uint32)
+    w = _c(weight, np.float64)
+    mu = np.zeros((a.size, n_leaves), dtype=np.float64)
+    _lib.mgo_symbolic_eval(a, b, w, a.size, n_leaves, mu.reshape(-1))
+    return mu
+
+
+def lookup(node_idx, c, n_threads=1):
+    """C_graph(v) = c[node_idx[v]], fp64 [..., 4]."""
+    idx = _c(node_idx, np.uint32)
+    c = _c(c, np.float64)
+    out = np.zeros(idx.shape + (4,), dtype=np.float64)
+    _lib.mgo_lookup(idx.reshape(-1), idx.size, c.reshape(-1), out.reshape(-1), n_threads)
+    return out
+
+
+def to_rgba8(c):
+    """uint8 [..., 4]: round_half_even(clamp(fp32(c), 0, 1) * 255), decision in fp32 (Q13)."""
+    c = _c(c, np.float64)
+    out = np.zeros(c.shape, dtype=np.uint8)
+    _lib.mgo_to_rgba8(c.reshape(-1), c.size // 4, out.reshape(-1))
+    return out
+
+
+def to_rgba16f(c):
+    """fp16 [..., 4]: RN(fp32(c)) (Q13)."""
+    return np.asarray(c, dtype=np.float64).astype(np.float32).astype(np.float16)
+
+
+def colourise_rgba8(node_idx, c, n_threads=0):
+    """lookup + to_rgba8 in one pass (timed CPU baseline of the colourise step)."""
+    idx = _c(node_idx, np.uint32)
+    c = _c(c, np.float64)
+    out = np.zeros(idx.shape + (4,), dtype=np.uint8)
+    used = _lib.mgo_colourise_rgba8(idx.reshape(-1), idx.size, c.reshape(-1), out.reshape(-1), n_threads)
+    return out, used
