@@ -1,0 +1,178 @@
+/*
+ * mg.h -- C ABI of the B200-native Mixture Graph transfer-function propagation library.
+ *
+ * Implements the hot path of "The Mixture Graph" (arXiv 2009.02702; "L<n>" = line n of PAPER.md):
+ *   a4  leaf assignment        c[k] = TF[k], bit-exact                         (L371)
+ *   a5  propagation            c[n] = (1 - w[n]) c[a[n]] + w[n] c[b[n]]        (L259, L269, L371)
+ *                              level-synchronous over the topological levels   (L211-L213)
+ *   a6  colourise              out[v] = convert(c[node_idx[v]])                (L221, L267)
+ *
+ * Conventions
+ *   - every call returns int: MG_OK (0) or a negative MG_ERR_*; mg_last_error() gives a
+ *     thread-local message for the last failing call on this thread.  No exceptions, no aborts.
+ *   - "host" / "device" is stated per pointer.  Device pointers must belong to the CUDA device that
+ *     was current when mg_load_graph was called.  `stream` is a cudaStream_t passed as void*
+ *     (NULL = the legacy default stream).
+ *   - mg_propagate / mg_colorize only ENQUEUE work on `stream`: no synchronisation and no
+ *     allocation (the first call on a graph may create cached launch state).
+ *     Caller-owned buffers must outlive the enqueued work.
+ *   - the library owns only its device copy of the graph (and per-graph scratch: 8-bit / 16-bit
+ *     palettes, a TF staging buffer), released by mg_free_graph.
+ *   - there is no CPU fallback: without a CUDA device every compute call fails with MG_ERR_CUDA.
+ */
+#ifndef MG_H_
+#define MG_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct mg_graph mg_graph;
+
+enum {
+    MG_OK = 0,
+    MG_ERR_INVALID_ARG = -1,   /* NULL pointer, bad enum, misaligned buffer ...            */
+    MG_ERR_INVALID_GRAPH = -2, /* the arrays do not describe a valid Mixture Graph         */
+    MG_ERR_CUDA = -3,          /* a CUDA runtime call failed (message has the CUDA error)  */
+    MG_ERR_OOM = -4            /* host or device allocation failed                         */
+};
+
+/* mg_load_graph flags */
+enum {
+    MG_RELABEL = 1u /* input is only children-before-parents (Eq. 8), not level-contiguous:
+                       the library computes the topological levels (L211), permutes the nodes so
+                       that every level is contiguous (leaves keep their numbers; inside a level
+                       nodes are ordered by their children's new numbers for L2 locality) and
+                       exposes the permutation through mg_node_permutation.                      */
+};
+
+/* mg_colorize output formats (bit mask) */
+enum {
+    MG_RGBA8 = 1u,         /* 4 x uint8 per voxel, R in byte 0: round_half_even(clamp(c,0,1)*255)  */
+    MG_RGBA16F = 2u,       /* 4 x IEEE fp16 per voxel (round to nearest even)                      */
+    MG_BOTH = 3u,          /* both; RGBA8 to out_rgba, fp16 to out_rgba_aux                        */
+    MG_FORCE_CONVERT = 16u /* do not reuse the palettes cached by mg_propagate (see mg_colorize)   */
+};
+
+typedef struct mg_info {
+    uint64_t n_nodes;       /* leaves + internal nodes                                        */
+    uint64_t n_internal;    /* n_nodes - n_leaves                                             */
+    uint32_t n_leaves;      /* sources = segment IDs (L130)                                   */
+    uint32_t depth;         /* topological depth = number of synchronisation points (L211)    */
+    uint32_t n_topo_levels; /* depth + 1                                                      */
+    uint32_t first_fused_level; /* levels >= this run inside ONE persistent CTA (0 = none)    */
+    uint32_t n_launches_propagate; /* kernel launches one mg_propagate enqueues               */
+    uint32_t relabelled;    /* 1 if the library permuted the nodes (MG_RELABEL)               */
+    uint64_t device_bytes;  /* device memory owned by the graph object                        */
+} mg_info;
+
+/*
+ * mg_load_graph -- validate a Mixture Graph given as HOST SoA arrays and copy it to the device.
+ *
+ *   child_a, child_b  host uint32[n_nodes]: the two predecessors of each node (stored as incoming
+ *                     edges, L140).  Entries of the leaves [0, n_leaves) are ignored.
+ *   weight            host float[n_nodes]: w of the triple (a, b, w) = (1-w) s_a + w s_b (L259):
+ *                     the weight multiplies child_b.  Must satisfy 0 < w < 1 (L176).
+ *   n_nodes, n_leaves leaves are nodes 0 .. n_leaves-1, in leaf_segment_id order; n_nodes < 2^32.
+ *   level_offsets     host uint64[n_topo_levels + 1], [0] = 0, [1] = n_leaves, [last] = n_nodes;
+ *                     nodes of topological level L occupy [off[L], off[L+1]) and both children of
+ *                     such a node lie below off[L], at least one of them at or above off[L-1]
+ *                     (level = max + 1, L211).  May be NULL together with flags & MG_RELABEL.
+ *   n_topo_levels     depth + 1 (ignored with MG_RELABEL when level_offsets is NULL).
+ *   leaf_segment_id   host uint32[n_leaves] or NULL: the segment ID of each leaf (kept for
+ *                     mg_graph_info consumers; strictly increasing if given).
+ *   flags             0 or MG_RELABEL.
+ *   out               receives the graph handle.
+ *
+ * All arrays are caller-owned and copied.  Errors: MG_ERR_INVALID_ARG (NULL, n_leaves = 0,
+ * n_nodes >= 2^32), MG_ERR_INVALID_GRAPH (a == b, child not below its level, level not max+1,
+ * w outside (0,1) or not finite, offsets not increasing), MG_ERR_OOM, MG_ERR_CUDA.
+ */
+int mg_load_graph(const uint32_t *child_a, const uint32_t *child_b, const float *weight,
+                  uint64_t n_nodes, uint32_t n_leaves, const uint64_t *level_offsets,
+                  uint32_t n_topo_levels, const uint32_t *leaf_segment_id, uint32_t flags,
+                  mg_graph **out);
+
+/* Release the handle and every device buffer it owns.  NULL is allowed. */
+void mg_free_graph(mg_graph *g);
+
+/* Fill *info.  Host only. */
+int mg_graph_info(const mg_graph *g, mg_info *info);
+
+/* level_offsets of the loaded (possibly relabelled) graph: host uint64[n_topo_levels + 1]. */
+int mg_level_offsets(const mg_graph *g, uint64_t *level_offsets_host);
+
+/* new_of_old_host: host uint32[n_nodes]; node `old` of the arrays given to mg_load_graph is node
+ * new_of_old[old] of the library's numbering (identity unless MG_RELABEL permuted the graph). */
+int mg_node_permutation(const mg_graph *g, uint32_t *new_of_old_host);
+
+/* One-off: rewrite a DEVICE array of n node indices in place from the caller's numbering to the
+ * library's (idx[i] = new_of_old[idx[i]]), so that builder-numbered node_idx volumes can be passed
+ * to mg_colorize.  No-op for a graph that was not relabelled. */
+int mg_relabel_indices(mg_graph *g, uint32_t *idx_device, uint64_t n, void *stream);
+
+/*
+ * mg_propagate -- one full transfer-function update (the paper performs full updates only, L221).
+ *
+ *   tf_rgba    DEVICE float[n_leaves][4], leaf order.  16-byte aligned.
+ *   node_rgba  DEVICE float[n_nodes][4], caller-allocated, 16-byte aligned.  On completion
+ *              node_rgba[k] == tf_rgba[k] bit-for-bit for k < n_leaves and every other entry holds
+ *              fma(w, c_b, fma(-w, c_a, c_a)) per channel in fp32, in the library's numbering.
+ *
+ * Enqueues: one kernel per large topological level (leaf copy fused into the first) and one
+ * persistent single-CTA kernel for the small top levels.  Every kernel also writes the 8-bit and
+ * 16-bit palettes that mg_colorize gathers from.
+ */
+int mg_propagate(mg_graph *g, const float *tf_rgba, float *node_rgba, void *stream);
+
+/* Same, with the TF in HOST memory (pinned for a truly asynchronous copy): enqueues the
+ * host-to-device copy of n_leaves float4 into a graph-owned staging buffer first -- the quantity
+ * the paper times ("GPU timings include the data upload of one float4 color per source", L371). */
+int mg_propagate_host(mg_graph *g, const float *tf_rgba_host, float *node_rgba, void *stream);
+
+/*
+ * mg_colorize -- materialise (part of) the pre-filtered RGBA mipmap: out[v] = convert(c[idx[v]]).
+ *
+ *   mip_level        informational (the operation is the same for every level); pass 0xFFFFFFFF
+ *                    when one call covers several concatenated levels.
+ *   node_idx_volume  DEVICE uint32[n_voxels], x fastest, values < n_nodes in the LIBRARY's
+ *                    numbering (see mg_relabel_indices).  4-byte aligned; the fast path needs the
+ *                    index and output pointers to have the same offset modulo 16 bytes in units of
+ *                    voxels (true for any two cudaMalloc'ed buffers indexed at the same voxel).
+ *   n_voxels         number of voxels; authoritative.  0 is allowed (no work).
+ *   node_rgba        DEVICE float[n_nodes][4] as filled by mg_propagate.  If it is the buffer most
+ *                    recently filled by mg_propagate on this graph, the 8/16-bit palettes derived
+ *                    there are reused; for any other pointer, or with MG_FORCE_CONVERT, the
+ *                    palettes are first re-derived from node_rgba (one extra kernel).
+ *   out_rgba         DEVICE output, n_voxels * 4 bytes (MG_RGBA8, MG_BOTH) or * 8 (MG_RGBA16F).
+ *   out_rgba_aux     DEVICE fp16 output for MG_BOTH, else ignored (may be NULL).
+ *   format           MG_RGBA8 | MG_RGBA16F | MG_BOTH, optionally | MG_FORCE_CONVERT.
+ */
+int mg_colorize(mg_graph *g, uint32_t mip_level, const uint32_t *node_idx_volume,
+                uint64_t n_voxels, const float *node_rgba, void *out_rgba, void *out_rgba_aux,
+                uint32_t format, void *stream);
+
+/*
+ * mg_tf_update_host -- the whole per-update path with HOST buffers at both ends:
+ * H2D of the TF, mg_propagate, mg_colorize over n_voxels (typically every mip level,
+ * concatenated), and -- if out_host is not NULL -- D2H of the colourised output.
+ * out_device is the DEVICE buffer the mipmap is materialised in (what a renderer would sample);
+ * out_host, if given, must hold n_voxels * 4 (MG_RGBA8) or * 8 (MG_RGBA16F) bytes (MG_BOTH is not
+ * accepted here).  Enqueue-only, like the calls it is made of.
+ */
+int mg_tf_update_host(mg_graph *g, const float *tf_rgba_host, float *node_rgba,
+                      const uint32_t *node_idx_volume, uint64_t n_voxels, void *out_device,
+                      void *out_host, uint32_t format, void *stream);
+
+/* Thread-local description of the last error returned on this thread ("" if none). */
+const char *mg_last_error(void);
+
+/* Number of kernels the library has launched since it was loaded (for gpu_launches accounting). */
+uint64_t mg_kernel_launch_count(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MG_H_ */

@@ -1,0 +1,243 @@
+// mg_api.cu -- graph object: validation, relabelling, device upload, info (include/mg.h).
+#include <atomic>
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+#include "mg_internal.h"
+
+namespace mg {
+
+static thread_local char g_err[512] = "";
+static std::atomic<uint64_t> g_launches{0};
+
+void set_error(const char* fmt, ...)
+{
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof(g_err), fmt, ap);
+    va_end(ap);
+}
+
+int cuda_fail(cudaError_t e, const char* what)
+{
+    set_error("CUDA error %d (%s) in %s", (int)e, cudaGetErrorString(e), what);
+    cudaGetLastError();   // clear the sticky-less error state
+    return e == cudaErrorMemoryAllocation ? MG_ERR_OOM : MG_ERR_CUDA;
+}
+
+void count_launch(unsigned n) { g_launches.fetch_add(n, std::memory_order_relaxed); }
+
+// Levels >= first_fused_level run inside one persistent CTA.  A level goes to that CTA when it and
+// every later level has at most kTailMaxLevelNodes nodes: below that size one more kernel launch
+// (a few microseconds of dependent-launch latency) costs more than the level itself.
+static const uint64_t kTailMaxLevelNodes = 8192;
+// Nodes of the fused tail whose colours are also kept in shared memory (float4 each).
+static const uint32_t kTailSmemNodes = 12288;   // 192 KB
+
+static void plan_launches(mg_graph* g)
+{
+    uint32_t first = g->n_levels;   // none
+    for (uint32_t L = g->n_levels; L-- > 1;) {
+        if (g->level_off[L + 1] - g->level_off[L] <= kTailMaxLevelNodes) first = L; else break;
+    }
+    g->first_fused_level = (first < g->n_levels) ? first : 0;
+    g->tail_smem_nodes = 0;
+    if (g->first_fused_level) {
+        uint64_t tail_nodes = g->n_nodes - g->level_off[g->first_fused_level];
+        g->tail_smem_nodes = (uint32_t)(tail_nodes < kTailSmemNodes ? tail_nodes : kTailSmemNodes);
+    }
+}
+
+template <typename T>
+static int dev_alloc(mg_graph* g, T** p, uint64_t count)
+{
+    size_t bytes = (size_t)(count ? count : 1) * sizeof(T);
+    bytes = (bytes + 255) & ~(size_t)255;
+    MG_CUDA(cudaMalloc((void**)p, bytes));
+    g->device_bytes += bytes;
+    return MG_OK;
+}
+
+}  // namespace mg
+
+using namespace mg;
+
+extern "C" const char* mg_last_error(void) { return g_err; }
+extern "C" uint64_t mg_kernel_launch_count(void) { return g_launches.load(); }
+
+extern "C" void mg_free_graph(mg_graph* g)
+{
+    if (!g) return;
+    int prev = 0;
+    bool have = cudaGetDevice(&prev) == cudaSuccess;
+    if (have) cudaSetDevice(g->device);
+    cudaFree(g->d_a); cudaFree(g->d_b); cudaFree(g->d_w); cudaFree(g->d_level_off);
+    cudaFree(g->d_new_of_old); cudaFree(g->d_tf_stage); cudaFree(g->d_pal8); cudaFree(g->d_pal16);
+    if (have) cudaSetDevice(prev);
+    cudaGetLastError();
+    delete g;
+}
+
+extern "C" int mg_load_graph(const uint32_t* child_a, const uint32_t* child_b, const float* weight,
+                             uint64_t n_nodes, uint32_t n_leaves, const uint64_t* level_offsets,
+                             uint32_t n_topo_levels, const uint32_t* leaf_segment_id, uint32_t flags,
+                             mg_graph** out)
+{
+    g_err[0] = 0;
+    if (!out) { set_error("mg_load_graph: out is NULL"); return MG_ERR_INVALID_ARG; }
+    *out = nullptr;
+    if (n_leaves == 0 || n_nodes < n_leaves) { set_error("mg_load_graph: need 0 < n_leaves <= n_nodes"); return MG_ERR_INVALID_ARG; }
+    if (n_nodes >= (1ull << 32)) { set_error("mg_load_graph: n_nodes must be < 2^32"); return MG_ERR_INVALID_ARG; }
+    if (flags & ~(uint32_t)MG_RELABEL) { set_error("mg_load_graph: unknown flags 0x%x", flags); return MG_ERR_INVALID_ARG; }
+    if (n_nodes > n_leaves && (!child_a || !child_b || !weight)) { set_error("mg_load_graph: NULL graph array"); return MG_ERR_INVALID_ARG; }
+    const bool relabel = (flags & MG_RELABEL) != 0;
+    if (!relabel && !level_offsets) { set_error("mg_load_graph: level_offsets is NULL without MG_RELABEL"); return MG_ERR_INVALID_ARG; }
+
+    // ---- validation that does not depend on the numbering (I2: a != b, children precede, 0 < w < 1)
+    for (uint64_t n = n_leaves; n < n_nodes; n++) {
+        uint32_t a = child_a[n], b = child_b[n];
+        float w = weight[n];
+        if (a >= n || b >= n) { set_error("node %llu: child (%u, %u) does not precede it (Eq. 8)", (unsigned long long)n, a, b); return MG_ERR_INVALID_GRAPH; }
+        if (a == b) { set_error("node %llu: both children are node %u", (unsigned long long)n, a); return MG_ERR_INVALID_GRAPH; }
+        if (!(w > 0.0f && w < 1.0f)) { set_error("node %llu: weight %g outside the open interval (0,1) (L176)", (unsigned long long)n, (double)w); return MG_ERR_INVALID_GRAPH; }
+    }
+    if (leaf_segment_id)
+        for (uint32_t k = 1; k < n_leaves; k++)
+            if (leaf_segment_id[k] <= leaf_segment_id[k - 1]) { set_error("leaf_segment_id not strictly increasing at %u", k); return MG_ERR_INVALID_GRAPH; }
+
+    mg_graph* g = new (std::nothrow) mg_graph();
+    if (!g) { set_error("mg_load_graph: host allocation failed"); return MG_ERR_OOM; }
+    g->n_nodes = n_nodes;
+    g->n_leaves = n_leaves;
+    if (leaf_segment_id) g->leaf_segment_id.assign(leaf_segment_id, leaf_segment_id + n_leaves);
+
+    std::vector<uint32_t> ha, hb;
+    std::vector<float> hw;
+    try {
+        if (relabel) {
+            if (relabel_by_level(child_a, child_b, n_nodes, n_leaves, g->new_of_old, g->level_off) != 0) {
+                set_error("mg_load_graph: relabel failed (graph not children-before-parents)");
+                delete g; return MG_ERR_INVALID_GRAPH;
+            }
+            g->n_levels = (uint32_t)g->level_off.size() - 1;
+            ha.assign(n_nodes, 0); hb.assign(n_nodes, 0); hw.assign(n_nodes, 0.0f);
+            const std::vector<uint32_t>& p = g->new_of_old;
+#pragma omp parallel for schedule(static)
+            for (int64_t n = n_leaves; n < (int64_t)n_nodes; n++) {
+                uint32_t q = p[n];
+                ha[q] = p[child_a[n]]; hb[q] = p[child_b[n]]; hw[q] = weight[n];
+            }
+        } else {
+            if (n_topo_levels == 0) { set_error("mg_load_graph: n_topo_levels is 0"); delete g; return MG_ERR_INVALID_ARG; }
+            g->n_levels = n_topo_levels;
+            g->level_off.assign(level_offsets, level_offsets + n_topo_levels + 1);
+            if (g->level_off[0] != 0 || g->level_off[1] != n_leaves || g->level_off[n_topo_levels] != n_nodes) {
+                set_error("level_offsets must start 0, n_leaves and end n_nodes"); delete g; return MG_ERR_INVALID_GRAPH;
+            }
+            for (uint32_t L = 0; L < n_topo_levels; L++)
+                if (g->level_off[L + 1] <= g->level_off[L]) { set_error("level %u is empty or offsets decrease", L); delete g; return MG_ERR_INVALID_GRAPH; }
+            // level = max(level(a), level(b)) + 1 (L211): both children below off[L], one at or above off[L-1]
+            for (uint32_t L = 1; L < n_topo_levels; L++) {
+                uint64_t lo = g->level_off[L], prev = g->level_off[L - 1];
+                for (uint64_t n = lo; n < g->level_off[L + 1]; n++) {
+                    uint32_t a = child_a[n], b = child_b[n];
+                    uint32_t mx = a > b ? a : b;
+                    if (mx >= lo || mx < prev) {
+                        set_error("node %llu (level %u): children (%u, %u) violate level = max + 1 (L211)", (unsigned long long)n, L, a, b);
+                        delete g; return MG_ERR_INVALID_GRAPH;
+                    }
+                }
+            }
+            ha.assign(child_a, child_a + n_nodes); hb.assign(child_b, child_b + n_nodes); hw.assign(weight, weight + n_nodes);
+            for (uint32_t n = 0; n < n_leaves; n++) { ha[n] = 0; hb[n] = 0; hw[n] = 0.0f; }
+        }
+    } catch (const std::bad_alloc&) {
+        set_error("mg_load_graph: host allocation failed"); delete g; return MG_ERR_OOM;
+    }
+    plan_launches(g);
+
+    // ---- device upload
+    int rc = MG_OK;
+    cudaError_t e = cudaGetDevice(&g->device);
+    if (e != cudaSuccess) { rc = cuda_fail(e, "cudaGetDevice"); delete g; return rc; }
+    std::vector<uint32_t> off32(g->level_off.begin(), g->level_off.end());
+#define MG_TRY(x) do { rc = (x); if (rc != MG_OK) { mg_free_graph(g); return rc; } } while (0)
+#define MG_TRY_CUDA(x) do { cudaError_t e2 = (x); if (e2 != cudaSuccess) { rc = cuda_fail(e2, #x); mg_free_graph(g); return rc; } } while (0)
+    MG_TRY(dev_alloc(g, &g->d_a, n_nodes + 4));       // +4: vector loads of the last partial group
+    MG_TRY(dev_alloc(g, &g->d_b, n_nodes + 4));
+    MG_TRY(dev_alloc(g, &g->d_w, n_nodes + 4));
+    MG_TRY(dev_alloc(g, &g->d_level_off, off32.size()));
+    MG_TRY(dev_alloc(g, &g->d_tf_stage, (uint64_t)n_leaves * 4));
+    MG_TRY(dev_alloc(g, &g->d_pal8, n_nodes + 4));
+    MG_TRY(dev_alloc(g, &g->d_pal16, n_nodes + 4));
+    MG_TRY_CUDA(cudaMemset(g->d_a, 0, (n_nodes + 4) * 4));
+    MG_TRY_CUDA(cudaMemset(g->d_b, 0, (n_nodes + 4) * 4));
+    MG_TRY_CUDA(cudaMemset(g->d_w, 0, (n_nodes + 4) * 4));
+    MG_TRY_CUDA(cudaMemcpy(g->d_a, ha.data(), n_nodes * 4, cudaMemcpyHostToDevice));
+    MG_TRY_CUDA(cudaMemcpy(g->d_b, hb.data(), n_nodes * 4, cudaMemcpyHostToDevice));
+    MG_TRY_CUDA(cudaMemcpy(g->d_w, hw.data(), n_nodes * 4, cudaMemcpyHostToDevice));
+    MG_TRY_CUDA(cudaMemcpy(g->d_level_off, off32.data(), off32.size() * 4, cudaMemcpyHostToDevice));
+    if (relabel) {
+        MG_TRY(dev_alloc(g, &g->d_new_of_old, n_nodes));
+        MG_TRY_CUDA(cudaMemcpy(g->d_new_of_old, g->new_of_old.data(), n_nodes * 4, cudaMemcpyHostToDevice));
+    }
+#undef MG_TRY
+#undef MG_TRY_CUDA
+    *out = g;
+    return MG_OK;
+}
+
+extern "C" int mg_graph_info(const mg_graph* g, mg_info* info)
+{
+    if (!g || !info) { set_error("mg_graph_info: NULL argument"); return MG_ERR_INVALID_ARG; }
+    info->n_nodes = g->n_nodes;
+    info->n_internal = g->n_nodes - g->n_leaves;
+    info->n_leaves = g->n_leaves;
+    info->depth = g->n_levels - 1;
+    info->n_topo_levels = g->n_levels;
+    info->first_fused_level = g->first_fused_level;
+    uint32_t big = (g->first_fused_level ? g->first_fused_level : g->n_levels) - 1;   // levels 1 .. first_fused-1
+    info->n_launches_propagate = (big ? big : 0) + (g->first_fused_level ? 1 : 0) + ((big == 0 && !g->first_fused_level) ? 1 : 0);
+    info->relabelled = g->new_of_old.empty() ? 0 : 1;
+    info->device_bytes = g->device_bytes;
+    return MG_OK;
+}
+
+extern "C" int mg_level_offsets(const mg_graph* g, uint64_t* level_offsets_host)
+{
+    if (!g || !level_offsets_host) { set_error("mg_level_offsets: NULL argument"); return MG_ERR_INVALID_ARG; }
+    memcpy(level_offsets_host, g->level_off.data(), g->level_off.size() * sizeof(uint64_t));
+    return MG_OK;
+}
+
+extern "C" int mg_node_permutation(const mg_graph* g, uint32_t* new_of_old_host)
+{
+    if (!g || !new_of_old_host) { set_error("mg_node_permutation: NULL argument"); return MG_ERR_INVALID_ARG; }
+    if (g->new_of_old.empty())
+        for (uint64_t n = 0; n < g->n_nodes; n++) new_of_old_host[n] = (uint32_t)n;
+    else
+        memcpy(new_of_old_host, g->new_of_old.data(), g->n_nodes * sizeof(uint32_t));
+    return MG_OK;
+}
+
+__global__ void __launch_bounds__(256) k_relabel_indices(uint32_t* __restrict__ idx, uint64_t n,
+                                                          const uint32_t* __restrict__ new_of_old)
+{
+    for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (uint64_t)gridDim.x * blockDim.x)
+        idx[i] = __ldg(new_of_old + idx[i]);
+}
+
+extern "C" int mg_relabel_indices(mg_graph* g, uint32_t* idx_device, uint64_t n, void* stream)
+{
+    if (!g || (!idx_device && n)) { set_error("mg_relabel_indices: NULL argument"); return MG_ERR_INVALID_ARG; }
+    if (!g->d_new_of_old || n == 0) return MG_OK;
+    uint64_t blocks = (n + 255) / 256;
+    if (blocks > 148ull * 64) blocks = 148ull * 64;
+    k_relabel_indices<<<(unsigned)blocks, 256, 0, (cudaStream_t)stream>>>(idx_device, n, g->d_new_of_old);
+    count_launch();
+    MG_CUDA(cudaGetLastError());
+    return MG_OK;
+}

@@ -1,0 +1,58 @@
+// Internal declarations shared by the translation units of libmg.so (NOT part of the C ABI,
+// not used by oracle/).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <string>
+#include <vector>
+
+#include "../../include/mg.h"
+
+namespace mg {
+
+void set_error(const char* fmt, ...);
+int cuda_fail(cudaError_t e, const char* what);   // records the message, returns MG_ERR_CUDA / MG_ERR_OOM
+void count_launch(unsigned n = 1);
+
+#define MG_CUDA(call)                                         \
+    do {                                                      \
+        cudaError_t e__ = (call);                             \
+        if (e__ != cudaSuccess) return mg::cuda_fail(e__, #call); \
+    } while (0)
+
+// Host-side relabelling (csrc/relabel.cpp, also linked into the builder library).
+// Input: any children-before-parents graph.  Output: level-contiguous numbering.
+//   new_of_old[n]  new index of node n (leaves keep their index)
+//   level_off      [depth + 2] offsets of the levels in the new numbering
+// Returns 0, or -1 if a child does not precede its parent / equals its sibling.
+int relabel_by_level(const uint32_t* child_a, const uint32_t* child_b, uint64_t n_nodes,
+                     uint32_t n_leaves, std::vector<uint32_t>& new_of_old,
+                     std::vector<uint64_t>& level_off);
+
+}  // namespace mg
+
+struct mg_graph {
+    int device = 0;
+    uint64_t n_nodes = 0;
+    uint32_t n_leaves = 0;
+    uint32_t n_levels = 0;                 // depth + 1
+    std::vector<uint64_t> level_off;       // [n_levels + 1], library numbering
+    std::vector<uint32_t> leaf_segment_id; // may be empty
+    std::vector<uint32_t> new_of_old;      // empty = identity
+    // device SoA (library numbering); leaves' entries are zero
+    uint32_t* d_a = nullptr;
+    uint32_t* d_b = nullptr;
+    float* d_w = nullptr;
+    uint32_t* d_level_off = nullptr;       // [n_levels + 1] as uint32 (n_nodes < 2^32)
+    uint32_t* d_new_of_old = nullptr;      // only if relabelled
+    // per-graph scratch
+    float* d_tf_stage = nullptr;           // [n_leaves][4]
+    uint32_t* d_pal8 = nullptr;            // [n_nodes] RGBA8
+    uint2* d_pal16 = nullptr;              // [n_nodes] 4 x fp16
+    const float* pal_src = nullptr;        // node_rgba the palettes were last derived from
+    // launch plan
+    uint32_t first_fused_level = 0;        // levels >= this run in the single-CTA tail kernel (0 = none)
+    uint32_t tail_smem_nodes = 0;          // nodes of the tail staged in shared memory
+    uint64_t device_bytes = 0;
+};

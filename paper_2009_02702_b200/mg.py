@@ -1,0 +1,160 @@
+"""ctypes binding of the C-ABI library (include/mg.h): argument marshalling only.
+
+Every step of the path runs in the library's CUDA kernels; PyTorch is used by callers for device
+memory (``tensor.data_ptr()``) and streams (``torch.cuda.current_stream().cuda_stream``).  There is
+no CPU fallback: if ``libmg.so`` is missing this module raises at import time.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libmg.so")
+
+if not os.path.exists(LIB_PATH):
+    raise ImportError(f"{LIB_PATH} is missing: run `python -m paper_2009_02702_b200.build` "
+                      "(there is no CPU fallback for the CUDA path)")
+lib = C.CDLL(LIB_PATH)
+
+MG_OK, MG_ERR_INVALID_ARG, MG_ERR_INVALID_GRAPH, MG_ERR_CUDA, MG_ERR_OOM = 0, -1, -2, -3, -4
+MG_RELABEL = 1
+MG_RGBA8, MG_RGBA16F, MG_BOTH, MG_FORCE_CONVERT = 1, 2, 3, 16
+ALL_LEVELS = 0xFFFFFFFF
+
+# every symbol include/mg.h declares (tests check that the library exports all of them)
+SYMBOLS = ["mg_load_graph", "mg_free_graph", "mg_graph_info", "mg_level_offsets", "mg_node_permutation",
+           "mg_relabel_indices", "mg_propagate", "mg_propagate_host", "mg_colorize", "mg_tf_update_host",
+           "mg_last_error", "mg_kernel_launch_count"]
+
+
+class MgInfo(C.Structure):
+    _fields_ = [("n_nodes", C.c_uint64), ("n_internal", C.c_uint64), ("n_leaves", C.c_uint32),
+                ("depth", C.c_uint32), ("n_topo_levels", C.c_uint32), ("first_fused_level", C.c_uint32),
+                ("n_launches_propagate", C.c_uint32), ("relabelled", C.c_uint32), ("device_bytes", C.c_uint64)]
+
+
+_vp = C.c_void_p
+lib.mg_load_graph.argtypes = [_vp, _vp, _vp, C.c_uint64, C.c_uint32, _vp, C.c_uint32, _vp, C.c_uint32, C.POINTER(_vp)]
+lib.mg_load_graph.restype = C.c_int
+lib.mg_free_graph.argtypes = [_vp]
+lib.mg_free_graph.restype = None
+lib.mg_graph_info.argtypes = [_vp, C.POINTER(MgInfo)]
+lib.mg_graph_info.restype = C.c_int
+lib.mg_level_offsets.argtypes = [_vp, _vp]
+lib.mg_level_offsets.restype = C.c_int
+lib.mg_node_permutation.argtypes = [_vp, _vp]
+lib.mg_node_permutation.restype = C.c_int
+lib.mg_relabel_indices.argtypes = [_vp, _vp, C.c_uint64, _vp]
+lib.mg_relabel_indices.restype = C.c_int
+lib.mg_propagate.argtypes = [_vp, _vp, _vp, _vp]
+lib.mg_propagate.restype = C.c_int
+lib.mg_propagate_host.argtypes = [_vp, _vp, _vp, _vp]
+lib.mg_propagate_host.restype = C.c_int
+lib.mg_colorize.argtypes = [_vp, C.c_uint32, _vp, C.c_uint64, _vp, _vp, _vp, C.c_uint32, _vp]
+lib.mg_colorize.restype = C.c_int
+lib.mg_tf_update_host.argtypes = [_vp, _vp, _vp, _vp, C.c_uint64, _vp, _vp, C.c_uint32, _vp]
+lib.mg_tf_update_host.restype = C.c_int
+lib.mg_last_error.argtypes = []
+lib.mg_last_error.restype = C.c_char_p
+lib.mg_kernel_launch_count.argtypes = []
+lib.mg_kernel_launch_count.restype = C.c_uint64
+
+
+class MgError(RuntimeError):
+    def __init__(self, code: int, where: str):
+        self.code = code
+        super().__init__(f"{where} failed with {code}: {lib.mg_last_error().decode()}")
+
+
+def _check(rc: int, where: str) -> None:
+    if rc != MG_OK:
+        raise MgError(rc, where)
+
+
+def _ptr(x) -> int | None:
+    """Address of a torch tensor / numpy array / raw int (None -> NULL)."""
+    if x is None:
+        return None
+    if isinstance(x, int):
+        return x
+    if isinstance(x, np.ndarray):
+        return x.ctypes.data
+    return x.data_ptr()          # torch.Tensor
+
+
+def _np(a, dt):
+    return None if a is None else np.ascontiguousarray(a, dtype=dt)
+
+
+def kernel_launch_count() -> int:
+    return int(lib.mg_kernel_launch_count())
+
+
+class Graph:
+    """Handle of a loaded Mixture Graph (mg_load_graph ... mg_free_graph)."""
+
+    def __init__(self, child_a, child_b, weight, n_leaves: int, level_offsets=None,
+                 leaf_segment_id=None, flags: int = 0):
+        a, b = _np(child_a, np.uint32), _np(child_b, np.uint32)
+        w = _np(weight, np.float32)
+        off = _np(level_offsets, np.uint64)
+        seg = _np(leaf_segment_id, np.uint32)
+        n_nodes = int(a.size)
+        n_topo = 0 if off is None else int(off.size) - 1
+        h = _vp()
+        self._h = None
+        _check(lib.mg_load_graph(_ptr(a), _ptr(b), _ptr(w), n_nodes, int(n_leaves), _ptr(off), n_topo,
+                                 _ptr(seg), int(flags), C.byref(h)), "mg_load_graph")
+        self._h = h
+
+    def close(self) -> None:
+        if self._h is not None:
+            lib.mg_free_graph(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    @property
+    def info(self) -> MgInfo:
+        i = MgInfo()
+        _check(lib.mg_graph_info(self._h, C.byref(i)), "mg_graph_info")
+        return i
+
+    def level_offsets(self) -> np.ndarray:
+        out = np.zeros(self.info.n_topo_levels + 1, dtype=np.uint64)
+        _check(lib.mg_level_offsets(self._h, _ptr(out)), "mg_level_offsets")
+        return out
+
+    def node_permutation(self) -> np.ndarray:
+        out = np.zeros(self.info.n_nodes, dtype=np.uint32)
+        _check(lib.mg_node_permutation(self._h, _ptr(out)), "mg_node_permutation")
+        return out
+
+    def relabel_indices(self, idx_device, n: int, stream: int = 0) -> None:
+        _check(lib.mg_relabel_indices(self._h, _ptr(idx_device), int(n), stream or None), "mg_relabel_indices")
+
+    def propagate(self, tf_device, node_rgba_device, stream: int = 0) -> None:
+        _check(lib.mg_propagate(self._h, _ptr(tf_device), _ptr(node_rgba_device), stream or None), "mg_propagate")
+
+    def propagate_host(self, tf_host, node_rgba_device, stream: int = 0) -> None:
+        _check(lib.mg_propagate_host(self._h, _ptr(tf_host), _ptr(node_rgba_device), stream or None),
+               "mg_propagate_host")
+
+    def colorize(self, node_idx_device, n_voxels: int, node_rgba_device, out, out_aux=None,
+                 fmt: int = MG_RGBA8, mip_level: int = ALL_LEVELS, stream: int = 0) -> None:
+        _check(lib.mg_colorize(self._h, int(mip_level), _ptr(node_idx_device), int(n_voxels),
+                               _ptr(node_rgba_device), _ptr(out), _ptr(out_aux), int(fmt), stream or None),
+               "mg_colorize")
+
+    def tf_update_host(self, tf_host, node_rgba_device, node_idx_device, n_voxels: int, out_device,
+                       out_host=None, fmt: int = MG_RGBA8, stream: int = 0) -> None:
+        _check(lib.mg_tf_update_host(self._h, _ptr(tf_host), _ptr(node_rgba_device), _ptr(node_idx_device),
+                                     int(n_voxels), _ptr(out_device), _ptr(out_host), int(fmt), stream or None),
+               "mg_tf_update_host")

@@ -198,22 +198,17 @@ def cylinder_volume(dims_xyz, params: np.ndarray, region=None) -> np.ndarray:
 # config 5: synthetic DAG stress + random node-index volume
 # ----------------------------------------------------------------------------------------------
 
-def random_dag(n_nodes: int, n_levels: int, n_leaves: int, seed: int):
-    """Random binary-lerp DAG (config 5 recipe, any size).
-
-    Level 0 = ``n_leaves`` leaves; levels 1..n_levels-1 share the remaining nodes equally (the
-    remainder goes to the last level).  ``child_a`` is uniform in level L-1 (so the topological
+def random_dag_levels(level_sizes, seed: int):
+    """Random binary-lerp DAG with the given number of nodes per topological level
+    (level_sizes[0] = number of leaves).  ``child_a`` is uniform in level L-1 (so the topological
     level of the node is exactly L), ``child_b`` uniform over all levels < L, redrawn (next
-    counter value) while equal to ``child_a``; ``weight`` = fp32 U(0,1) with 0 excluded.
+    stream) while equal to ``child_a``; ``weight`` = fp32 U(0,1) with 0 excluded.
     Returns (child_a u32, child_b u32, weight f32, level_offsets u64 [n_levels+1]); entries of
     the leaves in child/weight are 0."""
-    n_int = n_nodes - n_leaves
-    per = n_int // (n_levels - 1)
+    n_levels = len(level_sizes)
     off = np.zeros(n_levels + 1, dtype=np.uint64)
-    off[1] = n_leaves
-    for L in range(1, n_levels):
-        off[L + 1] = int(off[L]) + per
-    off[n_levels] = n_nodes
+    off[1:] = np.cumsum(np.asarray(level_sizes, dtype=np.uint64))
+    n_nodes = int(off[-1])
     a = np.zeros(n_nodes, dtype=np.uint32)
     b = np.zeros(n_nodes, dtype=np.uint32)
     w = np.zeros(n_nodes, dtype=np.float32)
@@ -234,6 +229,15 @@ def random_dag(n_nodes: int, n_levels: int, n_leaves: int, seed: int):
         ww[ww == 0.0] = np.float32(2.0 ** -24)
         a[lo:hi], b[lo:hi], w[lo:hi] = ca, cb, ww
     return a, b, w, off
+
+
+def random_dag(n_nodes: int, n_levels: int, n_leaves: int, seed: int):
+    """Config 5 recipe at any size: level 0 = ``n_leaves`` leaves; levels 1..n_levels-1 share the
+    remaining nodes equally (the remainder goes to the last level).  See random_dag_levels."""
+    per = (n_nodes - n_leaves) // (n_levels - 1)
+    sizes = [n_leaves] + [per] * (n_levels - 1)
+    sizes[-1] += n_nodes - sum(sizes)
+    return random_dag_levels(sizes, seed)
 
 
 def random_node_idx(n_voxels: int, n_nodes: int, seed: int, chunk: int = 1 << 24) -> np.ndarray:
