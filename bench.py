@@ -1,0 +1,389 @@
+#!/usr/bin/env python
+"""bench.py -- TF-update latency of the Mixture Graph hot path on B200 (contract: see DESIGN.md §Measurement).
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config 3] [--format rgba8|rgba16f]
+  python bench.py --impl reference ...      # the CPU fp64 oracle, as it stands, on the host cores
+
+One "step" = one full transfer-function update = every §8(a) device row:
+  a4 leaf assignment + a5 level-synchronous propagation (mg_propagate, TF already in HBM)
+  a6 colourise of EVERY mip level (mg_colorize over the concatenated node-index mipmap).
+`value` = milliseconds per TF update with all inputs resident in HBM (CUDA events on the launch
+stream, barrier + synchronize on both sides, max over ranks).  `e2e` = the same update through
+mg_tf_update_host: TF from pinned HOST memory, colourised mipmap copied back to pinned HOST memory,
+both copies inside the timed region.  Prints ONE JSON line (rank 0).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "tf_update_latency_ms"
+UNIT = "ms"
+FALLBACK_HBM_GBS = 6650.0            # /opt/skills/guides/B200_PROFILING.md fallback ("of fallback")
+NOMINAL_HBM_GBS = 8000.0             # BASELINE.json north_star "~8 TB/s"
+BYTES_PER_VOXEL = {"rgba8": 8, "rgba16f": 12}       # 4 B index + 4 B (8 B) output
+BYTES_PER_NODE_L2 = 28               # 12 B a/b/w stream + 16 B colour store (gathers hit L2), §8(d)
+
+
+def parse_args():
+    p = argparse.ArgumentParser()
+    p.add_argument("--gpus", type=int, default=1)
+    p.add_argument("--steps", type=int, default=300)
+    p.add_argument("--warmup", type=int, default=10)
+    p.add_argument("--impl", choices=["b200", "reference"], default="b200")
+    p.add_argument("--config", type=int, default=3, help="BASELINE.json config 1-5 (default 3: 2048x2048x300)")
+    p.add_argument("--scale", type=float, default=1.0, help="geometric down-scale of the config (debugging only)")
+    p.add_argument("--format", choices=["rgba8", "rgba16f"], default="rgba8")
+    p.add_argument("--e2e-steps", type=int, default=0, help="0 = min(steps, 8)")
+    p.add_argument("--no-cpu-baseline", action="store_true")
+    p.add_argument("--no-e2e", action="store_true")
+    p.add_argument("--cpu-sample-voxels", type=int, default=1 << 31, help="oracle sample size (>= the mipmap = whole workload)")
+    p.add_argument("--reference-budget-s", type=float, default=90.0)
+    return p.parse_args()
+
+
+# ------------------------------------------------------------------------------------------------
+# clocks: sample SM clock + throttle reasons DURING the timed region (NVML in a thread)
+# ------------------------------------------------------------------------------------------------
+
+class ClockSampler:
+    def __init__(self, device_index: int, period_s: float = 0.02):
+        self.samples, self.reasons, self.max_mhz = [], set(), None
+        self._stop = threading.Event()
+        self._thr = None
+        self._idx, self._period = device_index, period_s
+        self.error = None
+
+    def _visible_index(self) -> int:
+        vis = os.environ.get("CUDA_VISIBLE_DEVICES")
+        if vis:
+            ids = [v.strip() for v in vis.split(",") if v.strip()]
+            if self._idx < len(ids) and ids[self._idx].isdigit():
+                return int(ids[self._idx])
+        return self._idx
+
+    def _run(self):
+        try:
+            import pynvml as nv
+            nv.nvmlInit()
+            h = nv.nvmlDeviceGetHandleByIndex(self._visible_index())
+            self.max_mhz = int(nv.nvmlDeviceGetMaxClockInfo(h, nv.NVML_CLOCK_SM))
+            names = {"hw_slowdown": 0x8, "sw_thermal_slowdown": 0x20, "hw_thermal_slowdown": 0x40,
+                     "hw_power_brake_slowdown": 0x80, "sw_power_cap": 0x4, "sync_boost": 0x10,
+                     "applications_clocks_setting": 0x2}
+            while not self._stop.is_set():
+                self.samples.append(int(nv.nvmlDeviceGetClockInfo(h, nv.NVML_CLOCK_SM)))
+                try:
+                    r = int(nv.nvmlDeviceGetCurrentClocksEventReasons(h))
+                except Exception:
+                    r = int(nv.nvmlDeviceGetCurrentClocksThrottleReasons(h))
+                for k, bit in names.items():
+                    if r & bit:
+                        self.reasons.add(k)
+                time.sleep(self._period)
+        except Exception as exc:                      # noqa: BLE001 -- reported in the JSON, never fatal
+            self.error = repr(exc)
+
+    def __enter__(self):
+        self._thr = threading.Thread(target=self._run, daemon=True)
+        self._thr.start()
+        return self
+
+    def __exit__(self, *a):
+        self._stop.set()
+        self._thr.join(timeout=5)
+
+    def summary(self) -> dict:
+        out = {"sm_mhz": (float(np.median(self.samples)) if self.samples else None), "sm_max_mhz": self.max_mhz,
+               "reasons": sorted(self.reasons), "samples": len(self.samples)}
+        if self.error:
+            out["error"] = self.error
+        return out
+
+
+# ------------------------------------------------------------------------------------------------
+# the oracle as a timed CPU baseline (cpu_baseline leg and --impl reference): test infrastructure,
+# executed here only, as it stands (oracle/__init__.py: graph_eval_levels + colourise_rgba8)
+# ------------------------------------------------------------------------------------------------
+
+def _sample_plan(w, n_sample: int):
+    """Leading voxels of every mip level, in proportion to the level's size (>= 1 voxel each)."""
+    frac = min(1.0, n_sample / max(1, w.n_voxels))
+    return [max(1, int(np.ceil(v * frac))) if v else 0 for v in w.level_voxels]
+
+
+def oracle_step(w, tf64, plan, chunk: int = 1 << 25):
+    """One TF update by the oracle on a sample: (propagate seconds, colourise seconds, threads)."""
+    import oracle
+    g = w.host_graph
+    t0 = time.perf_counter()
+    c, used = oracle.graph_eval_levels(g["child_a"], g["child_b"], g["weight"], g["n_leaves"], tf64, n_threads=0)
+    t1 = time.perf_counter()
+    for lvl, n in zip(w.host_idx, plan):
+        flat = lvl.reshape(-1)
+        for o in range(0, n, chunk):
+            oracle.colourise_rgba8(flat[o:min(n, o + chunk)], c, n_threads=0)
+    t2 = time.perf_counter()
+    return t1 - t0, t2 - t1, int(used)
+
+
+def cpu_baseline(w, n_sample: int) -> dict:
+    plan = _sample_plan(w, n_sample)
+    tf64 = w.tf(0).astype(np.float64)
+    tp, tc, used = oracle_step(w, tf64, plan)
+    n_s = sum(plan)
+    ms = 1e3 * (tp + tc * (w.n_voxels / n_s))
+    return {"value": ms, "unit": UNIT, "cores": used, "kind": "oracle",
+            "sample": f"full fp64 level-synchronous propagation of all {w.stats['n_nodes']} nodes ({1e3 * tp:.1f} ms) + "
+                      f"fp64 lookup/RGBA8 conversion of the leading {n_s} of {w.n_voxels} voxels (same share of every "
+                      f"mip level, {1e3 * tc:.1f} ms), colourise time scaled to the whole mipmap",
+            "propagate_ms": 1e3 * tp, "colorize_sample_ms": 1e3 * tc, "sample_voxels": n_s}
+
+
+def workload_config(w, args, n_gpus: int) -> dict:
+    s = w.stats
+    cfg = {"workload": w.name, "baseline_config": args.config, "mip_voxels": w.n_voxels, "mip_levels": len(w.level_voxels),
+           "nodes": s["n_nodes"], "leaves": s["n_leaves"], "topo_depth": s["depth"], "output": args.format,
+           "parallelism": "single GPU" if n_gpus == 1 else f"{n_gpus} independent replicas (no collective)",
+           "l2": "inputs larger than L2 (node-index stream %.2f GB per step, L2 126 MB); no explicit flush" % (4e-9 * w.n_voxels)}
+    if "quant_bits" in s:
+        cfg["quant_bits"] = s["quant_bits"]
+    if args.scale != 1.0:
+        cfg["scale"] = args.scale
+    return cfg
+
+
+# ------------------------------------------------------------------------------------------------
+# distributed plumbing: one process per GPU, replicas only -- the only
+# cross-rank traffic is the timing reduction (max over ranks)
+# ------------------------------------------------------------------------------------------------
+
+def dist_env():
+    return int(os.environ.get("RANK", "0")), int(os.environ.get("LOCAL_RANK", "0")), int(os.environ.get("WORLD_SIZE", "1"))
+
+
+def peak_hbm_gbs():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(path) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs, burst copy)"
+    except Exception:                                   # noqa: BLE001
+        return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+def ncu_traffic(workload: str, kernel: str):
+    """dram bytes per launch of the dominant kernel from the committed ncu capture (profiles/), or None."""
+    path = os.path.join(ROOT, "profiles", "roofline_traffic.csv")
+    try:
+        with open(path) as f:
+            for line in f:
+                p = [x.strip() for x in line.split(",")]
+                if len(p) >= 4 and p[0] == workload and p[1] == kernel:
+                    return float(p[2]) + float(p[3])
+    except OSError:
+        pass
+    return None
+
+
+def run_b200(args) -> dict:
+    import torch
+    import torch.distributed as dist
+
+    rank, local_rank, world = dist_env()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the hot path has no CPU fallback)")
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    from paper_2009_02702_b200 import mg, workload
+
+    w = workload.make(args.config, args.scale)
+    g = w.graph
+    info = g.info
+    n_nodes, n_internal = int(info.n_nodes), int(info.n_internal)
+    fmt = mg.MG_RGBA8 if args.format == "rgba8" else mg.MG_RGBA16F
+    out_bytes = 4 if args.format == "rgba8" else 8
+    nodes = torch.empty((n_nodes, 4), dtype=torch.float32, device="cuda")
+    out = torch.empty(w.n_voxels_padded * out_bytes, dtype=torch.uint8, device="cuda")
+    n_tf = max(1, min(args.steps + args.warmup, 16))
+    tfs = [torch.from_numpy(w.tf(u)).cuda() for u in range(n_tf)]          # resident in HBM before the timed region
+    stream = torch.cuda.current_stream()
+    st = stream.cuda_stream
+
+    def step(k: int):
+        g.propagate(tfs[k % n_tf], nodes, st)
+        g.colorize(w.d_idx, w.n_voxels_padded, nodes, out, fmt=fmt, stream=st)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for k in range(args.warmup):
+        step(k)
+    barrier()
+    K = args.steps
+    ev = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(K)]
+    t_begin, t_end = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    launches0 = mg.kernel_launch_count()
+    with ClockSampler(local_rank) as clocks:
+        barrier()
+        t_begin.record(stream)
+        for k in range(K):
+            e = ev[k]
+            e[0].record(stream)
+            g.propagate(tfs[(args.warmup + k) % n_tf], nodes, st)
+            e[1].record(stream)
+            g.colorize(w.d_idx, w.n_voxels_padded, nodes, out, fmt=fmt, stream=st)
+            e[2].record(stream)
+        t_end.record(stream)
+        barrier()
+    launches = mg.kernel_launch_count() - launches0
+    total_ms = t_begin.elapsed_time(t_end)
+    prop_ms = np.array([e[0].elapsed_time(e[1]) for e in ev])
+    col_ms = np.array([e[1].elapsed_time(e[2]) for e in ev])
+    if world > 1:
+        t = torch.tensor([total_ms], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        total_ms = float(t.item())
+    ms_per_step = total_ms / K
+
+    # ---- e2e: host TF in, host mipmap out, through the public C-ABI call (rank-local, then max)
+    e2e = None
+    if not args.no_e2e:
+        ke = args.e2e_steps or min(K, 8)
+        tf_pinned = [torch.from_numpy(w.tf(u)).pin_memory() for u in range(min(n_tf, ke))]
+        out_host = torch.empty(w.n_voxels_padded * out_bytes, dtype=torch.uint8).pin_memory()
+        for k in range(2):
+            g.tf_update_host(tf_pinned[k % len(tf_pinned)], nodes, w.d_idx, w.n_voxels_padded, out, out_host, fmt=fmt, stream=st)
+        barrier()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        for k in range(ke):
+            g.tf_update_host(tf_pinned[k % len(tf_pinned)], nodes, w.d_idx, w.n_voxels_padded, out, out_host, fmt=fmt, stream=st)
+        e1.record(stream)
+        barrier()
+        e2e_ms = e0.elapsed_time(e1)
+        if world > 1:
+            t = torch.tensor([e2e_ms], dtype=torch.float64, device="cuda")
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            e2e_ms = float(t.item())
+        e2e = {"value": e2e_ms / ke / world, "unit": UNIT, "h2d_bytes_per_step": int(w.n_leaves * 16),
+               "d2h_bytes_per_step": int(w.n_voxels_padded * out_bytes), "steps": ke,
+               "what": "mg_tf_update_host: pinned-host TF -> H2D -> propagate -> colourise all levels -> D2H of the whole "
+                       "mipmap into pinned host memory (PCIe-bound)"}
+        del out_host
+
+    if rank != 0:
+        if world > 1:
+            dist.barrier()
+            dist.destroy_process_group()
+        return {}
+
+    peak, peak_src = peak_hbm_gbs()
+    bpv = BYTES_PER_VOXEL[args.format]
+    col_avg = float(col_ms.mean())
+    prop_avg = float(prop_ms.mean())
+    algo_bytes = float(bpv) * w.n_voxels
+    achieved = algo_bytes / (col_avg * 1e-3) / 1e9
+    kernel = "k_colorize"
+    res = {
+        "metric": METRIC, "value": ms_per_step / world, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": args.warmup,
+        "ms_per_step": ms_per_step, "higher_is_better": False, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f32", "data": "synthetic", "config": workload_config(w, args, world),
+        "propagate_ms": prop_avg, "colorize_ms": col_avg, "propagate_ms_min": float(prop_ms.min()), "colorize_ms_min": float(col_ms.min()),
+        "nodes_per_s": n_internal / (prop_avg * 1e-3), "voxels_per_s": w.n_voxels / (col_avg * 1e-3),
+        "hbm_gbs_step": (algo_bytes + BYTES_PER_NODE_L2 * n_internal) / (ms_per_step * 1e-3) / 1e9,
+        "frac_of_nominal_8TBs": achieved / NOMINAL_HBM_GBS,
+        "roofline": {"bound": "hbm", "kernel": kernel, "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                     "traffic": ncu_traffic(w.name, kernel), "algorithmic_bytes_per_launch": algo_bytes,
+                     "avg_launch_ms": col_avg, "peak_source": peak_src,
+                     "timing": "CUDA events on the launch stream around every mg_colorize of the timed region"},
+        "gpu_launches": int(launches), "clocks": clocks.summary(),
+        "paper_context": "RTX Titan palette update (propagation only, incl. TF upload): 3.5 / 11.3 / 12.1 ms for 1.03 / 5.20 / 1.93 M "
+                         "nodes (PAPER.md L373); the paper never materialises the RGBA mipmap (L221)",
+        "setup_s": {k: round(v, 3) for k, v in w.stats.items() if k.endswith("_s")},
+    }
+    if e2e is not None:
+        res["e2e"] = e2e
+    if world == 1 and not args.no_cpu_baseline and w.host_idx is not None:
+        res["cpu_baseline"] = cpu_baseline(w, args.cpu_sample_voxels)
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+    return res
+
+
+# ------------------------------------------------------------------------------------------------
+# --impl reference: there is no reference implementation (the paper ships no code), so this arm
+# times the CPU fp64 oracle, as it stands, on the host cores; each step a bounded sample
+# ------------------------------------------------------------------------------------------------
+
+def run_reference(args) -> dict:
+    rank, local_rank, world = dist_env()
+    if rank != 0:
+        return {}
+    import torch
+    if torch.cuda.is_available():
+        torch.cuda.set_device(local_rank)
+    from paper_2009_02702_b200 import workload
+    # the oracle's inputs (graph + node-index mipmap) come from the same seeded assembly as the GPU arm
+    w = workload.make(args.config, args.scale, device_synth=torch.cuda.is_available())
+    if w.graph is not None:
+        w.graph.close()
+        w.graph = None
+    w.d_idx = None
+    tf64 = [w.tf(u).astype(np.float64) for u in range(4)]
+    # calibrate the per-step sample so that steps + warmup fit the budget
+    probe = _sample_plan(w, 1 << 22)
+    tp, tc, used = oracle_step(w, tf64[0], probe)
+    per_voxel = tc / sum(probe)
+    n_total = args.steps + args.warmup
+    budget_per_step = max(0.05, args.reference_budget_s / max(1, n_total) - tp)
+    n_sample = int(min(w.n_voxels, max(1 << 16, budget_per_step / per_voxel)))
+    plan = _sample_plan(w, n_sample)
+    n_s = sum(plan)
+    for k in range(args.warmup):
+        oracle_step(w, tf64[k % 4], plan)
+    t0 = time.perf_counter()
+    tps, tcs = [], []
+    for k in range(args.steps):
+        a, b, used = oracle_step(w, tf64[(args.warmup + k) % 4], plan)
+        tps.append(a)
+        tcs.append(b)
+    wall = time.perf_counter() - t0
+    tp, tc = float(np.mean(tps)), float(np.mean(tcs))
+    ms = 1e3 * (tp + tc * (w.n_voxels / n_s))
+    sample = (f"per step: full fp64 propagation of {w.stats['n_nodes']} nodes + lookup/RGBA8 of the leading {n_s} of "
+              f"{w.n_voxels} voxels (same share of every mip level); colourise time scaled to the whole mipmap")
+    cfg = workload_config(w, args, 1)
+    cfg["output"] = "rgba8"
+    return {"impl": "reference", "metric": METRIC, "value": ms, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": 1e3 * wall / max(1, args.steps), "higher_is_better": False, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic", "config": cfg,
+            "cpu_baseline": {"value": ms, "unit": UNIT, "cores": used, "kind": "oracle", "sample": sample},
+            "e2e": {"value": ms, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0, "propagate_ms": 1e3 * tp, "colorize_sample_ms": 1e3 * tc,
+            "note": "no reference implementation exists for this paper; this arm is the repo's CPU fp64 oracle (test "
+                    "infrastructure), a deliberately plain program: the ratio against it is not the headline"}
+
+
+def main():
+    args = parse_args()
+    res = run_reference(args) if args.impl == "reference" else run_b200(args)
+    if res:
+        print(json.dumps(res), flush=True)
+
+
+if __name__ == "__main__":
+    main()

@@ -1,0 +1,168 @@
+"""Assemble one of the BASELINE.json configs end to end on the current CUDA device.
+
+Plumbing only (none of the method's arithmetic): volume generator (synth / synth_gpu) -> host
+builder (libmg_builder.so: a0-a2) -> mg_load_graph (a3) -> the per-voxel node indices of every
+mip level uploaded into ONE device buffer.  Used by bench.py, by the full-size parity tests and
+by __graft_entry__; nothing here imports ``oracle/``.
+
+Device layout of the mipmap (indices and outputs alike): the mip levels are concatenated finest
+first; level l starts at voxel ``level_start[l]``, a multiple of 64 voxels (256 B for the uint32
+indices and the RGBA8 output, 512 B for fp16), so that every level is a self-contained, vector-
+aligned sub-buffer a renderer can bind on its own, and ONE mg_colorize call over
+``n_voxels_padded`` voxels covers all levels.  Padding voxels hold node index 0.
+"""
+from __future__ import annotations
+
+import time
+
+import numpy as np
+
+from . import builder, mg, synth
+
+LEVEL_ALIGN = 64          # voxels
+
+
+class Workload:
+    """A loaded graph plus its device-resident node-index mipmap."""
+
+    def __init__(self, name: str):
+        self.name = name
+        self.graph: mg.Graph | None = None
+        self.host_graph: dict | None = None       # child_a, child_b, weight, level_offsets, n_leaves (builder numbering = library numbering)
+        self.mip_dims: list = []                  # [(X_l, Y_l, Z_l)]
+        self.level_start: list = []               # first voxel of level l in the concatenated buffers
+        self.level_voxels: list = []              # voxels of level l
+        self.n_voxels = 0                         # real voxels (sum of level_voxels)
+        self.n_voxels_padded = 0                  # extent of the concatenated buffers
+        self.d_idx = None                         # torch int32 [n_voxels_padded] (uint32 values)
+        self.host_idx = None                      # list of numpy uint32 views per level (builder-owned) or arrays
+        self.build_result = None                  # keeps the builder-owned arrays alive
+        self.stats: dict = {}
+        self.n_leaves = 0
+        self.cfg: dict = {}
+
+    def tf(self, update: int = 0) -> np.ndarray:
+        """fp32 [n_leaves, 4] transfer function number ``update`` of this config (synth recipe)."""
+        c = self.cfg
+        return synth.random_tf(self.n_leaves, c.get("seed", 0), update=update,
+                               alpha_zero_frac=c.get("alpha_zero_frac", 0.0))
+
+    def close(self) -> None:
+        if self.graph is not None:
+            self.graph.close()
+            self.graph = None
+        self.d_idx = None
+        self.host_idx = None
+        if self.build_result is not None:
+            self.build_result.close()
+            self.build_result = None
+
+
+def _layout(level_voxels):
+    start, pos = [], 0
+    for n in level_voxels:
+        start.append(pos)
+        pos += -(-n // LEVEL_ALIGN) * LEVEL_ALIGN
+    return start, pos
+
+
+def _upload_levels(w: Workload, levels) -> None:
+    import torch
+    w.level_voxels = [int(a.size) for a in levels]
+    w.level_start, w.n_voxels_padded = _layout(w.level_voxels)
+    w.n_voxels = sum(w.level_voxels)
+    d = torch.zeros(max(w.n_voxels_padded, 1), dtype=torch.int32, device="cuda")
+    chunk = 1 << 27                                # 512 MB pieces through pageable memory
+    for s, a in zip(w.level_start, levels):
+        flat = a.reshape(-1).view(np.int32)
+        for o in range(0, flat.size, chunk):
+            e = min(flat.size, o + chunk)
+            d[s + o:s + e].copy_(torch.from_numpy(flat[o:e]))
+    w.d_idx = d
+    w.host_idx = levels
+
+
+def from_volume(seg: np.ndarray, name: str = "volume", cfg: dict | None = None, keep_host: bool = True,
+                **builder_params) -> Workload:
+    """Builder + load + upload for a uint32 [Z, Y, X] segment-ID volume."""
+    w = Workload(name)
+    w.cfg = dict(cfg or {})
+    t0 = time.perf_counter()
+    r = builder.build(seg, **builder_params)
+    t1 = time.perf_counter()
+    g = r.graph()
+    w.host_graph = g
+    w.n_leaves = g["n_leaves"]
+    w.mip_dims = r.mip_dims
+    w.graph = mg.Graph(g["child_a"], g["child_b"], g["weight"], g["n_leaves"], level_offsets=g["level_offsets"],
+                       leaf_segment_id=g["leaf_segment_id"])
+    t2 = time.perf_counter()
+    levels = [r.node_idx(l, copy=False) for l in range(r.info.n_mip_levels)]
+    _upload_levels(w, levels)
+    t3 = time.perf_counter()
+    i = r.info
+    w.stats = dict(builder_s=t1 - t0, load_graph_s=t2 - t1, upload_idx_s=t3 - t2, n_nodes=int(i.n_nodes),
+                   n_leaves=int(i.n_leaves), depth=int(i.depth), quant_bits=int(i.quant_bits),
+                   n_distinct_mixtures=int(i.n_distinct_mixtures), nnz_per_voxel=i.nnz_total / max(1, i.n_voxels_total),
+                   n_mip_levels=int(i.n_mip_levels), builder_mipmap_s=i.seconds_mipmap,
+                   builder_factorise_s=i.seconds_factorise, builder_finalise_s=i.seconds_finalise,
+                   phi2_exact=int(i.phi2_exact), n_stage1=int(i.n_stage1), n_stage2=int(i.n_stage2), n_big=int(i.n_big),
+                   level_sizes=np.diff(g["level_offsets"].astype(np.int64)).tolist())
+    if keep_host:
+        w.build_result = r
+    else:
+        w.host_idx = None
+        r.close()
+    return w
+
+
+def from_dag(child_a, child_b, weight, level_offsets, n_leaves: int, node_idx: np.ndarray, name: str = "dag",
+             cfg: dict | None = None) -> Workload:
+    """A ready-made level-contiguous DAG plus ONE node-index volume (config 5)."""
+    w = Workload(name)
+    w.cfg = dict(cfg or {})
+    w.n_leaves = int(n_leaves)
+    t0 = time.perf_counter()
+    w.graph = mg.Graph(child_a, child_b, weight, n_leaves, level_offsets=level_offsets)
+    t1 = time.perf_counter()
+    w.host_graph = dict(child_a=child_a, child_b=child_b, weight=weight, level_offsets=np.asarray(level_offsets),
+                        n_leaves=int(n_leaves))
+    w.mip_dims = [(int(node_idx.size), 1, 1)]
+    _upload_levels(w, [node_idx.reshape(-1)])
+    t2 = time.perf_counter()
+    off = np.asarray(level_offsets, dtype=np.int64)
+    w.stats = dict(load_graph_s=t1 - t0, upload_idx_s=t2 - t1, n_nodes=int(child_a.size), n_leaves=int(n_leaves),
+                   depth=int(off.size - 2), level_sizes=np.diff(off).tolist())
+    return w
+
+
+def make(cfg_id: int, scale: float = 1.0, device_synth: bool = True, **builder_params) -> Workload:
+    """BASELINE.json config ``cfg_id`` (1-5); ``scale`` < 1 gives a geometrically similar smaller
+    instance (tests).  Volumes are generated on the GPU (bit-identical to synth.py) unless
+    ``device_synth`` is False."""
+    if cfg_id == 5:
+        c = dict(synth.CONFIGS[5])
+        n_nodes = max(1 << 10, int(round(c["n_nodes"] * scale)))
+        n_leaves = max(16, int(round(c["n_leaves"] * scale)))
+        n_vox = max(1 << 10, int(round(c["volume_voxels"] * scale)))
+        t0 = time.perf_counter()
+        a, b, wt, off = synth.random_dag(n_nodes, c["n_levels"], n_leaves, c["seed"])
+        idx = synth.random_node_idx(n_vox, n_nodes, c["seed"])
+        t1 = time.perf_counter()
+        w = from_dag(a, b, wt, off, n_leaves, idx, name=c["name"] + (f"_x{scale:g}" if scale != 1.0 else ""), cfg=c)
+        w.stats["synth_s"] = t1 - t0
+        return w
+    c = synth.scaled_config(cfg_id, scale)
+    t0 = time.perf_counter()
+    if device_synth:
+        import torch
+        from . import synth_gpu
+        seg = synth_gpu.make_volume(c).cpu().numpy().view(np.uint32)
+        torch.cuda.empty_cache()
+    else:
+        seg = synth.make_volume(c)
+    t1 = time.perf_counter()
+    w = from_volume(seg, name=c["name"], cfg=c, **builder_params)
+    del seg
+    w.stats["synth_s"] = t1 - t0
+    return w
