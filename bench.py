@@ -172,6 +172,22 @@ def dist_env():
     return int(os.environ.get("RANK", "0")), int(os.environ.get("LOCAL_RANK", "0")), int(os.environ.get("WORLD_SIZE", "1"))
 
 
+def max_over_ranks(value: float, world: int, device="cpu") -> float:
+    """MAX over all ranks of a per-rank duration (the only cross-rank traffic of a replica run)."""
+    if world <= 1:
+        return float(value)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([value], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def aggregate_value(ms_per_step: float, world: int) -> float:
+    """Whole-job milliseconds per TF update: `world` independent replicas finish `world` updates per step."""
+    return ms_per_step / max(1, world)
+
+
 def peak_hbm_gbs():
     path = os.path.join(ROOT, "MEASURED_PEAKS.json")
     try:
@@ -252,10 +268,7 @@ def run_b200(args) -> dict:
     total_ms = t_begin.elapsed_time(t_end)
     prop_ms = np.array([e[0].elapsed_time(e[1]) for e in ev])
     col_ms = np.array([e[1].elapsed_time(e[2]) for e in ev])
-    if world > 1:
-        t = torch.tensor([total_ms], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        total_ms = float(t.item())
+    total_ms = max_over_ranks(total_ms, world, "cuda")
     ms_per_step = total_ms / K
 
     # ---- e2e: host TF in, host mipmap out, through the public C-ABI call (rank-local, then max)
@@ -274,11 +287,8 @@ def run_b200(args) -> dict:
         e1.record(stream)
         barrier()
         e2e_ms = e0.elapsed_time(e1)
-        if world > 1:
-            t = torch.tensor([e2e_ms], dtype=torch.float64, device="cuda")
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            e2e_ms = float(t.item())
-        e2e = {"value": e2e_ms / ke / world, "unit": UNIT, "h2d_bytes_per_step": int(w.n_leaves * 16),
+        e2e_ms = max_over_ranks(e2e_ms, world, "cuda")
+        e2e = {"value": aggregate_value(e2e_ms / ke, world), "unit": UNIT, "h2d_bytes_per_step": int(w.n_leaves * 16),
                "d2h_bytes_per_step": int(w.n_voxels_padded * out_bytes), "steps": ke,
                "what": "mg_tf_update_host: pinned-host TF -> H2D -> propagate -> colourise all levels -> D2H of the whole "
                        "mipmap into pinned host memory (PCIe-bound)"}
@@ -298,7 +308,7 @@ def run_b200(args) -> dict:
     achieved = algo_bytes / (col_avg * 1e-3) / 1e9
     kernel = "k_colorize"
     res = {
-        "metric": METRIC, "value": ms_per_step / world, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": args.warmup,
+        "metric": METRIC, "value": aggregate_value(ms_per_step, world), "unit": UNIT, "n_gpus": world, "steps": K, "warmup": args.warmup,
         "ms_per_step": ms_per_step, "higher_is_better": False, "scaling": "weak", "vs_baseline": None,
         "dtype": "f32", "data": "synthetic", "config": workload_config(w, args, world),
         "propagate_ms": prop_avg, "colorize_ms": col_avg, "propagate_ms_min": float(prop_ms.min()), "colorize_ms_min": float(col_ms.min()),

@@ -40,6 +40,7 @@ class Workload:
         self.stats: dict = {}
         self.n_leaves = 0
         self.cfg: dict = {}
+        self.seg = None                           # uint32 [Z, Y, X] segmentation (only with keep_seg)
 
     def tf(self, update: int = 0) -> np.ndarray:
         """fp32 [n_leaves, 4] transfer function number ``update`` of this config (synth recipe)."""
@@ -136,10 +137,11 @@ def from_dag(child_a, child_b, weight, level_offsets, n_leaves: int, node_idx: n
     return w
 
 
-def make(cfg_id: int, scale: float = 1.0, device_synth: bool = True, **builder_params) -> Workload:
+def make(cfg_id: int, scale: float = 1.0, device_synth: bool = True, keep_seg: bool = False,
+         **builder_params) -> Workload:
     """BASELINE.json config ``cfg_id`` (1-5); ``scale`` < 1 gives a geometrically similar smaller
     instance (tests).  Volumes are generated on the GPU (bit-identical to synth.py) unless
-    ``device_synth`` is False."""
+    ``device_synth`` is False.  ``keep_seg`` keeps the generated volume in ``Workload.seg``."""
     if cfg_id == 5:
         c = dict(synth.CONFIGS[5])
         n_nodes = max(1 << 10, int(round(c["n_nodes"] * scale)))
@@ -163,6 +165,8 @@ def make(cfg_id: int, scale: float = 1.0, device_synth: bool = True, **builder_p
         seg = synth.make_volume(c)
     t1 = time.perf_counter()
     w = from_volume(seg, name=c["name"], cfg=c, **builder_params)
+    if keep_seg:
+        w.seg = seg                                # the generator's volume (tests: input of the oracle)
     del seg
     w.stats["synth_s"] = t1 - t0
     return w

@@ -1,0 +1,55 @@
+"""The N > 1 path of bench.py is "replicas only": no data-path collective, the only
+cross-rank traffic is the MAX reduction of the per-rank step time.  World size 2 over gloo on CPU."""
+import os
+import socket
+import sys
+
+import pytest
+
+torch = pytest.importorskip("torch")
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def _free_port():
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        return s.getsockname()[1]
+
+
+def _worker(rank, world, port, q):
+    import torch.distributed as dist
+    sys.path.insert(0, ROOT)
+    import bench
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), LOCAL_RANK=str(rank),
+                      WORLD_SIZE=str(world))
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    assert bench.dist_env() == (rank, rank, world)
+    mine = 1.5 + rank                      # rank 1 is the slow replica
+    total = bench.max_over_ranks(mine, world, "cpu")
+    dist.barrier()
+    q.put((rank, total, bench.aggregate_value(total, world)))
+    dist.destroy_process_group()
+
+
+def test_max_over_ranks_and_aggregate_world2():
+    import torch.multiprocessing as mp
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = _free_port()
+    procs = [ctx.Process(target=_worker, args=(r, 2, port, q)) for r in range(2)]
+    for p in procs:
+        p.start()
+    res = sorted(q.get(timeout=120) for _ in procs)
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    assert [r[1] for r in res] == [2.5, 2.5]            # both ranks see the slowest replica's time
+    assert [r[2] for r in res] == [1.25, 1.25]          # 2 replicas -> 2 updates per step time
+
+
+def test_single_rank_is_identity():
+    sys.path.insert(0, ROOT)
+    import bench
+    assert bench.max_over_ranks(3.25, 1) == 3.25 and bench.aggregate_value(3.25, 1) == 3.25
+    assert bench.dist_env()[2] >= 1

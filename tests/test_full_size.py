@@ -1,0 +1,219 @@
+"""Full-size parity: BASELINE.json's configs in the launch configuration bench.py times.
+
+The whole workload is assembled exactly as bench.py does (workload.make: GPU volume generator ->
+host builder -> mg_load_graph -> ONE concatenated node-index mipmap, ONE mg_colorize call over all
+levels).  The oracle cannot colourise 1.4 G voxels element by element in seconds, so:
+  * node colours: EVERY node against the same-graph oracle (O-4), leaves bit-exact, max-abs <= 1e-5;
+  * level 0 (87 % of the voxels): EVERY voxel -- its colour must be the RGBA8 code of TF[S(v)] (I5, L223),
+    with S from the input generator (not from the builder) and the 4 x n_leaves codes from the oracle;
+  * every other level: seeded random samples + the first/last voxels of the level against the oracle's
+    lookup/conversion on the same graph, and padding voxels against node 0;
+  * quantised-graph colour vs the DIRECT histogram (O-3 brute force on the generator's volume) on
+    sampled mixed voxels of levels 1-7: max-abs <= 2e-3 (north_star).
+"""
+import numpy as np
+import pytest
+
+import oracle
+from paper_2009_02702_b200 import synth
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+TOL = 1e-5
+TOL_DIRECT = 2e-3
+
+
+@pytest.fixture(scope="module")
+def libs():
+    if not torch.cuda.is_available():
+        pytest.fail("the gpu-marked tests need a CUDA device (no CPU fallback exists)")
+    from paper_2009_02702_b200 import mg, workload
+    torch.cuda.set_device(0)
+    return mg, workload
+
+
+def _leaf_index_chunked(S):
+    """Sorted distinct IDs and per-voxel leaf number of a big volume (same result as oracle.leaf_index,
+    slab by slab to bound memory)."""
+    mx = int(S.max())
+    cnt = np.zeros(mx + 1, dtype=np.int64)
+    for z in range(S.shape[0]):
+        cnt += np.bincount(S[z].reshape(-1), minlength=mx + 1)
+    ids = np.flatnonzero(cnt).astype(np.uint32)
+    lut = np.zeros(mx + 1, dtype=np.uint32)
+    lut[ids] = np.arange(ids.size, dtype=np.uint32)
+    out = np.empty(S.shape, dtype=np.uint32)
+    for z in range(S.shape[0]):
+        out[z] = lut[S[z]]
+    return ids, out
+
+
+def _rgba8_close(got, ref_c):
+    """got uint8 [n,4] vs oracle colours fp64 [n,4]: equal codes, or +-1 next to a rounding boundary."""
+    code = oracle.to_rgba8(ref_c).astype(np.int64)
+    diff = got.astype(np.int64) - code
+    if not diff.any():
+        return True
+    scaled = np.clip(ref_c, 0.0, 1.0) * 255.0
+    near = np.abs(scaled - np.floor(scaled) - 0.5) <= 255 * TOL + 1e-4
+    return bool(((diff == 0) | ((np.abs(diff) == 1) & near)).all())
+
+
+def _run_update(mg, w, tf, fmt):
+    g = w.graph
+    nodes = torch.full((g.info.n_nodes, 4), float("nan"), dtype=torch.float32, device="cuda")
+    bpv = 4 if fmt == mg.MG_RGBA8 else 8
+    out = torch.full((w.n_voxels_padded * bpv,), 0xAB, dtype=torch.uint8, device="cuda")
+    st = torch.cuda.current_stream().cuda_stream
+    g.propagate(torch.from_numpy(tf).cuda(), nodes, st)
+    g.colorize(w.d_idx, w.n_voxels_padded, nodes, out, fmt=fmt, stream=st)
+    torch.cuda.synchronize()
+    return nodes, out
+
+
+def _check_nodes(w, nodes, tf):
+    hg = w.host_graph
+    ref = oracle.graph_eval(hg["child_a"], hg["child_b"], hg["weight"], hg["n_leaves"], tf.astype(np.float64))
+    got = nodes.cpu().numpy()
+    nl = hg["n_leaves"]
+    assert np.array_equal(got[:nl].view(np.uint32), tf.view(np.uint32)), "leaves not bit-exact"
+    err = float(np.abs(got - ref).max())
+    assert err <= TOL, err
+    return ref
+
+
+def _sample_positions(n, k, seed, stream):
+    k = min(k, n)
+    pos = (synth.u64(seed, stream, np.arange(k, dtype=np.uint64)) % np.uint64(n)).astype(np.int64)
+    edge = np.concatenate([np.arange(min(n, 70)), np.arange(max(0, n - 70), n)])
+    return np.unique(np.concatenate([pos, edge]))
+
+
+@pytest.mark.parametrize("cfg_id", [3, 2, 4])
+def test_volume_config_full_size(libs, cfg_id):
+    mg, workload = libs
+    w = workload.make(cfg_id, keep_seg=True)
+    try:
+        c = synth.CONFIGS[cfg_id]
+        X, Y, Z = c["dims"]
+        assert w.mip_dims == oracle.mip_dims((X, Y, Z))                     # O-1 at full size (Table 2 totals)
+        assert w.n_voxels == sum(x * y * z for x, y, z in w.mip_dims)
+        tf = w.tf(1)
+        nodes, out = _run_update(mg, w, tf, mg.MG_RGBA8)
+        ref_nodes = _check_nodes(w, nodes, tf)
+        out4 = out.view(-1, 4)
+
+        # ---- level 0, every voxel: out == code(TF[S(v)])  (I5; S from the generator)
+        ids, seg_index = _leaf_index_chunked(w.seg)
+        assert np.array_equal(ids, w.host_graph["leaf_segment_id"])
+        code_tf = torch.from_numpy(oracle.to_rgba8(tf.astype(np.float64)).view(np.uint32).reshape(-1).astype(np.int64)).cuda()
+        n0 = w.level_voxels[0]
+        flat = seg_index.reshape(-1)
+        out32 = out.view(torch.int32)
+        bad = 0
+        step = 1 << 27
+        for o in range(0, n0, step):
+            e = min(n0, o + step)
+            s = torch.from_numpy(flat[o:e].astype(np.int64)).cuda()
+            exp = code_tf[s]
+            got = out32[o:e].to(torch.int64) & 0xFFFFFFFF
+            bad += int((got != exp).sum().item())
+        assert bad == 0, f"{bad} level-0 voxels differ from code(TF[S(v)])"
+
+        # ---- every level: samples + edges against the oracle's lookup on the same graph
+        out_host_levels = []
+        for l, (s0, nv) in enumerate(zip(w.level_start, w.level_voxels)):
+            pos = _sample_positions(nv, 200000, 77 + cfg_id, l)
+            got = out4[torch.from_numpy(pos + s0).cuda()].cpu().numpy()
+            idx = w.host_idx[l].reshape(-1)[pos]
+            assert _rgba8_close(got, oracle.lookup(idx, ref_nodes)), f"level {l}"
+            out_host_levels.append((pos, got))
+            pad_end = w.level_start[l + 1] if l + 1 < len(w.level_start) else w.n_voxels_padded
+            if pad_end > s0 + nv:                                            # padding voxels: node 0
+                padv = out4[s0 + nv:pad_end].cpu().numpy()
+                assert _rgba8_close(padv, np.broadcast_to(ref_nodes[0], padv.shape).copy())
+
+        # ---- quantised graph vs the DIRECT histogram on sampled mixed voxels (levels 1-7)
+        nl = ids.size
+        tf64 = tf.astype(np.float64)
+        nodes_host = nodes.cpu().numpy().astype(np.float64)
+        worst = 0.0
+        for l in range(1, min(8, len(w.mip_dims))):
+            xl, yl, zl = w.mip_dims[l]
+            idx_l = w.host_idx[l].reshape(-1)
+            mixed = np.flatnonzero(idx_l >= nl)
+            if mixed.size == 0:
+                continue
+            pick = mixed[(synth.u64(5, 300 + l, np.arange(6, dtype=np.uint64)) % np.uint64(mixed.size)).astype(np.int64)]
+            for v in pick:
+                k, rem = divmod(int(v), xl * yl)
+                j, i = divmod(rem, xl)
+                h = oracle.brute_force_histogram(seg_index, nl, l, i, j, k)
+                assert abs(h.sum() - 1.0) < 1e-12
+                direct = h @ tf64
+                worst = max(worst, float(np.abs(nodes_host[idx_l[v]] - direct).max()))
+        assert worst <= TOL_DIRECT, worst
+        print(f"cfg {cfg_id}: {w.stats['n_nodes']} nodes depth {w.stats['depth']}, max |graph - direct| on samples = {worst:.2e}")
+    finally:
+        w.close()
+
+
+def test_config3_fp16_output_full_size(libs):
+    """Same launch configuration with the fp16 output: sampled voxels within 1 fp16 ulp of RN(oracle)."""
+    mg, workload = libs
+    w = workload.make(3)
+    try:
+        tf = w.tf(2)
+        nodes, out = _run_update(mg, w, tf, mg.MG_RGBA16F)
+        ref_nodes = _check_nodes(w, nodes, tf)
+        out4 = out.view(torch.float16).view(-1, 4)
+        for l, (s0, nv) in enumerate(zip(w.level_start, w.level_voxels)):
+            pos = _sample_positions(nv, 100000, 91, l)
+            got = out4[torch.from_numpy(pos + s0).cuda()].cpu().numpy()
+            ref = oracle.to_rgba16f(oracle.lookup(w.host_idx[l].reshape(-1)[pos], ref_nodes))
+            gi, ri = got.view(np.int16).astype(np.int64), ref.view(np.int16).astype(np.int64)
+            assert (np.abs(gi - ri) <= 1).all(), f"level {l}"
+    finally:
+        w.close()
+
+
+def test_config5_dag_stress_full_size(libs):
+    """2^26 nodes, 24 levels, 2^14 leaves, random children; 512^3 random node-index volume."""
+    mg, workload = libs
+    w = workload.make(5)
+    try:
+        assert w.graph.info.n_nodes == 1 << 26 and w.graph.info.depth == 23 and w.n_voxels == 512 ** 3
+        tf = w.tf(0)
+        nodes, out = _run_update(mg, w, tf, mg.MG_RGBA8)
+        ref_nodes = _check_nodes(w, nodes, tf)                               # every one of the 2^26 nodes
+        out4 = out.view(-1, 4)
+        pos = _sample_positions(w.n_voxels, 2000000, 93, 0)
+        got = out4[torch.from_numpy(pos).cuda()].cpu().numpy()
+        assert _rgba8_close(got, oracle.lookup(w.host_idx[0][pos], ref_nodes))
+    finally:
+        w.close()
+
+
+def test_config1_every_voxel_every_level(libs):
+    """Config 1 (64^3, 16 segments): element-by-element on all 299,593 voxels, unquantised and b = 9,
+    both against the same-graph oracle and against the direct histogram (dense O-2)."""
+    mg, workload = libs
+    for bits, tol_direct in ((0, 1e-5), (9, TOL_DIRECT)):
+        w = workload.make(1, keep_seg=True, quant_bits=bits)
+        try:
+            tf = w.tf(0)
+            nodes, out = _run_update(mg, w, tf, mg.MG_RGBA8)
+            ref_nodes = _check_nodes(w, nodes, tf)
+            ids, seg_index = oracle.leaf_index(w.seg)
+            H = oracle.histogram_mipmap(seg_index, ids.size)
+            out4 = out.view(-1, 4).cpu().numpy()
+            got_nodes = nodes.cpu().numpy().astype(np.float64)
+            for l, counts in enumerate(H):
+                s0, nv = w.level_start[l], w.level_voxels[l]
+                idx = w.host_idx[l].reshape(-1)
+                assert _rgba8_close(out4[s0:s0 + nv], oracle.lookup(idx, ref_nodes))
+                direct = oracle.direct_colour(counts, l, tf.astype(np.float64)).reshape(-1, 4)
+                assert np.abs(got_nodes[idx] - direct).max() <= tol_direct
+        finally:
+            w.close()
