@@ -1,4 +1,5 @@
 // mg_api.cu -- graph object: validation, relabelling, device upload, info (include/mg.h).
+#include <algorithm>
 #include <atomic>
 #include <cmath>
 #include <cstdarg>
@@ -30,25 +31,52 @@ int cuda_fail(cudaError_t e, const char* what)
 
 void count_launch(unsigned n) { g_launches.fetch_add(n, std::memory_order_relaxed); }
 
-// Levels >= first_fused_level run inside one persistent CTA.  A level goes to that CTA when it and
-// every later level has at most kTailMaxLevelNodes nodes: below that size one more kernel launch
-// (a few microseconds of dependent-launch latency) costs more than the level itself.
+// Levels >= first_fused_level run inside ONE persistent CTA (k_tail) that works entirely in shared
+// memory: the distinct "external" children (below the tail) are gathered once, then every level is
+// smem gathers + a __syncthreads().  The tail is the longest suffix of levels whose working set fits:
+//   16 B x (external children + tail nodes)  +  12 B x tail nodes (a, b, w staged)  <=  kTailSmemBytes
+// and whose levels have at most kTailMaxLevelNodes nodes each (a bigger level is worth a full-grid launch).
 static const uint64_t kTailMaxLevelNodes = 8192;
-// Nodes of the fused tail whose colours are also kept in shared memory (float4 each).
-static const uint32_t kTailSmemNodes = 12288;   // 192 KB
+static const uint64_t kTailSmemBytes = MG_TAIL_SMEM_BYTES;
 
-static void plan_launches(mg_graph* g)
+// ha / hb: host child arrays in library numbering.  Fills the plan and the local-index arrays.
+static void plan_launches(mg_graph* g, const std::vector<uint32_t>& ha, const std::vector<uint32_t>& hb,
+                          std::vector<uint32_t>& ext, std::vector<uint32_t>& la, std::vector<uint32_t>& lb)
 {
-    uint32_t first = g->n_levels;   // none
+    g->first_fused_level = 0;
+    g->tail_base = (uint32_t)g->n_nodes;
+    g->tail_n = g->tail_n_ext = 0;
+    ext.clear(); la.clear(); lb.clear();
+    // grow the tail downwards one level at a time, tracking the set of external children
+    std::vector<uint32_t> cur_ext;                       // sorted distinct children below the current tail start
+    uint32_t first = g->n_levels;
     for (uint32_t L = g->n_levels; L-- > 1;) {
-        if (g->level_off[L + 1] - g->level_off[L] <= kTailMaxLevelNodes) first = L; else break;
+        const uint64_t lo = g->level_off[L], hi = g->level_off[L + 1];
+        if (hi - lo > kTailMaxLevelNodes || g->n_levels - L > MG_TAIL_MAX_LEVELS) break;
+        std::vector<uint32_t> cand;
+        cand.reserve(cur_ext.size() + 2 * (hi - lo));
+        for (uint32_t e : cur_ext)
+            if (e < lo) cand.push_back(e);               // nodes of level L stop being external
+        for (uint64_t n = lo; n < hi; n++) { cand.push_back(ha[n]); cand.push_back(hb[n]); }   // all below lo (validated)
+        std::sort(cand.begin(), cand.end());
+        cand.erase(std::unique(cand.begin(), cand.end()), cand.end());
+        const uint64_t T = g->n_nodes - lo;
+        if (16 * (cand.size() + T) + 12 * T > kTailSmemBytes) break;
+        cur_ext.swap(cand);
+        first = L;
     }
-    g->first_fused_level = (first < g->n_levels) ? first : 0;
-    g->tail_smem_nodes = 0;
-    if (g->first_fused_level) {
-        uint64_t tail_nodes = g->n_nodes - g->level_off[g->first_fused_level];
-        g->tail_smem_nodes = (uint32_t)(tail_nodes < kTailSmemNodes ? tail_nodes : kTailSmemNodes);
-    }
+    if (first >= g->n_levels) return;                    // no tail
+    g->first_fused_level = first;
+    g->tail_base = (uint32_t)g->level_off[first];
+    g->tail_n = (uint32_t)(g->n_nodes - g->tail_base);
+    g->tail_n_ext = (uint32_t)cur_ext.size();
+    ext = cur_ext;
+    la.resize(g->tail_n); lb.resize(g->tail_n);
+    auto local = [&](uint32_t c) -> uint32_t {
+        if (c >= g->tail_base) return g->tail_n_ext + (c - g->tail_base);
+        return (uint32_t)(std::lower_bound(ext.begin(), ext.end(), c) - ext.begin());
+    };
+    for (uint32_t t = 0; t < g->tail_n; t++) { la[t] = local(ha[g->tail_base + t]); lb[t] = local(hb[g->tail_base + t]); }
 }
 
 template <typename T>
@@ -76,6 +104,7 @@ extern "C" void mg_free_graph(mg_graph* g)
     if (have) cudaSetDevice(g->device);
     cudaFree(g->d_a); cudaFree(g->d_b); cudaFree(g->d_w); cudaFree(g->d_level_off);
     cudaFree(g->d_new_of_old); cudaFree(g->d_tf_stage); cudaFree(g->d_pal8); cudaFree(g->d_pal16);
+    cudaFree(g->d_tail_ext); cudaFree(g->d_tail_a); cudaFree(g->d_tail_b);
     if (have) cudaSetDevice(prev);
     cudaGetLastError();
     delete g;
@@ -157,7 +186,12 @@ extern "C" int mg_load_graph(const uint32_t* child_a, const uint32_t* child_b, c
     } catch (const std::bad_alloc&) {
         set_error("mg_load_graph: host allocation failed"); delete g; return MG_ERR_OOM;
     }
-    plan_launches(g);
+    std::vector<uint32_t> t_ext, t_a, t_b;
+    try {
+        plan_launches(g, ha, hb, t_ext, t_a, t_b);
+    } catch (const std::bad_alloc&) {
+        set_error("mg_load_graph: host allocation failed"); delete g; return MG_ERR_OOM;
+    }
 
     // ---- device upload
     int rc = MG_OK;
@@ -180,6 +214,14 @@ extern "C" int mg_load_graph(const uint32_t* child_a, const uint32_t* child_b, c
     MG_TRY_CUDA(cudaMemcpy(g->d_b, hb.data(), n_nodes * 4, cudaMemcpyHostToDevice));
     MG_TRY_CUDA(cudaMemcpy(g->d_w, hw.data(), n_nodes * 4, cudaMemcpyHostToDevice));
     MG_TRY_CUDA(cudaMemcpy(g->d_level_off, off32.data(), off32.size() * 4, cudaMemcpyHostToDevice));
+    if (g->tail_n) {
+        MG_TRY(dev_alloc(g, &g->d_tail_ext, t_ext.size()));
+        MG_TRY(dev_alloc(g, &g->d_tail_a, t_a.size()));
+        MG_TRY(dev_alloc(g, &g->d_tail_b, t_b.size()));
+        if (!t_ext.empty()) MG_TRY_CUDA(cudaMemcpy(g->d_tail_ext, t_ext.data(), t_ext.size() * 4, cudaMemcpyHostToDevice));
+        MG_TRY_CUDA(cudaMemcpy(g->d_tail_a, t_a.data(), t_a.size() * 4, cudaMemcpyHostToDevice));
+        MG_TRY_CUDA(cudaMemcpy(g->d_tail_b, t_b.data(), t_b.size() * 4, cudaMemcpyHostToDevice));
+    }
     if (relabel) {
         MG_TRY(dev_alloc(g, &g->d_new_of_old, n_nodes));
         MG_TRY_CUDA(cudaMemcpy(g->d_new_of_old, g->new_of_old.data(), n_nodes * 4, cudaMemcpyHostToDevice));

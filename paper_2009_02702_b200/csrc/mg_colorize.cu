@@ -16,7 +16,6 @@ namespace {
 
 constexpr int kThreads = 256;
 constexpr int kVec = 2;                       // 16-byte index vectors per thread
-constexpr int kTileVox = kThreads * kVec * 4; // voxels per CTA tile
 
 __device__ __forceinline__ uint4 ld_cs_u4(const uint4* p)
 {
@@ -126,6 +125,9 @@ int launch_colorize(const mg_graph* g, const uint32_t* idx, uint64_t n, uint32_t
     if (n_vec) {
         const uint64_t blocks = (n_vec + (uint64_t)kThreads * kVec - 1) / ((uint64_t)kThreads * kVec);
         if (blocks > 0x7fffffffull) { mg::set_error("mg_colorize: too many voxels for one launch"); return MG_ERR_INVALID_ARG; }
+        // A NORMAL launch (no programmatic dependent launch): the palette gathers use the non-coherent
+        // path (ld.global.nc, L1-cached), which is only safe behind a full kernel boundary -- measured: with
+        // PDL a back-to-back update read stale palette lines (tests/test_gpu_parity.py::test_back_to_back...).
         k_colorize<W8, W16><<<(unsigned)blocks, kThreads, 0, st>>>(
             reinterpret_cast<const uint4*>(idx + head), n_vec, g->d_pal8, g->d_pal16,
             reinterpret_cast<uint4*>(W8 ? out8 + head : nullptr), reinterpret_cast<uint4*>(W16 ? out16 + head : nullptr));

@@ -9,6 +9,10 @@
 
 #include "../../include/mg.h"
 
+// Single-CTA tail kernel limits (mg_api.cu plans against them, mg_propagate.cu sizes its buffers with them).
+#define MG_TAIL_SMEM_BYTES (224 * 1024)
+#define MG_TAIL_MAX_LEVELS 128
+
 namespace mg {
 
 void set_error(const char* fmt, ...);
@@ -51,8 +55,15 @@ struct mg_graph {
     uint32_t* d_pal8 = nullptr;            // [n_nodes] RGBA8
     uint2* d_pal16 = nullptr;              // [n_nodes] 4 x fp16
     const float* pal_src = nullptr;        // node_rgba the palettes were last derived from
-    // launch plan
-    uint32_t first_fused_level = 0;        // levels >= this run in the single-CTA tail kernel (0 = none)
-    uint32_t tail_smem_nodes = 0;          // nodes of the tail staged in shared memory
+    // launch plan: levels >= first_fused_level run in the single-CTA tail kernel (0 = none).  The tail
+    // works entirely in shared memory on LOCAL indices: [0, tail_n_ext) = the distinct children that lie
+    // below the tail ("external": gathered once), [tail_n_ext, tail_n_ext + tail_n) = the tail's nodes.
+    uint32_t first_fused_level = 0;
+    uint32_t tail_base = 0;                // library index of the first tail node (= level_off[first_fused_level])
+    uint32_t tail_n = 0;                   // nodes in the tail
+    uint32_t tail_n_ext = 0;               // distinct external children
+    uint32_t* d_tail_ext = nullptr;        // [tail_n_ext] library indices of the external children
+    uint32_t* d_tail_a = nullptr;          // [tail_n] children in local indices
+    uint32_t* d_tail_b = nullptr;
     uint64_t device_bytes = 0;
 };

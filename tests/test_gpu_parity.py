@@ -275,3 +275,46 @@ def test_error_paths(mg):
     with pytest.raises(mg.MgError):
         mg.Graph(bad, b, w, 4, level_offsets=off)
     assert mg.kernel_launch_count() > 0
+
+
+@pytest.mark.parametrize("profile,n_vox", [("big_then_tail", 200003), ("big_levels", 3000001), ("tiny_all_tail", 4099)])
+def test_back_to_back_updates_without_sync(mg, profile, n_vox):
+    """Programmatic dependent launch lets a kernel become resident before its predecessor has finished
+    (griddepcontrol.wait orders them).  Many TF updates enqueued back to back, each with its own TF and
+    its own output buffers, no host synchronisation in between: every update must see exactly its own
+    palette (no stale cached colours from the previous update, no early reads)."""
+    sizes = PROFILES[profile]
+    a, b, w, off = synth.random_dag_levels(sizes, seed=21)
+    g = mg.Graph(a, b, w, sizes[0], level_offsets=off)
+    n = sum(sizes)
+    n_upd = 12
+    idx = synth.random_node_idx(n_vox, n, 60)
+    d_idx = _dev(idx)
+    tfs = [synth.random_tf(sizes[0], 61, update=u) for u in range(n_upd)]
+    d_tfs = [_dev(t) for t in tfs]
+    nodes = torch.zeros((n, 4), dtype=torch.float32, device="cuda")          # ONE palette buffer, reused
+    outs = [torch.zeros((n_vox, 4), dtype=torch.uint8, device="cuda") for _ in range(n_upd)]
+    snaps = [torch.zeros((n, 4), dtype=torch.float32, device="cuda") for _ in range(n_upd)]
+    st = torch.cuda.current_stream().cuda_stream
+    for u in range(n_upd):
+        g.propagate(d_tfs[u], nodes, st)
+        g.colorize(d_idx, n_vox, nodes, outs[u], fmt=mg.MG_RGBA8, stream=st)
+        snaps[u].copy_(nodes)                                                 # stream-ordered snapshot
+    torch.cuda.synchronize()
+    for u in range(n_upd):
+        ref = oracle.graph_eval(a, b, w, sizes[0], tfs[u].astype(np.float64))
+        got = snaps[u].cpu().numpy()
+        assert np.array_equal(got[:sizes[0]], tfs[u])
+        assert np.abs(got - ref).max() <= TOL, u
+        assert _rgba8_ok(outs[u].cpu().numpy(), oracle.lookup(idx, ref)), u
+
+
+def test_tail_plan_limits(mg):
+    """The single-CTA tail takes the longest suffix of levels that fits its shared-memory budget."""
+    sizes = [500, 30000, 9000, 8000, 3000, 900, 200, 40, 8, 1]
+    a, b, w, off = synth.random_dag_levels(sizes, seed=22)
+    tf = synth.random_tf(sizes[0], 62)
+    g, out = _propagate(mg, a, b, w, off, sizes[0], tf)
+    info = g.info
+    assert 2 <= info.first_fused_level <= 5 and info.n_launches_propagate == info.first_fused_level
+    _check_nodes(out, a, b, w, sizes[0], tf)
