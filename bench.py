@@ -47,6 +47,7 @@ def parse_args():
     p.add_argument("--e2e-steps", type=int, default=0, help="0 = min(steps, 8)")
     p.add_argument("--no-cpu-baseline", action="store_true")
     p.add_argument("--no-e2e", action="store_true")
+    p.add_argument("--no-packed", action="store_true", help="skip the extra NEXT-3 measurement (bit-packed node IDs)")
     p.add_argument("--cpu-sample-voxels", type=int, default=1 << 31, help="oracle sample size (>= the mipmap = whole workload)")
     p.add_argument("--reference-budget-s", type=float, default=90.0)
     return p.parse_args()
@@ -271,6 +272,34 @@ def run_b200(args) -> dict:
     total_ms = max_over_ranks(total_ms, world, "cuda")
     ms_per_step = total_ms / K
 
+    # ---- NEXT-3 variant: the same update with the node IDs bit-packed at r(l) bits per voxel (Table 1)
+    packed = None
+    if not args.no_packed and rank == 0:
+        w.pack()
+        lv = w.packed_levels
+        for k in range(3):
+            g.propagate(tfs[k % n_tf], nodes, st)
+            g.colorize_packed(w.d_packed, lv, nodes, out, fmt=fmt, stream=st)
+        torch.cuda.synchronize()
+        kp = min(K, 100)
+        evp = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(kp)]
+        for k in range(kp):
+            evp[k][0].record(stream)
+            g.propagate(tfs[k % n_tf], nodes, st)
+            evp[k][1].record(stream)
+            g.colorize_packed(w.d_packed, lv, nodes, out, fmt=fmt, stream=st)
+            evp[k][2].record(stream)
+        torch.cuda.synchronize()
+        pc = float(np.mean([e[1].elapsed_time(e[2]) for e in evp]))
+        pt = float(np.mean([e[0].elapsed_time(e[2]) for e in evp]))
+        in_bytes = sum(l["bits"] * l["n_voxels"] for l in lv) / 8.0
+        algo = in_bytes + out_bytes * w.n_voxels
+        packed = {"tf_update_ms": pt, "colorize_ms": pc, "bits_per_voxel": 8.0 * in_bytes / w.n_voxels,
+                  "bits_per_level": [l["bits"] for l in lv], "algorithmic_bytes_per_launch": algo,
+                  "achieved_gbs": algo / (pc * 1e-3) / 1e9, "steps": kp, "kernel": "k_colorize_packed",
+                  "what": "NEXT-3: node IDs stored as (id - i_min(l)) at r(l) bits per voxel (PAPER.md Table 1, Eq. 15-16)"}
+        w.d_packed = None
+
     # ---- e2e: host TF in, host mipmap out, through the public C-ABI call (rank-local, then max)
     e2e = None
     if not args.no_e2e:
@@ -324,6 +353,9 @@ def run_b200(args) -> dict:
                          "nodes (PAPER.md L373); the paper never materialises the RGBA mipmap (L221)",
         "setup_s": {k: round(v, 3) for k, v in w.stats.items() if k.endswith("_s")},
     }
+    if packed is not None:
+        packed["frac"] = packed["achieved_gbs"] / peak
+        res["packed"] = packed
     if e2e is not None:
         res["e2e"] = e2e
     if world == 1 and not args.no_cpu_baseline and w.host_idx is not None:

@@ -166,6 +166,51 @@ int mg_tf_update_host(mg_graph *g, const float *tf_rgba_host, float *node_rgba,
                       const uint32_t *node_idx_volume, uint64_t n_voxels, void *out_device,
                       void *out_host, uint32_t format, void *stream);
 
+/* ------------------------------------------------------------------------------------------------
+ * NEXT-3: bit-packed node-ID volumes (Table 1 rows (8), (9), (A); Eq. 15-16).
+ *
+ * Per mip level l the paper stores i_min(l) and, for every voxel, (node ID - i_min(l)) at the fixed
+ * bitrate r(l) = ceil(log2(i_max(l) - i_min(l) + 1)); the shader addresses the stream by bit address
+ * (L267).  Bit order (not fixed by the paper; reading Q18): voxel v of the level occupies
+ * stream bits [v r, (v+1) r), stream bit q is bit (q mod 8) of byte q / 8, value bit k goes to
+ * stream bit v r + k (LSB first, little endian).
+ * ------------------------------------------------------------------------------------------------ */
+#define MG_MAX_PACKED_LEVELS 32
+
+typedef struct mg_packed_level {
+    uint64_t n_voxels;    /* voxels of the level (0 = skip)                                          */
+    uint64_t out_offset;  /* first voxel of the level in the output buffers; multiple of 4            */
+    uint64_t byte_offset; /* start of the level's stream inside the packed buffer; multiple of 16     */
+    uint32_t bits;        /* r(l), 0 .. 32 (0: every voxel is node i_min)                             */
+    uint32_t i_min;       /* i_min(l)                                                                 */
+} mg_packed_level;
+
+/* r = ceil(log2(i_max - i_min + 1)), Eq. 16.  Host only. */
+uint32_t mg_bits_per_voxel(uint32_t i_min, uint32_t i_max);
+
+/* Bytes to allocate for the stream of one level: ceil(n r / 8) rounded up to 16, plus 16.  Host only. */
+uint64_t mg_packed_stream_bytes(uint64_t n_voxels, uint32_t bits);
+
+/* i_min / i_max of Eq. 15 for a DEVICE index volume (n > 0).  Returns the two values to the HOST:
+ * this call synchronises `stream`. */
+int mg_index_range(const uint32_t *idx_device, uint64_t n, uint32_t *i_min, uint32_t *i_max, void *stream);
+
+/* One-off encoder step (Table 1 row (A)): pack DEVICE uint32 indices (every value in
+ * [i_min, i_min + 2^bits)) into the DEVICE stream `packed_device` (16-byte aligned,
+ * mg_packed_stream_bytes(n, bits) bytes, fully written incl. zero padding).  Enqueue-only. */
+int mg_pack_indices(const uint32_t *idx_device, uint64_t n, uint32_t i_min, uint32_t bits,
+                    void *packed_device, void *stream);
+
+/* mg_colorize with packed input, ALL levels in one launch: for every level l and voxel v < n_voxels,
+ * out[out_offset + v] = convert(c[i_min + bits(v)]).  `levels` is a HOST array of n_levels
+ * (<= MG_MAX_PACKED_LEVELS) descriptors, copied at enqueue.  packed_device, out_rgba, out_rgba_aux
+ * are DEVICE, 16-byte aligned.  node_rgba must be the buffer most recently filled by mg_propagate
+ * on this graph (its derived 8/16-bit palettes are gathered); otherwise MG_ERR_INVALID_ARG.
+ * format: MG_RGBA8 | MG_RGBA16F | MG_BOTH.  Enqueue-only. */
+int mg_colorize_packed(mg_graph *g, const void *packed_device, const mg_packed_level *levels,
+                       uint32_t n_levels, const float *node_rgba, void *out_rgba, void *out_rgba_aux,
+                       uint32_t format, void *stream);
+
 /* Thread-local description of the last error returned on this thread ("" if none). */
 const char *mg_last_error(void);
 

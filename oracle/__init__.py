@@ -17,6 +17,7 @@ Function -> passage (PAPER.md line):
   symbolic_eval        O-5  L321, L375
   lookup               L221, L267
   to_rgba8 / to_rgba16f  Q13 (defined by this repo; not in the paper)
+  bits_per_voxel, index_range, pack_level, unpack_level   NEXT-3: Table 1 (8),(9),(A), Eq. 15-16
 All functions are pinned by tests/test_oracle_pins.py; none is "parity unpinned".
 """
 from __future__ import annotations
@@ -60,6 +61,14 @@ _lib.mgo_to_rgba8.argtypes = [_f64p, _u64, _u8p]
 _lib.mgo_to_rgba8.restype = None
 _lib.mgo_colourise_rgba8.argtypes = [_u32p, _u64, _f64p, _u8p, C.c_int]
 _lib.mgo_colourise_rgba8.restype = C.c_int
+
+
+_lib.mgo_bits_per_voxel.argtypes = [_u32, _u32]
+_lib.mgo_bits_per_voxel.restype = _u32
+_lib.mgo_pack_bits.argtypes = [_u32p, _u64, _u32, _u32, _u8p]
+_lib.mgo_pack_bits.restype = None
+_lib.mgo_unpack_bits.argtypes = [_u8p, _u64, _u32, _u32, _u32p]
+_lib.mgo_unpack_bits.restype = None
 
 
 def _c(a, dt):
@@ -195,3 +204,34 @@ def colourise_rgba8(node_idx, c, n_threads=0):
     out = np.zeros(idx.shape + (4,), dtype=np.uint8)
     used = _lib.mgo_colourise_rgba8(idx.reshape(-1), idx.size, c.reshape(-1), out.reshape(-1), n_threads)
     return out, used
+
+
+# ---- NEXT-3: bit-packed node-ID volumes (Table 1 rows (8), (9), (A); Eq. 15-16) ------------------
+
+def index_range(node_idx):
+    """(i_min(l), i_max(l)) of Eq. 15, read per level (Q10): min / max node ID referenced by the level."""
+    idx = np.asarray(node_idx)
+    return int(idx.min()), int(idx.max())
+
+
+def bits_per_voxel(i_min, i_max):
+    """r(l) = ceil(log2(i_max - i_min + 1)), Eq. 16."""
+    return int(_lib.mgo_bits_per_voxel(int(i_min), int(i_max)))
+
+
+def pack_level(node_idx, i_min, r):
+    """uint8 stream of ceil(n r / 8) bytes: voxel v holds (node_idx[v] - i_min) in bits [v r, (v+1) r),
+    LSB first (reading Q18)."""
+    idx = _c(node_idx, np.uint32).reshape(-1)
+    out = np.zeros((idx.size * int(r) + 7) // 8, dtype=np.uint8)
+    _lib.mgo_pack_bits(idx, idx.size, int(i_min), int(r), out)
+    return out
+
+
+def unpack_level(stream, n_vox, i_min, r):
+    """Inverse of pack_level: uint32 [n_vox]."""
+    st = _c(stream, np.uint8).reshape(-1)
+    assert st.size * 8 >= int(n_vox) * int(r)
+    out = np.zeros(int(n_vox), dtype=np.uint32)
+    _lib.mgo_unpack_bits(st, int(n_vox), int(i_min), int(r), out)
+    return out

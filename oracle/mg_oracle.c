@@ -279,3 +279,52 @@ int mgo_colourise_rgba8(const uint32_t *node_idx, uint64_t n_vox, const double *
         mgo_to_rgba8(c + 4 * (uint64_t)node_idx[v], 1, out + 4 * v);
     return used;
 }
+
+/* ==== NEXT-3: bit-packed node-ID volumes (Table 1 rows (8), (9), (A); Eq. 15-16) ====
+ *
+ * "For each level of H, we compute the minimum and maximum ID of all nodes referenced in this
+ * level ... We store i_min(l) in the bitstream's header for each l.  For each voxel, we then store
+ * its node ID minus the minimum node ID of that level, again, using a fixed bitrate of
+ * r(l) = ceil(log2(i_max(l) - i_min(l) + 1)) for each voxel in this level" (Eq. 15 read per level,
+ * Q10; Eq. 16).  The shader addresses the stream by BIT address with 64-bit arithmetic (L267).
+ * The paper does not fix the bit order; reading Q18: voxel v of the level occupies bits
+ * [v r, (v+1) r) of the level's stream, bit q of the stream is bit (q mod 8) of byte q / 8 (LSB
+ * first, little endian), and bit k of the stored value goes to stream bit v r + k. */
+
+/* Eq. 16.  r = 0 when the level references a single node. */
+uint32_t mgo_bits_per_voxel(uint32_t i_min, uint32_t i_max)
+{
+    uint64_t range = (uint64_t)i_max - (uint64_t)i_min + 1; /* number of representable IDs needed */
+    uint32_t r = 0;
+    while (((uint64_t)1 << r) < range)
+        r++;
+    return r;
+}
+
+/* Write value - i_min of every voxel, one bit at a time.  stream must be zero-initialised and hold
+ * at least ceil(n r / 8) bytes. */
+void mgo_pack_bits(const uint32_t *node_idx, uint64_t n_vox, uint32_t i_min, uint32_t r, uint8_t *stream)
+{
+    for (uint64_t v = 0; v < n_vox; v++) {
+        uint32_t val = node_idx[v] - i_min;
+        for (uint32_t k = 0; k < r; k++) {
+            uint64_t q = v * (uint64_t)r + k;
+            if ((val >> k) & 1u)
+                stream[q >> 3] |= (uint8_t)(1u << (q & 7));
+        }
+    }
+}
+
+/* Inverse: node_idx[v] = i_min + the r-bit value at bit address v r. */
+void mgo_unpack_bits(const uint8_t *stream, uint64_t n_vox, uint32_t i_min, uint32_t r, uint32_t *node_idx)
+{
+    for (uint64_t v = 0; v < n_vox; v++) {
+        uint32_t val = 0;
+        for (uint32_t k = 0; k < r; k++) {
+            uint64_t q = v * (uint64_t)r + k;
+            if ((stream[q >> 3] >> (q & 7)) & 1u)
+                val |= 1u << k;
+        }
+        node_idx[v] = i_min + val;
+    }
+}

@@ -1,0 +1,266 @@
+// mg_packed.cu -- NEXT-3: bit-packed node-ID volumes as colourise input.
+//
+// The paper stores, per mip level l, i_min(l) and for every voxel (node ID - i_min(l)) at a fixed
+// bitrate r(l) = ceil(log2(i_max(l) - i_min(l) + 1)) (Table 1 rows (8), (9), (A); Eq. 15-16,
+// L199-L207) and addresses the stream by bit address in the shader (L267).  Reading Q18:
+// voxel v occupies bits [v r, (v+1) r) of its level's stream, LSB first, little endian.
+// This cuts the colourise input from 32 bits per voxel to r(l) (11 bits on level 0 of config 3).
+//
+//   k_index_range      min / max of a node-index volume (i_min, i_max of Eq. 15)
+//   k_pack_bits        one thread = one 32-bit word of the stream (no atomics)
+//   k_colorize_packed  one CTA = one tile of 2048 voxels of ONE level (uniform switch on the level's
+//                      bitrate into a compile-time-R body, see colorize_tile).  All levels of a mipmap
+//                      go in ONE launch: the per-level table travels as a __grid_constant__ parameter.
+#include <cuda_fp16.h>
+
+#include <cstring>
+
+#include "mg_internal.h"
+
+namespace {
+
+constexpr int kThreads = 256;
+constexpr int kTileVox = 2048;                 // voxels per CTA: 2 groups of 4 per thread
+constexpr int kMaxLevels = MG_MAX_PACKED_LEVELS;
+
+struct PackedLevel {
+    const uint32_t* words;   // level stream (16-byte aligned)
+    uint64_t n_vox;
+    uint64_t out_off;        // first voxel of the level in the outputs (multiple of 4)
+    uint32_t bits;
+    uint32_t i_min;
+    uint32_t tile_begin;     // first CTA of the level
+    uint32_t pad;
+};
+struct PackedParams {
+    PackedLevel lv[kMaxLevels];
+    uint32_t n_levels;
+};
+
+__device__ __forceinline__ uint4 ld_cs_u4(const uint4* p)
+{
+    uint4 r;
+    asm volatile("ld.global.cs.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "l"(p));
+    return r;
+}
+__device__ __forceinline__ void st_cs_u4(uint4* p, uint4 v)
+{
+    asm volatile("st.global.cs.v4.u32 [%0], {%1,%2,%3,%4};" :: "l"(p), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
+}
+
+__global__ void __launch_bounds__(256) k_index_range(const uint32_t* __restrict__ idx, uint64_t n, uint32_t* __restrict__ mm)
+{
+    uint32_t lo = 0xFFFFFFFFu, hi = 0u;
+    for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (uint64_t)gridDim.x * blockDim.x) {
+        const uint32_t v = idx[i];
+        lo = min(lo, v); hi = max(hi, v);
+    }
+    lo = __reduce_min_sync(0xFFFFFFFFu, lo);
+    hi = __reduce_max_sync(0xFFFFFFFFu, hi);
+    if ((threadIdx.x & 31) == 0) { atomicMin(mm, lo); atomicMax(mm + 1, hi); }
+}
+
+// word w of the stream holds stream bits [32 w, 32 w + 32): the voxels that overlap it are
+// floor(32 w / r) .. floor((32 w + 31) / r).
+__global__ void __launch_bounds__(256)
+k_pack_bits(const uint32_t* __restrict__ idx, uint64_t n, uint32_t i_min, uint32_t r, uint32_t* __restrict__ words, uint64_t n_words)
+{
+    const uint64_t w = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (w >= n_words) return;
+    uint32_t out = 0;
+    if (r) {
+        const uint64_t b0 = 32 * w, b1 = b0 + 32;
+        uint64_t v = b0 / r;
+        for (; v < n && v * r < b1; v++) {
+            const uint64_t val = (uint64_t)(idx[v] - i_min);
+            const int64_t sh = (int64_t)(v * r) - (int64_t)b0;          // position of the value's bit 0 inside the word
+            out |= (sh >= 0) ? (uint32_t)(val << sh) : (uint32_t)(val >> (-sh));
+        }
+    }
+    words[w] = out;
+}
+
+// One tile (2048 voxels of one level) at the compile-time bitrate R.  A lane handles groups of 4
+// consecutive voxels (4 R bits, one 16-byte RGBA8 store): it loads the NW aligned 32-bit words that
+// cover the group (neighbouring lanes overlap: the same sectors, served by L1), realigns them by the
+// group's bit offset (a runtime funnel shift) and extracts the four values at COMPILE-TIME positions
+// j R -- no shared memory, no barrier, word selection never depends on runtime data.
+template <int R, bool W8, bool W16>
+__device__ __forceinline__ void colorize_tile(const uint32_t* __restrict__ words, uint32_t i_min, uint32_t nv, uint64_t o0,
+                                              const uint32_t* __restrict__ pal8, const uint2* __restrict__ pal16,
+                                              uint32_t* __restrict__ out8, uint2* __restrict__ out16)
+{
+    constexpr int NW = (R == 0) ? 0 : (4 * R + 62) / 32;               // words that can hold 4 R bits at any bit offset
+    constexpr int NG = kTileVox / (4 * kThreads);                       // groups per thread
+    constexpr uint32_t mask = R >= 32 ? 0xFFFFFFFFu : ((1u << R) - 1u);
+    uint32_t a[NG][NW + 1];
+#pragma unroll
+    for (int k = 0; k < NG; k++) {
+        const uint32_t vb = (threadIdx.x + k * kThreads) * 4;
+        const uint32_t i0 = (vb * R) >> 5;
+#pragma unroll
+        for (int q = 0; q < NW; q++) a[k][q] = (vb < nv) ? __ldg(words + i0 + q) : 0u;
+        a[k][NW] = 0u;
+    }
+#pragma unroll
+    for (int k = 0; k < NG; k++) {
+        const uint32_t vb = (threadIdx.x + k * kThreads) * 4;
+        if (vb >= nv) continue;
+        const uint32_t sh = (vb * R) & 31;
+        uint32_t w[NW + 1];                                             // the group's bits, realigned to bit 0
+#pragma unroll
+        for (int q = 0; q < NW; q++) w[q] = __funnelshift_r(a[k][q], a[k][q + 1], sh);
+        w[NW] = 0u;
+        uint32_t id[4];
+#pragma unroll
+        for (int j = 0; j < 4; j++) {
+            constexpr int dummy = 0; (void)dummy;
+            const int p = j * R;                                        // compile-time after unrolling
+            uint32_t v = 0;
+            if (R > 0) v = (p & 31) ? __funnelshift_r(w[p >> 5], w[(p >> 5) + 1 <= NW ? (p >> 5) + 1 : NW], p & 31) : w[p >> 5];
+            id[j] = i_min + (v & mask);
+        }
+        const uint64_t o = o0 + vb;
+        if (vb + 4 <= nv) {
+            if (W8) st_cs_u4(reinterpret_cast<uint4*>(out8 + o),
+                             make_uint4(__ldg(pal8 + id[0]), __ldg(pal8 + id[1]), __ldg(pal8 + id[2]), __ldg(pal8 + id[3])));
+            if (W16) {
+                const uint2 h0 = __ldg(pal16 + id[0]), h1 = __ldg(pal16 + id[1]), h2 = __ldg(pal16 + id[2]), h3 = __ldg(pal16 + id[3]);
+                st_cs_u4(reinterpret_cast<uint4*>(out16 + o), make_uint4(h0.x, h0.y, h1.x, h1.y));
+                st_cs_u4(reinterpret_cast<uint4*>(out16 + o) + 1, make_uint4(h2.x, h2.y, h3.x, h3.y));
+            }
+        } else {
+#pragma unroll
+            for (int j = 0; j < 4; j++)
+                if (vb + j < nv) {
+                    if (W8) out8[o + j] = __ldg(pal8 + id[j]);
+                    if (W16) out16[o + j] = __ldg(pal16 + id[j]);
+                }
+        }
+    }
+}
+
+template <bool W8, bool W16>
+__global__ void __launch_bounds__(kThreads)
+k_colorize_packed(const __grid_constant__ PackedParams P, const uint32_t* __restrict__ pal8, const uint2* __restrict__ pal16,
+                  uint32_t* __restrict__ out8, uint2* __restrict__ out16)
+{
+    uint32_t l = 0;
+    while (l + 1 < P.n_levels && blockIdx.x >= P.lv[l + 1].tile_begin) l++;
+    const PackedLevel& L = P.lv[l];
+    const uint64_t tile = blockIdx.x - L.tile_begin;
+    const uint64_t v0 = tile * kTileVox;
+    const uint32_t nv = (uint32_t)min((uint64_t)kTileVox, L.n_vox - v0);
+    const uint32_t* words = L.words + tile * (uint64_t)(kTileVox / 32) * L.bits;   // a tile starts on a word boundary
+    const uint64_t o0 = L.out_off + v0;
+#define MG_CASE(R) case R: colorize_tile<R, W8, W16>(words, L.i_min, nv, o0, pal8, pal16, out8, out16); break;
+    switch (L.bits) {                                                    // uniform per CTA
+        MG_CASE(0) MG_CASE(1) MG_CASE(2) MG_CASE(3) MG_CASE(4) MG_CASE(5) MG_CASE(6) MG_CASE(7) MG_CASE(8)
+        MG_CASE(9) MG_CASE(10) MG_CASE(11) MG_CASE(12) MG_CASE(13) MG_CASE(14) MG_CASE(15) MG_CASE(16)
+        MG_CASE(17) MG_CASE(18) MG_CASE(19) MG_CASE(20) MG_CASE(21) MG_CASE(22) MG_CASE(23) MG_CASE(24)
+        MG_CASE(25) MG_CASE(26) MG_CASE(27) MG_CASE(28) MG_CASE(29) MG_CASE(30) MG_CASE(31) MG_CASE(32)
+        default: break;
+    }
+#undef MG_CASE
+}
+
+}  // namespace
+
+using namespace mg;
+
+extern "C" uint64_t mg_packed_stream_bytes(uint64_t n_voxels, uint32_t bits)
+{
+    const uint64_t payload = (n_voxels * (uint64_t)bits + 7) / 8;
+    return ((payload + 15) & ~(uint64_t)15) + 16;
+}
+
+extern "C" uint32_t mg_bits_per_voxel(uint32_t i_min, uint32_t i_max)
+{
+    if (i_max < i_min) return 0;
+    const uint64_t range = (uint64_t)i_max - i_min + 1;
+    uint32_t r = 0;
+    while ((1ull << r) < range) r++;
+    return r;
+}
+
+extern "C" int mg_index_range(const uint32_t* idx_device, uint64_t n, uint32_t* i_min, uint32_t* i_max, void* stream)
+{
+    if (!idx_device || !i_min || !i_max || n == 0) { set_error("mg_index_range: NULL argument or n = 0"); return MG_ERR_INVALID_ARG; }
+    cudaStream_t st = (cudaStream_t)stream;
+    uint32_t* d_mm = nullptr;
+    MG_CUDA(cudaMalloc((void**)&d_mm, 8));
+    const uint32_t init[2] = {0xFFFFFFFFu, 0u};
+    cudaError_t e = cudaMemcpyAsync(d_mm, init, 8, cudaMemcpyHostToDevice, st);
+    if (e == cudaSuccess) {
+        uint64_t blocks = (n + 255) / 256;
+        if (blocks > 148ull * 16) blocks = 148ull * 16;
+        k_index_range<<<(unsigned)blocks, 256, 0, st>>>(idx_device, n, d_mm);
+        count_launch();
+        uint32_t out[2] = {0, 0};
+        e = cudaMemcpyAsync(out, d_mm, 8, cudaMemcpyDeviceToHost, st);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+        *i_min = out[0]; *i_max = out[1];
+    }
+    cudaFree(d_mm);
+    if (e != cudaSuccess) return cuda_fail(e, "mg_index_range");
+    return MG_OK;
+}
+
+extern "C" int mg_pack_indices(const uint32_t* idx_device, uint64_t n, uint32_t i_min, uint32_t bits, void* packed_device, void* stream)
+{
+    if ((!idx_device && n) || !packed_device) { set_error("mg_pack_indices: NULL argument"); return MG_ERR_INVALID_ARG; }
+    if (bits > 32) { set_error("mg_pack_indices: bits must be <= 32"); return MG_ERR_INVALID_ARG; }
+    if ((uintptr_t)packed_device & 15) { set_error("mg_pack_indices: the stream must be 16-byte aligned"); return MG_ERR_INVALID_ARG; }
+    const uint64_t n_words = mg_packed_stream_bytes(n, bits) / 4;
+    const uint64_t blocks = (n_words + 255) / 256;
+    if (blocks > 0x7fffffffull) { set_error("mg_pack_indices: too many voxels for one launch"); return MG_ERR_INVALID_ARG; }
+    k_pack_bits<<<(unsigned)blocks, 256, 0, (cudaStream_t)stream>>>(idx_device, n, i_min, bits, (uint32_t*)packed_device, n_words);
+    count_launch();
+    MG_CUDA(cudaGetLastError());
+    return MG_OK;
+}
+
+extern "C" int mg_colorize_packed(mg_graph* g, const void* packed_device, const mg_packed_level* levels, uint32_t n_levels,
+                                  const float* node_rgba, void* out_rgba, void* out_rgba_aux, uint32_t format, void* stream)
+{
+    if (!g || !node_rgba || !levels || !packed_device || !out_rgba) { set_error("mg_colorize_packed: NULL argument"); return MG_ERR_INVALID_ARG; }
+    const uint32_t fmt = format & 3u;
+    if (fmt == 0 || (format & ~3u)) { set_error("mg_colorize_packed: bad format 0x%x", format); return MG_ERR_INVALID_ARG; }
+    if (fmt == MG_BOTH && !out_rgba_aux) { set_error("mg_colorize_packed: MG_BOTH needs out_rgba_aux"); return MG_ERR_INVALID_ARG; }
+    if (n_levels == 0 || n_levels > (uint32_t)kMaxLevels) { set_error("mg_colorize_packed: n_levels must be 1..%d", kMaxLevels); return MG_ERR_INVALID_ARG; }
+    if (((uintptr_t)packed_device & 15) || ((uintptr_t)out_rgba & 15) || (fmt == MG_BOTH && ((uintptr_t)out_rgba_aux & 15)) || ((uintptr_t)node_rgba & 15)) {
+        set_error("mg_colorize_packed: buffers must be 16-byte aligned"); return MG_ERR_INVALID_ARG;
+    }
+    if (g->pal_src != node_rgba) {
+        set_error("mg_colorize_packed: node_rgba must be the buffer most recently filled by mg_propagate on this graph");
+        return MG_ERR_INVALID_ARG;
+    }
+    PackedParams P;
+    memset(&P, 0, sizeof(P));
+    uint64_t tiles = 0;
+    uint32_t m = 0;
+    for (uint32_t l = 0; l < n_levels; l++) {
+        const mg_packed_level& s = levels[l];
+        if (s.bits > 32 || (s.out_offset & 3) || (s.byte_offset & 15)) {
+            set_error("mg_colorize_packed: level %u: bits <= 32, out_offset %% 4 == 0 and byte_offset %% 16 == 0 are required", l);
+            return MG_ERR_INVALID_ARG;
+        }
+        if (s.n_voxels == 0) continue;
+        PackedLevel& d = P.lv[m++];
+        d.words = reinterpret_cast<const uint32_t*>(static_cast<const char*>(packed_device) + s.byte_offset);
+        d.n_vox = s.n_voxels; d.out_off = s.out_offset; d.bits = s.bits; d.i_min = s.i_min;
+        d.tile_begin = (uint32_t)tiles;
+        tiles += (s.n_voxels + kTileVox - 1) / kTileVox;
+        if (tiles > 0x7fffffffull) { set_error("mg_colorize_packed: too many voxels for one launch"); return MG_ERR_INVALID_ARG; }
+    }
+    P.n_levels = m;
+    if (m == 0) return MG_OK;
+    cudaStream_t st = (cudaStream_t)stream;
+    // normal launches: the palette gathers use the non-coherent path (see mg_colorize.cu)
+    if (fmt == MG_RGBA8) k_colorize_packed<true, false><<<(unsigned)tiles, kThreads, 0, st>>>(P, g->d_pal8, g->d_pal16, (uint32_t*)out_rgba, nullptr);
+    else if (fmt == MG_RGBA16F) k_colorize_packed<false, true><<<(unsigned)tiles, kThreads, 0, st>>>(P, g->d_pal8, g->d_pal16, nullptr, (uint2*)out_rgba);
+    else k_colorize_packed<true, true><<<(unsigned)tiles, kThreads, 0, st>>>(P, g->d_pal8, g->d_pal16, (uint32_t*)out_rgba, (uint2*)out_rgba_aux);
+    count_launch();
+    MG_CUDA(cudaGetLastError());
+    return MG_OK;
+}

@@ -27,7 +27,8 @@ ALL_LEVELS = 0xFFFFFFFF
 # every symbol include/mg.h declares (tests check that the library exports all of them)
 SYMBOLS = ["mg_load_graph", "mg_free_graph", "mg_graph_info", "mg_level_offsets", "mg_node_permutation",
            "mg_relabel_indices", "mg_propagate", "mg_propagate_host", "mg_colorize", "mg_tf_update_host",
-           "mg_last_error", "mg_kernel_launch_count"]
+           "mg_last_error", "mg_kernel_launch_count",
+           "mg_bits_per_voxel", "mg_packed_stream_bytes", "mg_index_range", "mg_pack_indices", "mg_colorize_packed"]
 
 
 class MgInfo(C.Structure):
@@ -36,6 +37,12 @@ class MgInfo(C.Structure):
                 ("n_launches_propagate", C.c_uint32), ("relabelled", C.c_uint32), ("device_bytes", C.c_uint64)]
 
 
+class MgPackedLevel(C.Structure):
+    _fields_ = [("n_voxels", C.c_uint64), ("out_offset", C.c_uint64), ("byte_offset", C.c_uint64),
+                ("bits", C.c_uint32), ("i_min", C.c_uint32)]
+
+
+MG_MAX_PACKED_LEVELS = 32
 _vp = C.c_void_p
 lib.mg_load_graph.argtypes = [_vp, _vp, _vp, C.c_uint64, C.c_uint32, _vp, C.c_uint32, _vp, C.c_uint32, C.POINTER(_vp)]
 lib.mg_load_graph.restype = C.c_int
@@ -61,6 +68,18 @@ lib.mg_last_error.argtypes = []
 lib.mg_last_error.restype = C.c_char_p
 lib.mg_kernel_launch_count.argtypes = []
 lib.mg_kernel_launch_count.restype = C.c_uint64
+
+
+lib.mg_bits_per_voxel.argtypes = [C.c_uint32, C.c_uint32]
+lib.mg_bits_per_voxel.restype = C.c_uint32
+lib.mg_packed_stream_bytes.argtypes = [C.c_uint64, C.c_uint32]
+lib.mg_packed_stream_bytes.restype = C.c_uint64
+lib.mg_index_range.argtypes = [_vp, C.c_uint64, C.POINTER(C.c_uint32), C.POINTER(C.c_uint32), _vp]
+lib.mg_index_range.restype = C.c_int
+lib.mg_pack_indices.argtypes = [_vp, C.c_uint64, C.c_uint32, C.c_uint32, _vp, _vp]
+lib.mg_pack_indices.restype = C.c_int
+lib.mg_colorize_packed.argtypes = [_vp, _vp, C.POINTER(MgPackedLevel), C.c_uint32, _vp, _vp, _vp, C.c_uint32, _vp]
+lib.mg_colorize_packed.restype = C.c_int
 
 
 class MgError(RuntimeError):
@@ -91,6 +110,35 @@ def _np(a, dt):
 
 def kernel_launch_count() -> int:
     return int(lib.mg_kernel_launch_count())
+
+
+def bits_per_voxel(i_min: int, i_max: int) -> int:
+    return int(lib.mg_bits_per_voxel(int(i_min), int(i_max)))
+
+
+def packed_stream_bytes(n_voxels: int, bits: int) -> int:
+    return int(lib.mg_packed_stream_bytes(int(n_voxels), int(bits)))
+
+
+def index_range(idx_device, n: int, stream: int = 0):
+    lo, hi = C.c_uint32(), C.c_uint32()
+    _check(lib.mg_index_range(_ptr(idx_device), int(n), C.byref(lo), C.byref(hi), stream or None), "mg_index_range")
+    return int(lo.value), int(hi.value)
+
+
+def pack_indices(idx_device, n: int, i_min: int, bits: int, packed_device, stream: int = 0) -> None:
+    _check(lib.mg_pack_indices(_ptr(idx_device), int(n), int(i_min), int(bits), _ptr(packed_device), stream or None),
+           "mg_pack_indices")
+
+
+def packed_levels(levels) -> "C.Array":
+    """ctypes array of MgPackedLevel from dicts / tuples (n_voxels, out_offset, byte_offset, bits, i_min)."""
+    arr = (MgPackedLevel * len(levels))()
+    for i, l in enumerate(levels):
+        if isinstance(l, dict):
+            l = (l["n_voxels"], l["out_offset"], l["byte_offset"], l["bits"], l["i_min"])
+        arr[i] = MgPackedLevel(*[int(x) for x in l])
+    return arr
 
 
 class Graph:
@@ -152,6 +200,12 @@ class Graph:
         _check(lib.mg_colorize(self._h, int(mip_level), _ptr(node_idx_device), int(n_voxels),
                                _ptr(node_rgba_device), _ptr(out), _ptr(out_aux), int(fmt), stream or None),
                "mg_colorize")
+
+    def colorize_packed(self, packed_device, levels, node_rgba_device, out, out_aux=None, fmt: int = MG_RGBA8,
+                        stream: int = 0) -> None:
+        arr = levels if isinstance(levels, C.Array) else packed_levels(levels)
+        _check(lib.mg_colorize_packed(self._h, _ptr(packed_device), arr, len(arr), _ptr(node_rgba_device), _ptr(out),
+                                      _ptr(out_aux), int(fmt), stream or None), "mg_colorize_packed")
 
     def tf_update_host(self, tf_host, node_rgba_device, node_idx_device, n_voxels: int, out_device,
                        out_host=None, fmt: int = MG_RGBA8, stream: int = 0) -> None:

@@ -41,6 +41,9 @@ class Workload:
         self.n_leaves = 0
         self.cfg: dict = {}
         self.seg = None                           # uint32 [Z, Y, X] segmentation (only with keep_seg)
+        self.d_packed = None                      # torch uint8: bit-packed streams of all levels (after pack())
+        self.packed_levels = None                 # list of dicts (n_voxels, out_offset, byte_offset, bits, i_min)
+        self.packed_bytes = 0
 
     def tf(self, update: int = 0) -> np.ndarray:
         """fp32 [n_leaves, 4] transfer function number ``update`` of this config (synth recipe)."""
@@ -48,7 +51,26 @@ class Workload:
         return synth.random_tf(self.n_leaves, c.get("seed", 0), update=update,
                                alpha_zero_frac=c.get("alpha_zero_frac", 0.0))
 
+    def pack(self) -> None:
+        """NEXT-3: derive the bit-packed form of the device mipmap (Table 1 (8), (9), (A)): per level
+        i_min(l), r(l) (Eq. 15-16) and one packed stream; fills d_packed / packed_levels."""
+        import torch
+        st = torch.cuda.current_stream().cuda_stream
+        levels, pos = [], 0
+        for s0, nv in zip(self.level_start, self.level_voxels):
+            lo, hi = mg.index_range(self.d_idx[s0:s0 + nv], nv, st)
+            bits = mg.bits_per_voxel(lo, hi)
+            levels.append(dict(n_voxels=nv, out_offset=s0, byte_offset=pos, bits=bits, i_min=lo))
+            pos += mg.packed_stream_bytes(nv, bits)
+        self.d_packed = torch.empty(pos, dtype=torch.uint8, device="cuda")
+        for l, (s0, nv) in zip(levels, zip(self.level_start, self.level_voxels)):
+            mg.pack_indices(self.d_idx[s0:s0 + nv], nv, l["i_min"], l["bits"], self.d_packed[l["byte_offset"]:], st)
+        torch.cuda.synchronize()
+        self.packed_levels = levels
+        self.packed_bytes = pos
+
     def close(self) -> None:
+        self.d_packed = None
         if self.graph is not None:
             self.graph.close()
             self.graph = None

@@ -178,6 +178,41 @@ def test_config3_fp16_output_full_size(libs):
         w.close()
 
 
+@pytest.mark.parametrize("cfg_id", [3, 4])
+def test_packed_mipmap_full_size(libs, cfg_id):
+    """NEXT-3 at full size: the bit-packed mipmap (Table 1 (8), (9), (A)) colourises to EXACTLY the bytes of
+    the uint32 path on all voxels of all levels; per-level i_min / r(l) match the oracle's Eq. 15-16 on the
+    builder's indices; the device stream of a whole level equals the oracle's stream bit for bit."""
+    mg, workload = libs
+    w = workload.make(cfg_id)
+    try:
+        tf = w.tf(3)
+        nodes, out = _run_update(mg, w, tf, mg.MG_RGBA8)
+        w.pack()
+        out_p = torch.full_like(out, 0xAB)
+        st = torch.cuda.current_stream().cuda_stream
+        w.graph.colorize_packed(w.d_packed, w.packed_levels, nodes, out_p, fmt=mg.MG_RGBA8, stream=st)
+        torch.cuda.synchronize()
+        o4, p4 = out.view(-1, 4), out_p.view(-1, 4)
+        for s0, nv in zip(w.level_start, w.level_voxels):                      # every voxel of every level
+            assert torch.equal(o4[s0:s0 + nv], p4[s0:s0 + nv])
+        total_bits = 0
+        for l, lv in enumerate(w.packed_levels):
+            lo, hi = oracle.index_range(w.host_idx[l])
+            assert (lv["i_min"], lv["bits"]) == (lo, oracle.bits_per_voxel(lo, hi)), l
+            total_bits += lv["bits"] * lv["n_voxels"]
+        assert w.packed_levels[0]["bits"] == oracle.bits_per_voxel(0, w.n_leaves - 1)   # level 0 references leaves only (I5)
+        l = 2                                                                  # one whole level, bit for bit
+        lv = w.packed_levels[l]
+        ref = oracle.pack_level(w.host_idx[l], lv["i_min"], lv["bits"])
+        got = w.d_packed[lv["byte_offset"]:lv["byte_offset"] + ref.size].cpu().numpy()
+        assert np.array_equal(got, ref)
+        print(f"cfg {cfg_id}: packed mipmap {w.packed_bytes / 1e9:.3f} GB = {total_bits / w.n_voxels:.2f} bits/voxel "
+              f"(uint32: {4 * w.n_voxels / 1e9:.3f} GB); r(l) = {[lv['bits'] for lv in w.packed_levels]}")
+    finally:
+        w.close()
+
+
 def test_config5_dag_stress_full_size(libs):
     """2^26 nodes, 24 levels, 2^14 leaves, random children; 512^3 random node-index volume."""
     mg, workload = libs

@@ -294,3 +294,58 @@ def test_rgba16f_is_round_to_nearest():
     v = np.array([[0.1, 1 / 3, 1.0, 65504.0]])
     assert (oracle.to_rgba16f(v) == v.astype(np.float16)).all()
     assert oracle.to_rgba16f(v).dtype == np.float16
+
+
+# ------------------------------------------------------------------------------------------ NEXT-3
+def _golden_packed(golden_dir):
+    for line in open(os.path.join(golden_dir, "packed_bits.txt")):
+        if line.startswith("#") or not line.strip():
+            continue
+        head, ids, hexbytes = [p.strip() for p in line.split("|")]
+        i_min, r = (int(x) for x in head.split())
+        yield i_min, r, [int(x) for x in ids.split()], bytes(int(x, 16) for x in hexbytes.split())
+
+
+def test_pack_level_reproduces_hand_worked_streams(golden_dir):
+    """Table 1 row (A) with the Q18 bit order: streams worked by hand (tests/golden/packed_bits.txt)."""
+    n = 0
+    for i_min, r, ids, stream in _golden_packed(golden_dir):
+        got = oracle.pack_level(ids, i_min, r)
+        assert got.tobytes() == stream[:got.size], (i_min, r, ids)
+        assert all(b == 0 for b in stream[got.size:])
+        assert oracle.unpack_level(np.frombuffer(stream, dtype=np.uint8) if stream else np.zeros(0, np.uint8),
+                                   len(ids), i_min, r).tolist() == ids
+        n += 1
+    assert n == 4
+
+
+def test_bits_per_voxel_is_the_minimal_sufficient_bitrate():
+    """Eq. 16 (L205): r = ceil(log2(range)) <=> 2^r >= range > 2^(r-1); printed-size anchors."""
+    assert oracle.bits_per_voxel(0, 1181) == 11          # 1,182 sources -> 11 bits (config 3, level 0)
+    assert oracle.bits_per_voxel(0, 352) == 9            # 353 sources
+    assert oracle.bits_per_voxel(0, 15917) == 14         # 15,918 leaves
+    assert oracle.bits_per_voxel(7, 7) == 0 and oracle.bits_per_voxel(7, 8) == 1
+    assert oracle.bits_per_voxel(0, 2 ** 32 - 1) == 32
+    for rng in list(range(1, 70)) + [255, 256, 257, 2 ** 20, 2 ** 20 + 1, 2 ** 31, 2 ** 31 + 1]:
+        for i_min in (0, 5, 1000):
+            r = oracle.bits_per_voxel(i_min, i_min + rng - 1)
+            assert 2 ** r >= rng and (r == 0 or 2 ** (r - 1) < rng)
+
+
+@pytest.mark.parametrize("r", [0, 1, 3, 7, 8, 11, 13, 16, 21, 31, 32])
+def test_pack_unpack_round_trip_and_numpy_bit_view(r):
+    """Round trip, stream length ceil(n r / 8), and an independent decode through numpy's unpackbits."""
+    n = 1013
+    i_min = 12345 if r < 32 else 0
+    span = np.uint64(1) << np.uint64(r)
+    vals = (synth.u64(3, 70 + r, np.arange(n, dtype=np.uint64)) % span).astype(np.uint64)
+    ids = (vals + np.uint64(i_min)).astype(np.uint32)
+    stream = oracle.pack_level(ids, i_min, r)
+    assert stream.size == (n * r + 7) // 8
+    assert np.array_equal(oracle.unpack_level(stream, n, i_min, r), ids)
+    if r:
+        bits = np.unpackbits(stream, bitorder="little")[:n * r].reshape(n, r).astype(np.uint64)
+        dec = (bits << np.arange(r, dtype=np.uint64)).sum(axis=1)
+        assert np.array_equal(dec, vals)
+    lo, hi = oracle.index_range(ids)
+    assert lo == int(ids.min()) and hi == int(ids.max()) and oracle.bits_per_voxel(lo, hi) <= r
