@@ -211,6 +211,28 @@ int mg_colorize_packed(mg_graph *g, const void *packed_device, const mg_packed_l
                        uint32_t n_levels, const float *node_rgba, void *out_rgba, void *out_rgba_aux,
                        uint32_t format, void *stream);
 
+/* ------------------------------------------------------------------------------------------------
+ * NEXT-1: propagation of any numeric segment attribute ("the Mixture Graph allows the
+ * efficient computation of any kind of numeric segmentation attribute"): opacity alone for
+ * empty-space skipping (L271 (i)-(ii)), diffuse / specular light contributions (L277), or K transfer
+ * functions batched as 4 K channels -- one pass over the graph arrays for all channels.
+ *
+ *   leaf_attr   DEVICE float[n_leaves][n_channels], leaf order, channel fastest.
+ *   node_attr   DEVICE float[n_nodes][n_channels], caller-allocated, must not alias leaf_attr.
+ *               On completion node_attr[k][:] == leaf_attr[k][:] bit-for-bit for k < n_leaves; every
+ *               other entry holds fma(w, x_b, fma(-w, x_a, x_a)) per channel in fp32 (the arithmetic
+ *               of mg_propagate), in the library's numbering.
+ *   n_channels  1 .. MG_MAX_ATTR_CHANNELS.  Both buffers 4-byte aligned; 16-byte (8-byte) aligned
+ *               buffers with n_channels % 4 == 0 (% 2 == 0) take the vectorised path.
+ *
+ * Enqueue-only, no allocation.  Does not touch the 8/16-bit palettes of mg_propagate (mg_colorize on
+ * a 4-channel node_attr re-derives them, as for any foreign node_rgba).
+ * Errors: MG_ERR_INVALID_ARG (NULL, aliasing, misalignment, n_channels out of range), MG_ERR_CUDA.
+ * ------------------------------------------------------------------------------------------------ */
+#define MG_MAX_ATTR_CHANNELS 64
+int mg_propagate_attr(mg_graph *g, const float *leaf_attr, float *node_attr, uint32_t n_channels,
+                      void *stream);
+
 /* Thread-local description of the last error returned on this thread ("" if none). */
 const char *mg_last_error(void);
 

@@ -12,6 +12,7 @@ Function -> passage (PAPER.md line):
   direct_colour        O-2  L66 (<m, x>)
   brute_force_histogram O-3 Eq. 4 unrolled
   graph_eval           O-4  L259, L269, L371, Eq. 8
+  graph_eval_attr      NEXT-1: any numeric attribute, n_ch channels (L269, L271 (i)-(ii), L277)
   topo_levels          L211
   graph_eval_levels    L213, L373 (the paper's OpenMP CPU baseline shape)
   symbolic_eval        O-5  L321, L375
@@ -49,6 +50,8 @@ _lib.mgo_brute_force_histogram.argtypes = [_u32p, _u64, _u64, _u64, _u32, _u32, 
 _lib.mgo_brute_force_histogram.restype = None
 _lib.mgo_graph_eval.argtypes = [_u32p, _u32p, _f64p, _u64, _u64, _f64p, _f64p]
 _lib.mgo_graph_eval.restype = None
+_lib.mgo_graph_eval_attr.argtypes = [_u32p, _u32p, _f64p, _u64, _u64, _u32, _f64p, _f64p]
+_lib.mgo_graph_eval_attr.restype = None
 _lib.mgo_topo_levels.argtypes = [_u32p, _u32p, _u64, _u64, _u32p]
 _lib.mgo_topo_levels.restype = C.c_int64
 _lib.mgo_graph_eval_levels.argtypes = [_u32p, _u32p, _f64p, _u64, _u64p, _u64p, _u32, _f64p, _f64p, C.c_int]
@@ -138,6 +141,20 @@ def graph_eval(child_a, child_b, weight, n_leaves, tf):
     assert b.size == n and w.size == n and tf.shape == (n_leaves, 4)
     c = np.zeros((n, 4), dtype=np.float64)
     _lib.mgo_graph_eval(a, b, w, n, n_leaves, tf.reshape(-1), c.reshape(-1))
+    return c
+
+
+def graph_eval_attr(child_a, child_b, weight, n_leaves, attr):
+    """NEXT-1: c fp64 [n_nodes, n_ch] for an arbitrary per-leaf attribute ``attr`` [n_leaves, n_ch]
+    (opacity alone: n_ch = 1, L271; light contributions, L277; K batched TFs: n_ch = 4 K)."""
+    a, b = _c(child_a, np.uint32), _c(child_b, np.uint32)
+    w = _c(weight, np.float64)
+    attr = _c(attr, np.float64)
+    n = a.size
+    assert attr.ndim == 2 and attr.shape[0] == n_leaves and b.size == n and w.size == n
+    n_ch = attr.shape[1]
+    c = np.zeros((n, n_ch), dtype=np.float64)
+    _lib.mgo_graph_eval_attr(a, b, w, n, n_leaves, n_ch, attr.reshape(-1), c.reshape(-1))
     return c
 
 

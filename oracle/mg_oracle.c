@@ -159,6 +159,28 @@ void mgo_graph_eval(const uint32_t *child_a, const uint32_t *child_b, const doub
     }
 }
 
+/* ---- NEXT-1: the same evaluation for ANY numeric segment attribute with n_ch channels per node.
+ * "the Mixture Graph allows the efficient computation of any kind of numeric segmentation
+ * attribute" (L269); the paper's own uses besides RGBA: opacity alone for empty-space skipping
+ * (L271 (i)-(ii): "assigns opacity values of the current transfer function to the leafs,
+ * propagates these values through the Mixture Graph") and diffuse / specular light contributions
+ * (L277).  attr and c are [node][n_ch], channel fastest.  Same recurrence as mgo_graph_eval. */
+void mgo_graph_eval_attr(const uint32_t *child_a, const uint32_t *child_b, const double *weight,
+                         uint64_t n_nodes, uint64_t n_leaves, uint32_t n_ch, const double *attr,
+                         double *c)
+{
+    for (uint64_t n = 0; n < n_leaves; n++)
+        for (uint32_t ch = 0; ch < n_ch; ch++)
+            c[n * n_ch + ch] = attr[n * n_ch + ch];
+    for (uint64_t n = n_leaves; n < n_nodes; n++) {
+        double w = weight[n];
+        const double *ca = c + (uint64_t)child_a[n] * n_ch;
+        const double *cb = c + (uint64_t)child_b[n] * n_ch;
+        for (uint32_t ch = 0; ch < n_ch; ch++)
+            c[n * n_ch + ch] = (1.0 - w) * ca[ch] + w * cb[ch];
+    }
+}
+
 /* ---- Topological level (L211): sources 0; a node with predecessor values v1, v2 gets
  * max(v1, v2) + 1; "this amounts to a linear scan of all nodes".  Returns the depth (max level),
  * or -1 if a child index does not precede its parent (Eq. 8 violated). */

@@ -28,7 +28,8 @@ ALL_LEVELS = 0xFFFFFFFF
 SYMBOLS = ["mg_load_graph", "mg_free_graph", "mg_graph_info", "mg_level_offsets", "mg_node_permutation",
            "mg_relabel_indices", "mg_propagate", "mg_propagate_host", "mg_colorize", "mg_tf_update_host",
            "mg_last_error", "mg_kernel_launch_count",
-           "mg_bits_per_voxel", "mg_packed_stream_bytes", "mg_index_range", "mg_pack_indices", "mg_colorize_packed"]
+           "mg_bits_per_voxel", "mg_packed_stream_bytes", "mg_index_range", "mg_pack_indices", "mg_colorize_packed",
+           "mg_propagate_attr"]
 
 
 class MgInfo(C.Structure):
@@ -80,6 +81,11 @@ lib.mg_pack_indices.argtypes = [_vp, C.c_uint64, C.c_uint32, C.c_uint32, _vp, _v
 lib.mg_pack_indices.restype = C.c_int
 lib.mg_colorize_packed.argtypes = [_vp, _vp, C.POINTER(MgPackedLevel), C.c_uint32, _vp, _vp, _vp, C.c_uint32, _vp]
 lib.mg_colorize_packed.restype = C.c_int
+
+
+MG_MAX_ATTR_CHANNELS = 64
+lib.mg_propagate_attr.argtypes = [_vp, _vp, _vp, C.c_uint32, _vp]
+lib.mg_propagate_attr.restype = C.c_int
 
 
 class MgError(RuntimeError):
@@ -194,6 +200,10 @@ class Graph:
     def propagate_host(self, tf_host, node_rgba_device, stream: int = 0) -> None:
         _check(lib.mg_propagate_host(self._h, _ptr(tf_host), _ptr(node_rgba_device), stream or None),
                "mg_propagate_host")
+
+    def propagate_attr(self, leaf_attr_device, node_attr_device, n_channels: int, stream: int = 0) -> None:
+        _check(lib.mg_propagate_attr(self._h, _ptr(leaf_attr_device), _ptr(node_attr_device), int(n_channels),
+                                     stream or None), "mg_propagate_attr")
 
     def colorize(self, node_idx_device, n_voxels: int, node_rgba_device, out, out_aux=None,
                  fmt: int = MG_RGBA8, mip_level: int = ALL_LEVELS, stream: int = 0) -> None:

@@ -68,6 +68,14 @@ def random_tf(n_segments: int, seed: int, update: int = 0, alpha_zero_frac: floa
     return tf
 
 
+def random_attr(n_segments: int, n_channels: int, seed: int, lo: float = 0.0, hi: float = 1.0) -> np.ndarray:
+    """fp32 [n_segments, n_channels] uniform in [lo, hi): a generic per-segment attribute
+    (opacity alone, light contributions, K batched TFs as 4 K channels; NEXT-1)."""
+    i = np.arange(n_segments * n_channels, dtype=np.uint64)
+    u = uniform01(seed, 300 + n_channels, i).reshape(n_segments, n_channels)
+    return (np.float32(lo) + u * np.float32(hi - lo)).astype(np.float32)
+
+
 def single_segment_update(tf: np.ndarray, seed: int, update: int) -> np.ndarray:
     """Config 4: each update re-draws ONE random segment's RGBA; returns a new array."""
     out = tf.copy()

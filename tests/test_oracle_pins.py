@@ -236,6 +236,36 @@ def test_constant_tf_and_linearity():
     np.testing.assert_allclose(lhs, rhs, rtol=0, atol=1e-13)
 
 
+def test_graph_eval_attr_fig2_chain_and_matmul(golden_dir):
+    """NEXT-1 (L269 "any kind of numeric segmentation attribute", L271, L277): for every channel
+    count the root of Fig. 2 is m . attr, a chain follows the geometric closed form, and on a random
+    DAG the result is the numpy matmul mu @ attr with mu from the (separately pinned) symbolic
+    evaluation -- a transposed operand, a dropped (1 - w) or a wrong channel stride fails one."""
+    nodes, mix = _load_fig2(golden_dir)
+    a, b, w = _graph_from_fig(nodes, 7)
+    for n_ch in (1, 2, 3, 4, 7, 16):
+        attr = (synth.uniform01(31, n_ch, np.arange(4 * n_ch, dtype=np.uint64)).reshape(4, n_ch) * 3.0 - 1.0)
+        c = oracle.graph_eval_attr(a, b, w, 4, attr)
+        assert c.shape == (7, n_ch) and (c[:4] == attr).all()
+        np.testing.assert_allclose(c[6], np.array(mix["m"]) @ attr, rtol=0, atol=1e-15)
+    # chain closed form, 5 channels with distinct values per channel
+    K, wv = 25, 0.125
+    ca = np.zeros(K + 2, dtype=np.uint32); cb = np.zeros(K + 2, dtype=np.uint32); cw = np.zeros(K + 2)
+    for k in range(1, K + 1):
+        ca[k + 1], cb[k + 1], cw[k + 1] = (0 if k == 1 else k), 1, wv
+    attr = np.array([[1.0, -2.0, 0.5, 8.0, 0.0], [0.0, 4.0, 0.25, -8.0, 1.0]])
+    c = oracle.graph_eval_attr(ca, cb, cw, 2, attr)
+    for k in (1, 3, K):
+        g = (1 - wv) ** k
+        np.testing.assert_allclose(c[k + 1], g * attr[0] + (1 - g) * attr[1], rtol=0, atol=1e-14)
+    # random DAG: library matmul with the mixture lookup table
+    a, b, w, off, nl = _small_dag(seed=26)
+    mu = oracle.symbolic_eval(a, b, w, nl)
+    for n_ch in (1, 6):
+        attr = synth.uniform01(32, n_ch, np.arange(nl * n_ch, dtype=np.uint64)).reshape(nl, n_ch)
+        np.testing.assert_allclose(oracle.graph_eval_attr(a, b, w, nl, attr), mu @ attr, rtol=0, atol=1e-13)
+
+
 def test_topo_levels_definition():
     """L211: sources 0, node = max(v1, v2) + 1; Fig. 2 graph has levels 1, 2, 3."""
     a = np.array([0, 0, 0, 0, 0, 2, 3], dtype=np.uint32)
