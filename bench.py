@@ -47,6 +47,7 @@ def parse_args():
     p.add_argument("--e2e-steps", type=int, default=0, help="0 = min(steps, 8)")
     p.add_argument("--no-cpu-baseline", action="store_true")
     p.add_argument("--no-e2e", action="store_true")
+    p.add_argument("--no-attr", action="store_true", help="skip the extra NEXT-1 measurement (multi-attribute propagation)")
     p.add_argument("--no-packed", action="store_true", help="skip the extra NEXT-3 measurement (bit-packed node IDs)")
     p.add_argument("--cpu-sample-voxels", type=int, default=1 << 31, help="oracle sample size (>= the mipmap = whole workload)")
     p.add_argument("--reference-budget-s", type=float, default=90.0)
@@ -300,6 +301,26 @@ def run_b200(args) -> dict:
                   "what": "NEXT-3: node IDs stored as (id - i_min(l)) at r(l) bits per voxel (PAPER.md Table 1, Eq. 15-16)"}
         w.d_packed = None
 
+    # ---- NEXT-1 variant: the same graph pass for other attributes (opacity alone; 4 TFs batched as 16 channels)
+    attr = None
+    if not args.no_attr and rank == 0:
+        attr = {"what": "NEXT-1 mg_propagate_attr: C channels per node in ONE pass over the graph arrays (PAPER.md L269, L271, L277)",
+                "steps": min(K, 100)}
+        for C_, label in ((1, "opacity_only_c1_ms"), (16, "four_tfs_batched_c16_ms")):
+            leaf = torch.rand((int(info.n_leaves), C_), dtype=torch.float32, device="cuda")
+            xa = torch.empty((n_nodes, C_), dtype=torch.float32, device="cuda")
+            for _ in range(3):
+                g.propagate_attr(leaf, xa, C_, st)
+            torch.cuda.synchronize()
+            a0, a1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a0.record(stream)
+            for _ in range(attr["steps"]):
+                g.propagate_attr(leaf, xa, C_, st)
+            a1.record(stream)
+            torch.cuda.synchronize()
+            attr[label] = a0.elapsed_time(a1) / attr["steps"]
+            del leaf, xa
+
     # ---- e2e: host TF in, host mipmap out, through the public C-ABI call (rank-local, then max)
     e2e = None
     if not args.no_e2e:
@@ -356,6 +377,8 @@ def run_b200(args) -> dict:
     if packed is not None:
         packed["frac"] = packed["achieved_gbs"] / peak
         res["packed"] = packed
+    if attr is not None:
+        res["attr"] = attr
     if e2e is not None:
         res["e2e"] = e2e
     if world == 1 and not args.no_cpu_baseline and w.host_idx is not None:

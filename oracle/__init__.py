@@ -19,7 +19,8 @@ Function -> passage (PAPER.md line):
   lookup               L221, L267
   to_rgba8 / to_rgba16f  Q13 (defined by this repo; not in the paper)
   bits_per_voxel, index_range, pack_level, unpack_level   NEXT-3: Table 1 (8),(9),(A), Eq. 15-16
-All functions are pinned by tests/test_oracle_pins.py; none is "parity unpinned".
+  pixel_ray, sample_lod, render   NEXT-2: ray-marching the paletted mipmap, readings R1-R6 (L265-L271, L414)
+All functions are pinned by tests/test_oracle_pins.py / tests/test_oracle_render.py; none is "parity unpinned".
 """
 from __future__ import annotations
 
@@ -72,6 +73,12 @@ _lib.mgo_pack_bits.argtypes = [_u32p, _u64, _u32, _u32, _u8p]
 _lib.mgo_pack_bits.restype = None
 _lib.mgo_unpack_bits.argtypes = [_u8p, _u64, _u32, _u32, _u32p]
 _lib.mgo_unpack_bits.restype = None
+_lib.mgo_sample_lod.argtypes = [_u32p, _u64p, _u32p, _u32, _f64p, _f64p, C.c_double, _f64p]
+_lib.mgo_sample_lod.restype = None
+_lib.mgo_pixel_ray.argtypes = [_f64p, C.c_double, _u32, _u32, _u32, _u32, _f64p]
+_lib.mgo_pixel_ray.restype = None
+_lib.mgo_render.argtypes = [_u32p, _u64p, _u32p, _u32, _f64p, _f64p, _f64p, _u32, _u32, _f64p, _u64p]
+_lib.mgo_render.restype = None
 
 
 def _c(a, dt):
@@ -252,3 +259,53 @@ def unpack_level(stream, n_vox, i_min, r):
     out = np.zeros(int(n_vox), dtype=np.uint32)
     _lib.mgo_unpack_bits(st, int(n_vox), int(i_min), int(r), out)
     return out
+
+
+# ---- NEXT-2: ray-marching the paletted mipmap (section 4; readings R1-R6 in mg_oracle.c) ----
+
+def _pyramid(levels):
+    """levels: list of uint32 [Z_l, Y_l, X_l] node-index volumes, finest first -> (idx, offsets, dims)."""
+    offs, dims, flat, o = [], [], [], 0
+    for lv in levels:
+        lv = np.asarray(lv)
+        offs.append(o)
+        dims.append((lv.shape[2], lv.shape[1], lv.shape[0]))
+        flat.append(_c(lv, np.uint32).reshape(-1))
+        o += lv.size
+    return np.concatenate(flat), np.array(offs, dtype=np.uint64), np.array(dims, dtype=np.uint32).reshape(-1)
+
+
+def _cam_par(view):
+    cam = np.concatenate([np.asarray(view[k], dtype=np.float64).reshape(3) for k in ("eye", "right", "up", "forward")])
+    par = np.array([view["tan_half_fov"], *np.asarray(view["spacing"], dtype=np.float64).reshape(3), view["step_voxels"],
+                    view["ref_step_voxels"], view["lod_bias"], view["ess_threshold"], view["alpha_cutoff"]], dtype=np.float64)
+    return np.ascontiguousarray(cam), par
+
+
+def pixel_ray(view, i, j):
+    """R1: unit direction of pixel (i, j) (j = row from the top)."""
+    cam, par = _cam_par(view)
+    d = np.zeros(3)
+    _lib.mgo_pixel_ray(cam, par[0], int(view["width"]), int(view["height"]), int(i), int(j), d)
+    return d
+
+
+def sample_lod(levels, palette, p_vox, lam):
+    """R3: trilinear + inter-level blend at p_vox (level-0 voxel coordinates) for fractional level lam."""
+    idx, offs, dims = _pyramid(levels)
+    out = np.zeros(4)
+    _lib.mgo_sample_lod(idx, offs, dims, len(levels), _c(palette, np.float64).reshape(-1),
+                        np.ascontiguousarray(p_vox, dtype=np.float64), float(lam), out)
+    return out
+
+
+def render(levels, palette, view):
+    """R1-R6: fp64 image [H, W, 4] = (C_rgb associated, A) and (samples evaluated, samples skipped)."""
+    idx, offs, dims = _pyramid(levels)
+    cam, par = _cam_par(view)
+    W, H = int(view["width"]), int(view["height"])
+    out = np.zeros((H, W, 4), dtype=np.float64)
+    stats = np.zeros(2, dtype=np.uint64)
+    _lib.mgo_render(idx, offs, dims, len(levels), _c(palette, np.float64).reshape(-1), cam, par, W, H,
+                    out.reshape(-1), stats)
+    return out, (int(stats[0]), int(stats[1]))

@@ -350,3 +350,250 @@ void mgo_unpack_bits(const uint8_t *stream, uint64_t n_vox, uint32_t i_min, uint
         node_idx[v] = i_min + val;
     }
 }
+
+/* ==== NEXT-2: ray-marching the paletted histogram mipmap (section 4) ====
+ *
+ * "rendering from the Mixture Graph is the same as rendering from a paletted texture" (L267): a
+ * sample fetches node IDs, looks their colours up in the palette, and "we still have to perform the
+ * computation of the mip level as well as the interpolation in the shader manually" (L269).
+ * The paper gives the ingredients, not formulas; the readings (R1-R8) are:
+ *  R1 camera     pinhole; pixel (i, j) of a W x H image looks along
+ *                d = normalise(forward + u right + v up), u = (2 (i + 1/2) / W - 1) tan_half_fov W / H,
+ *                v = (1 - 2 (j + 1/2) / H) tan_half_fov; world units, voxel (x,y,z) of level 0
+ *                occupies [x sx, (x+1) sx] x ... (spacing s; "anisotropic voxels up to 1:1:7", L277).
+ *  R2 LOD        "the pixel coverage of a voxel is linear in viewspace depth z" (L269, GL 4.5 8.14):
+ *                rho = z_view (2 tan_half_fov / H) / s_ref voxels per pixel, s_ref = min spacing,
+ *                lambda = clamp(log2(rho) + lod_bias, 0, l_max).
+ *  R3 sample     GL_LINEAR_MIPMAP_LINEAR by hand: l0 = floor(lambda), f = lambda - l0, l1 = min(l0+1, l_max);
+ *                colour = (1 - f) tri(l0) + f tri(l1); tri(l) = trilinear interpolation of the 8
+ *                palette colours around p, voxel i of level l centred at (i + 1/2) 2^l level-0 voxels,
+ *                indices clamped to the level's extent; the four floats are interpolated as given (Q11).
+ *  R4 step       "the step size of a volume raymarcher can be adjusted to the LOD, which requires opacity
+ *                correction" (L269): Delta = step_voxels s_ref 2^lambda (0.5-voxel steps at full
+ *                resolution, L414); alpha' = 1 - (1 - alpha)^(Delta / (ref_step_voxels s_ref)).
+ *  R5 march      t from the entry of the volume's box; lambda and Delta from the interval start t, the
+ *                last interval is clipped to the exit, the sample sits at the interval's mid-point;
+ *                front-to-back: C += (1 - A) alpha' rgb, A += (1 - A) alpha'; stop at A >= alpha_cutoff.
+ *  R6 ESS        (L271) the opacity hierarchy is the A channel of the palette on the coarser mip levels.
+ *                From level l1 + 1 upwards, "as long as the opacity value in parent voxels falls below
+ *                a certain threshold" climb; the largest such block [lo, hi) is remembered and every
+ *                sample whose 16-voxel footprint lies inside it is skipped: trilinear at level l reads
+ *                voxels floor(p / 2^l - 1/2) and the next one, both inside the block iff
+ *                lo + 2^l / 2 <= p < hi - 2^l / 2; l = l1 is the binding level (no shrinking at faces
+ *                on the volume's boundary, where the fetch clamps to the edge).
+ * Output: [H][W][4] = (C_r, C_g, C_b, A), associated colour over a transparent background. */
+
+typedef struct mgo_view {
+    const uint32_t *node_idx;      /* all levels concatenated */
+    const uint64_t *level_offset;  /* [n_levels] first voxel of each level */
+    const uint32_t *level_dim;     /* [n_levels][3] = X_l, Y_l, Z_l */
+    uint32_t n_levels;
+    const double *palette;         /* [n_nodes][4] */
+} mgo_view;
+
+static const double *mgo_voxel_colour(const mgo_view *v, uint32_t l, int64_t i, int64_t j, int64_t k)
+{
+    const uint32_t *d = v->level_dim + 3 * l;
+    if (i < 0) i = 0;
+    if (j < 0) j = 0;
+    if (k < 0) k = 0;
+    if (i > (int64_t)d[0] - 1) i = (int64_t)d[0] - 1;
+    if (j > (int64_t)d[1] - 1) j = (int64_t)d[1] - 1;
+    if (k > (int64_t)d[2] - 1) k = (int64_t)d[2] - 1;
+    uint64_t lin = ((uint64_t)k * d[1] + (uint64_t)j) * d[0] + (uint64_t)i;
+    return v->palette + 4 * (uint64_t)v->node_idx[v->level_offset[l] + lin];
+}
+
+/* R3, one level: trilinear interpolation at p (level-0 voxel coordinates). */
+static void mgo_trilinear(const mgo_view *v, uint32_t l, const double p[3], double out[4])
+{
+    double scale = ldexp(1.0, -(int)l);
+    double u[3], fr[3];
+    int64_t i0[3];
+    for (int a = 0; a < 3; a++) {
+        u[a] = p[a] * scale - 0.5;
+        double fl = floor(u[a]);
+        i0[a] = (int64_t)fl;
+        fr[a] = u[a] - fl;
+    }
+    for (int ch = 0; ch < 4; ch++)
+        out[ch] = 0.0;
+    for (int dz = 0; dz < 2; dz++)
+        for (int dy = 0; dy < 2; dy++)
+            for (int dx = 0; dx < 2; dx++) {
+                double wgt = (dx ? fr[0] : 1.0 - fr[0]) * (dy ? fr[1] : 1.0 - fr[1]) * (dz ? fr[2] : 1.0 - fr[2]);
+                const double *c = mgo_voxel_colour(v, l, i0[0] + dx, i0[1] + dy, i0[2] + dz);
+                for (int ch = 0; ch < 4; ch++)
+                    out[ch] += wgt * c[ch];
+            }
+}
+
+/* R3: colour at p for a fractional level lambda in [0, l_max]. */
+void mgo_sample_lod(const uint32_t *node_idx, const uint64_t *level_offset, const uint32_t *level_dim,
+                    uint32_t n_levels, const double *palette, const double *p_vox, double lambda,
+                    double *out)
+{
+    mgo_view v = {node_idx, level_offset, level_dim, n_levels, palette};
+    uint32_t l_max = n_levels - 1;
+    if (lambda < 0.0) lambda = 0.0;
+    if (lambda > (double)l_max) lambda = (double)l_max;
+    uint32_t l0 = (uint32_t)floor(lambda);
+    uint32_t l1 = l0 + 1 > l_max ? l_max : l0 + 1;
+    double f = lambda - (double)l0;
+    double c0[4], c1[4];
+    mgo_trilinear(&v, l0, p_vox, c0);
+    mgo_trilinear(&v, l1, p_vox, c1);
+    for (int ch = 0; ch < 4; ch++)
+        out[ch] = (1.0 - f) * c0[ch] + f * c1[ch];
+}
+
+/* R1: direction of pixel (i, j).  cam = eye[3], right[3], up[3], forward[3]. */
+void mgo_pixel_ray(const double *cam, double tan_half_fov, uint32_t W, uint32_t H, uint32_t i, uint32_t j,
+                   double *dir)
+{
+    double u = (2.0 * ((double)i + 0.5) / (double)W - 1.0) * tan_half_fov * (double)W / (double)H;
+    double v = (1.0 - 2.0 * ((double)j + 0.5) / (double)H) * tan_half_fov;
+    double n = 0.0;
+    for (int a = 0; a < 3; a++) {
+        dir[a] = cam[9 + a] + u * cam[3 + a] + v * cam[6 + a];
+        n += dir[a] * dir[a];
+    }
+    n = sqrt(n);
+    for (int a = 0; a < 3; a++)
+        dir[a] /= n;
+}
+
+/* Slab test of the ray eye + t dir against the box [0, ext].  Returns 0 on a miss. */
+static int mgo_ray_box(const double *eye, const double *dir, const double *ext, double *t_near, double *t_far)
+{
+    double tn = 0.0, tf = INFINITY;
+    for (int a = 0; a < 3; a++) {
+        if (dir[a] == 0.0) {
+            if (eye[a] < 0.0 || eye[a] > ext[a])
+                return 0;
+        } else {
+            double t1 = (0.0 - eye[a]) / dir[a], t2 = (ext[a] - eye[a]) / dir[a];
+            double lo = t1 < t2 ? t1 : t2, hi = t1 < t2 ? t2 : t1;
+            if (lo > tn) tn = lo;
+            if (hi < tf) tf = hi;
+        }
+    }
+    if (!(tn < tf))
+        return 0;
+    *t_near = tn;
+    *t_far = tf;
+    return 1;
+}
+
+/* R2-R6 for one ray.  par = tan_half_fov, sx, sy, sz, step_voxels, ref_step_voxels, lod_bias,
+ * ess_threshold (< 0: no empty-space skipping), alpha_cutoff.  stats[0] += samples evaluated,
+ * stats[1] += samples skipped. */
+static void mgo_march(const mgo_view *v, const double *cam, const double *par, uint32_t H, const double *dir,
+                      double *rgba, uint64_t *stats)
+{
+    const double tanh_ = par[0], *s = par + 1, step = par[4], ref = par[5], bias = par[6], thr = par[7], cutoff = par[8];
+    const uint32_t l_max = v->n_levels - 1;
+    const double s_ref = fmin(s[0], fmin(s[1], s[2]));
+    double ext[3];
+    for (int a = 0; a < 3; a++)
+        ext[a] = (double)v->level_dim[a] * s[a];
+    double C[3] = {0, 0, 0}, A = 0.0;
+    rgba[0] = rgba[1] = rgba[2] = rgba[3] = 0.0;
+    double t_near, t_far;
+    if (!mgo_ray_box(cam, dir, ext, &t_near, &t_far))
+        return;
+    double cos_view = dir[0] * cam[9] + dir[1] * cam[10] + dir[2] * cam[11];
+    int box_valid = 0;
+    double box_lo[3] = {0, 0, 0}, box_hi[3] = {0, 0, 0};
+    int box_open_lo[3] = {0, 0, 0}, box_open_hi[3] = {0, 0, 0};     /* face on the volume's boundary */
+    double t = t_near;
+    while (t < t_far && A < cutoff) {
+        double rho = t * cos_view * (2.0 * tanh_ / (double)H) / s_ref;              /* R2 */
+        double lambda = rho > 0.0 ? log2(rho) + bias : 0.0;
+        if (lambda < 0.0) lambda = 0.0;
+        if (lambda > (double)l_max) lambda = (double)l_max;
+        double delta = step * s_ref * exp2(lambda);                                 /* R4 */
+        double de = delta < t_far - t ? delta : t_far - t;                          /* R5 */
+        double ts = t + 0.5 * de;
+        double p[3];
+        for (int a = 0; a < 3; a++)
+            p[a] = (cam[a] + ts * dir[a]) / s[a];
+        uint32_t l0 = (uint32_t)floor(lambda);
+        uint32_t l1 = l0 + 1 > l_max ? l_max : l0 + 1;
+        double f = lambda - (double)l0;
+        t += delta;
+        if (thr >= 0.0) {                                                           /* R6 */
+            double m = 0.5 * ldexp(1.0, (int)l1);
+            int inside = 0;
+            if (box_valid) {
+                inside = 1;
+                for (int a = 0; a < 3; a++)
+                    if ((!box_open_lo[a] && p[a] < box_lo[a] + m) || (!box_open_hi[a] && p[a] >= box_hi[a] - m))
+                        inside = 0;
+            }
+            if (!inside) {
+                box_valid = 0;
+                for (uint32_t L = l1 + 1; L <= l_max; L++) {
+                    const uint32_t *d = v->level_dim + 3 * L;
+                    int64_t q[3];
+                    for (int a = 0; a < 3; a++) {
+                        q[a] = (int64_t)floor(ldexp(p[a], -(int)L));
+                        if (q[a] < 0) q[a] = 0;
+                        if (q[a] > (int64_t)d[a] - 1) q[a] = (int64_t)d[a] - 1;
+                    }
+                    if (!(mgo_voxel_colour(v, L, q[0], q[1], q[2])[3] < thr))
+                        break;
+                    box_valid = 1;
+                    for (int a = 0; a < 3; a++) {
+                        box_lo[a] = ldexp((double)q[a], (int)L);
+                        box_hi[a] = ldexp((double)(q[a] + 1), (int)L);
+                        box_open_lo[a] = q[a] == 0;
+                        box_open_hi[a] = q[a] == (int64_t)d[a] - 1;
+                    }
+                }
+                if (box_valid) {
+                    inside = 1;
+                    for (int a = 0; a < 3; a++)
+                        if ((!box_open_lo[a] && p[a] < box_lo[a] + m) || (!box_open_hi[a] && p[a] >= box_hi[a] - m))
+                            inside = 0;
+                }
+            }
+            if (inside) {
+                if (stats) stats[1]++;
+                continue;
+            }
+        }
+        double c0[4], c1[4], c[4];
+        mgo_trilinear(v, l0, p, c0);
+        mgo_trilinear(v, l1, p, c1);
+        for (int ch = 0; ch < 4; ch++)
+            c[ch] = (1.0 - f) * c0[ch] + f * c1[ch];
+        double alpha = c[3] < 0.0 ? 0.0 : (c[3] > 1.0 ? 1.0 : c[3]);
+        double ac = 1.0 - pow(1.0 - alpha, de / (ref * s_ref));                      /* R4 */
+        for (int ch = 0; ch < 3; ch++)
+            C[ch] += (1.0 - A) * ac * c[ch];
+        A += (1.0 - A) * ac;
+        if (stats) stats[0]++;
+    }
+    rgba[0] = C[0]; rgba[1] = C[1]; rgba[2] = C[2]; rgba[3] = A;
+}
+
+/* The image: every pixel (i, j), j = row from the top.  out = [H][W][4] doubles. */
+void mgo_render(const uint32_t *node_idx, const uint64_t *level_offset, const uint32_t *level_dim,
+                uint32_t n_levels, const double *palette, const double *cam, const double *par,
+                uint32_t W, uint32_t H, double *out, uint64_t *stats)
+{
+    mgo_view v = {node_idx, level_offset, level_dim, n_levels, palette};
+    uint64_t st[2] = {0, 0};
+#pragma omp parallel for schedule(dynamic, 1) reduction(+ : st[:2])
+    for (int64_t j = 0; j < (int64_t)H; j++)
+        for (uint32_t i = 0; i < W; i++) {
+            double dir[3];
+            uint64_t loc[2] = {0, 0};
+            mgo_pixel_ray(cam, par[0], W, H, i, (uint32_t)j, dir);
+            mgo_march(&v, cam, par, H, dir, out + 4 * ((uint64_t)j * W + i), loc);
+            st[0] += loc[0];
+            st[1] += loc[1];
+        }
+    if (stats) { stats[0] = st[0]; stats[1] = st[1]; }
+}

@@ -76,6 +76,30 @@ def random_attr(n_segments: int, n_channels: int, seed: int, lo: float = 0.0, hi
     return (np.float32(lo) + u * np.float32(hi - lo)).astype(np.float32)
 
 
+def orbit_view(dims_xyz, spacing=(1.0, 1.0, 1.0), azimuth_deg: float = 30.0, elevation_deg: float = 20.0,
+               distance: float = 1.6, fov_deg: float = 40.0, width: int = 64, height: int = 48,
+               step_voxels: float = 0.5, ref_step_voxels: float = 1.0, lod_bias: float = 0.0,
+               ess_threshold: float = 1e-8, alpha_cutoff: float = 1.0) -> dict:
+    """A pinhole view of the volume for the ray-marcher (NEXT-2): the eye orbits the volume's centre at
+    ``distance`` x the box diagonal, looking at the centre.  Pure input construction (an orthonormal
+    camera basis); the meaning of every field is defined by the renderer (include/mg.h, oracle R1-R6).
+    The paper renders 1600 x 1200 at 0.5-voxel steps (L414) with an ESS threshold of 1e-8 (L271)."""
+    ext = np.asarray(dims_xyz, dtype=np.float64) * np.asarray(spacing, dtype=np.float64)
+    centre = 0.5 * ext
+    az, el = np.deg2rad(azimuth_deg), np.deg2rad(elevation_deg)
+    back = np.array([np.cos(el) * np.cos(az), np.cos(el) * np.sin(az), np.sin(el)])
+    eye = centre + back * distance * float(np.linalg.norm(ext))
+    forward = -back
+    world_up = np.array([0.0, 0.0, 1.0]) if abs(back[2]) < 0.99 else np.array([0.0, 1.0, 0.0])
+    right = np.cross(forward, world_up)
+    right /= np.linalg.norm(right)
+    up = np.cross(right, forward)
+    return dict(width=int(width), height=int(height), eye=eye, right=right, up=up, forward=forward,
+                tan_half_fov=float(np.tan(np.deg2rad(fov_deg) / 2)), spacing=np.asarray(spacing, dtype=np.float64),
+                step_voxels=float(step_voxels), ref_step_voxels=float(ref_step_voxels), lod_bias=float(lod_bias),
+                ess_threshold=float(ess_threshold), alpha_cutoff=float(alpha_cutoff))
+
+
 def single_segment_update(tf: np.ndarray, seed: int, update: int) -> np.ndarray:
     """Config 4: each update re-draws ONE random segment's RGBA; returns a new array."""
     out = tf.copy()
