@@ -233,6 +233,68 @@ int mg_colorize_packed(mg_graph *g, const void *packed_device, const mg_packed_l
 int mg_propagate_attr(mg_graph *g, const float *leaf_attr, float *node_attr, uint32_t n_channels,
                       void *stream);
 
+/* ------------------------------------------------------------------------------------------------
+ * NEXT-2: headless ray-marcher over the paletted histogram mipmap (section 4,
+ * L414): "rendering from the Mixture Graph is the same as rendering from a paletted texture" (L267);
+ * "we still have to perform the computation of the mip level as well as the interpolation in the
+ * shader manually" (L269).  The paper gives the ingredients, not formulas; the readings R1-R6 are
+ * listed in DESIGN.md section 3:
+ *   R1 pinhole camera: pixel (i, j) (j = row from the top) looks along
+ *      normalise(forward + u right + v up), u = (2 (i + 1/2) / W - 1) tan_half_fov W / H,
+ *      v = (1 - 2 (j + 1/2) / H) tan_half_fov; voxel (x, y, z) of level 0 occupies
+ *      [x sx, (x + 1) sx] x ... in world units (anisotropic spacing, L277).
+ *   R2 LOD linear in view depth (L269): rho = z_view (2 tan_half_fov / H) / s_ref, s_ref = min spacing,
+ *      lambda = clamp(log2(rho) + lod_bias, 0, l_max).
+ *   R3 manual trilinear interpolation of palette colours on levels floor(lambda) and floor(lambda)+1
+ *      (voxel i of level l centred at (i + 1/2) 2^l, indices clamped to the level), blended by frac(lambda).
+ *   R4 step Delta = step_voxels s_ref 2^lambda with opacity correction
+ *      alpha' = 1 - (1 - alpha)^(Delta / (ref_step_voxels s_ref)) (L269; 0.5-voxel steps, L414).
+ *   R5 front-to-back compositing from the entry of the volume's box, sample at the interval mid-point,
+ *      last interval clipped to the exit, stop at A >= alpha_cutoff.
+ *   R6 hierarchical empty-space skipping (L271): from level floor(lambda)+2 upwards climb while the
+ *      parent voxel's palette opacity is < ess_threshold; samples whose whole 2 x 8-voxel footprint
+ *      lies in the largest such block are not fetched.  ess_threshold < 0 disables it.
+ * Arithmetic: ray geometry (t, step, sample position, trilinear fractions, block tests) in fp64;
+ * fractional LOD, interpolation weights, colours, opacity correction and compositing in fp32.
+ * ------------------------------------------------------------------------------------------------ */
+#define MG_MAX_MIP_LEVELS 24
+
+typedef struct mg_mipmap_desc {
+    uint32_t n_levels;                             /* 1 .. MG_MAX_MIP_LEVELS                              */
+    uint32_t reserved;                             /* 0                                                   */
+    uint64_t level_offset[MG_MAX_MIP_LEVELS];      /* first voxel of level l in node_idx_mipmap           */
+    uint32_t level_dim[MG_MAX_MIP_LEVELS][3];      /* X_l, Y_l, Z_l; level l+1 = ceil(level l / 2), L80   */
+} mg_mipmap_desc;
+
+typedef struct mg_view {
+    double eye[3], right[3], up[3], forward[3];    /* world units; right/up/forward orthonormal           */
+    double tan_half_fov;                           /* vertical half field of view                         */
+    double spacing[3];                             /* world size of a level-0 voxel along x, y, z (> 0)    */
+    double step_voxels;                            /* > 0; step at full resolution in units of s_ref       */
+    double ref_step_voxels;                        /* > 0; step the TF opacities refer to                  */
+    double lod_bias;
+    double ess_threshold;                          /* < 0: no empty-space skipping (paper: 1e-8)           */
+    double alpha_cutoff;                           /* early ray termination (1.0 = never)                  */
+    uint32_t width, height;                        /* image size in pixels (> 0)                           */
+} mg_view;
+
+/*
+ * mg_render -- one image.  Enqueue-only, no allocation, one kernel launch.
+ *   node_idx_mipmap  DEVICE uint32, every level concatenated as `mip` describes, x fastest, values
+ *                    < n_nodes in the library's numbering (not checked).
+ *   mip, view        HOST, copied at enqueue.
+ *   node_rgba        DEVICE float[n_nodes][4], 16-byte aligned: the palette (any mg_propagate output).
+ *   out_rgba         DEVICE float[height][width][4], 16-byte aligned: (C_r, C_g, C_b, A), associated
+ *                    colour over a transparent background; rays missing the volume give zeros.
+ *   stats_device     DEVICE uint64[2] or NULL: += samples evaluated, += samples skipped by R6
+ *                    (the caller zeroes it).
+ * Errors: MG_ERR_INVALID_ARG (NULL, misalignment, bad sizes, level dims that are not the ceil-halving
+ * chain of L80, offsets overlapping), MG_ERR_CUDA.
+ */
+int mg_render(mg_graph *g, const uint32_t *node_idx_mipmap, const mg_mipmap_desc *mip,
+              const float *node_rgba, const mg_view *view, float *out_rgba, uint64_t *stats_device,
+              void *stream);
+
 /* Thread-local description of the last error returned on this thread ("" if none). */
 const char *mg_last_error(void);
 

@@ -1,0 +1,301 @@
+// mg_render.cu -- NEXT-2: headless ray-marcher over the paletted histogram mipmap.
+//
+// PAPER.md section 4 (L265-L271, L414): the renderer treats the histogram mipmap as a paletted
+// texture (L267): a sample fetches node IDs and looks their colours up in the palette that
+// mg_propagate wrote; "the computation of the mip level as well as the interpolation" are done by
+// hand (L269), the step grows with the LOD and opacities are corrected for it (L269), and the A
+// channel of the coarser levels drives hierarchical empty-space skipping (L271).  Readings R1-R6:
+// include/mg.h, DESIGN.md section 3.
+//
+// Mapping: one thread per ray; a CTA is an 8 x 8 pixel tile (each warp an 8 x 4 tile, so the 32
+// rays of a warp walk through neighbouring voxels and their gathers share sectors).  Per sample at
+// most 2 x (8 index gathers + 8 palette gathers): the index volume streams through L2 from HBM, the
+// palette (16 B per node, tens of MB) stays L2-resident.  Three data-dependent shortcuts that do
+// not change the value beyond rounding: the second level is not fetched when frac(lambda) == 0; a
+// footprint whose 8 voxels name the same node costs one palette gather; skipped samples (R6) cost
+// no memory access at all.
+// Arithmetic: t, the step, the sample position, the trilinear fractions and the block tests in fp64
+// (the B200's fp64 pipe is half the fp32 rate and the loop is gather-latency-bound, so this is free
+// and keeps sample positions within 1e-12 voxels of the oracle's); the fractional LOD, the weights,
+// colours, opacity correction and compositing in fp32.
+#include <math.h>
+
+#include <cstring>
+
+#include "mg_internal.h"
+
+namespace {
+
+constexpr int kTileX = 8, kTileY = 8;
+
+struct RenderParams {
+    const uint32_t* idx;
+    const float4* pal;
+    float4* out;
+    unsigned long long* stats;
+    unsigned long long off[MG_MAX_MIP_LEVELS];
+    int dim[MG_MAX_MIP_LEVELS][3];
+    int n_levels;
+    unsigned W, H;
+    double eye[3], right[3], up[3], fwd[3];
+    double inv_s[3], ext[3];
+    double tan_half_fov, pix;       // pix = 2^lod_bias (2 tan_half_fov / H) / s_ref
+    double pow_lmax;                // 2^l_max
+    double thr;                     // ess threshold (< 0: off)
+    double step_ref;                // step_voxels * s_ref
+    float inv_ref;                  // 1 / (ref_step_voxels * s_ref)
+    float cutoff;
+};
+
+__device__ __forceinline__ int clampi(int v, int hi) { return v < 0 ? 0 : (v > hi ? hi : v); }
+
+__device__ __forceinline__ void tap(float4& acc, const float4* __restrict__ pal, uint32_t n, float wgt)
+{
+    const float4 c = __ldg(pal + n);
+    acc.x = fmaf(wgt, c.x, acc.x); acc.y = fmaf(wgt, c.y, acc.y);
+    acc.z = fmaf(wgt, c.z, acc.z); acc.w = fmaf(wgt, c.w, acc.w);
+}
+
+// R3, one level: trilinear interpolation of the palette at p (level-0 voxel coordinates).
+__device__ __forceinline__ float4 trilinear(const RenderParams& P, int l, double px, double py, double pz)
+{
+    const double sc = __hiloint2double((1023 - l) << 20, 0);            // 2^-l
+    const double ux = fma(px, sc, -0.5), uy = fma(py, sc, -0.5), uz = fma(pz, sc, -0.5);
+    const double flx = floor(ux), fly = floor(uy), flz = floor(uz);
+    const float fx = (float)(ux - flx), fy = (float)(uy - fly), fz = (float)(uz - flz);
+    const int X = P.dim[l][0], Y = P.dim[l][1], Z = P.dim[l][2];
+    const int ix = (int)flx, iy = (int)fly, iz = (int)flz;
+    const int x0 = clampi(ix, X - 1), x1 = clampi(ix + 1, X - 1);
+    const int y0 = clampi(iy, Y - 1), y1 = clampi(iy + 1, Y - 1);
+    const int z0 = clampi(iz, Z - 1), z1 = clampi(iz + 1, Z - 1);
+    const uint32_t* base = P.idx + P.off[l];
+    const uint32_t* r00 = base + ((size_t)z0 * Y + y0) * X;
+    const uint32_t* r01 = base + ((size_t)z0 * Y + y1) * X;
+    const uint32_t* r10 = base + ((size_t)z1 * Y + y0) * X;
+    const uint32_t* r11 = base + ((size_t)z1 * Y + y1) * X;
+    const uint32_t n000 = __ldg(r00 + x0), n001 = __ldg(r00 + x1), n010 = __ldg(r01 + x0), n011 = __ldg(r01 + x1);
+    const uint32_t n100 = __ldg(r10 + x0), n101 = __ldg(r10 + x1), n110 = __ldg(r11 + x0), n111 = __ldg(r11 + x1);
+    const uint32_t same = (n000 ^ n001) | (n000 ^ n010) | (n000 ^ n011) | (n000 ^ n100) | (n000 ^ n101) |
+                          (n000 ^ n110) | (n000 ^ n111);
+    if (same == 0) return __ldg(P.pal + n000);                           // segment interior
+    const float gx = 1.f - fx, gy = 1.f - fy, gz = 1.f - fz;
+    float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+    tap(acc, P.pal, n000, gx * gy * gz); tap(acc, P.pal, n001, fx * gy * gz);
+    tap(acc, P.pal, n010, gx * fy * gz); tap(acc, P.pal, n011, fx * fy * gz);
+    tap(acc, P.pal, n100, gx * gy * fz); tap(acc, P.pal, n101, fx * gy * fz);
+    tap(acc, P.pal, n110, gx * fy * fz); tap(acc, P.pal, n111, fx * fy * fz);
+    return acc;
+}
+
+// R6 block: voxel-aligned box [lo, hi) in level-0 coordinates; bit a of open_lo / open_hi = the face
+// lies on the volume's boundary (the trilinear fetch clamps there, so no margin is needed).
+struct EssBlock {
+    int lo[3], hi[3];
+    unsigned open_lo, open_hi;
+    bool valid;
+};
+
+__device__ __forceinline__ bool inside_block(const EssBlock& B, double m, double px, double py, double pz)
+{
+    const double p[3] = {px, py, pz};
+    bool in = true;
+#pragma unroll
+    for (int a = 0; a < 3; a++) {
+        if (!((B.open_lo >> a) & 1u) && p[a] < (double)B.lo[a] + m) in = false;
+        if (!((B.open_hi >> a) & 1u) && p[a] >= (double)B.hi[a] - m) in = false;
+    }
+    return in;
+}
+
+__global__ void __launch_bounds__(kTileX * kTileY)
+k_render(const __grid_constant__ RenderParams P)
+{
+    const unsigned i = blockIdx.x * kTileX + (threadIdx.x & (kTileX - 1));
+    const unsigned j = blockIdx.y * kTileY + threadIdx.x / kTileX;
+    const bool live = i < P.W && j < P.H;
+    unsigned n_eval = 0, n_skip = 0;
+    float Cr = 0.f, Cg = 0.f, Cb = 0.f, A = 0.f;
+    if (live) {
+        // R1: pixel ray
+        const double u = (2.0 * ((double)i + 0.5) / (double)P.W - 1.0) * P.tan_half_fov * (double)P.W / (double)P.H;
+        const double v = (1.0 - 2.0 * ((double)j + 0.5) / (double)P.H) * P.tan_half_fov;
+        double d[3], nrm = 0.0;
+#pragma unroll
+        for (int a = 0; a < 3; a++) {
+            d[a] = P.fwd[a] + u * P.right[a] + v * P.up[a];
+            nrm += d[a] * d[a];
+        }
+        nrm = sqrt(nrm);
+#pragma unroll
+        for (int a = 0; a < 3; a++) d[a] /= nrm;
+        // slab test against [0, ext]
+        double tn = 0.0, tf = INFINITY;
+        bool hit = true;
+#pragma unroll
+        for (int a = 0; a < 3; a++) {
+            if (d[a] == 0.0) {
+                if (P.eye[a] < 0.0 || P.eye[a] > P.ext[a]) hit = false;
+            } else {
+                const double t1 = (0.0 - P.eye[a]) / d[a], t2 = (P.ext[a] - P.eye[a]) / d[a];
+                tn = fmax(tn, fmin(t1, t2));
+                tf = fmin(tf, fmax(t1, t2));
+            }
+        }
+        if (!(tn < tf)) hit = false;
+        if (hit) {
+            const double cos_view = d[0] * P.fwd[0] + d[1] * P.fwd[1] + d[2] * P.fwd[2];
+            const double rho_t = cos_view * P.pix;                              // rho 2^bias = t * rho_t (R2)
+            const int l_max = P.n_levels - 1;
+            const bool ess = P.thr >= 0.0;
+            EssBlock B;
+            B.valid = false;
+            B.open_lo = B.open_hi = 0;
+#pragma unroll
+            for (int a = 0; a < 3; a++) B.lo[a] = B.hi[a] = 0;
+            double t = tn;
+            while (t < tf && A < P.cutoff) {
+                // R2 + R4 without transcendentals on the ray parameter: 2^lambda = clamp(rho 2^bias, 1, 2^l_max),
+                // so Delta = step s_ref 2^lambda is a product in fp64 and t follows the oracle's to rounding.
+                const double pow_lambda = fmin(fmax(t * rho_t, 1.0), P.pow_lmax);
+                const float lambda = fminf(log2f((float)pow_lambda), (float)l_max);
+                const double delta = P.step_ref * pow_lambda;                    // R4
+                const double de = fmin(delta, tf - t);                           // R5
+                const double ts = fma(0.5, de, t);
+                const double px = fma(ts, d[0], P.eye[0]) * P.inv_s[0];
+                const double py = fma(ts, d[1], P.eye[1]) * P.inv_s[1];
+                const double pz = fma(ts, d[2], P.eye[2]) * P.inv_s[2];
+                const float fl = floorf(lambda);
+                const int l0 = (int)fl;
+                const int l1 = min(l0 + 1, l_max);
+                const float f = lambda - fl;
+                t += delta;
+                if (ess) {                                                       // R6
+                    const double m = __hiloint2double((1022 + l1) << 20, 0);     // 2^l1 / 2
+                    bool inside = B.valid && inside_block(B, m, px, py, pz);
+                    if (!inside) {
+                        B.valid = false;
+                        for (int L = l1 + 1; L <= l_max; L++) {
+                            const double sc = __hiloint2double((1023 - L) << 20, 0);
+                            const int qx = clampi((int)floor(px * sc), P.dim[L][0] - 1);
+                            const int qy = clampi((int)floor(py * sc), P.dim[L][1] - 1);
+                            const int qz = clampi((int)floor(pz * sc), P.dim[L][2] - 1);
+                            const uint32_t n = __ldg(P.idx + P.off[L] + ((size_t)qz * P.dim[L][1] + qy) * P.dim[L][0] + qx);
+                            const float alpha_parent = __ldg(reinterpret_cast<const float*>(P.pal + n) + 3);
+                            if (!((double)alpha_parent < P.thr)) break;
+                            B.valid = true;
+                            B.lo[0] = qx << L; B.lo[1] = qy << L; B.lo[2] = qz << L;
+                            B.hi[0] = (qx + 1) << L; B.hi[1] = (qy + 1) << L; B.hi[2] = (qz + 1) << L;
+                            B.open_lo = (qx == 0) | ((qy == 0) << 1) | ((qz == 0) << 2);
+                            B.open_hi = (qx == P.dim[L][0] - 1) | ((qy == P.dim[L][1] - 1) << 1) | ((qz == P.dim[L][2] - 1) << 2);
+                        }
+                        inside = B.valid && inside_block(B, m, px, py, pz);
+                    }
+                    if (inside) {
+                        n_skip++;
+                        continue;
+                    }
+                }
+                float4 c = trilinear(P, l0, px, py, pz);                          // R3
+                if (f != 0.f) {
+                    const float4 c1 = trilinear(P, l1, px, py, pz);
+                    const float g = 1.f - f;
+                    c.x = fmaf(f, c1.x, g * c.x); c.y = fmaf(f, c1.y, g * c.y);
+                    c.z = fmaf(f, c1.z, g * c.z); c.w = fmaf(f, c1.w, g * c.w);
+                }
+                const float alpha = fminf(fmaxf(c.w, 0.f), 1.f);
+                const float e = (float)de * P.inv_ref;
+                const float ac = -expm1f(e * log1pf(-alpha));                     // 1 - (1 - alpha)^e
+                const float wgt = (1.f - A) * ac;
+                Cr = fmaf(wgt, c.x, Cr); Cg = fmaf(wgt, c.y, Cg); Cb = fmaf(wgt, c.z, Cb);
+                A += wgt;
+                n_eval++;
+            }
+        }
+        P.out[(size_t)j * P.W + i] = make_float4(Cr, Cg, Cb, A);
+    }
+    if (P.stats) {
+        const unsigned e = __reduce_add_sync(0xffffffffu, n_eval);
+        const unsigned s = __reduce_add_sync(0xffffffffu, n_skip);
+        if ((threadIdx.x & 31) == 0) {
+            if (e) atomicAdd(P.stats, (unsigned long long)e);
+            if (s) atomicAdd(P.stats + 1, (unsigned long long)s);
+        }
+    }
+}
+
+}  // namespace
+
+extern "C" int mg_render(mg_graph* g, const uint32_t* node_idx_mipmap, const mg_mipmap_desc* mip,
+                         const float* node_rgba, const mg_view* view, float* out_rgba, uint64_t* stats_device,
+                         void* stream)
+{
+    if (!g || !node_idx_mipmap || !mip || !node_rgba || !view || !out_rgba) {
+        mg::set_error("mg_render: NULL argument");
+        return MG_ERR_INVALID_ARG;
+    }
+    if (((uintptr_t)node_rgba & 15) || ((uintptr_t)out_rgba & 15) || ((uintptr_t)node_idx_mipmap & 3) ||
+        ((uintptr_t)stats_device & 7)) {
+        mg::set_error("mg_render: node_rgba / out_rgba must be 16-byte aligned (stats 8, indices 4)");
+        return MG_ERR_INVALID_ARG;
+    }
+    if (mip->n_levels == 0 || mip->n_levels > MG_MAX_MIP_LEVELS) {
+        mg::set_error("mg_render: n_levels = %u not in 1..%d", mip->n_levels, MG_MAX_MIP_LEVELS);
+        return MG_ERR_INVALID_ARG;
+    }
+    if (view->width == 0 || view->height == 0 || view->width > 65536u || view->height > 65536u) {
+        mg::set_error("mg_render: image size %u x %u out of range", view->width, view->height);
+        return MG_ERR_INVALID_ARG;
+    }
+    const double* s = view->spacing;
+    if (!(s[0] > 0.0) || !(s[1] > 0.0) || !(s[2] > 0.0) || !(view->step_voxels > 0.0) || !(view->ref_step_voxels > 0.0) ||
+        !(view->tan_half_fov > 0.0) || !isfinite(view->lod_bias) || !isfinite(view->step_voxels) ||
+        !isfinite(view->tan_half_fov) || isnan(view->ess_threshold) || isnan(view->alpha_cutoff)) {
+        mg::set_error("mg_render: spacing, step_voxels, ref_step_voxels and tan_half_fov must be positive and finite");
+        return MG_ERR_INVALID_ARG;
+    }
+    RenderParams P;
+    memset(&P, 0, sizeof(P));
+    for (uint32_t l = 0; l < mip->n_levels; l++) {
+        for (int a = 0; a < 3; a++) {
+            const uint32_t dl = mip->level_dim[l][a];
+            if (dl == 0 || dl > (1u << 20) || (l > 0 && dl != (mip->level_dim[l - 1][a] + 1) / 2)) {
+                mg::set_error("mg_render: level %u axis %d has %u voxels: not the ceil-halving chain of L80", l, a, dl);
+                return MG_ERR_INVALID_ARG;
+            }
+            P.dim[l][a] = (int)dl;
+        }
+        if (l > 0) {
+            const uint64_t prev = (uint64_t)mip->level_dim[l - 1][0] * mip->level_dim[l - 1][1] * mip->level_dim[l - 1][2];
+            if (mip->level_offset[l] < mip->level_offset[l - 1] + prev) {
+                mg::set_error("mg_render: level %u starts inside level %u", l, l - 1);
+                return MG_ERR_INVALID_ARG;
+            }
+        }
+        P.off[l] = mip->level_offset[l];
+    }
+    P.idx = node_idx_mipmap;
+    P.pal = reinterpret_cast<const float4*>(node_rgba);
+    P.out = reinterpret_cast<float4*>(out_rgba);
+    P.stats = reinterpret_cast<unsigned long long*>(stats_device);
+    P.n_levels = (int)mip->n_levels;
+    P.W = view->width;
+    P.H = view->height;
+    const double s_ref = fmin(s[0], fmin(s[1], s[2]));
+    for (int a = 0; a < 3; a++) {
+        P.eye[a] = view->eye[a]; P.right[a] = view->right[a]; P.up[a] = view->up[a]; P.fwd[a] = view->forward[a];
+        P.inv_s[a] = 1.0 / s[a];
+        P.ext[a] = (double)mip->level_dim[0][a] * s[a];
+    }
+    P.tan_half_fov = view->tan_half_fov;
+    P.pix = exp2(view->lod_bias) * (2.0 * view->tan_half_fov / (double)view->height) / s_ref;
+    P.pow_lmax = ldexp(1.0, (int)mip->n_levels - 1);
+    P.thr = view->ess_threshold;
+    P.step_ref = view->step_voxels * s_ref;
+    P.inv_ref = (float)(1.0 / (view->ref_step_voxels * s_ref));
+    P.cutoff = (float)view->alpha_cutoff;
+    const dim3 grid((P.W + kTileX - 1) / kTileX, (P.H + kTileY - 1) / kTileY);
+    k_render<<<grid, kTileX * kTileY, 0, (cudaStream_t)stream>>>(P);
+    MG_CUDA(cudaGetLastError());
+    mg::count_launch();
+    return MG_OK;
+}

@@ -29,7 +29,7 @@ SYMBOLS = ["mg_load_graph", "mg_free_graph", "mg_graph_info", "mg_level_offsets"
            "mg_relabel_indices", "mg_propagate", "mg_propagate_host", "mg_colorize", "mg_tf_update_host",
            "mg_last_error", "mg_kernel_launch_count",
            "mg_bits_per_voxel", "mg_packed_stream_bytes", "mg_index_range", "mg_pack_indices", "mg_colorize_packed",
-           "mg_propagate_attr"]
+           "mg_propagate_attr", "mg_render"]
 
 
 class MgInfo(C.Structure):
@@ -86,6 +86,25 @@ lib.mg_colorize_packed.restype = C.c_int
 MG_MAX_ATTR_CHANNELS = 64
 lib.mg_propagate_attr.argtypes = [_vp, _vp, _vp, C.c_uint32, _vp]
 lib.mg_propagate_attr.restype = C.c_int
+
+
+MG_MAX_MIP_LEVELS = 24
+
+
+class MgMipmapDesc(C.Structure):
+    _fields_ = [("n_levels", C.c_uint32), ("reserved", C.c_uint32), ("level_offset", C.c_uint64 * MG_MAX_MIP_LEVELS),
+                ("level_dim", (C.c_uint32 * 3) * MG_MAX_MIP_LEVELS)]
+
+
+class MgView(C.Structure):
+    _fields_ = [("eye", C.c_double * 3), ("right", C.c_double * 3), ("up", C.c_double * 3), ("forward", C.c_double * 3),
+                ("tan_half_fov", C.c_double), ("spacing", C.c_double * 3), ("step_voxels", C.c_double),
+                ("ref_step_voxels", C.c_double), ("lod_bias", C.c_double), ("ess_threshold", C.c_double),
+                ("alpha_cutoff", C.c_double), ("width", C.c_uint32), ("height", C.c_uint32)]
+
+
+lib.mg_render.argtypes = [_vp, _vp, C.POINTER(MgMipmapDesc), _vp, C.POINTER(MgView), _vp, _vp, _vp]
+lib.mg_render.restype = C.c_int
 
 
 class MgError(RuntimeError):
@@ -145,6 +164,31 @@ def packed_levels(levels) -> "C.Array":
             l = (l["n_voxels"], l["out_offset"], l["byte_offset"], l["bits"], l["i_min"])
         arr[i] = MgPackedLevel(*[int(x) for x in l])
     return arr
+
+
+def mipmap_desc(level_offsets, level_dims_xyz) -> MgMipmapDesc:
+    """level_offsets[l] = first voxel of level l, level_dims_xyz[l] = (X_l, Y_l, Z_l)."""
+    d = MgMipmapDesc()
+    d.n_levels = len(level_offsets)
+    if d.n_levels > MG_MAX_MIP_LEVELS:
+        raise ValueError(f"at most {MG_MAX_MIP_LEVELS} mip levels")
+    for l, (o, dims) in enumerate(zip(level_offsets, level_dims_xyz)):
+        d.level_offset[l] = int(o)
+        for a in range(3):
+            d.level_dim[l][a] = int(dims[a])
+    return d
+
+
+def view_struct(view: dict) -> MgView:
+    """Marshal a view dictionary (the fields of mg_view; synth.orbit_view builds one)."""
+    v = MgView()
+    for k in ("eye", "right", "up", "forward", "spacing"):
+        for a in range(3):
+            getattr(v, k)[a] = float(view[k][a])
+    for k in ("tan_half_fov", "step_voxels", "ref_step_voxels", "lod_bias", "ess_threshold", "alpha_cutoff"):
+        setattr(v, k, float(view[k]))
+    v.width, v.height = int(view["width"]), int(view["height"])
+    return v
 
 
 class Graph:
@@ -222,3 +266,10 @@ class Graph:
         _check(lib.mg_tf_update_host(self._h, _ptr(tf_host), _ptr(node_rgba_device), _ptr(node_idx_device),
                                      int(n_voxels), _ptr(out_device), _ptr(out_host), int(fmt), stream or None),
                "mg_tf_update_host")
+
+    def render(self, node_idx_device, mip, node_rgba_device, view, out_rgba_device, stats_device=None,
+               stream: int = 0) -> None:
+        m = mip if isinstance(mip, MgMipmapDesc) else mipmap_desc(*mip)
+        v = view if isinstance(view, MgView) else view_struct(view)
+        _check(lib.mg_render(self._h, _ptr(node_idx_device), C.byref(m), _ptr(node_rgba_device), C.byref(v),
+                             _ptr(out_rgba_device), _ptr(stats_device), stream or None), "mg_render")

@@ -51,6 +51,10 @@ class Workload:
         return synth.random_tf(self.n_leaves, c.get("seed", 0), update=update,
                                alpha_zero_frac=c.get("alpha_zero_frac", 0.0))
 
+    def mip_desc(self) -> "mg.MgMipmapDesc":
+        """The mg_mipmap_desc of the concatenated device mipmap (input of mg_render)."""
+        return mg.mipmap_desc(self.level_start, self.mip_dims)
+
     def pack(self) -> None:
         """NEXT-3: derive the bit-packed form of the device mipmap (Table 1 (8), (9), (A)): per level
         i_min(l), r(l) (Eq. 15-16) and one packed stream; fills d_packed / packed_levels."""
