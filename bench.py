@@ -48,6 +48,7 @@ def parse_args():
     p.add_argument("--no-cpu-baseline", action="store_true")
     p.add_argument("--no-e2e", action="store_true")
     p.add_argument("--no-attr", action="store_true", help="skip the extra NEXT-1 measurement (multi-attribute propagation)")
+    p.add_argument("--no-render", action="store_true", help="skip the extra NEXT-2 measurement (ray-marcher over the paletted mipmap)")
     p.add_argument("--no-packed", action="store_true", help="skip the extra NEXT-3 measurement (bit-packed node IDs)")
     p.add_argument("--cpu-sample-voxels", type=int, default=1 << 31, help="oracle sample size (>= the mipmap = whole workload)")
     p.add_argument("--reference-budget-s", type=float, default=90.0)
@@ -321,6 +322,40 @@ def run_b200(args) -> dict:
             attr[label] = a0.elapsed_time(a1) / attr["steps"]
             del leaf, xa
 
+    # ---- NEXT-2: ray-march the paletted mipmap (1600 x 1200, 0.5-voxel steps: L414), with and without ESS (L271)
+    render = None
+    if not args.no_render and rank == 0 and len(w.mip_dims) > 1:
+        from paper_2009_02702_b200 import synth
+        view = synth.render_view(w.cfg)
+        g.propagate(torch.from_numpy(synth.render_tf(w.tf(0))).cuda(), nodes, st)
+        img = torch.empty((view["height"], view["width"], 4), dtype=torch.float32, device="cuda")
+        desc = w.mip_desc()
+        render = {"what": "NEXT-2 mg_render: pinhole ray-marcher over the node-index mipmap + fp32 palette, per-sample LOD, "
+                          "manual trilinear + inter-level blend, opacity correction, hierarchical empty-space skipping "
+                          "(PAPER.md L267-L271, L414)", "width": view["width"], "height": view["height"],
+                  "step_voxels": view["step_voxels"], "tf": f"config TF, opacities x {synth.RENDER_ALPHA_SCALE}", "frames": 10}
+        for label, thr, fl in (("ess", view["ess_threshold"], view["flags"]), ("no_ess", -1.0, view["flags"]),
+                               ("ess_generic_mipmap", view["ess_threshold"], 0), ("no_ess_generic_mipmap", -1.0, 0)):
+            v = mg.view_struct(dict(view, ess_threshold=thr, flags=fl))
+            stats = torch.zeros(4, dtype=torch.int64, device="cuda")
+            for _ in range(2):
+                g.render(w.d_idx, desc, nodes, v, img, None, st)
+            torch.cuda.synchronize()
+            r0, r1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            r0.record(stream)
+            for _ in range(render["frames"]):
+                g.render(w.d_idx, desc, nodes, v, img, None, st)
+            r1.record(stream)
+            g.render(w.d_idx, desc, nodes, v, img, stats, st)
+            torch.cuda.synchronize()
+            ms = r0.elapsed_time(r1) / render["frames"]
+            ev_, sk_, un_, _ = (int(x) for x in stats.cpu().numpy())
+            render[label] = {"ms_per_frame": ms, "fps": 1e3 / ms, "samples_composited": ev_, "samples_skipped": sk_,
+                             "samples_one_leaf_shortcut": un_, "samples_per_s": (ev_ + sk_) / (ms * 1e-3)}
+        render["histogram_mipmap_flag_speedup"] = render["no_ess_generic_mipmap"]["ms_per_frame"] / render["no_ess"]["ms_per_frame"]
+        render["coverage"] = float((img[..., 3] > 0).float().mean().item())
+        del img
+
     # ---- e2e: host TF in, host mipmap out, through the public C-ABI call (rank-local, then max)
     e2e = None
     if not args.no_e2e:
@@ -379,6 +414,8 @@ def run_b200(args) -> dict:
         res["packed"] = packed
     if attr is not None:
         res["attr"] = attr
+    if render is not None:
+        res["render"] = render
     if e2e is not None:
         res["e2e"] = e2e
     if world == 1 and not args.no_cpu_baseline and w.host_idx is not None:

@@ -276,7 +276,20 @@ typedef struct mg_view {
     double ess_threshold;                          /* < 0: no empty-space skipping (paper: 1e-8)           */
     double alpha_cutoff;                           /* early ray termination (1.0 = never)                  */
     uint32_t width, height;                        /* image size in pixels (> 0)                           */
+    uint32_t flags;                                /* 0 or MG_VIEW_HISTOGRAM_MIPMAP                        */
+    uint32_t reserved;                             /* 0                                                    */
 } mg_view;
+
+/* mg_view.flags */
+enum {
+    MG_VIEW_HISTOGRAM_MIPMAP = 1u /* the caller asserts that node_idx_mipmap is the histogram mipmap of THIS graph
+                                     (Eq. 4; what the builder emits): a voxel whose node is a leaf (< n_leaves) holds
+                                     a pure mixture e_k, hence every voxel below it names the same leaf (L223).  The
+                                     marcher then fetches the coarse level of a sample first; if its 8 voxels name
+                                     one leaf, the 8 voxels of the fine level (their children) do too and the sample
+                                     takes that leaf's palette colour without the second fetch.  The image is
+                                     unchanged up to rounding (the 16 taps would all return that colour). */
+};
 
 /*
  * mg_render -- one image.  Enqueue-only, no allocation, one kernel launch.
@@ -286,8 +299,9 @@ typedef struct mg_view {
  *   node_rgba        DEVICE float[n_nodes][4], 16-byte aligned: the palette (any mg_propagate output).
  *   out_rgba         DEVICE float[height][width][4], 16-byte aligned: (C_r, C_g, C_b, A), associated
  *                    colour over a transparent background; rays missing the volume give zeros.
- *   stats_device     DEVICE uint64[2] or NULL: += samples evaluated, += samples skipped by R6
- *                    (the caller zeroes it).
+ *   stats_device     DEVICE uint64[4] or NULL (the caller zeroes it): [0] += samples composited,
+ *                    [1] += samples skipped by R6, [2] += those of [0] whose coarse level named one leaf
+ *                    (MG_VIEW_HISTOGRAM_MIPMAP: fine level not fetched), [3] unused.
  * Errors: MG_ERR_INVALID_ARG (NULL, misalignment, bad sizes, level dims that are not the ceil-halving
  * chain of L80, offsets overlapping), MG_ERR_CUDA.
  */

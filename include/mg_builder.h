@@ -100,6 +100,11 @@ int mgb_mip_dims(const mgb_result *r, uint64_t *dims_out);
 int mgb_get_graph(const mgb_result *r, uint32_t *child_a, uint32_t *child_b, float *weight,
                   double *weight_exact, uint64_t *level_offsets, uint32_t *leaf_segment_id);
 
+/* delta w of Eq. 18 per node: float[n_nodes], the empirical standard deviation of the quantiser bin the
+ * node's codeword was taken from (L176: "we store an empirical standard deviation sigma for each bin to
+ * facilitate estimating the error"); 0 for leaves and for unquantised builds. */
+int mgb_get_weight_sigma(const mgb_result *r, float *weight_sigma);
+
 /* Node index (in the numbering of mgb_get_graph) of every voxel of one mip level:
  * uint32[Z_l * Y_l * X_l].  mgb_node_idx_ptr returns the builder-owned array (valid until
  * mgb_free), mgb_get_node_idx copies it. */

@@ -79,6 +79,8 @@ _lib.mgo_pixel_ray.argtypes = [_f64p, C.c_double, _u32, _u32, _u32, _u32, _f64p]
 _lib.mgo_pixel_ray.restype = None
 _lib.mgo_render.argtypes = [_u32p, _u64p, _u32p, _u32, _f64p, _f64p, _f64p, _u32, _u32, _f64p, _u64p]
 _lib.mgo_render.restype = None
+_lib.mgo_render_pixels.argtypes = [_u32p, _u64p, _u32p, _u32, _f64p, _f64p, _f64p, _u32, _u32, _u32p, _u64, _f64p, _u64p]
+_lib.mgo_render_pixels.restype = None
 
 
 def _c(a, dt):
@@ -308,4 +310,23 @@ def render(levels, palette, view):
     stats = np.zeros(2, dtype=np.uint64)
     _lib.mgo_render(idx, offs, dims, len(levels), _c(palette, np.float64).reshape(-1), cam, par, W, H,
                     out.reshape(-1), stats)
+    return out, (int(stats[0]), int(stats[1]))
+
+
+def render_pixels(levels, palette, view, pixels_ij, flat=None):
+    """The same rays as ``render`` for selected pixels only: pixels_ij = [(column i, row j)] -> fp64 [n, 4] and
+    the (evaluated, skipped) counters.  ``flat`` = (node_idx, level_offset, level_dim_xyz) passes an already
+    concatenated pyramid (full-size volumes) instead of ``levels``."""
+    if flat is None:
+        idx, offs, dims = _pyramid(levels)
+    else:
+        idx = _c(flat[0], np.uint32).reshape(-1)
+        offs = np.ascontiguousarray(flat[1], dtype=np.uint64)
+        dims = np.ascontiguousarray(flat[2], dtype=np.uint32).reshape(-1)
+    cam, par = _cam_par(view)
+    ij = np.ascontiguousarray(pixels_ij, dtype=np.uint32).reshape(-1, 2)
+    out = np.zeros((ij.shape[0], 4), dtype=np.float64)
+    stats = np.zeros(2, dtype=np.uint64)
+    _lib.mgo_render_pixels(idx, offs, dims, offs.size, _c(palette, np.float64).reshape(-1), cam, par,
+                           int(view["width"]), int(view["height"]), ij.reshape(-1), ij.shape[0], out.reshape(-1), stats)
     return out, (int(stats[0]), int(stats[1]))

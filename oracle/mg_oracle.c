@@ -597,3 +597,23 @@ void mgo_render(const uint32_t *node_idx, const uint64_t *level_offset, const ui
         }
     if (stats) { stats[0] = st[0]; stats[1] = st[1]; }
 }
+
+/* Selected pixels of the same image (full-size parity on sampled outputs): pixel q = (ij[2q], ij[2q+1])
+ * = (column i, row j) of the W x H image; out = [n_pix][4].  Same per-ray code as mgo_render. */
+void mgo_render_pixels(const uint32_t *node_idx, const uint64_t *level_offset, const uint32_t *level_dim,
+                       uint32_t n_levels, const double *palette, const double *cam, const double *par,
+                       uint32_t W, uint32_t H, const uint32_t *ij, uint64_t n_pix, double *out, uint64_t *stats)
+{
+    mgo_view v = {node_idx, level_offset, level_dim, n_levels, palette};
+    uint64_t st[2] = {0, 0};
+#pragma omp parallel for schedule(dynamic, 1) reduction(+ : st[:2])
+    for (int64_t q = 0; q < (int64_t)n_pix; q++) {
+        double dir[3];
+        uint64_t loc[2] = {0, 0};
+        mgo_pixel_ray(cam, par[0], W, H, ij[2 * q], ij[2 * q + 1], dir);
+        mgo_march(&v, cam, par, H, dir, out + 4 * q, loc);
+        st[0] += loc[0];
+        st[1] += loc[1];
+    }
+    if (stats) { stats[0] = st[0]; stats[1] = st[1]; }
+}

@@ -21,7 +21,7 @@ PICK_SMALLEST_INDEX, PICK_SMALLEST_MASS = 0, 1
 
 SYMBOLS = ["mgb_default_params", "mgb_build", "mgb_build_from_mixtures", "mgb_free", "mgb_get_info",
            "mgb_mip_dims", "mgb_get_graph", "mgb_node_idx_ptr", "mgb_get_node_idx", "mgb_get_codebook",
-           "mgb_last_error"]
+           "mgb_get_weight_sigma", "mgb_last_error"]
 
 
 class Params(C.Structure):
@@ -59,6 +59,8 @@ lib.mgb_node_idx_ptr.argtypes = [_vp, C.c_uint32]
 lib.mgb_node_idx_ptr.restype = _vp
 lib.mgb_get_node_idx.argtypes = [_vp, C.c_uint32, _vp]
 lib.mgb_get_node_idx.restype = C.c_int
+lib.mgb_get_weight_sigma.argtypes = [_vp, _vp]
+lib.mgb_get_weight_sigma.restype = C.c_int
 lib.mgb_get_codebook.argtypes = [_vp, _vp, _vp, _vp]
 lib.mgb_get_codebook.restype = C.c_int
 lib.mgb_last_error.argtypes = []
@@ -118,6 +120,8 @@ class Result:
                                             ("child_a", "child_b", "weight", "weight_exact", "level_offsets",
                                              "leaf_segment_id"))), "mgb_get_graph")
         out["n_leaves"] = int(self.info.n_leaves)
+        out["weight_sigma"] = np.zeros(n, np.float32)
+        _check(lib.mgb_get_weight_sigma(self._h, out["weight_sigma"].ctypes.data), "mgb_get_weight_sigma")
         return out
 
     def n_voxels(self, level: int) -> int:

@@ -62,6 +62,7 @@ int finalise_graph(const Factorised& F, uint32_t n_leaves, const mgb_params& p, 
     std::vector<uint32_t> ca(n_nodes, 0), cb(n_nodes, 0);
     std::vector<float> w32(n_nodes, 0.0f);
     std::vector<double> wex(n_nodes, 0.0);
+    std::vector<float> wsg(n_nodes, 0.0f);           // sigma of the bin the node's codeword came from (L176, Eq. 18)
     const uint32_t b = p.quant_bits;
     R.codeword.clear(); R.sigma.clear(); R.bin_count.clear();
     R.info.max_bin_sigma = 0.0;
@@ -102,8 +103,8 @@ int finalise_graph(const Factorised& F, uint32_t n_leaves, const mgb_params& p, 
             if (k2 >= nb) k2 = nb - 1;
             const double e1 = std::fabs((double)R.codeword[k1] - wm);
             const double e2 = std::fabs((double)R.codeword[k2] - (1.0 - wm));
-            if (e2 < e1) { ca[n] = F.b[q]; cb[n] = F.a[q]; w32[n] = R.codeword[k2]; wex[n] = 1.0 - wm; }
-            else { ca[n] = F.a[q]; cb[n] = F.b[q]; w32[n] = R.codeword[k1]; wex[n] = wm; }
+            if (e2 < e1) { ca[n] = F.b[q]; cb[n] = F.a[q]; w32[n] = R.codeword[k2]; wex[n] = 1.0 - wm; wsg[n] = R.sigma[k2]; }
+            else { ca[n] = F.a[q]; cb[n] = F.b[q]; w32[n] = R.codeword[k1]; wex[n] = wm; wsg[n] = R.sigma[k1]; }
         }
     } else {
 #pragma omp parallel for schedule(static)
@@ -123,15 +124,15 @@ int finalise_graph(const Factorised& F, uint32_t n_leaves, const mgb_params& p, 
     R.info.depth = (uint32_t)level_off.size() - 2;
     if (p.relabel) {
         R.child_a.assign(n_nodes, 0); R.child_b.assign(n_nodes, 0);
-        R.weight.assign(n_nodes, 0.0f); R.weight_exact.assign(n_nodes, 0.0);
+        R.weight.assign(n_nodes, 0.0f); R.weight_exact.assign(n_nodes, 0.0); R.weight_sigma.assign(n_nodes, 0.0f);
 #pragma omp parallel for schedule(static)
         for (int64_t n = n_leaves; n < (int64_t)n_nodes; n++) {
             const uint32_t q = new_of_old[n];
             R.child_a[q] = new_of_old[ca[n]]; R.child_b[q] = new_of_old[cb[n]];
-            R.weight[q] = w32[n]; R.weight_exact[q] = wex[n];
+            R.weight[q] = w32[n]; R.weight_exact[q] = wex[n]; R.weight_sigma[q] = wsg[n];
         }
     } else {
-        R.child_a.swap(ca); R.child_b.swap(cb); R.weight.swap(w32); R.weight_exact.swap(wex);
+        R.child_a.swap(ca); R.child_b.swap(cb); R.weight.swap(w32); R.weight_exact.swap(wex); R.weight_sigma.swap(wsg);
         for (uint64_t n = 0; n < n_nodes; n++) new_of_old[n] = (uint32_t)n;
     }
     R.info.n_nodes = n_nodes;
@@ -359,6 +360,13 @@ extern "C" int mgb_get_node_idx(const mgb_result* r, uint32_t level, uint32_t* o
 {
     if (!r || !out || level >= r->node_idx.size()) { set_error("mgb_get_node_idx: bad argument"); return MGB_ERR_INVALID_ARG; }
     memcpy(out, r->node_idx[level].data(), r->node_idx[level].size() * sizeof(uint32_t));
+    return MGB_OK;
+}
+
+extern "C" int mgb_get_weight_sigma(const mgb_result* r, float* weight_sigma)
+{
+    if (!r || !weight_sigma) { set_error("mgb_get_weight_sigma: NULL argument"); return MGB_ERR_INVALID_ARG; }
+    memcpy(weight_sigma, r->weight_sigma.data(), r->weight_sigma.size() * sizeof(float));
     return MGB_OK;
 }
 

@@ -63,6 +63,7 @@ struct mgb_result {
     std::vector<uint32_t> child_a, child_b;
     std::vector<float> weight;
     std::vector<double> weight_exact;
+    std::vector<float> weight_sigma;     // per node: sigma of its weight's quantiser bin (0 when unquantised)
     std::vector<uint64_t> level_off;
     std::vector<uint32_t> leaf_segment_id;
     std::vector<std::vector<uint32_t>> node_idx;   // per mip level, final numbering

@@ -13,11 +13,18 @@
 // palette (16 B per node, tens of MB) stays L2-resident.  Three data-dependent shortcuts that do
 // not change the value beyond rounding: the second level is not fetched when frac(lambda) == 0; a
 // footprint whose 8 voxels name the same node costs one palette gather; skipped samples (R6) cost
-// no memory access at all.
+// no memory access at all.  Two more: the parent voxel at which the last climb of R6 stopped is
+// remembered (consecutive samples share it, so most samples climb without a gather), and with
+// MG_VIEW_HISTOGRAM_MIPMAP the COARSE level is fetched first -- its 8 voxels cover the children
+// holding the fine level's 8 voxels, and a leaf node in a histogram mipmap is a pure voxel, so if
+// the 8 coarse voxels name one leaf all 16 taps are that leaf: segment interiors cost 8 index
+// gathers + 1 palette gather instead of 16 + 2.  The block tests of R6 run on floor(2 p) in
+// integers (exactly the oracle's comparisons, see Block).
 // Arithmetic: t, the step, the sample position, the trilinear fractions and the block tests in fp64
 // (the B200's fp64 pipe is half the fp32 rate and the loop is gather-latency-bound, so this is free
 // and keeps sample positions within 1e-12 voxels of the oracle's); the fractional LOD, the weights,
-// colours, opacity correction and compositing in fp32.
+// colours and opacity correction in fp32; the compositing sums C and A in fp64 (thousands of
+// samples per ray would otherwise add their fp32 rounding errors).
 #include <math.h>
 
 #include <cstring>
@@ -43,26 +50,26 @@ struct RenderParams {
     double pow_lmax;                // 2^l_max
     double thr;                     // ess threshold (< 0: off)
     double step_ref;                // step_voxels * s_ref
+    double cutoff;
     float inv_ref;                  // 1 / (ref_step_voxels * s_ref)
-    float cutoff;
+    uint32_t n_leaves;              // > 0: MG_VIEW_HISTOGRAM_MIPMAP (nodes below it are pure voxels)
 };
 
 __device__ __forceinline__ int clampi(int v, int hi) { return v < 0 ? 0 : (v > hi ? hi : v); }
 
-__device__ __forceinline__ void tap(float4& acc, const float4* __restrict__ pal, uint32_t n, float wgt)
-{
-    const float4 c = __ldg(pal + n);
-    acc.x = fmaf(wgt, c.x, acc.x); acc.y = fmaf(wgt, c.y, acc.y);
-    acc.z = fmaf(wgt, c.z, acc.z); acc.w = fmaf(wgt, c.w, acc.w);
-}
+// The 2 x 2 x 2 voxels around p on level l (R3: voxel i of level l is centred at (i + 1/2) 2^l, indices
+// clamped to the level) and the interpolation fractions.
+struct Cell {
+    uint32_t n[8];          // node of voxel (dz, dy, dx) at n[4 dz + 2 dy + dx]
+    float fx, fy, fz;
+};
 
-// R3, one level: trilinear interpolation of the palette at p (level-0 voxel coordinates).
-__device__ __forceinline__ float4 trilinear(const RenderParams& P, int l, double px, double py, double pz)
+__device__ __forceinline__ void fetch_cell(const RenderParams& P, int l, double px, double py, double pz, Cell& c)
 {
     const double sc = __hiloint2double((1023 - l) << 20, 0);            // 2^-l
     const double ux = fma(px, sc, -0.5), uy = fma(py, sc, -0.5), uz = fma(pz, sc, -0.5);
     const double flx = floor(ux), fly = floor(uy), flz = floor(uz);
-    const float fx = (float)(ux - flx), fy = (float)(uy - fly), fz = (float)(uz - flz);
+    c.fx = (float)(ux - flx); c.fy = (float)(uy - fly); c.fz = (float)(uz - flz);
     const int X = P.dim[l][0], Y = P.dim[l][1], Z = P.dim[l][2];
     const int ix = (int)flx, iy = (int)fly, iz = (int)flz;
     const int x0 = clampi(ix, X - 1), x1 = clampi(ix + 1, X - 1);
@@ -73,36 +80,63 @@ __device__ __forceinline__ float4 trilinear(const RenderParams& P, int l, double
     const uint32_t* r01 = base + ((size_t)z0 * Y + y1) * X;
     const uint32_t* r10 = base + ((size_t)z1 * Y + y0) * X;
     const uint32_t* r11 = base + ((size_t)z1 * Y + y1) * X;
-    const uint32_t n000 = __ldg(r00 + x0), n001 = __ldg(r00 + x1), n010 = __ldg(r01 + x0), n011 = __ldg(r01 + x1);
-    const uint32_t n100 = __ldg(r10 + x0), n101 = __ldg(r10 + x1), n110 = __ldg(r11 + x0), n111 = __ldg(r11 + x1);
-    const uint32_t same = (n000 ^ n001) | (n000 ^ n010) | (n000 ^ n011) | (n000 ^ n100) | (n000 ^ n101) |
-                          (n000 ^ n110) | (n000 ^ n111);
-    if (same == 0) return __ldg(P.pal + n000);                           // segment interior
-    const float gx = 1.f - fx, gy = 1.f - fy, gz = 1.f - fz;
+    c.n[0] = __ldg(r00 + x0); c.n[1] = __ldg(r00 + x1); c.n[2] = __ldg(r01 + x0); c.n[3] = __ldg(r01 + x1);
+    c.n[4] = __ldg(r10 + x0); c.n[5] = __ldg(r10 + x1); c.n[6] = __ldg(r11 + x0); c.n[7] = __ldg(r11 + x1);
+}
+
+__device__ __forceinline__ bool one_node(const Cell& c)
+{
+    return ((c.n[0] ^ c.n[1]) | (c.n[0] ^ c.n[2]) | (c.n[0] ^ c.n[3]) | (c.n[0] ^ c.n[4]) | (c.n[0] ^ c.n[5]) |
+            (c.n[0] ^ c.n[6]) | (c.n[0] ^ c.n[7])) == 0;
+}
+
+__device__ __forceinline__ void tap(float4& acc, const float4* __restrict__ pal, uint32_t n, float wgt)
+{
+    const float4 c = __ldg(pal + n);
+    acc.x = fmaf(wgt, c.x, acc.x); acc.y = fmaf(wgt, c.y, acc.y);
+    acc.z = fmaf(wgt, c.z, acc.z); acc.w = fmaf(wgt, c.w, acc.w);
+}
+
+// Trilinear interpolation of the palette over a fetched cell; a cell naming one node costs one gather.
+__device__ __forceinline__ float4 shade_cell(const RenderParams& P, const Cell& c)
+{
+    if (one_node(c)) return __ldg(P.pal + c.n[0]);
+    const float fx = c.fx, fy = c.fy, fz = c.fz, gx = 1.f - fx, gy = 1.f - fy, gz = 1.f - fz;
     float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
-    tap(acc, P.pal, n000, gx * gy * gz); tap(acc, P.pal, n001, fx * gy * gz);
-    tap(acc, P.pal, n010, gx * fy * gz); tap(acc, P.pal, n011, fx * fy * gz);
-    tap(acc, P.pal, n100, gx * gy * fz); tap(acc, P.pal, n101, fx * gy * fz);
-    tap(acc, P.pal, n110, gx * fy * fz); tap(acc, P.pal, n111, fx * fy * fz);
+    tap(acc, P.pal, c.n[0], gx * gy * gz); tap(acc, P.pal, c.n[1], fx * gy * gz);
+    tap(acc, P.pal, c.n[2], gx * fy * gz); tap(acc, P.pal, c.n[3], fx * fy * gz);
+    tap(acc, P.pal, c.n[4], gx * gy * fz); tap(acc, P.pal, c.n[5], fx * gy * fz);
+    tap(acc, P.pal, c.n[6], gx * fy * fz); tap(acc, P.pal, c.n[7], fx * fy * fz);
     return acc;
 }
 
-// R6 block: voxel-aligned box [lo, hi) in level-0 coordinates; bit a of open_lo / open_hi = the face
-// lies on the volume's boundary (the trilinear fetch clamps there, so no margin is needed).
-struct EssBlock {
-    int lo[3], hi[3];
-    unsigned open_lo, open_hi;
+// R6 block: voxel-aligned box in level-0 coordinates, kept in HALF-voxel integers so that the oracle's
+// tests on p become integer tests on h = floor(2 p):  p < lo + m  <=>  h < 2 lo + 2 m  and
+// p >= hi - m  <=>  h >= 2 hi - 2 m  (2 lo, 2 hi, 2 m = 2^l1 are integers).  A face on the volume's
+// boundary needs no margin (the fetch clamps there): its bound is pushed out of reach instead.
+struct Block {
+    int lo2[3], hi2[3];     // 2 lo, 2 hi
+    unsigned open;          // bit a: lo face of axis a is open; bit 3 + a: hi face
     bool valid;
 };
 
-__device__ __forceinline__ bool inside_block(const EssBlock& B, double m, double px, double py, double pz)
+__device__ __forceinline__ void set_block(Block& B, int qx, int qy, int qz, int L, const int* dim)
 {
-    const double p[3] = {px, py, pz};
-    bool in = true;
+    B.valid = true;
+    B.lo2[0] = qx << (L + 1); B.lo2[1] = qy << (L + 1); B.lo2[2] = qz << (L + 1);
+    B.hi2[0] = (qx + 1) << (L + 1); B.hi2[1] = (qy + 1) << (L + 1); B.hi2[2] = (qz + 1) << (L + 1);
+    B.open = (qx == 0) | ((qy == 0) << 1) | ((qz == 0) << 2) | ((qx == dim[0] - 1) << 3) | ((qy == dim[1] - 1) << 4) |
+             ((qz == dim[2] - 1) << 5);
+}
+
+__device__ __forceinline__ bool inside_block(const Block& B, int m2, int hx, int hy, int hz)
+{
+    const int h[3] = {hx, hy, hz};
+    bool in = B.valid;
 #pragma unroll
     for (int a = 0; a < 3; a++) {
-        if (!((B.open_lo >> a) & 1u) && p[a] < (double)B.lo[a] + m) in = false;
-        if (!((B.open_hi >> a) & 1u) && p[a] >= (double)B.hi[a] - m) in = false;
+        if (!((B.open >> a) & 1u) && h[a] < B.lo2[a] + m2) in = false;
+        if (!((B.open >> (3 + a)) & 1u) && h[a] >= B.hi2[a] - m2) in = false;
     }
     return in;
 }
@@ -113,8 +147,8 @@ k_render(const __grid_constant__ RenderParams P)
     const unsigned i = blockIdx.x * kTileX + (threadIdx.x & (kTileX - 1));
     const unsigned j = blockIdx.y * kTileY + threadIdx.x / kTileX;
     const bool live = i < P.W && j < P.H;
-    unsigned n_eval = 0, n_skip = 0;
-    float Cr = 0.f, Cg = 0.f, Cb = 0.f, A = 0.f;
+    unsigned n_eval = 0, n_skip = 0, n_uni = 0;
+    double Cr = 0.0, Cg = 0.0, Cb = 0.0, A = 0.0;
     if (live) {
         // R1: pixel ray
         const double u = (2.0 * ((double)i + 0.5) / (double)P.W - 1.0) * P.tan_half_fov * (double)P.W / (double)P.H;
@@ -147,11 +181,13 @@ k_render(const __grid_constant__ RenderParams P)
             const double rho_t = cos_view * P.pix;                              // rho 2^bias = t * rho_t (R2)
             const int l_max = P.n_levels - 1;
             const bool ess = P.thr >= 0.0;
-            EssBlock B;
-            B.valid = false;
-            B.open_lo = B.open_hi = 0;
+            const bool uni = P.n_leaves != 0;                                    // MG_VIEW_HISTOGRAM_MIPMAP
+            Block E;                                                             // the empty block of R6
+            E.valid = false;
+            E.open = 0;
 #pragma unroll
-            for (int a = 0; a < 3; a++) B.lo[a] = B.hi[a] = 0;
+            for (int a = 0; a < 3; a++) E.lo2[a] = E.hi2[a] = 0;
+            int miss_L = -1, miss_x = 0, miss_y = 0, miss_z = 0;                 // last parent voxel found not empty
             double t = tn;
             while (t < tf && A < P.cutoff) {
                 // R2 + R4 without transcendentals on the ray parameter: 2^lambda = clamp(rho 2^bias, 1, 2^l_max),
@@ -169,56 +205,90 @@ k_render(const __grid_constant__ RenderParams P)
                 const int l1 = min(l0 + 1, l_max);
                 const float f = lambda - fl;
                 t += delta;
-                if (ess) {                                                       // R6
-                    const double m = __hiloint2double((1022 + l1) << 20, 0);     // 2^l1 / 2
-                    bool inside = B.valid && inside_block(B, m, px, py, pz);
-                    if (!inside) {
-                        B.valid = false;
-                        for (int L = l1 + 1; L <= l_max; L++) {
-                            const double sc = __hiloint2double((1023 - L) << 20, 0);
-                            const int qx = clampi((int)floor(px * sc), P.dim[L][0] - 1);
-                            const int qy = clampi((int)floor(py * sc), P.dim[L][1] - 1);
-                            const int qz = clampi((int)floor(pz * sc), P.dim[L][2] - 1);
-                            const uint32_t n = __ldg(P.idx + P.off[L] + ((size_t)qz * P.dim[L][1] + qy) * P.dim[L][0] + qx);
-                            const float alpha_parent = __ldg(reinterpret_cast<const float*>(P.pal + n) + 3);
-                            if (!((double)alpha_parent < P.thr)) break;
-                            B.valid = true;
-                            B.lo[0] = qx << L; B.lo[1] = qy << L; B.lo[2] = qz << L;
-                            B.hi[0] = (qx + 1) << L; B.hi[1] = (qy + 1) << L; B.hi[2] = (qz + 1) << L;
-                            B.open_lo = (qx == 0) | ((qy == 0) << 1) | ((qz == 0) << 2);
-                            B.open_hi = (qx == P.dim[L][0] - 1) | ((qy == P.dim[L][1] - 1) << 1) | ((qz == P.dim[L][2] - 1) << 2);
-                        }
-                        inside = B.valid && inside_block(B, m, px, py, pz);
-                    }
-                    if (inside) {
+                int hx = 0, hy = 0, hz = 0;
+                const int m2 = 1 << l1;                                          // 2 m, m = 2^l1 / 2
+                if (ess) {                                                       // R6, in half-voxel integers
+                    hx = (int)floor(px + px); hy = (int)floor(py + py); hz = (int)floor(pz + pz);
+                    if (inside_block(E, m2, hx, hy, hz)) {
                         n_skip++;
                         continue;
                     }
                 }
-                float4 c = trilinear(P, l0, px, py, pz);                          // R3
-                if (f != 0.f) {
-                    const float4 c1 = trilinear(P, l1, px, py, pz);
-                    const float g = 1.f - f;
-                    c.x = fmaf(f, c1.x, g * c.x); c.y = fmaf(f, c1.y, g * c.y);
-                    c.z = fmaf(f, c1.z, g * c.z); c.w = fmaf(f, c1.w, g * c.w);
+                // The level needed first: with MG_VIEW_HISTOGRAM_MIPMAP the COARSE one -- its 8 voxels cover the
+                // children that hold the fine level's 8 voxels, so if they all name ONE LEAF (a pure voxel of a
+                // histogram mipmap) every tap of both levels is that leaf.  Its index gathers are issued before the
+                // climb of R6 so that the two dependent chains overlap.
+                Cell cell;
+                fetch_cell(P, uni ? l1 : l0, px, py, pz, cell);
+                if (ess) {
+                    // The oracle forgets its block here and climbs again from level l1 + 1.  The climb is a pure
+                    // function of the parent voxels, so a parent already found not empty is not fetched again
+                    // (consecutive samples share it).
+                    E.valid = false;
+                    for (int L = l1 + 1; L <= l_max; L++) {
+                        const int qx = clampi(hx >> (L + 1), P.dim[L][0] - 1);
+                        const int qy = clampi(hy >> (L + 1), P.dim[L][1] - 1);
+                        const int qz = clampi(hz >> (L + 1), P.dim[L][2] - 1);
+                        if (L == miss_L && qx == miss_x && qy == miss_y && qz == miss_z) break;
+                        const uint32_t n = __ldg(P.idx + P.off[L] + ((size_t)qz * P.dim[L][1] + qy) * P.dim[L][0] + qx);
+                        const float alpha_parent = __ldg(reinterpret_cast<const float*>(P.pal + n) + 3);
+                        if (!((double)alpha_parent < P.thr)) {
+                            miss_L = L; miss_x = qx; miss_y = qy; miss_z = qz;
+                            break;
+                        }
+                        set_block(E, qx, qy, qz, L, P.dim[L]);
+                    }
+                    if (inside_block(E, m2, hx, hy, hz)) {
+                        n_skip++;
+                        continue;
+                    }
+                }
+                float4 c;                                                        // R3
+                if (uni && one_node(cell) && cell.n[0] < P.n_leaves) {
+                    c = __ldg(P.pal + cell.n[0]);
+                    n_uni++;
+                } else {
+                    float4 c1 = make_float4(0.f, 0.f, 0.f, 0.f);
+                    if (uni) {                                                   // cell = coarse level
+                        if (f != 0.f || l0 == l1) c1 = shade_cell(P, cell);
+                        if (l0 != l1) {
+                            fetch_cell(P, l0, px, py, pz, cell);
+                            c = shade_cell(P, cell);
+                        } else {
+                            c = c1;
+                        }
+                    } else {                                                     // cell = fine level
+                        c = shade_cell(P, cell);
+                        if (f != 0.f) {
+                            fetch_cell(P, l1, px, py, pz, cell);
+                            c1 = shade_cell(P, cell);
+                        }
+                    }
+                    if (f != 0.f) {
+                        const float g = 1.f - f;
+                        c.x = fmaf(f, c1.x, g * c.x); c.y = fmaf(f, c1.y, g * c.y);
+                        c.z = fmaf(f, c1.z, g * c.z); c.w = fmaf(f, c1.w, g * c.w);
+                    }
                 }
                 const float alpha = fminf(fmaxf(c.w, 0.f), 1.f);
                 const float e = (float)de * P.inv_ref;
                 const float ac = -expm1f(e * log1pf(-alpha));                     // 1 - (1 - alpha)^e
-                const float wgt = (1.f - A) * ac;
-                Cr = fmaf(wgt, c.x, Cr); Cg = fmaf(wgt, c.y, Cg); Cb = fmaf(wgt, c.z, Cb);
+                const double wgt = (1.0 - A) * (double)ac;                        // R5, accumulated in fp64
+                Cr = fma(wgt, (double)c.x, Cr); Cg = fma(wgt, (double)c.y, Cg); Cb = fma(wgt, (double)c.z, Cb);
                 A += wgt;
                 n_eval++;
             }
         }
-        P.out[(size_t)j * P.W + i] = make_float4(Cr, Cg, Cb, A);
+        P.out[(size_t)j * P.W + i] = make_float4((float)Cr, (float)Cg, (float)Cb, (float)A);
     }
     if (P.stats) {
         const unsigned e = __reduce_add_sync(0xffffffffu, n_eval);
         const unsigned s = __reduce_add_sync(0xffffffffu, n_skip);
+        const unsigned u = __reduce_add_sync(0xffffffffu, n_uni);
         if ((threadIdx.x & 31) == 0) {
             if (e) atomicAdd(P.stats, (unsigned long long)e);
             if (s) atomicAdd(P.stats + 1, (unsigned long long)s);
+            if (u) atomicAdd(P.stats + 2, (unsigned long long)u);
         }
     }
 }
@@ -240,6 +310,10 @@ extern "C" int mg_render(mg_graph* g, const uint32_t* node_idx_mipmap, const mg_
     }
     if (mip->n_levels == 0 || mip->n_levels > MG_MAX_MIP_LEVELS) {
         mg::set_error("mg_render: n_levels = %u not in 1..%d", mip->n_levels, MG_MAX_MIP_LEVELS);
+        return MG_ERR_INVALID_ARG;
+    }
+    if (view->flags & ~(uint32_t)MG_VIEW_HISTOGRAM_MIPMAP) {
+        mg::set_error("mg_render: unknown view flags 0x%x", view->flags);
         return MG_ERR_INVALID_ARG;
     }
     if (view->width == 0 || view->height == 0 || view->width > 65536u || view->height > 65536u) {
@@ -292,7 +366,8 @@ extern "C" int mg_render(mg_graph* g, const uint32_t* node_idx_mipmap, const mg_
     P.thr = view->ess_threshold;
     P.step_ref = view->step_voxels * s_ref;
     P.inv_ref = (float)(1.0 / (view->ref_step_voxels * s_ref));
-    P.cutoff = (float)view->alpha_cutoff;
+    P.cutoff = view->alpha_cutoff;
+    P.n_leaves = (view->flags & MG_VIEW_HISTOGRAM_MIPMAP) ? g->n_leaves : 0u;
     const dim3 grid((P.W + kTileX - 1) / kTileX, (P.H + kTileY - 1) / kTileY);
     k_render<<<grid, kTileX * kTileY, 0, (cudaStream_t)stream>>>(P);
     MG_CUDA(cudaGetLastError());

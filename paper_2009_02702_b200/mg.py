@@ -89,6 +89,7 @@ lib.mg_propagate_attr.restype = C.c_int
 
 
 MG_MAX_MIP_LEVELS = 24
+MG_VIEW_HISTOGRAM_MIPMAP = 1
 
 
 class MgMipmapDesc(C.Structure):
@@ -100,7 +101,8 @@ class MgView(C.Structure):
     _fields_ = [("eye", C.c_double * 3), ("right", C.c_double * 3), ("up", C.c_double * 3), ("forward", C.c_double * 3),
                 ("tan_half_fov", C.c_double), ("spacing", C.c_double * 3), ("step_voxels", C.c_double),
                 ("ref_step_voxels", C.c_double), ("lod_bias", C.c_double), ("ess_threshold", C.c_double),
-                ("alpha_cutoff", C.c_double), ("width", C.c_uint32), ("height", C.c_uint32)]
+                ("alpha_cutoff", C.c_double), ("width", C.c_uint32), ("height", C.c_uint32), ("flags", C.c_uint32),
+                ("reserved", C.c_uint32)]
 
 
 lib.mg_render.argtypes = [_vp, _vp, C.POINTER(MgMipmapDesc), _vp, C.POINTER(MgView), _vp, _vp, _vp]
@@ -188,6 +190,7 @@ def view_struct(view: dict) -> MgView:
     for k in ("tan_half_fov", "step_voxels", "ref_step_voxels", "lod_bias", "ess_threshold", "alpha_cutoff"):
         setattr(v, k, float(view[k]))
     v.width, v.height = int(view["width"]), int(view["height"])
+    v.flags = int(view.get("flags", 0))
     return v
 
 

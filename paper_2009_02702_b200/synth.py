@@ -100,6 +100,27 @@ def orbit_view(dims_xyz, spacing=(1.0, 1.0, 1.0), azimuth_deg: float = 30.0, ele
                 ess_threshold=float(ess_threshold), alpha_cutoff=float(alpha_cutoff))
 
 
+RENDER_ALPHA_SCALE = 0.04      # render inputs: TF opacities scaled so that rays travel ~25+ voxels before saturating
+
+
+def render_view(c: dict, width: int = 1600, height: int = 1200, **overrides) -> dict:
+    """The view bench.py and the full-size parity test render a config with: the paper's 1600 x 1200
+    viewport at 0.5-voxel steps (L414), ESS threshold 1e-8 (L271), voxel spacing 1 : 1 : zscale (L277),
+    the volume filling most of the frame."""
+    kw = dict(azimuth_deg=35.0, elevation_deg=30.0, distance=0.75, fov_deg=45.0)
+    kw.update(overrides)
+    v = orbit_view(c["dims"], spacing=(1.0, 1.0, float(c.get("zscale", 1))), width=width, height=height, **kw)
+    v["flags"] = 1          # MG_VIEW_HISTOGRAM_MIPMAP: the configs' mipmaps come from the builder
+    return v
+
+
+def render_tf(tf: np.ndarray) -> np.ndarray:
+    """The config's TF with its opacities scaled by RENDER_ALPHA_SCALE (exact zeros stay zero)."""
+    out = tf.copy()
+    out[:, 3] *= np.float32(RENDER_ALPHA_SCALE)
+    return out
+
+
 def single_segment_update(tf: np.ndarray, seed: int, update: int) -> np.ndarray:
     """Config 4: each update re-draws ONE random segment's RGBA; returns a new array."""
     out = tf.copy()

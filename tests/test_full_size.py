@@ -155,8 +155,55 @@ def test_volume_config_full_size(libs, cfg_id):
                 worst = max(worst, float(np.abs(nodes_host[idx_l[v]] - direct).max()))
         assert worst <= TOL_DIRECT, worst
         print(f"cfg {cfg_id}: {w.stats['n_nodes']} nodes depth {w.stats['depth']}, max |graph - direct| on samples = {worst:.2e}")
+        if cfg_id == 3:
+            _check_render_full_size(mg, w, tf)
     finally:
         w.close()
+
+
+def _check_render_full_size(mg, w, tf):
+    """NEXT-2 in bench.py's launch configuration (synth.render_view: 1600 x 1200, 0.5-voxel steps, ESS 1e-8,
+    spacing 1:1:7): sampled pixels + the image corners against the oracle's per-ray march on the same
+    pyramid (tolerance: tests/test_gpu_render.py), and the ESS-off image must equal the ESS-on image."""
+    g = w.graph
+    rtf = synth.render_tf(tf)
+    nodes = torch.empty((g.info.n_nodes, 4), dtype=torch.float32, device="cuda")
+    g.propagate(torch.from_numpy(rtf).cuda(), nodes)
+    view = synth.render_view(w.cfg)
+    W, H = view["width"], view["height"]
+    img = torch.full((H, W, 4), float("nan"), dtype=torch.float32, device="cuda")
+    img_off = torch.full((H, W, 4), float("nan"), dtype=torch.float32, device="cuda")
+    img_plain = torch.full((H, W, 4), float("nan"), dtype=torch.float32, device="cuda")
+    stats = torch.zeros(12, dtype=torch.int64, device="cuda")
+    desc = w.mip_desc()
+    assert view["flags"] == mg.MG_VIEW_HISTOGRAM_MIPMAP            # what bench.py times
+    g.render(w.d_idx, desc, nodes, view, img, stats[0:4])
+    g.render(w.d_idx, desc, nodes, dict(view, ess_threshold=-1.0), img_off, stats[4:8])
+    g.render(w.d_idx, desc, nodes, dict(view, flags=0), img_plain, stats[8:12])
+    torch.cuda.synchronize()
+    got, got_off = img.cpu().numpy().astype(np.float64), img_off.cpu().numpy().astype(np.float64)
+    st = stats.cpu().numpy().reshape(3, 4)
+    assert np.isfinite(got).all() and got[..., 3].max() > 0.5
+    assert st[0, 1] > 0 and st[1, 1] == 0 and st[0, 0] < st[1, 0] and st[0, 2] > 0 and st[2, 2] == 0
+    assert st[0, :2].sum() == st[1, :2].sum() == st[2, :2].sum()
+    assert np.abs(got - got_off).max() <= 1e-5                     # skipped samples were (numerically) transparent
+    assert np.abs(got - img_plain.cpu().numpy()).max() <= 1e-6     # one-leaf blocks do not change the image
+    k = 300
+    pi = (synth.u64(3, 400, np.arange(k, dtype=np.uint64)) % np.uint64(W)).astype(np.int64)
+    pj = (synth.u64(3, 401, np.arange(k, dtype=np.uint64)) % np.uint64(H)).astype(np.int64)
+    ij = np.concatenate([np.stack([pi, pj], 1), [[0, 0], [W - 1, 0], [0, H - 1], [W - 1, H - 1], [W // 2, H // 2]]])
+    hg = w.host_graph
+    pal = oracle.graph_eval(hg["child_a"], hg["child_b"], hg["weight"], hg["n_leaves"], rtf.astype(np.float64))
+    flat = np.zeros(w.n_voxels_padded, dtype=np.uint32)
+    for s0, lv in zip(w.level_start, w.host_idx):
+        flat[s0:s0 + lv.size] = lv.reshape(-1)
+    ref, _ = oracle.render_pixels(None, pal, view, ij, flat=(flat, w.level_start, np.array(w.mip_dims)))
+    err = np.abs(got[ij[:, 1], ij[:, 0]] - ref).max()
+    hit = (ref[:, 3] > 0).mean()
+    print(f"render 1600x1200 cfg3: max|err| on {ij.shape[0]} sampled pixels = {err:.2e} ({hit:.0%} hit the volume); "
+          f"samples composited/skipped/from one-leaf blocks: {st[0, :3].tolist()}, without ESS {st[1, :3].tolist()}, "
+          f"without the histogram-mipmap flag {st[2, :3].tolist()}")
+    assert hit > 0.3 and err <= 5e-6, err
 
 
 def test_config3_fp16_output_full_size(libs):

@@ -206,3 +206,21 @@ def test_empty_space_skipping_never_changes_the_image():
     assert s0 == 0 and s1 > 0 and e1 + s1 == e0 and s1 > 0.2 * e0, (e0, e1, s1)
     np.testing.assert_allclose(img1, img0, rtol=0, atol=1e-13)
     assert img0[..., 3].max() > 0.5 and (img0[..., 3] == 0).any()
+
+
+def test_render_pixels_is_render_restricted_to_those_pixels():
+    dims = (13, 7, 5)
+    levels, n = [], 0
+    for (x, y, z) in oracle.mip_dims(dims):
+        levels.append((np.arange(x * y * z, dtype=np.uint32) + n).reshape(z, y, x))
+        n += x * y * z
+    pal = synth.random_attr(n, 4, seed=5).astype(np.float64)
+    view = synth.orbit_view(dims, width=9, height=7, distance=0.8)
+    img, st = oracle.render(levels, pal, view)
+    ij = [(0, 0), (8, 6), (4, 3), (2, 5)]
+    px, _ = oracle.render_pixels(levels, pal, view, ij)
+    np.testing.assert_array_equal(px, np.stack([img[j, i] for i, j in ij]))
+    every = [(i, j) for j in range(7) for i in range(9)]
+    px_all, st_all = oracle.render_pixels(levels, pal, view, every)
+    np.testing.assert_array_equal(px_all.reshape(7, 9, 4), img)
+    assert st_all == st
