@@ -81,6 +81,14 @@ _lib.mgo_render.argtypes = [_u32p, _u64p, _u32p, _u32, _f64p, _f64p, _f64p, _u32
 _lib.mgo_render.restype = None
 _lib.mgo_render_pixels.argtypes = [_u32p, _u64p, _u32p, _u32, _f64p, _f64p, _f64p, _u32, _u32, _u32p, _u64, _f64p, _u64p]
 _lib.mgo_render_pixels.restype = None
+_lib.mgo_mixture_lut.argtypes = [_u32p, _u32p, _f64p, _f64p, _u64, _u64, _f64p, _f64p]
+_lib.mgo_mixture_lut.restype = None
+_lib.mgo_fa_axis.argtypes = [_u64, _u64, _u32, _u64p, _u32p]
+_lib.mgo_fa_axis.restype = _u32
+_lib.mgo_range_query_fa.argtypes = [_u32p, _u64p, _u32p, _u32, _f64p, _f64p, _u64, _u64p, _f64p, _f64p]
+_lib.mgo_range_query_fa.restype = _u64
+_lib.mgo_range_query_naive.argtypes = [_u32p, _u32p, _f64p, _u64, _u64p, _f64p]
+_lib.mgo_range_query_naive.restype = _u64
 
 
 def _c(a, dt):
@@ -330,3 +338,45 @@ def render_pixels(levels, palette, view, pixels_ij, flat=None):
     _lib.mgo_render_pixels(idx, offs, dims, offs.size, _c(palette, np.float64).reshape(-1), cam, par,
                            int(view["width"]), int(view["height"]), ij.reshape(-1), ij.shape[0], out.reshape(-1), stats)
     return out, (int(stats[0]), int(stats[1]))
+
+
+# ---- NEXT-4: mixture lookup table with Eq. 18 errors; footprint-assembly range queries (sections 3.5-3.6) ----
+
+def mixture_lut(child_a, child_b, weight, weight_sigma, n_leaves):
+    """(mu, dmu) fp64 [n_nodes, n_leaves]: e_i with error 0 on leaf i, propagated with Eq. 18 (L375)."""
+    a, b = _c(child_a, np.uint32), _c(child_b, np.uint32)
+    w, sg = _c(weight, np.float64), _c(weight_sigma, np.float64)
+    mu = np.zeros((a.size, n_leaves), dtype=np.float64)
+    dmu = np.zeros((a.size, n_leaves), dtype=np.float64)
+    _lib.mgo_mixture_lut(a, b, w, sg, a.size, n_leaves, mu.reshape(-1), dmu.reshape(-1))
+    return mu, dmu
+
+
+def fa_axis(lo, hi, max_level):
+    """1D decomposition of [lo, hi) into aligned power-of-two pieces (section 3.6): [(start, level)]."""
+    start = np.zeros(130, dtype=np.uint64)
+    level = np.zeros(130, dtype=np.uint32)
+    n = _lib.mgo_fa_axis(int(lo), int(hi), int(max_level), start, level)
+    return [(int(start[i]), int(level[i])) for i in range(n)]
+
+
+def range_query_fa(levels, mu, dmu, box):
+    """Footprint assembly over box = (x0, y0, z0, x1, y1, z1): (expected voxels per leaf, error per leaf, fetches)."""
+    idx, offs, dims = _pyramid(levels)
+    mu, dmu = _c(mu, np.float64), _c(dmu, np.float64)
+    nl = mu.shape[1]
+    e, d = np.zeros(nl), np.zeros(nl)
+    n = _lib.mgo_range_query_fa(idx, offs, dims, len(levels), mu.reshape(-1), dmu.reshape(-1), nl,
+                                np.ascontiguousarray(box, dtype=np.uint64), e, d)
+    return e, d, int(n)
+
+
+def range_query_naive(level0, mu, box):
+    """Sum of mu over every finest-level voxel of the box (L377): (expected voxels per leaf, fetches)."""
+    l0 = _c(level0, np.uint32)
+    dims = np.array([l0.shape[2], l0.shape[1], l0.shape[0]], dtype=np.uint32)
+    mu = _c(mu, np.float64)
+    e = np.zeros(mu.shape[1])
+    n = _lib.mgo_range_query_naive(l0.reshape(-1), dims, mu.reshape(-1), mu.shape[1],
+                                   np.ascontiguousarray(box, dtype=np.uint64), e)
+    return e, int(n)

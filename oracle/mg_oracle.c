@@ -617,3 +617,114 @@ void mgo_render_pixels(const uint32_t *node_idx, const uint64_t *level_offset, c
     }
     if (stats) { stats[0] = st[0]; stats[1] = st[1]; }
 }
+
+/* ==== NEXT-4: mixture lookup table with error propagation, and sub-volume (range) queries ====
+ * PAPER.md section 3.5 (Eq. 17-18), section 3.6 (L243-L253), L375-L377, Table 4.
+ *
+ * Mixture lookup table (L375): "assigning a mixture e_i with variance 0 to each leaf node i ... we
+ * propagate this information through the DAG, including the error described in Eq. (18).  Each node
+ * thus stores ... the expected value mu and its variance delta mu."  Dense here: mu, dmu = [n_nodes][n_leaves].
+ *   mu_i  = (1 - w) a_i + w b_i
+ *   dmu_i = sqrt( mu_i^2 ( (da_i / a_i)^2 + (db_i / b_i)^2 + 2 (dw / w)^2 ) )            (Eq. 18, as printed)
+ * dw = the standard deviation stored with the weight's quantiser bin (L176).  Reading Q19: a ratio
+ * whose denominator is 0 (the component is absent from that child, so its uncertainty is 0 too) is
+ * dropped from the sum. */
+void mgo_mixture_lut(const uint32_t *child_a, const uint32_t *child_b, const double *weight, const double *weight_sigma,
+                     uint64_t n_nodes, uint64_t n_leaves, double *mu, double *dmu)
+{
+    memset(mu, 0, (size_t)n_nodes * n_leaves * sizeof(double));
+    memset(dmu, 0, (size_t)n_nodes * n_leaves * sizeof(double));
+    for (uint64_t n = 0; n < n_leaves; n++)
+        mu[n * n_leaves + n] = 1.0;
+    for (uint64_t n = n_leaves; n < n_nodes; n++) {
+        double w = weight[n], rw = weight_sigma[n] / w;
+        const double *ma = mu + (uint64_t)child_a[n] * n_leaves, *da = dmu + (uint64_t)child_a[n] * n_leaves;
+        const double *mb = mu + (uint64_t)child_b[n] * n_leaves, *db = dmu + (uint64_t)child_b[n] * n_leaves;
+        for (uint64_t i = 0; i < n_leaves; i++) {
+            double m = (1.0 - w) * ma[i] + w * mb[i];
+            double rel2 = 2.0 * rw * rw;
+            if (ma[i] != 0.0) rel2 += (da[i] / ma[i]) * (da[i] / ma[i]);
+            if (mb[i] != 0.0) rel2 += (db[i] / mb[i]) * (db[i] / mb[i]);
+            mu[n * n_leaves + i] = m;
+            dmu[n * n_leaves + i] = sqrt(m * m * rel2);
+        }
+    }
+}
+
+/* Section 3.6: "we decompose the 1D ranges along x, y and z according to their alignment with the mip
+ * levels".  [lo, hi) is cut, left to right, into the largest aligned power-of-two pieces: a piece
+ * starts at x, has length 2^l, x is a multiple of 2^l, and l <= max_level.  Returns the number of pieces. */
+uint32_t mgo_fa_axis(uint64_t lo, uint64_t hi, uint32_t max_level, uint64_t *start, uint32_t *level)
+{
+    uint32_t n = 0;
+    uint64_t x = lo;
+    while (x < hi) {
+        uint32_t l = 0;
+        while (l + 1 <= max_level && x % ((uint64_t)1 << (l + 1)) == 0 && x + ((uint64_t)1 << (l + 1)) <= hi)
+            l++;
+        start[n] = x;
+        level[n] = l;
+        n++;
+        x += (uint64_t)1 << l;
+    }
+    return n;
+}
+
+/* Footprint assembly (L245-L247): "the tensor product of these ranges is comprised of rectangular boxes
+ * ... Each of these boxes is tesselated by cubes of a side length l equal to the shortest of the three
+ * box extents.  Each cube represents a single sample from H at level log2(l).  The contribution of each
+ * sample ... is denormalized (multiplication by l^3) before being accumulated."  Errors add in quadrature
+ * (Eq. 17).  box = x0, y0, z0, x1, y1, z1 (half-open, inside the volume).  expect / err = [n_leaves].
+ * Returns the number of samples fetched. */
+uint64_t mgo_range_query_fa(const uint32_t *node_idx, const uint64_t *level_offset, const uint32_t *level_dim,
+                            uint32_t n_levels, const double *mu, const double *dmu, uint64_t n_leaves,
+                            const uint64_t *box, double *expect, double *err)
+{
+    uint64_t sx[130], sy[130], sz[130], fetches = 0;
+    uint32_t lx[130], ly[130], lz[130];
+    uint32_t nx = mgo_fa_axis(box[0], box[3], n_levels - 1, sx, lx);
+    uint32_t ny = mgo_fa_axis(box[1], box[4], n_levels - 1, sy, ly);
+    uint32_t nz = mgo_fa_axis(box[2], box[5], n_levels - 1, sz, lz);
+    for (uint64_t i = 0; i < n_leaves; i++)
+        expect[i] = err[i] = 0.0;
+    for (uint32_t c = 0; c < nz; c++)
+        for (uint32_t b = 0; b < ny; b++)
+            for (uint32_t a = 0; a < nx; a++) {
+                uint32_t l = lx[a] < ly[b] ? lx[a] : ly[b];
+                if (lz[c] < l) l = lz[c];
+                double scale = ldexp(1.0, 3 * (int)l);                       /* l^3 voxels per cube */
+                const uint32_t *d = level_dim + 3 * l;
+                for (uint64_t z = sz[c] >> l; z < (sz[c] + ((uint64_t)1 << lz[c])) >> l; z++)
+                    for (uint64_t y = sy[b] >> l; y < (sy[b] + ((uint64_t)1 << ly[b])) >> l; y++)
+                        for (uint64_t x = sx[a] >> l; x < (sx[a] + ((uint64_t)1 << lx[a])) >> l; x++) {
+                            uint64_t node = node_idx[level_offset[l] + (z * d[1] + y) * d[0] + x];
+                            const double *m = mu + node * n_leaves, *dm = dmu + node * n_leaves;
+                            for (uint64_t i = 0; i < n_leaves; i++) {
+                                expect[i] += scale * m[i];
+                                err[i] += (scale * dm[i]) * (scale * dm[i]);
+                            }
+                            fetches++;
+                        }
+            }
+    for (uint64_t i = 0; i < n_leaves; i++)
+        err[i] = sqrt(err[i]);
+    return fetches;
+}
+
+/* The naive approach of L377: "adds the contributions of each voxel at the finest level". */
+uint64_t mgo_range_query_naive(const uint32_t *node_idx0, const uint32_t *dim0, const double *mu, uint64_t n_leaves,
+                               const uint64_t *box, double *expect)
+{
+    uint64_t fetches = 0;
+    for (uint64_t i = 0; i < n_leaves; i++)
+        expect[i] = 0.0;
+    for (uint64_t z = box[2]; z < box[5]; z++)
+        for (uint64_t y = box[1]; y < box[4]; y++)
+            for (uint64_t x = box[0]; x < box[3]; x++) {
+                const double *m = mu + (uint64_t)node_idx0[(z * dim0[1] + y) * dim0[0] + x] * n_leaves;
+                for (uint64_t i = 0; i < n_leaves; i++)
+                    expect[i] += m[i];
+                fetches++;
+            }
+    return fetches;
+}
