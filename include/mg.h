@@ -309,6 +309,65 @@ int mg_render(mg_graph *g, const uint32_t *node_idx_mipmap, const mg_mipmap_desc
               const float *node_rgba, const mg_view *view, float *out_rgba, uint64_t *stats_device,
               void *stream);
 
+/* ------------------------------------------------------------------------------------------------
+ * NEXT-4: mixture lookup table with error propagation and sub-volume (range) queries
+ * (section 3.5 Eq. 17-18, section 3.6, Table 4).
+ *
+ * The table stores, per node, the sparse mixture mu (expected share of every leaf / segment) and its
+ * uncertainty dmu: leaf i holds e_i with error 0; an internal node (a, b, w +- dw) holds
+ *   mu_i = (1 - w) a_i + w b_i,   dmu_i = sqrt(mu_i^2 ((da_i / a_i)^2 + (db_i / b_i)^2 + 2 (dw / w)^2))   (Eq. 18)
+ * where a ratio with a zero denominator (component absent from that child) is dropped (reading Q19) and
+ * dw is the standard deviation of the weight's quantiser bin (L176).  fp64 throughout, w = (double) of
+ * the graph's fp32 weight.  Device layout: CSR rows sorted by leaf index.
+ *
+ * A range query returns, for a box of the level-0 grid, the expected number of voxels of every leaf and
+ * its error.  MG_QUERY_FA is the paper's footprint assembly: each axis range is cut into the largest
+ * aligned power-of-two pieces, every box of the tensor product is tesselated by cubes whose side is its
+ * shortest extent, each cube is ONE sample of the histogram mipmap at level log2(side), denormalised by
+ * side^3; errors add in quadrature (Eq. 17).  MG_QUERY_NAIVE adds every level-0 voxel of the box (L377).
+ * ------------------------------------------------------------------------------------------------ */
+typedef struct mg_mixture_lut mg_mixture_lut;
+
+typedef struct mg_lut_info {
+    uint64_t n_nodes;      /* rows                                                        */
+    uint64_t nnz;          /* stored (leaf, mu, dmu) entries                              */
+    uint64_t capacity;     /* entries allocated (an upper bound computed before the build) */
+    uint64_t device_bytes; /* device memory owned by the table                            */
+    uint32_t n_leaves;
+    uint32_t max_row_nnz;  /* longest row                                                 */
+} mg_lut_info;
+
+enum { MG_QUERY_FA = 0u, MG_QUERY_NAIVE = 1u };
+
+/* Build the table for a loaded graph.  weight_sigma: HOST float[n_nodes] in the library's numbering
+ * (entries of the leaves ignored), or NULL for dw = 0 everywhere.  Allocates device memory and
+ * synchronises `stream` (a one-off at load time, L375).  Errors: MG_ERR_INVALID_ARG, MG_ERR_OOM
+ * (the entry bound sum_n min(n_leaves, nnz(a) + nnz(b)) does not fit), MG_ERR_CUDA. */
+int mg_mixture_lut_build(mg_graph *g, const float *weight_sigma, mg_mixture_lut **out, void *stream);
+void mg_mixture_lut_free(mg_mixture_lut *lut);
+int mg_mixture_lut_info(const mg_mixture_lut *lut, mg_lut_info *info);
+
+/* Copy the table to the HOST (tests, export): row_ptr uint64[n_nodes + 1], then leaf uint32[nnz],
+ * mu double[nnz], dmu double[nnz] in row order.  Any pointer may be NULL.  Synchronises. */
+int mg_mixture_lut_export(const mg_mixture_lut *lut, uint64_t *row_ptr, uint32_t *leaf, double *mu, double *dmu);
+
+/*
+ * mg_range_query -- n_queries boxes in one launch sequence (zero, accumulate, finish).
+ *   node_idx_mipmap  DEVICE uint32, all levels as `mip` describes (MG_QUERY_NAIVE reads level 0 only).
+ *   boxes            HOST uint64[n_queries][6] = x0, y0, z0, x1, y1, z1, half-open, non-empty, inside
+ *                    level 0 (validated); copied into a table-owned staging buffer at enqueue (the
+ *                    buffer grows, i.e. allocates, when n_queries exceeds every earlier call's).
+ *   expect, err      DEVICE double[n_queries][n_leaves]: expected voxels per leaf and its error
+ *                    (err may be NULL).  sum_i expect[q][i] = volume of box q (L251).
+ *   fetches          DEVICE uint64[n_queries] or NULL: samples fetched per query (Table 4).
+ *   mode             MG_QUERY_FA or MG_QUERY_NAIVE.
+ * Enqueue-only apart from the staging copy.  Accumulation uses fp64 atomics: the result is the oracle's
+ * up to summation order.
+ */
+int mg_range_query(mg_mixture_lut *lut, const uint32_t *node_idx_mipmap, const mg_mipmap_desc *mip,
+                   const uint64_t *boxes, uint32_t n_queries, double *expect, double *err,
+                   uint64_t *fetches, uint32_t mode, void *stream);
+
 /* Thread-local description of the last error returned on this thread ("" if none). */
 const char *mg_last_error(void);
 

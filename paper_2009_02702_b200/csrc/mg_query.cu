@@ -1,0 +1,444 @@
+// mg_query.cu -- NEXT-4: mixture lookup table (Eq. 17-18) and sub-volume (range) queries.
+//
+// PAPER.md section 3.5 (L225-L241), section 3.6 (L243-L253), L375-L377, Table 4.  The paper builds
+// the table on the CPU and calls range queries "not well suited for the GPU, since the number of
+// non-zero entries in the sparse mixtures is hard to predict" (L253).  Here both run on the device:
+//   * the table is a CSR (leaf, mu, dmu) per node whose row CAPACITIES are known before any value is:
+//     cap(n) = min(n_leaves, cap(a) + cap(b)) -- exact for graphs made by the factorisation (the two
+//     children of a node carry disjoint parts of a mixture), an upper bound for any other DAG -- so one
+//     allocation and one merge kernel per topological level suffice (no count/scan/fill passes);
+//   * a query is spread over several CTAs; each warp takes boxes of the footprint's tensor product,
+//     its lanes take the cubes of the box, every cube is one mipmap sample whose sparse row is added
+//     into the dense per-query result with fp64 atomics in L2.  Samples that are pure voxels (row =
+//     one leaf, the bulk of every query) are pre-aggregated per warp with __match_any_sync so that a
+//     homogeneous region costs one atomic per warp instead of 32 on the same address.
+// fp64 throughout (the B200's fp64 pipe is half the fp32 rate; the work is gather/atomic-bound).
+#include <math.h>
+
+#include <algorithm>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "mg_internal.h"
+
+struct mg_mixture_lut {
+    int device = 0;
+    uint64_t n_nodes = 0;
+    uint32_t n_leaves = 0;
+    uint64_t capacity = 0, nnz = 0;
+    uint32_t max_row = 0;
+    uint64_t* d_row_ptr = nullptr;    // [n_nodes + 1] row starts (capacity layout)
+    uint32_t* d_row_len = nullptr;    // [n_nodes] entries in use
+    uint32_t* d_col = nullptr;        // [capacity] leaf index, ascending inside a row
+    double* d_mu = nullptr;           // [capacity]
+    double* d_dmu = nullptr;          // [capacity]
+    uint64_t* d_boxes = nullptr;      // staging for mg_range_query
+    uint32_t boxes_cap = 0;
+    uint64_t device_bytes = 0;
+};
+
+namespace {
+
+constexpr int kBuildThreads = 128;
+constexpr int kQueryThreads = 256;
+constexpr int kMaxPieces = 2 * MG_MAX_MIP_LEVELS + 2;     // pieces of one axis: at most 2 per level
+
+__global__ void k_lut_leaves(uint32_t n_leaves, const uint64_t* __restrict__ row_ptr, uint32_t* row_len, uint32_t* col,
+                             double* mu, double* dmu)
+{
+    const uint32_t n = blockIdx.x * blockDim.x + threadIdx.x;
+    if (n >= n_leaves) return;
+    const uint64_t r = row_ptr[n];
+    row_len[n] = 1;
+    col[r] = n;
+    mu[r] = 1.0;          // e_i ...
+    dmu[r] = 0.0;         // ... "with variance 0" (L375)
+}
+
+// One topological level [lo, hi): thread per node, a two-way merge of the children's sorted rows.
+__global__ void __launch_bounds__(kBuildThreads)
+k_lut_level(const uint32_t* __restrict__ ga, const uint32_t* __restrict__ gb, const float* __restrict__ gw,
+            const float* __restrict__ gsig, uint32_t lo, uint32_t hi, const uint64_t* __restrict__ row_ptr,
+            uint32_t* row_len, uint32_t* col, double* mu, double* dmu)
+{
+    const uint32_t n = lo + blockIdx.x * kBuildThreads + threadIdx.x;
+    if (n >= hi) return;
+    const uint32_t a = ga[n], b = gb[n];
+    const double w = (double)gw[n];
+    const double rw = gsig ? (double)gsig[n] / w : 0.0;
+    const double rw2 = 2.0 * rw * rw;                                    // 2 (dw / w)^2
+    uint64_t pa = row_ptr[a], pb = row_ptr[b];
+    const uint64_t ea = pa + row_len[a], eb = pb + row_len[b];
+    uint64_t o = row_ptr[n];
+    const uint64_t o0 = o;
+    while (pa < ea || pb < eb) {
+        const uint32_t ca = pa < ea ? col[pa] : 0xFFFFFFFFu, cb = pb < eb ? col[pb] : 0xFFFFFFFFu;
+        const uint32_t c = ca < cb ? ca : cb;
+        double va = 0.0, da = 0.0, vb = 0.0, db = 0.0;
+        if (ca == c) { va = mu[pa]; da = dmu[pa]; pa++; }
+        if (cb == c) { vb = mu[pb]; db = dmu[pb]; pb++; }
+        const double m = (1.0 - w) * va + w * vb;
+        double rel2 = rw2;                                               // Eq. 18; absent component: no ratio (Q19)
+        if (va != 0.0) rel2 += (da / va) * (da / va);
+        if (vb != 0.0) rel2 += (db / vb) * (db / vb);
+        col[o] = c;
+        mu[o] = m;
+        dmu[o] = sqrt(m * m * rel2);
+        o++;
+    }
+    row_len[n] = (uint32_t)(o - o0);
+}
+
+}  // namespace
+
+extern "C" void mg_mixture_lut_free(mg_mixture_lut* lut)
+{
+    if (!lut) return;
+    cudaFree(lut->d_row_ptr); cudaFree(lut->d_row_len); cudaFree(lut->d_col);
+    cudaFree(lut->d_mu); cudaFree(lut->d_dmu); cudaFree(lut->d_boxes);
+    delete lut;
+}
+
+extern "C" int mg_mixture_lut_build(mg_graph* g, const float* weight_sigma, mg_mixture_lut** out, void* stream)
+{
+    if (!g || !out) { mg::set_error("mg_mixture_lut_build: NULL argument"); return MG_ERR_INVALID_ARG; }
+    *out = nullptr;
+    cudaStream_t st = (cudaStream_t)stream;
+    const uint64_t n = g->n_nodes;
+    const uint32_t nl = g->n_leaves;
+    // row capacities on the host: cap(n) = min(n_leaves, cap(a) + cap(b))
+    std::vector<uint32_t> ha(n), hb(n);
+    if (n > nl) {
+        MG_CUDA(cudaMemcpyAsync(ha.data(), g->d_a, n * sizeof(uint32_t), cudaMemcpyDeviceToHost, st));
+        MG_CUDA(cudaMemcpyAsync(hb.data(), g->d_b, n * sizeof(uint32_t), cudaMemcpyDeviceToHost, st));
+    }
+    MG_CUDA(cudaStreamSynchronize(st));
+    std::vector<uint32_t> cap(n);
+    std::vector<uint64_t> row_ptr(n + 1);
+    uint64_t total = 0;
+    for (uint64_t i = 0; i < n; i++) {
+        const uint64_t c = i < nl ? 1 : std::min<uint64_t>(nl, (uint64_t)cap[ha[i]] + cap[hb[i]]);
+        cap[i] = (uint32_t)c;
+        row_ptr[i] = total;
+        total += c;
+    }
+    row_ptr[n] = total;
+    size_t free_b = 0, total_b = 0;
+    MG_CUDA(cudaMemGetInfo(&free_b, &total_b));
+    const uint64_t need = total * 20 + (n + 1) * 8 + n * 4 + (weight_sigma ? n * 4 : 0);
+    if (need > free_b) {
+        mg::set_error("mg_mixture_lut_build: the table needs %llu entries (%.1f GB), %.1f GB are free",
+                      (unsigned long long)total, need / 1e9, free_b / 1e9);
+        return MG_ERR_OOM;
+    }
+    mg_mixture_lut* lut = new (std::nothrow) mg_mixture_lut;
+    if (!lut) { mg::set_error("mg_mixture_lut_build: out of host memory"); return MG_ERR_OOM; }
+    lut->device = g->device;
+    lut->n_nodes = n;
+    lut->n_leaves = nl;
+    lut->capacity = total;
+    float* d_sig = nullptr;
+    auto fail = [&](int rc) { cudaFree(d_sig); mg_mixture_lut_free(lut); return rc; };
+#define LUT_CUDA(call)                                                              \
+    do {                                                                            \
+        cudaError_t e__ = (call);                                                   \
+        if (e__ != cudaSuccess) return fail(mg::cuda_fail(e__, #call));             \
+    } while (0)
+    LUT_CUDA(cudaMalloc(&lut->d_row_ptr, (n + 1) * sizeof(uint64_t)));
+    LUT_CUDA(cudaMalloc(&lut->d_row_len, n * sizeof(uint32_t)));
+    LUT_CUDA(cudaMalloc(&lut->d_col, std::max<uint64_t>(total, 1) * sizeof(uint32_t)));
+    LUT_CUDA(cudaMalloc(&lut->d_mu, std::max<uint64_t>(total, 1) * sizeof(double)));
+    LUT_CUDA(cudaMalloc(&lut->d_dmu, std::max<uint64_t>(total, 1) * sizeof(double)));
+    lut->device_bytes = (n + 1) * 8 + n * 4 + total * 20;
+    LUT_CUDA(cudaMemcpyAsync(lut->d_row_ptr, row_ptr.data(), (n + 1) * sizeof(uint64_t), cudaMemcpyHostToDevice, st));
+    if (weight_sigma) {
+        LUT_CUDA(cudaMalloc(&d_sig, n * sizeof(float)));
+        LUT_CUDA(cudaMemcpyAsync(d_sig, weight_sigma, n * sizeof(float), cudaMemcpyHostToDevice, st));
+    }
+    k_lut_leaves<<<(nl + 255) / 256, 256, 0, st>>>(nl, lut->d_row_ptr, lut->d_row_len, lut->d_col, lut->d_mu, lut->d_dmu);
+    LUT_CUDA(cudaGetLastError());
+    mg::count_launch();
+    for (uint32_t L = 1; L < g->n_levels; L++) {
+        const uint32_t lo = (uint32_t)g->level_off[L], hi = (uint32_t)g->level_off[L + 1];
+        if (hi == lo) continue;
+        k_lut_level<<<(hi - lo + kBuildThreads - 1) / kBuildThreads, kBuildThreads, 0, st>>>(
+            g->d_a, g->d_b, g->d_w, d_sig, lo, hi, lut->d_row_ptr, lut->d_row_len, lut->d_col, lut->d_mu, lut->d_dmu);
+        LUT_CUDA(cudaGetLastError());
+        mg::count_launch();
+    }
+    std::vector<uint32_t> len(n);
+    LUT_CUDA(cudaMemcpyAsync(len.data(), lut->d_row_len, n * sizeof(uint32_t), cudaMemcpyDeviceToHost, st));
+    LUT_CUDA(cudaStreamSynchronize(st));
+#undef LUT_CUDA
+    cudaFree(d_sig);
+    for (uint64_t i = 0; i < n; i++) {
+        lut->nnz += len[i];
+        lut->max_row = std::max(lut->max_row, len[i]);
+    }
+    *out = lut;
+    return MG_OK;
+}
+
+extern "C" int mg_mixture_lut_info(const mg_mixture_lut* lut, mg_lut_info* info)
+{
+    if (!lut || !info) { mg::set_error("mg_mixture_lut_info: NULL argument"); return MG_ERR_INVALID_ARG; }
+    info->n_nodes = lut->n_nodes;
+    info->nnz = lut->nnz;
+    info->capacity = lut->capacity;
+    info->device_bytes = lut->device_bytes;
+    info->n_leaves = lut->n_leaves;
+    info->max_row_nnz = lut->max_row;
+    return MG_OK;
+}
+
+extern "C" int mg_mixture_lut_export(const mg_mixture_lut* lut, uint64_t* row_ptr, uint32_t* leaf, double* mu, double* dmu)
+{
+    if (!lut) { mg::set_error("mg_mixture_lut_export: NULL table"); return MG_ERR_INVALID_ARG; }
+    const uint64_t n = lut->n_nodes;
+    std::vector<uint64_t> cap_ptr(n + 1);
+    std::vector<uint32_t> len(n);
+    MG_CUDA(cudaMemcpy(cap_ptr.data(), lut->d_row_ptr, (n + 1) * sizeof(uint64_t), cudaMemcpyDeviceToHost));
+    MG_CUDA(cudaMemcpy(len.data(), lut->d_row_len, n * sizeof(uint32_t), cudaMemcpyDeviceToHost));
+    std::vector<uint32_t> c;
+    std::vector<double> m, d;
+    if (leaf) { c.resize(lut->capacity); MG_CUDA(cudaMemcpy(c.data(), lut->d_col, lut->capacity * sizeof(uint32_t), cudaMemcpyDeviceToHost)); }
+    if (mu) { m.resize(lut->capacity); MG_CUDA(cudaMemcpy(m.data(), lut->d_mu, lut->capacity * sizeof(double), cudaMemcpyDeviceToHost)); }
+    if (dmu) { d.resize(lut->capacity); MG_CUDA(cudaMemcpy(d.data(), lut->d_dmu, lut->capacity * sizeof(double), cudaMemcpyDeviceToHost)); }
+    uint64_t o = 0;
+    for (uint64_t i = 0; i < n; i++) {                                   // compact: capacity layout -> exact CSR
+        if (row_ptr) row_ptr[i] = o;
+        const uint64_t s = cap_ptr[i];
+        if (leaf) memcpy(leaf + o, c.data() + s, len[i] * sizeof(uint32_t));
+        if (mu) memcpy(mu + o, m.data() + s, len[i] * sizeof(double));
+        if (dmu) memcpy(dmu + o, d.data() + s, len[i] * sizeof(double));
+        o += len[i];
+    }
+    if (row_ptr) row_ptr[n] = o;
+    return MG_OK;
+}
+
+namespace {
+
+struct QueryParams {
+    const uint32_t* idx;
+    unsigned long long off[MG_MAX_MIP_LEVELS];
+    int dim[MG_MAX_MIP_LEVELS][3];
+    int n_levels;
+    uint32_t n_leaves;
+    const uint64_t* row_ptr;
+    const uint32_t* row_len;
+    const uint32_t* col;
+    const double* mu;
+    const double* dmu;
+    const uint64_t* boxes;
+    double* expect;
+    double* var;                     // may be NULL
+    unsigned long long* fetches;     // may be NULL
+};
+
+// Add one mipmap sample (node, denormalised by `scale` voxels) to query q's dense result.  Called by all
+// 32 lanes of a warp (`active` says which hold a sample).  Leaves (pure voxels: mu = e_node, dmu = 0) are
+// grouped by node across the warp first, so a homogeneous region costs one atomic per warp.
+__device__ __forceinline__ void add_sample(const QueryParams& P, double* expect, double* var, bool active, uint32_t node,
+                                           double scale)
+{
+    const unsigned lane = threadIdx.x & 31;
+    const bool pure = active && node < P.n_leaves;
+    const unsigned pm = __ballot_sync(0xffffffffu, pure);
+    if (pure) {
+        const unsigned grp = __match_any_sync(pm, node);
+        if (lane == (unsigned)(__ffs(grp) - 1)) atomicAdd(expect + node, scale * (double)__popc(grp));
+    } else if (active) {
+        const uint64_t r = P.row_ptr[node];
+        const uint32_t len = P.row_len[node];
+        for (uint32_t k = 0; k < len; k++) {
+            const uint32_t c = P.col[r + k];
+            atomicAdd(expect + c, scale * P.mu[r + k]);
+            if (var) {
+                const double d = scale * P.dmu[r + k];
+                if (d != 0.0) atomicAdd(var + c, d * d);
+            }
+        }
+    }
+}
+
+// Section 3.6, one axis: [lo, hi) cut left to right into the largest aligned power-of-two pieces.
+__device__ int fa_axis(uint32_t lo, uint32_t hi, int max_level, uint32_t* start, int* level)
+{
+    int n = 0;
+    uint32_t x = lo;
+    while (x < hi) {
+        int l = 0;
+        while (l + 1 <= max_level && (x & ((2u << l) - 1u)) == 0 && x + (2u << l) <= hi) l++;
+        start[n] = x;
+        level[n] = l;
+        n++;
+        x += 1u << l;
+    }
+    return n;
+}
+
+// grid = (n_queries, splits); the warps of all CTAs of a query share its boxes: chunk c (32 cubes) of box t
+// goes to warp (t + c) mod n_warps, which spreads both many one-cube boxes and few huge ones.
+__global__ void __launch_bounds__(kQueryThreads)
+k_range_query_fa(const __grid_constant__ QueryParams P)
+{
+    __shared__ uint32_t s_start[3][kMaxPieces];
+    __shared__ int s_level[3][kMaxPieces];
+    __shared__ int s_n[3];
+    const uint32_t q = blockIdx.x;
+    const uint64_t* box = P.boxes + 6ull * q;
+    if (threadIdx.x < 3)
+        s_n[threadIdx.x] = fa_axis((uint32_t)box[threadIdx.x], (uint32_t)box[3 + threadIdx.x], P.n_levels - 1,
+                                   s_start[threadIdx.x], s_level[threadIdx.x]);
+    __syncthreads();
+    const int nx = s_n[0], ny = s_n[1], nz = s_n[2];
+    const unsigned lane = threadIdx.x & 31;
+    const unsigned n_warps = gridDim.y * (kQueryThreads / 32), warp = blockIdx.y * (kQueryThreads / 32) + threadIdx.x / 32;
+    double* expect = P.expect + (uint64_t)q * P.n_leaves;
+    double* var = P.var ? P.var + (uint64_t)q * P.n_leaves : nullptr;
+    unsigned long long n_fetch = 0;
+    const unsigned n_boxes = (unsigned)(nx * ny * nz);
+    for (unsigned t = 0; t < n_boxes; t++) {
+        const int a = t % nx, b = (t / nx) % ny, c = t / (nx * ny);
+        const int lx = s_level[0][a], ly = s_level[1][b], lz = s_level[2][c];
+        const int l = min(lx, min(ly, lz));                              // cube side = the shortest extent
+        const int ex = lx - l, ey = ly - l, ez = lz - l;                 // cubes per axis = 2^e
+        const unsigned long long n_cubes = 1ull << (ex + ey + ez);
+        const unsigned long long n_chunks = (n_cubes + 31) >> 5;
+        const double scale = __hiloint2double((1023 + 3 * l) << 20, 0);  // side^3 = 8^l
+        const int X = P.dim[l][0], Y = P.dim[l][1];
+        const uint32_t* lvl = P.idx + P.off[l];
+        const uint32_t bx = s_start[0][a] >> l, by = s_start[1][b] >> l, bz = s_start[2][c] >> l;
+        for (unsigned long long ch = (warp + n_warps - t % n_warps) % n_warps; ch < n_chunks; ch += n_warps) {
+            const unsigned long long k = (ch << 5) + lane;
+            const bool active = k < n_cubes;
+            uint32_t node = 0;
+            if (active) {
+                const uint32_t ix = (uint32_t)(k & ((1ull << ex) - 1)), iy = (uint32_t)((k >> ex) & ((1ull << ey) - 1)),
+                               iz = (uint32_t)(k >> (ex + ey));
+                node = __ldg(lvl + ((size_t)(bz + iz) * Y + (by + iy)) * X + (bx + ix));
+            }
+            add_sample(P, expect, var, active, node, scale);
+            if (lane == 0) n_fetch += min(32ull, n_cubes - (ch << 5));
+        }
+    }
+    if (P.fetches && lane == 0 && n_fetch) atomicAdd(P.fetches + q, n_fetch);
+}
+
+// The naive approach (L377): every level-0 voxel of the box is one sample.
+__global__ void __launch_bounds__(kQueryThreads)
+k_range_query_naive(const __grid_constant__ QueryParams P)
+{
+    const uint32_t q = blockIdx.x;
+    const uint64_t* box = P.boxes + 6ull * q;
+    const uint32_t x0 = (uint32_t)box[0], y0 = (uint32_t)box[1], z0 = (uint32_t)box[2];
+    const uint32_t dx = (uint32_t)box[3] - x0, dy = (uint32_t)box[4] - y0, dz = (uint32_t)box[5] - z0;
+    const unsigned long long n_vox = (unsigned long long)dx * dy * dz;
+    const int X = P.dim[0][0], Y = P.dim[0][1];
+    double* expect = P.expect + (uint64_t)q * P.n_leaves;
+    double* var = P.var ? P.var + (uint64_t)q * P.n_leaves : nullptr;
+    const unsigned long long stride = (unsigned long long)gridDim.y * kQueryThreads;
+    const unsigned long long first = (unsigned long long)blockIdx.y * kQueryThreads + threadIdx.x;
+    for (unsigned long long base = first - (threadIdx.x & 31); base < n_vox; base += stride) {   // warp-uniform trip count
+        const unsigned long long v = base + (threadIdx.x & 31);
+        const bool active = v < n_vox;
+        uint32_t node = 0;
+        if (active) {
+            const uint32_t ix = (uint32_t)(v % dx), iy = (uint32_t)((v / dx) % dy), iz = (uint32_t)(v / ((unsigned long long)dx * dy));
+            node = __ldg(P.idx + P.off[0] + ((size_t)(z0 + iz) * Y + (y0 + iy)) * X + (x0 + ix));
+        }
+        add_sample(P, expect, var, active, node, 1.0);
+    }
+    if (P.fetches && blockIdx.y == 0 && threadIdx.x == 0) atomicAdd(P.fetches + q, n_vox);
+}
+
+__global__ void k_query_finish(double* var, uint64_t n)
+{
+    const uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) var[i] = sqrt(var[i]);                                    // Eq. 17: errors add in quadrature
+}
+
+}  // namespace
+
+extern "C" int mg_range_query(mg_mixture_lut* lut, const uint32_t* node_idx_mipmap, const mg_mipmap_desc* mip,
+                              const uint64_t* boxes, uint32_t n_queries, double* expect, double* err, uint64_t* fetches,
+                              uint32_t mode, void* stream)
+{
+    if (!lut || !node_idx_mipmap || !mip || !expect || (n_queries && !boxes)) {
+        mg::set_error("mg_range_query: NULL argument");
+        return MG_ERR_INVALID_ARG;
+    }
+    if (mode != MG_QUERY_FA && mode != MG_QUERY_NAIVE) { mg::set_error("mg_range_query: unknown mode %u", mode); return MG_ERR_INVALID_ARG; }
+    if (((uintptr_t)expect & 7) || ((uintptr_t)err & 7) || ((uintptr_t)fetches & 7) || ((uintptr_t)node_idx_mipmap & 3)) {
+        mg::set_error("mg_range_query: misaligned buffer");
+        return MG_ERR_INVALID_ARG;
+    }
+    if (mip->n_levels == 0 || mip->n_levels > MG_MAX_MIP_LEVELS) {
+        mg::set_error("mg_range_query: n_levels = %u not in 1..%d", mip->n_levels, MG_MAX_MIP_LEVELS);
+        return MG_ERR_INVALID_ARG;
+    }
+    QueryParams P;
+    memset(&P, 0, sizeof(P));
+    for (uint32_t l = 0; l < mip->n_levels; l++) {
+        for (int a = 0; a < 3; a++) {
+            const uint32_t dl = mip->level_dim[l][a];
+            if (dl == 0 || dl > (1u << 20) || (l > 0 && dl != (mip->level_dim[l - 1][a] + 1) / 2)) {
+                mg::set_error("mg_range_query: level %u axis %d has %u voxels: not the ceil-halving chain of L80", l, a, dl);
+                return MG_ERR_INVALID_ARG;
+            }
+            P.dim[l][a] = (int)dl;
+        }
+        P.off[l] = mip->level_offset[l];
+    }
+    const uint32_t* top = mip->level_dim[mip->n_levels - 1];
+    if (top[0] != 1 || top[1] != 1 || top[2] != 1) {
+        mg::set_error("mg_range_query: the mipmap must run up to its 1 x 1 x 1 level");
+        return MG_ERR_INVALID_ARG;
+    }
+    for (uint32_t q = 0; q < n_queries; q++) {
+        const uint64_t* b = boxes + 6ull * q;
+        for (int a = 0; a < 3; a++)
+            if (!(b[a] < b[3 + a]) || b[3 + a] > mip->level_dim[0][a]) {
+                mg::set_error("mg_range_query: box %u is empty or leaves the volume along axis %d", q, a);
+                return MG_ERR_INVALID_ARG;
+            }
+    }
+    if (n_queries == 0) return MG_OK;
+    cudaStream_t st = (cudaStream_t)stream;
+    if (n_queries > lut->boxes_cap) {
+        MG_CUDA(cudaStreamSynchronize(st));                              // earlier queries may still read the old buffer
+        cudaFree(lut->d_boxes);
+        lut->d_boxes = nullptr;
+        lut->boxes_cap = 0;
+        MG_CUDA(cudaMalloc(&lut->d_boxes, (size_t)n_queries * 6 * sizeof(uint64_t)));
+        lut->boxes_cap = n_queries;
+    }
+    MG_CUDA(cudaMemcpyAsync(lut->d_boxes, boxes, (size_t)n_queries * 6 * sizeof(uint64_t), cudaMemcpyHostToDevice, st));
+    const uint64_t n_out = (uint64_t)n_queries * lut->n_leaves;
+    MG_CUDA(cudaMemsetAsync(expect, 0, n_out * sizeof(double), st));
+    if (err) MG_CUDA(cudaMemsetAsync(err, 0, n_out * sizeof(double), st));
+    if (fetches) MG_CUDA(cudaMemsetAsync(fetches, 0, (size_t)n_queries * sizeof(uint64_t), st));
+    P.idx = node_idx_mipmap;
+    P.n_levels = (int)mip->n_levels;
+    P.n_leaves = lut->n_leaves;
+    P.row_ptr = lut->d_row_ptr; P.row_len = lut->d_row_len; P.col = lut->d_col; P.mu = lut->d_mu; P.dmu = lut->d_dmu;
+    P.boxes = lut->d_boxes;
+    P.expect = expect;
+    P.var = err;
+    P.fetches = reinterpret_cast<unsigned long long*>(fetches);
+    // spread a query over enough CTAs to fill the machine when there are few queries (148 SMs x 8 CTAs)
+    const uint32_t splits = std::max<uint32_t>(1, std::min<uint32_t>(64, (148 * 8 + n_queries - 1) / n_queries));
+    const dim3 grid(n_queries, splits);
+    if (mode == MG_QUERY_FA) k_range_query_fa<<<grid, kQueryThreads, 0, st>>>(P);
+    else k_range_query_naive<<<grid, kQueryThreads, 0, st>>>(P);
+    MG_CUDA(cudaGetLastError());
+    mg::count_launch();
+    if (err) {
+        k_query_finish<<<(unsigned)((n_out + 255) / 256), 256, 0, st>>>(err, n_out);
+        MG_CUDA(cudaGetLastError());
+        mg::count_launch();
+    }
+    return MG_OK;
+}

@@ -29,7 +29,8 @@ SYMBOLS = ["mg_load_graph", "mg_free_graph", "mg_graph_info", "mg_level_offsets"
            "mg_relabel_indices", "mg_propagate", "mg_propagate_host", "mg_colorize", "mg_tf_update_host",
            "mg_last_error", "mg_kernel_launch_count",
            "mg_bits_per_voxel", "mg_packed_stream_bytes", "mg_index_range", "mg_pack_indices", "mg_colorize_packed",
-           "mg_propagate_attr", "mg_render"]
+           "mg_propagate_attr", "mg_render",
+           "mg_mixture_lut_build", "mg_mixture_lut_free", "mg_mixture_lut_info", "mg_mixture_lut_export", "mg_range_query"]
 
 
 class MgInfo(C.Structure):
@@ -107,6 +108,24 @@ class MgView(C.Structure):
 
 lib.mg_render.argtypes = [_vp, _vp, C.POINTER(MgMipmapDesc), _vp, C.POINTER(MgView), _vp, _vp, _vp]
 lib.mg_render.restype = C.c_int
+
+
+class MgLutInfo(C.Structure):
+    _fields_ = [("n_nodes", C.c_uint64), ("nnz", C.c_uint64), ("capacity", C.c_uint64), ("device_bytes", C.c_uint64),
+                ("n_leaves", C.c_uint32), ("max_row_nnz", C.c_uint32)]
+
+
+MG_QUERY_FA, MG_QUERY_NAIVE = 0, 1
+lib.mg_mixture_lut_build.argtypes = [_vp, _vp, C.POINTER(_vp), _vp]
+lib.mg_mixture_lut_build.restype = C.c_int
+lib.mg_mixture_lut_free.argtypes = [_vp]
+lib.mg_mixture_lut_free.restype = None
+lib.mg_mixture_lut_info.argtypes = [_vp, C.POINTER(MgLutInfo)]
+lib.mg_mixture_lut_info.restype = C.c_int
+lib.mg_mixture_lut_export.argtypes = [_vp, _vp, _vp, _vp, _vp]
+lib.mg_mixture_lut_export.restype = C.c_int
+lib.mg_range_query.argtypes = [_vp, _vp, C.POINTER(MgMipmapDesc), _vp, C.c_uint32, _vp, _vp, _vp, C.c_uint32, _vp]
+lib.mg_range_query.restype = C.c_int
 
 
 class MgError(RuntimeError):
@@ -276,3 +295,49 @@ class Graph:
         v = view if isinstance(view, MgView) else view_struct(view)
         _check(lib.mg_render(self._h, _ptr(node_idx_device), C.byref(m), _ptr(node_rgba_device), C.byref(v),
                              _ptr(out_rgba_device), _ptr(stats_device), stream or None), "mg_render")
+
+    def mixture_lut(self, weight_sigma=None, stream: int = 0) -> "MixtureLut":
+        """NEXT-4: build the mixture lookup table (mu, dmu per node) of this graph on the device."""
+        return MixtureLut(self, weight_sigma, stream)
+
+
+class MixtureLut:
+    """Handle of a device mixture lookup table (mg_mixture_lut_build ... mg_mixture_lut_free)."""
+
+    def __init__(self, graph: Graph, weight_sigma=None, stream: int = 0):
+        sg = _np(weight_sigma, np.float32)
+        if sg is not None and sg.size != graph.info.n_nodes:
+            raise ValueError("weight_sigma must have n_nodes entries")
+        h = _vp()
+        _check(lib.mg_mixture_lut_build(graph._h, _ptr(sg), C.byref(h), stream or None), "mg_mixture_lut_build")
+        self._h = h
+        self.info = MgLutInfo()
+        _check(lib.mg_mixture_lut_info(self._h, C.byref(self.info)), "mg_mixture_lut_info")
+
+    def close(self) -> None:
+        if getattr(self, "_h", None):
+            lib.mg_mixture_lut_free(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def export(self):
+        """(row_ptr u64 [n_nodes + 1], leaf u32 [nnz], mu f64 [nnz], dmu f64 [nnz]) on the host."""
+        n, nnz = int(self.info.n_nodes), int(self.info.nnz)
+        rp, leaf = np.zeros(n + 1, np.uint64), np.zeros(nnz, np.uint32)
+        mu, dmu = np.zeros(nnz, np.float64), np.zeros(nnz, np.float64)
+        _check(lib.mg_mixture_lut_export(self._h, rp.ctypes.data, leaf.ctypes.data, mu.ctypes.data, dmu.ctypes.data),
+               "mg_mixture_lut_export")
+        return rp, leaf, mu, dmu
+
+    def range_query(self, node_idx_device, mip, boxes, expect_device, err_device=None, fetches_device=None,
+                    mode: int = MG_QUERY_FA, stream: int = 0) -> None:
+        m = mip if isinstance(mip, MgMipmapDesc) else mipmap_desc(*mip)
+        b = np.ascontiguousarray(boxes, dtype=np.uint64).reshape(-1, 6)
+        _check(lib.mg_range_query(self._h, _ptr(node_idx_device), C.byref(m), b.ctypes.data, b.shape[0],
+                                  _ptr(expect_device), _ptr(err_device), _ptr(fetches_device), int(mode), stream or None),
+               "mg_range_query")
