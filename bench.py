@@ -48,6 +48,8 @@ def parse_args():
     p.add_argument("--no-cpu-baseline", action="store_true")
     p.add_argument("--no-e2e", action="store_true")
     p.add_argument("--no-attr", action="store_true", help="skip the extra NEXT-1 measurement (multi-attribute propagation)")
+    p.add_argument("--relabel", action="store_true", help="config 5: load the DAG with MG_RELABEL (levels sorted by children)")
+    p.add_argument("--no-query", action="store_true", help="skip the extra NEXT-4 measurement (mixture LUT + range queries)")
     p.add_argument("--no-render", action="store_true", help="skip the extra NEXT-2 measurement (ray-marcher over the paletted mipmap)")
     p.add_argument("--no-packed", action="store_true", help="skip the extra NEXT-3 measurement (bit-packed node IDs)")
     p.add_argument("--cpu-sample-voxels", type=int, default=1 << 31, help="oracle sample size (>= the mipmap = whole workload)")
@@ -226,7 +228,7 @@ def run_b200(args) -> dict:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
     from paper_2009_02702_b200 import mg, workload
 
-    w = workload.make(args.config, args.scale)
+    w = workload.make(args.config, args.scale, relabel=args.relabel)
     g = w.graph
     info = g.info
     n_nodes, n_internal = int(info.n_nodes), int(info.n_internal)
@@ -356,6 +358,48 @@ def run_b200(args) -> dict:
         render["coverage"] = float((img[..., 3] > 0).float().mean().item())
         del img
 
+    # ---- NEXT-4: mixture lookup table + range queries (Table 4: random cubes of 16^3 .. 256^3 voxels, FA vs naive)
+    query = None
+    if not args.no_query and rank == 0 and len(w.mip_dims) > 1 and w.host_graph is not None and "weight_sigma" in w.host_graph:
+        from paper_2009_02702_b200 import synth
+        g.mixture_lut(w.host_graph["weight_sigma"]).close()          # warm-up build (module load, allocator state)
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        lut = g.mixture_lut(w.host_graph["weight_sigma"])
+        torch.cuda.synchronize()
+        t_build = time.perf_counter() - t0
+        nl = int(info.n_leaves)
+        nq = 64
+        query = {"what": "NEXT-4: device mixture LUT (mu, dmu per node, Eq. 18) and batched range queries, footprint assembly "
+                         "vs naive (PAPER.md sections 3.5-3.6, Table 4)", "lut_build_ms": 1e3 * t_build,
+                 "lut_entries": int(lut.info.nnz), "lut_mbytes": lut.info.device_bytes / 1e6, "queries_per_batch": nq,
+                 "paper_context": "Table 4 (10-core CPU, ms per query FA / naive): 16^3 0.11-0.15 / 0.40-0.44; 64^3 1.3-2.1 / 12.9-29.5; "
+                                  "256^3 25-394 / 1200-70500", "sizes": {}}
+        desc = w.mip_desc()
+        e_buf = torch.empty((nq, nl), dtype=torch.float64, device="cuda")
+        d_buf = torch.empty((nq, nl), dtype=torch.float64, device="cuda")
+        f_buf = torch.empty((nq,), dtype=torch.int64, device="cuda")
+        c = w.cfg
+        for side in (16, 32, 64, 128, 256):
+            boxes = np.array(synth.query_boxes(c["dims"], side, nq, seed=c.get("seed", 0)), dtype=np.uint64)
+            row = {}
+            for label, mode, reps in (("fa", mg.MG_QUERY_FA, 10), ("naive", mg.MG_QUERY_NAIVE, 3)):
+                lut.range_query(w.d_idx, desc, boxes, e_buf, d_buf, f_buf, mode=mode, stream=st)
+                torch.cuda.synchronize()
+                q0, q1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                q0.record(stream)
+                for _ in range(reps):
+                    lut.range_query(w.d_idx, desc, boxes, e_buf, d_buf, f_buf, mode=mode, stream=st)
+                q1.record(stream)
+                torch.cuda.synchronize()
+                row[label + "_ms_per_query"] = q0.elapsed_time(q1) / reps / nq
+                row[label + "_fetches"] = float(f_buf.double().mean().item())
+            row["fetches_saved"] = 1.0 - row["fa_fetches"] / row["naive_fetches"]
+            row["speedup"] = row["naive_ms_per_query"] / row["fa_ms_per_query"]
+            query["sizes"][str(side)] = row
+        lut.close()
+        del e_buf, d_buf, f_buf
+
     # ---- e2e: host TF in, host mipmap out, through the public C-ABI call (rank-local, then max)
     e2e = None
     if not args.no_e2e:
@@ -416,6 +460,8 @@ def run_b200(args) -> dict:
         res["attr"] = attr
     if render is not None:
         res["render"] = render
+    if query is not None:
+        res["query"] = query
     if e2e is not None:
         res["e2e"] = e2e
     if world == 1 and not args.no_cpu_baseline and w.host_idx is not None:

@@ -300,18 +300,25 @@ k_range_query_fa(const __grid_constant__ QueryParams P)
     double* var = P.var ? P.var + (uint64_t)q * P.n_leaves : nullptr;
     unsigned long long n_fetch = 0;
     const unsigned n_boxes = (unsigned)(nx * ny * nz);
+    // every warp walks all boxes (a, b, c) = t in x-fastest order; (a, b, c) and t mod n_warps are carried along
+    // incrementally -- no divisions in the walk, most boxes are left after a few instructions
+    int a = -1, b = 0, c = 0;
+    unsigned tm = n_warps - 1;                                           // (t - 1) mod n_warps
     for (unsigned t = 0; t < n_boxes; t++) {
-        const int a = t % nx, b = (t / nx) % ny, c = t / (nx * ny);
+        if (++a == nx) { a = 0; if (++b == ny) { b = 0; ++c; } }
+        if (++tm == n_warps) tm = 0;
         const int lx = s_level[0][a], ly = s_level[1][b], lz = s_level[2][c];
         const int l = min(lx, min(ly, lz));                              // cube side = the shortest extent
         const int ex = lx - l, ey = ly - l, ez = lz - l;                 // cubes per axis = 2^e
         const unsigned long long n_cubes = 1ull << (ex + ey + ez);
         const unsigned long long n_chunks = (n_cubes + 31) >> 5;
+        const unsigned long long ch0 = warp >= tm ? warp - tm : warp + n_warps - tm;   // (warp - t) mod n_warps
+        if (ch0 >= n_chunks) continue;
         const double scale = __hiloint2double((1023 + 3 * l) << 20, 0);  // side^3 = 8^l
         const int X = P.dim[l][0], Y = P.dim[l][1];
         const uint32_t* lvl = P.idx + P.off[l];
         const uint32_t bx = s_start[0][a] >> l, by = s_start[1][b] >> l, bz = s_start[2][c] >> l;
-        for (unsigned long long ch = (warp + n_warps - t % n_warps) % n_warps; ch < n_chunks; ch += n_warps) {
+        for (unsigned long long ch = ch0; ch < n_chunks; ch += n_warps) {
             const unsigned long long k = (ch << 5) + lane;
             const bool active = k < n_cubes;
             uint32_t node = 0;

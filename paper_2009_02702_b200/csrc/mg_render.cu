@@ -219,7 +219,8 @@ k_render(const __grid_constant__ RenderParams P)
                 // histogram mipmap) every tap of both levels is that leaf.  Its index gathers are issued before the
                 // climb of R6 so that the two dependent chains overlap.
                 Cell cell;
-                fetch_cell(P, uni ? l1 : l0, px, py, pz, cell);
+                const bool coarse_first = uni && f != 0.f;                        // frac(lambda) = 0: only level l0 is needed
+                fetch_cell(P, coarse_first ? l1 : l0, px, py, pz, cell);
                 if (ess) {
                     // The oracle forgets its block here and climbs again from level l1 + 1.  The climb is a pure
                     // function of the parent voxels, so a parent already found not empty is not fetched again
@@ -244,19 +245,15 @@ k_render(const __grid_constant__ RenderParams P)
                     }
                 }
                 float4 c;                                                        // R3
-                if (uni && one_node(cell) && cell.n[0] < P.n_leaves) {
+                if (coarse_first && one_node(cell) && cell.n[0] < P.n_leaves) {
                     c = __ldg(P.pal + cell.n[0]);
                     n_uni++;
                 } else {
                     float4 c1 = make_float4(0.f, 0.f, 0.f, 0.f);
-                    if (uni) {                                                   // cell = coarse level
-                        if (f != 0.f || l0 == l1) c1 = shade_cell(P, cell);
-                        if (l0 != l1) {
-                            fetch_cell(P, l0, px, py, pz, cell);
-                            c = shade_cell(P, cell);
-                        } else {
-                            c = c1;
-                        }
+                    if (coarse_first) {                                          // cell = coarse level (f != 0, l0 < l1)
+                        c1 = shade_cell(P, cell);
+                        fetch_cell(P, l0, px, py, pz, cell);
+                        c = shade_cell(P, cell);
                     } else {                                                     // cell = fine level
                         c = shade_cell(P, cell);
                         if (f != 0.f) {

@@ -121,6 +121,19 @@ def render_tf(tf: np.ndarray) -> np.ndarray:
     return out
 
 
+def query_boxes(dims_xyz, side: int, n: int, seed: int) -> list:
+    """``n`` randomly aligned range queries of (up to) side^3 voxels inside the volume (Table 4: "randomly-
+    aligned range queries covering between 16^3 to 256^3 voxels"): [x0, y0, z0, x1, y1, z1], half-open.  An
+    axis shorter than ``side`` is covered whole."""
+    out = []
+    for q in range(n):
+        r = u64(seed, 600 + side, np.arange(3 * q, 3 * q + 3, dtype=np.uint64))
+        ext = [min(int(side), int(d)) for d in dims_xyz]
+        lo = [int(r[a] % np.uint64(int(dims_xyz[a]) - ext[a] + 1)) for a in range(3)]
+        out.append(lo + [lo[a] + ext[a] for a in range(3)])
+    return out
+
+
 def single_segment_update(tf: np.ndarray, seed: int, update: int) -> np.ndarray:
     """Config 4: each update re-draws ONE random segment's RGBA; returns a new array."""
     out = tf.copy()

@@ -44,6 +44,7 @@ class Workload:
         self.d_packed = None                      # torch uint8: bit-packed streams of all levels (after pack())
         self.packed_levels = None                 # list of dicts (n_voxels, out_offset, byte_offset, bits, i_min)
         self.packed_bytes = 0
+        self.perm = None                          # uint32 [n_nodes]: library index of the caller's node (only after MG_RELABEL)
 
     def tf(self, update: int = 0) -> np.ndarray:
         """fp32 [n_leaves, 4] transfer function number ``update`` of this config (synth recipe)."""
@@ -144,18 +145,26 @@ def from_volume(seg: np.ndarray, name: str = "volume", cfg: dict | None = None, 
 
 
 def from_dag(child_a, child_b, weight, level_offsets, n_leaves: int, node_idx: np.ndarray, name: str = "dag",
-             cfg: dict | None = None) -> Workload:
-    """A ready-made level-contiguous DAG plus ONE node-index volume (config 5)."""
+             cfg: dict | None = None, relabel: bool = False) -> Workload:
+    """A ready-made level-contiguous DAG plus ONE node-index volume (config 5).  ``relabel`` loads it with
+    MG_RELABEL (the library sorts every level by its children for gather locality) and renumbers the
+    device index volume accordingly; ``Workload.perm`` then maps the caller's node numbers to the library's."""
     w = Workload(name)
     w.cfg = dict(cfg or {})
     w.n_leaves = int(n_leaves)
     t0 = time.perf_counter()
-    w.graph = mg.Graph(child_a, child_b, weight, n_leaves, level_offsets=level_offsets)
+    w.graph = mg.Graph(child_a, child_b, weight, n_leaves, level_offsets=level_offsets,
+                       flags=mg.MG_RELABEL if relabel else 0)
     t1 = time.perf_counter()
     w.host_graph = dict(child_a=child_a, child_b=child_b, weight=weight, level_offsets=np.asarray(level_offsets),
                         n_leaves=int(n_leaves))
     w.mip_dims = [(int(node_idx.size), 1, 1)]
     _upload_levels(w, [node_idx.reshape(-1)])
+    if relabel:
+        import torch
+        w.perm = w.graph.node_permutation()
+        w.graph.relabel_indices(w.d_idx, w.n_voxels_padded, torch.cuda.current_stream().cuda_stream)
+        torch.cuda.synchronize()
     t2 = time.perf_counter()
     off = np.asarray(level_offsets, dtype=np.int64)
     w.stats = dict(load_graph_s=t1 - t0, upload_idx_s=t2 - t1, n_nodes=int(child_a.size), n_leaves=int(n_leaves),
@@ -164,7 +173,7 @@ def from_dag(child_a, child_b, weight, level_offsets, n_leaves: int, node_idx: n
 
 
 def make(cfg_id: int, scale: float = 1.0, device_synth: bool = True, keep_seg: bool = False,
-         **builder_params) -> Workload:
+         relabel: bool = False, **builder_params) -> Workload:
     """BASELINE.json config ``cfg_id`` (1-5); ``scale`` < 1 gives a geometrically similar smaller
     instance (tests).  Volumes are generated on the GPU (bit-identical to synth.py) unless
     ``device_synth`` is False.  ``keep_seg`` keeps the generated volume in ``Workload.seg``."""
@@ -177,7 +186,8 @@ def make(cfg_id: int, scale: float = 1.0, device_synth: bool = True, keep_seg: b
         a, b, wt, off = synth.random_dag(n_nodes, c["n_levels"], n_leaves, c["seed"])
         idx = synth.random_node_idx(n_vox, n_nodes, c["seed"])
         t1 = time.perf_counter()
-        w = from_dag(a, b, wt, off, n_leaves, idx, name=c["name"] + (f"_x{scale:g}" if scale != 1.0 else ""), cfg=c)
+        w = from_dag(a, b, wt, off, n_leaves, idx, name=c["name"] + (f"_x{scale:g}" if scale != 1.0 else ""), cfg=c,
+                     relabel=relabel)
         w.stats["synth_s"] = t1 - t0
         return w
     c = synth.scaled_config(cfg_id, scale)

@@ -277,6 +277,27 @@ def test_config5_dag_stress_full_size(libs):
         w.close()
 
 
+def test_config5_scaled_with_relabel(libs):
+    """Config 5 at 1/64 scale loaded with MG_RELABEL (bench.py --relabel): the library's numbering is a
+    permutation of the caller's; node colours and colourised voxels must equal the oracle's through it."""
+    mg, workload = libs
+    w = workload.make(5, scale=1.0 / 64, relabel=True)
+    try:
+        assert w.perm is not None and w.graph.info.relabelled == 1
+        assert np.array_equal(np.sort(w.perm), np.arange(w.perm.size))
+        tf = w.tf(0)
+        nodes, out = _run_update(mg, w, tf, mg.MG_RGBA8)
+        hg = w.host_graph
+        ref = oracle.graph_eval(hg["child_a"], hg["child_b"], hg["weight"], hg["n_leaves"], tf.astype(np.float64))
+        got = nodes.cpu().numpy()[w.perm]                                    # caller's node n lives at perm[n]
+        assert np.array_equal(got[:hg["n_leaves"]].view(np.uint32), tf.view(np.uint32))
+        assert float(np.abs(got - ref).max()) <= TOL
+        out4 = out.view(-1, 4).cpu().numpy()[:w.n_voxels]
+        assert _rgba8_close(out4, oracle.lookup(w.host_idx[0], ref))         # host_idx keeps the caller's numbering
+    finally:
+        w.close()
+
+
 def test_config1_every_voxel_every_level(libs):
     """Config 1 (64^3, 16 segments): element-by-element on all 299,593 voxels, unquantised and b = 9,
     both against the same-graph oracle and against the direct histogram (dense O-2)."""
@@ -299,3 +320,89 @@ def test_config1_every_voxel_every_level(libs):
                 assert np.abs(got_nodes[idx] - direct).max() <= tol_direct
         finally:
             w.close()
+
+
+def _sub_dag(hg, targets):
+    """The part of the graph below `targets`, renumbered (leaves first, children before parents), for the
+    dense oracle: returns (child_a, child_b, weight, sigma, n_sub_leaves, old ids of the sub-nodes)."""
+    a, b, nl = hg["child_a"], hg["child_b"], hg["n_leaves"]
+    seen, stack = set(), [int(t) for t in targets]
+    while stack:
+        n = stack.pop()
+        if n in seen:
+            continue
+        seen.add(n)
+        if n >= nl:
+            stack += [int(a[n]), int(b[n])]
+    old = np.array(sorted(seen), dtype=np.int64)                  # library numbering is children-before-parents
+    n_sub_leaves = int((old < nl).sum())
+    new = {int(o): i for i, o in enumerate(old)}
+    sa = np.array([new[int(a[o])] if o >= nl else 0 for o in old], dtype=np.uint32)
+    sb = np.array([new[int(b[o])] if o >= nl else 0 for o in old], dtype=np.uint32)
+    return sa, sb, hg["weight"][old].astype(np.float64), hg["weight_sigma"][old].astype(np.float64), n_sub_leaves, old
+
+
+def test_config3_mixture_lut_and_range_queries_full_size(libs):
+    """NEXT-4 at full size, in bench.py's launch configuration (batches of random cubes, Table 4's sizes).
+    The dense oracle cannot hold 1.7 M x 1182 entries, so: sampled rows of the table against the oracle run on
+    the sub-DAG below them; every row sums to 1; NAIVE == the plain per-segment voxel count of the generator's
+    volume (exact); FA fetch counts == the oracle's decomposition; FA sums to the box volume (L251) and stays
+    within 1 % of the volume of the true counts (L251: 'about 0.3 %')."""
+    mg, workload = libs
+    w = workload.make(3, keep_seg=True)
+    try:
+        hg, g = w.host_graph, w.graph
+        nl = hg["n_leaves"]
+        lut = g.mixture_lut(hg["weight_sigma"])
+        rp, leaf, mu, dmu = lut.export()
+        n = rp.size - 1
+        assert n == hg["child_a"].size and lut.info.nnz == leaf.size == lut.info.capacity     # builder graphs: disjoint children
+        sums = np.add.reduceat(mu, rp[:-1].astype(np.int64))
+        assert np.abs(sums - 1.0).max() <= 1e-12
+        # sampled rows (incl. the root and the deepest nodes) against the dense oracle on their sub-DAG
+        pick = np.unique(np.concatenate([(synth.u64(3, 500, np.arange(300, dtype=np.uint64)) % np.uint64(n)).astype(np.int64),
+                                         np.arange(n - 40, n)]))
+        sa, sb, sw, ssg, snl, old = _sub_dag(hg, pick)
+        omu, odmu = oracle.mixture_lut(sa, sb, sw, ssg, snl)
+        pos = {int(o): i for i, o in enumerate(old)}
+        for t in pick:
+            s, e = int(rp[t]), int(rp[t + 1])
+            row = pos[int(t)]
+            cols = np.array([pos[int(c)] for c in leaf[s:e]])               # sub-leaf index of each stored leaf
+            assert (np.flatnonzero(omu[row]) == np.sort(cols)).all()
+            np.testing.assert_allclose(mu[s:e], omu[row, cols], rtol=1e-12)
+            np.testing.assert_allclose(dmu[s:e], odmu[row, cols], rtol=1e-12, atol=1e-300)
+
+        dims = synth.CONFIGS[3]["dims"]
+        ids, seg_index = _leaf_index_chunked(w.seg)
+        desc = w.mip_desc()
+        l_max = len(w.mip_dims) - 1
+        worst = 0.0
+        for side in (16, 64, 256):
+            boxes = synth.query_boxes(dims, side, 24, seed=3)
+            nq = len(boxes)
+            e_fa = torch.empty((nq, nl), dtype=torch.float64, device="cuda")
+            d_fa = torch.empty((nq, nl), dtype=torch.float64, device="cuda")
+            f_fa = torch.empty((nq,), dtype=torch.int64, device="cuda")
+            e_nv = torch.empty((nq, nl), dtype=torch.float64, device="cuda")
+            f_nv = torch.empty((nq,), dtype=torch.int64, device="cuda")
+            lut.range_query(w.d_idx, desc, boxes, e_fa, d_fa, f_fa, mode=mg.MG_QUERY_FA)
+            lut.range_query(w.d_idx, desc, boxes, e_nv, None, f_nv, mode=mg.MG_QUERY_NAIVE)
+            torch.cuda.synchronize()
+            e_fa, d_fa, f_fa, e_nv, f_nv = (t.cpu().numpy() for t in (e_fa, d_fa, f_fa, e_nv, f_nv))
+            for q, (x0, y0, z0, x1, y1, z1) in enumerate(boxes):
+                vol = (x1 - x0) * (y1 - y0) * (z1 - z0)
+                truth = np.bincount(seg_index[z0:z1, y0:y1, x0:x1].reshape(-1), minlength=nl)
+                assert np.array_equal(e_nv[q], truth) and f_nv[q] == vol
+                segs = [oracle.fa_axis(lo, hi, l_max) for lo, hi in ((x0, x1), (y0, y1), (z0, z1))]
+                n_fetch = sum(1 << (lx + ly + lz - 3 * min(lx, ly, lz)) for _, lx in segs[0] for _, ly in segs[1] for _, lz in segs[2])
+                assert f_fa[q] == n_fetch
+                assert abs(e_fa[q].sum() - vol) <= 1e-9 * vol
+                assert (e_fa[q] >= 0).all() and (d_fa[q] >= 0).all()
+                worst = max(worst, float(np.abs(e_fa[q] - truth).max()) / vol)
+        print(f"cfg3 range queries: LUT {lut.info.nnz} entries ({lut.info.device_bytes / 1e6:.0f} MB, longest row "
+              f"{lut.info.max_row_nnz}); max |FA - true count| / volume = {worst:.2e}")
+        assert worst < 0.01, worst
+        lut.close()
+    finally:
+        w.close()
