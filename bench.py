@@ -486,11 +486,7 @@ def run_reference(args) -> dict:
         torch.cuda.set_device(local_rank)
     from paper_2009_02702_b200 import workload
     # the oracle's inputs (graph + node-index mipmap) come from the same seeded assembly as the GPU arm
-    w = workload.make(args.config, args.scale, device_synth=torch.cuda.is_available())
-    if w.graph is not None:
-        w.graph.close()
-        w.graph = None
-    w.d_idx = None
+    w = workload.make(args.config, args.scale, device_synth=torch.cuda.is_available(), load=False)
     tf64 = [w.tf(u).astype(np.float64) for u in range(4)]
     # calibrate the per-step sample so that steps + warmup fit the budget
     probe = _sample_plan(w, 1 << 22)

@@ -111,8 +111,9 @@ def _upload_levels(w: Workload, levels) -> None:
 
 
 def from_volume(seg: np.ndarray, name: str = "volume", cfg: dict | None = None, keep_host: bool = True,
-                **builder_params) -> Workload:
-    """Builder + load + upload for a uint32 [Z, Y, X] segment-ID volume."""
+                load: bool = True, **builder_params) -> Workload:
+    """Builder + load + upload for a uint32 [Z, Y, X] segment-ID volume.  ``load=False`` stops after the
+    builder (host arrays only: what bench.py's reference arm needs; no device is touched)."""
     w = Workload(name)
     w.cfg = dict(cfg or {})
     t0 = time.perf_counter()
@@ -122,11 +123,18 @@ def from_volume(seg: np.ndarray, name: str = "volume", cfg: dict | None = None, 
     w.host_graph = g
     w.n_leaves = g["n_leaves"]
     w.mip_dims = r.mip_dims
-    w.graph = mg.Graph(g["child_a"], g["child_b"], g["weight"], g["n_leaves"], level_offsets=g["level_offsets"],
-                       leaf_segment_id=g["leaf_segment_id"])
+    if load:
+        w.graph = mg.Graph(g["child_a"], g["child_b"], g["weight"], g["n_leaves"], level_offsets=g["level_offsets"],
+                           leaf_segment_id=g["leaf_segment_id"])
     t2 = time.perf_counter()
     levels = [r.node_idx(l, copy=False) for l in range(r.info.n_mip_levels)]
-    _upload_levels(w, levels)
+    if load:
+        _upload_levels(w, levels)
+    else:
+        w.level_voxels = [int(a.size) for a in levels]
+        w.level_start, w.n_voxels_padded = _layout(w.level_voxels)
+        w.n_voxels = sum(w.level_voxels)
+        w.host_idx = levels
     t3 = time.perf_counter()
     i = r.info
     w.stats = dict(builder_s=t1 - t0, load_graph_s=t2 - t1, upload_idx_s=t3 - t2, n_nodes=int(i.n_nodes),
@@ -145,7 +153,7 @@ def from_volume(seg: np.ndarray, name: str = "volume", cfg: dict | None = None, 
 
 
 def from_dag(child_a, child_b, weight, level_offsets, n_leaves: int, node_idx: np.ndarray, name: str = "dag",
-             cfg: dict | None = None, relabel: bool = False) -> Workload:
+             cfg: dict | None = None, relabel: bool = False, load: bool = True) -> Workload:
     """A ready-made level-contiguous DAG plus ONE node-index volume (config 5).  ``relabel`` loads it with
     MG_RELABEL (the library sorts every level by its children for gather locality) and renumbers the
     device index volume accordingly; ``Workload.perm`` then maps the caller's node numbers to the library's."""
@@ -153,14 +161,20 @@ def from_dag(child_a, child_b, weight, level_offsets, n_leaves: int, node_idx: n
     w.cfg = dict(cfg or {})
     w.n_leaves = int(n_leaves)
     t0 = time.perf_counter()
-    w.graph = mg.Graph(child_a, child_b, weight, n_leaves, level_offsets=level_offsets,
-                       flags=mg.MG_RELABEL if relabel else 0)
+    if load:
+        w.graph = mg.Graph(child_a, child_b, weight, n_leaves, level_offsets=level_offsets,
+                           flags=mg.MG_RELABEL if relabel else 0)
     t1 = time.perf_counter()
     w.host_graph = dict(child_a=child_a, child_b=child_b, weight=weight, level_offsets=np.asarray(level_offsets),
                         n_leaves=int(n_leaves))
     w.mip_dims = [(int(node_idx.size), 1, 1)]
-    _upload_levels(w, [node_idx.reshape(-1)])
-    if relabel:
+    if load:
+        _upload_levels(w, [node_idx.reshape(-1)])
+    else:
+        w.level_voxels, w.level_start = [int(node_idx.size)], [0]
+        w.n_voxels = w.n_voxels_padded = int(node_idx.size)
+        w.host_idx = [node_idx.reshape(-1)]
+    if relabel and load:
         import torch
         w.perm = w.graph.node_permutation()
         w.graph.relabel_indices(w.d_idx, w.n_voxels_padded, torch.cuda.current_stream().cuda_stream)
@@ -173,7 +187,7 @@ def from_dag(child_a, child_b, weight, level_offsets, n_leaves: int, node_idx: n
 
 
 def make(cfg_id: int, scale: float = 1.0, device_synth: bool = True, keep_seg: bool = False,
-         relabel: bool = False, **builder_params) -> Workload:
+         relabel: bool = False, load: bool = True, **builder_params) -> Workload:
     """BASELINE.json config ``cfg_id`` (1-5); ``scale`` < 1 gives a geometrically similar smaller
     instance (tests).  Volumes are generated on the GPU (bit-identical to synth.py) unless
     ``device_synth`` is False.  ``keep_seg`` keeps the generated volume in ``Workload.seg``."""
@@ -187,7 +201,7 @@ def make(cfg_id: int, scale: float = 1.0, device_synth: bool = True, keep_seg: b
         idx = synth.random_node_idx(n_vox, n_nodes, c["seed"])
         t1 = time.perf_counter()
         w = from_dag(a, b, wt, off, n_leaves, idx, name=c["name"] + (f"_x{scale:g}" if scale != 1.0 else ""), cfg=c,
-                     relabel=relabel)
+                     relabel=relabel, load=load)
         w.stats["synth_s"] = t1 - t0
         return w
     c = synth.scaled_config(cfg_id, scale)
@@ -200,7 +214,7 @@ def make(cfg_id: int, scale: float = 1.0, device_synth: bool = True, keep_seg: b
     else:
         seg = synth.make_volume(c)
     t1 = time.perf_counter()
-    w = from_volume(seg, name=c["name"], cfg=c, **builder_params)
+    w = from_volume(seg, name=c["name"], cfg=c, load=load, **builder_params)
     if keep_seg:
         w.seg = seg                                # the generator's volume (tests: input of the oracle)
     del seg
