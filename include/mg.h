@@ -251,9 +251,11 @@ int mg_propagate_attr(mg_graph *g, const float *leaf_attr, float *node_attr, uin
  *      alpha' = 1 - (1 - alpha)^(Delta / (ref_step_voxels s_ref)) (L269; 0.5-voxel steps, L414).
  *   R5 front-to-back compositing from the entry of the volume's box, sample at the interval mid-point,
  *      last interval clipped to the exit, stop at A >= alpha_cutoff.
- *   R6 hierarchical empty-space skipping (L271): from level floor(lambda)+2 upwards climb while the
- *      parent voxel's palette opacity is < ess_threshold; samples whose whole 2 x 8-voxel footprint
- *      lies in the largest such block are not fetched.  ess_threshold < 0 disables it.
+ *   R6 hierarchical empty-space skipping (L271): a ray is in "empty mode" when it enters the volume and after
+ *      every sample that was skipped or whose interpolated opacity was < ess_threshold.  In empty mode, before
+ *      a sample is fetched, climb from level floor(lambda)+2 upwards while the parent voxel's palette opacity
+ *      is < ess_threshold; samples whose whole 2 x 8-voxel footprint lies in the largest such block are not
+ *      fetched.  ess_threshold < 0 disables it.
  * Arithmetic: ray geometry (t, step, sample position, trilinear fractions, block tests) in fp64;
  * fractional LOD, interpolation weights, colours, opacity correction and compositing in fp32.
  * ------------------------------------------------------------------------------------------------ */

@@ -375,10 +375,14 @@ void mgo_unpack_bits(const uint8_t *stream, uint64_t n_vox, uint32_t i_min, uint
  *                last interval is clipped to the exit, the sample sits at the interval's mid-point;
  *                front-to-back: C += (1 - A) alpha' rgb, A += (1 - A) alpha'; stop at A >= alpha_cutoff.
  *  R6 ESS        (L271) the opacity hierarchy is the A channel of the palette on the coarser mip levels.
- *                From level l1 + 1 upwards, "as long as the opacity value in parent voxels falls below
- *                a certain threshold" climb; the largest such block [lo, hi) is remembered and every
- *                sample whose 16-voxel footprint lies inside it is skipped: trilinear at level l reads
- *                voxels floor(p / 2^l - 1/2) and the next one, both inside the block iff
+ *                A ray is in "empty mode" when it enters the volume and after every sample that was skipped or
+ *                whose interpolated opacity fell below the threshold; it leaves it with the first sample at or
+ *                above the threshold ("uses the hierarchy for skipping longer segments": the hierarchy is only
+ *                consulted where the ray is in empty space).  In empty mode, before a sample is fetched: from
+ *                level l1 + 1 upwards, "as long as the opacity value in parent voxels falls below a certain
+ *                threshold" climb; the largest such block [lo, hi) is remembered and every sample whose
+ *                16-voxel footprint lies inside it is skipped: trilinear at level l reads voxels
+ *                floor(p / 2^l - 1/2) and the next one, both inside the block iff
  *                lo + 2^l / 2 <= p < hi - 2^l / 2; l = l1 is the binding level (no shrinking at faces
  *                on the volume's boundary, where the fetch clamps to the edge).
  * Output: [H][W][4] = (C_r, C_g, C_b, A), associated colour over a transparent background. */
@@ -506,6 +510,7 @@ static void mgo_march(const mgo_view *v, const double *cam, const double *par, u
     int box_valid = 0;
     double box_lo[3] = {0, 0, 0}, box_hi[3] = {0, 0, 0};
     int box_open_lo[3] = {0, 0, 0}, box_open_hi[3] = {0, 0, 0};     /* face on the volume's boundary */
+    int empty_mode = 1;                                             /* R6: a ray enters the volume in empty mode */
     double t = t_near;
     while (t < t_far && A < cutoff) {
         double rho = t * cos_view * (2.0 * tanh_ / (double)H) / s_ref;              /* R2 */
@@ -522,7 +527,7 @@ static void mgo_march(const mgo_view *v, const double *cam, const double *par, u
         uint32_t l1 = l0 + 1 > l_max ? l_max : l0 + 1;
         double f = lambda - (double)l0;
         t += delta;
-        if (thr >= 0.0) {                                                           /* R6 */
+        if (thr >= 0.0 && empty_mode) {                                             /* R6 */
             double m = 0.5 * ldexp(1.0, (int)l1);
             int inside = 0;
             if (box_valid) {
@@ -569,6 +574,7 @@ static void mgo_march(const mgo_view *v, const double *cam, const double *par, u
         for (int ch = 0; ch < 4; ch++)
             c[ch] = (1.0 - f) * c0[ch] + f * c1[ch];
         double alpha = c[3] < 0.0 ? 0.0 : (c[3] > 1.0 ? 1.0 : c[3]);
+        empty_mode = alpha < thr;                                                   /* R6 */
         double ac = 1.0 - pow(1.0 - alpha, de / (ref * s_ref));                      /* R4 */
         for (int ch = 0; ch < 3; ch++)
             C[ch] += (1.0 - A) * ac * c[ch];

@@ -188,6 +188,7 @@ k_render(const __grid_constant__ RenderParams P)
 #pragma unroll
             for (int a = 0; a < 3; a++) E.lo2[a] = E.hi2[a] = 0;
             int miss_L = -1, miss_x = 0, miss_y = 0, miss_z = 0;                 // last parent voxel found not empty
+            bool empty_mode = true;                                              // R6: a ray enters the volume in empty mode
             double t = tn;
             while (t < tf && A < P.cutoff) {
                 // R2 + R4 without transcendentals on the ray parameter: 2^lambda = clamp(rho 2^bias, 1, 2^l_max),
@@ -207,7 +208,8 @@ k_render(const __grid_constant__ RenderParams P)
                 t += delta;
                 int hx = 0, hy = 0, hz = 0;
                 const int m2 = 1 << l1;                                          // 2 m, m = 2^l1 / 2
-                if (ess) {                                                       // R6, in half-voxel integers
+                const bool probe = ess && empty_mode;                            // R6: only where the ray is in empty space
+                if (probe) {                                                     // in half-voxel integers
                     hx = (int)floor(px + px); hy = (int)floor(py + py); hz = (int)floor(pz + pz);
                     if (inside_block(E, m2, hx, hy, hz)) {
                         n_skip++;
@@ -221,8 +223,9 @@ k_render(const __grid_constant__ RenderParams P)
                 Cell cell;
                 const bool coarse_first = uni && f != 0.f;                        // frac(lambda) = 0: only level l0 is needed
                 fetch_cell(P, coarse_first ? l1 : l0, px, py, pz, cell);
-                if (ess) {
-                    // The oracle forgets its block here and climbs again from level l1 + 1.  The climb is a pure
+                if (probe) {
+                    // Empty mode and not inside the remembered block: the oracle forgets its block and climbs again
+                    // from level l1 + 1.  The climb is a pure
                     // function of the parent voxels, so a parent already found not empty is not fetched again
                     // (consecutive samples share it).
                     E.valid = false;
@@ -268,6 +271,7 @@ k_render(const __grid_constant__ RenderParams P)
                     }
                 }
                 const float alpha = fminf(fmaxf(c.w, 0.f), 1.f);
+                empty_mode = (double)alpha < P.thr;                               // R6
                 const float e = (float)de * P.inv_ref;
                 const float ac = -expm1f(e * log1pf(-alpha));                     // 1 - (1 - alpha)^e
                 const double wgt = (1.0 - A) * (double)ac;                        // R5, accumulated in fp64

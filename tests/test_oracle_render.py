@@ -224,3 +224,26 @@ def test_render_pixels_is_render_restricted_to_those_pixels():
     px_all, st_all = oracle.render_pixels(levels, pal, view, every)
     np.testing.assert_array_equal(px_all.reshape(7, 9, 4), img)
     assert st_all == st
+
+
+def test_empty_mode_state_machine_hand_worked():
+    """R6: the hierarchy is consulted only in empty mode (on entry, and after a skipped or transparent sample).
+    32 x 1 x 1 voxels, opaque for x < 8 and x >= 24, exactly transparent in between; ray along +x, lambda = 0,
+    2-voxel steps: samples at x = 1, 3, ..., 31 (footprint = voxels floor(x - 1/2), +1; block margin 2^l1 / 2 = 1).
+      x = 1 .. 7   evaluated (x = 1 climbs first -- the ray enters in empty mode -- and finds [0, 4) occupied)
+      x = 9        evaluated although it lies in the empty block [8, 16): the sample before it was opaque;
+                   its opacity is 0, so the ray is in empty mode from here
+      x = 11, 13   skipped (9 <= x < 15);  x = 15 evaluated (outside the margin), transparent
+      x = 17       skipped at once: still in empty mode, new block [16, 24), 17 <= x < 23;  x = 19, 21 skipped
+      x = 23       evaluated (voxels 22, 23 are empty -> transparent), x = 25 .. 31 evaluated (opaque)
+    => 11 samples evaluated, 5 skipped; an eager climb before every sample would have skipped x = 9 too."""
+    x = np.arange(32)
+    S = np.where((x < 8) | (x >= 24), 1, 0).astype(np.uint32).reshape(1, 1, 32)
+    tf = np.array([[0.3, 0.3, 0.3, 0.0], [0.9, 0.2, 0.1, 0.5]])
+    levels, pal = _direct_pyramid(S, tf)
+    v = _view(eye=np.array([-1.0, 0.5, 0.5]), tan_half_fov=1e-4, step_voxels=2.0, ess_threshold=1e-8)
+    img, (n_eval, n_skip) = oracle.render(levels, pal, v)
+    assert (n_eval, n_skip) == (11, 5)
+    img0, (e0, s0) = oracle.render(levels, pal, dict(v, ess_threshold=-1.0))
+    assert (e0, s0) == (16, 0)
+    np.testing.assert_allclose(img, img0, atol=1e-15)
