@@ -79,6 +79,25 @@ void mgb_default_params(mgb_params *p);
 int mgb_build(const uint32_t *seg, uint64_t X, uint64_t Y, uint64_t Z, const mgb_params *params,
               mgb_result **out);
 
+/*
+ * mgb_build_from_level1 -- mgb_build for a volume whose two finest levels were classified elsewhere (the device
+ * front end mg_mipmap_leaf_index / mg_mipmap_front_level1 of include/mg.h: level 0 is 87 % of the mipmap and the
+ * classification is a pure stream).  The result is identical to mgb_build on the same volume, except that the node
+ * index of level 0 is not stored: it is the leaf number, which the caller already has (mgb_get_node_idx(level 0)
+ * fails, mgb_node_idx_ptr returns NULL).
+ *   X, Y, Z          dimensions of level 0
+ *   leaf_segment_id  uint32[n_leaves] sorted distinct segment IDs present (Q14)
+ *   level1           uint32[X_1 Y_1 Z_1] (ceil-halved dims): the leaf number of every parent whose existing children
+ *                    are one segment, 0xFFFFFFFF for every other parent; may be NULL for a 1 x 1 x 1 volume
+ *   mixed_voxel      uint32[n_mixed] level-1 voxel index of every 0xFFFFFFFF parent, each exactly once, any order
+ *   mixed_children   uint32[n_mixed][8] leaf numbers of its existing children (2, 4 or 8 of them, Eq. 4 / Q2),
+ *                    0xFFFFFFFF for children outside the volume; their order does not matter
+ * Errors: MGB_ERR_INVALID_ARG when the three arrays are inconsistent.
+ */
+int mgb_build_from_level1(uint64_t X, uint64_t Y, uint64_t Z, const uint32_t *leaf_segment_id, uint32_t n_leaves,
+                          const uint32_t *level1, const uint32_t *mixed_voxel, const uint32_t *mixed_children,
+                          uint64_t n_mixed, const mgb_params *params, mgb_result **out);
+
 /* Build from explicit mixtures instead of a volume (tests, Fig. 2): mixture m has entries
  * [offsets[m], offsets[m+1]) of (leaf[], count[]) with strictly increasing leaf numbers < n_leaves
  * and positive integer counts (any scale).  The result has one "mip level" holding n_mixtures

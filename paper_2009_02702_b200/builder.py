@@ -19,7 +19,7 @@ lib = C.CDLL(LIB_PATH)
 MGB_OK = 0
 PICK_SMALLEST_INDEX, PICK_SMALLEST_MASS = 0, 1
 
-SYMBOLS = ["mgb_default_params", "mgb_build", "mgb_build_from_mixtures", "mgb_free", "mgb_get_info",
+SYMBOLS = ["mgb_default_params", "mgb_build", "mgb_build_from_level1", "mgb_build_from_mixtures", "mgb_free", "mgb_get_info",
            "mgb_mip_dims", "mgb_get_graph", "mgb_node_idx_ptr", "mgb_get_node_idx", "mgb_get_codebook",
            "mgb_get_weight_sigma", "mgb_last_error"]
 
@@ -59,6 +59,9 @@ lib.mgb_node_idx_ptr.argtypes = [_vp, C.c_uint32]
 lib.mgb_node_idx_ptr.restype = _vp
 lib.mgb_get_node_idx.argtypes = [_vp, C.c_uint32, _vp]
 lib.mgb_get_node_idx.restype = C.c_int
+lib.mgb_build_from_level1.argtypes = [C.c_uint64, C.c_uint64, C.c_uint64, _vp, C.c_uint32, _vp, _vp, _vp, C.c_uint64,
+                                      C.POINTER(Params), C.POINTER(_vp)]
+lib.mgb_build_from_level1.restype = C.c_int
 lib.mgb_get_weight_sigma.argtypes = [_vp, _vp]
 lib.mgb_get_weight_sigma.restype = C.c_int
 lib.mgb_get_codebook.argtypes = [_vp, _vp, _vp, _vp]
@@ -158,6 +161,29 @@ def build(seg: np.ndarray, params: Params | None = None, **overrides) -> Result:
     h = _vp()
     Z, Y, X = seg.shape
     _check(lib.mgb_build(seg.ctypes.data, X, Y, Z, C.byref(p), C.byref(h)), "mgb_build")
+    return Result(h)
+
+
+def build_from_level1(dims_xyz, leaf_segment_id, level1, mixed_voxel, mixed_children, params: Params | None = None,
+                      **overrides) -> Result:
+    """Build from levels 0 / 1 classified by a front end (mg.mipmap_leaf_index + mg.mipmap_front_level1, or any
+    equivalent): ``level1`` uint32 [Z_1, Y_1, X_1] (leaf number of a pure parent, 0xFFFFFFFF otherwise),
+    ``mixed_voxel`` uint32 [n], ``mixed_children`` uint32 [n, 8].  Level 0's node index is not stored."""
+    X, Y, Z = (int(d) for d in dims_xyz)
+    ids = np.ascontiguousarray(leaf_segment_id, dtype=np.uint32)
+    l1 = np.ascontiguousarray(level1, dtype=np.uint32).reshape(-1)
+    mv = np.ascontiguousarray(mixed_voxel, dtype=np.uint32).reshape(-1)
+    mc = np.ascontiguousarray(mixed_children, dtype=np.uint32).reshape(-1, 8)
+    if mc.shape[0] != mv.size:
+        raise ValueError("mixed_children must be [n_mixed, 8]")
+    n1 = -(-X // 2) * -(-Y // 2) * -(-Z // 2)
+    if (X, Y, Z) != (1, 1, 1) and l1.size != n1:
+        raise ValueError(f"level1 must have {n1} voxels")
+    p = params if params is not None else default_params(**overrides)
+    h = _vp()
+    _check(lib.mgb_build_from_level1(X, Y, Z, ids.ctypes.data, ids.size, l1.ctypes.data if l1.size else None,
+                                     mv.ctypes.data if mv.size else None, mc.ctypes.data if mv.size else None, mv.size,
+                                     C.byref(p), C.byref(h)), "mgb_build_from_level1")
     return Result(h)
 
 

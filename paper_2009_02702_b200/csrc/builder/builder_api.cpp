@@ -169,13 +169,14 @@ extern "C" void mgb_default_params(mgb_params* p)
 
 extern "C" void mgb_free(mgb_result* r) { delete r; }
 
-extern "C" int mgb_build(const uint32_t* seg, uint64_t X, uint64_t Y, uint64_t Z, const mgb_params* params,
-                         mgb_result** out)
+// a0 - a2 for a volume: from the segment IDs (front == nullptr), or from levels 0 / 1 classified by a front end.
+static int build_volume(const uint32_t* seg, uint64_t X, uint64_t Y, uint64_t Z, const Level1Front* front,
+                        const mgb_params* params, mgb_result** out)
 {
     g_err[0] = 0;
     if (!out) { set_error("mgb_build: out is NULL"); return MGB_ERR_INVALID_ARG; }
     *out = nullptr;
-    if (!seg || X == 0 || Y == 0 || Z == 0) { set_error("mgb_build: NULL volume or zero dimension"); return MGB_ERR_INVALID_ARG; }
+    if ((!seg && !front) || X == 0 || Y == 0 || Z == 0) { set_error("mgb_build: NULL volume or zero dimension"); return MGB_ERR_INVALID_ARG; }
     if (X > 0x7fffffffull || Y > 0x7fffffffull || Z > 0x7fffffffull || X * Y * Z >= (1ull << 40)) {
         set_error("mgb_build: volume too large"); return MGB_ERR_INVALID_ARG;
     }
@@ -187,7 +188,7 @@ extern "C" int mgb_build(const uint32_t* seg, uint64_t X, uint64_t Y, uint64_t Z
         R = new mgb_result();
         const double t0 = now_s();
         Mipmap mm;
-        rc = build_mipmap(seg, X, Y, Z, (int)p.n_threads, mm);
+        rc = build_mipmap(seg, X, Y, Z, (int)p.n_threads, mm, front);
         if (rc != MGB_OK) { delete R; return rc; }
         const double t1 = now_s();
         Factorised F;
@@ -205,7 +206,7 @@ extern "C" int mgb_build(const uint32_t* seg, uint64_t X, uint64_t Y, uint64_t Z
         for (uint32_t l = 0; l < n_mip; l++) {
             std::vector<uint32_t>& ids = mm.level_ids[l];
             const int64_t nv = (int64_t)ids.size();
-            n_vox_total += (uint64_t)nv;
+            n_vox_total += (l == 0 && front) ? X * Y * Z : (uint64_t)nv;      // with a front end level 0 stays with the caller
             uint32_t* P = ids.data();
             const uint32_t* nom = F.node_of_mix.data();
             const uint32_t* perm = new_of_old.data();
@@ -238,6 +239,40 @@ extern "C" int mgb_build(const uint32_t* seg, uint64_t X, uint64_t Y, uint64_t Z
     }
     *out = R;
     return MGB_OK;
+}
+
+extern "C" int mgb_build(const uint32_t* seg, uint64_t X, uint64_t Y, uint64_t Z, const mgb_params* params,
+                         mgb_result** out)
+{
+    return build_volume(seg, X, Y, Z, nullptr, params, out);
+}
+
+extern "C" int mgb_build_from_level1(uint64_t X, uint64_t Y, uint64_t Z, const uint32_t* leaf_segment_id, uint32_t n_leaves,
+                                     const uint32_t* level1, const uint32_t* mixed_voxel, const uint32_t* mixed_children,
+                                     uint64_t n_mixed, const mgb_params* params, mgb_result** out)
+{
+    if (!leaf_segment_id || n_leaves == 0 || (n_mixed && (!mixed_voxel || !mixed_children))) {
+        g_err[0] = 0;
+        set_error("mgb_build_from_level1: NULL argument or no leaves");
+        if (out) *out = nullptr;
+        return MGB_ERR_INVALID_ARG;
+    }
+    const bool has_level1 = !(X == 1 && Y == 1 && Z == 1);
+    if (has_level1 && !level1) {
+        g_err[0] = 0;
+        set_error("mgb_build_from_level1: level1 is NULL");
+        if (out) *out = nullptr;
+        return MGB_ERR_INVALID_ARG;
+    }
+    for (uint32_t k = 1; k < n_leaves; k++)
+        if (leaf_segment_id[k] <= leaf_segment_id[k - 1]) {
+            g_err[0] = 0;
+            set_error("mgb_build_from_level1: leaf_segment_id must be strictly increasing");
+            if (out) *out = nullptr;
+            return MGB_ERR_INVALID_ARG;
+        }
+    Level1Front front{leaf_segment_id, n_leaves, level1, mixed_voxel, mixed_children, n_mixed};
+    return build_volume(nullptr, X, Y, Z, &front, params, out);
 }
 
 extern "C" int mgb_build_from_mixtures(uint32_t n_leaves, uint64_t n_mixtures, const uint64_t* offsets,
@@ -353,12 +388,14 @@ extern "C" int mgb_get_graph(const mgb_result* r, uint32_t* child_a, uint32_t* c
 extern "C" const uint32_t* mgb_node_idx_ptr(const mgb_result* r, uint32_t level)
 {
     if (!r || level >= r->node_idx.size()) { set_error("mgb_node_idx_ptr: bad level"); return nullptr; }
+    if (r->node_idx[level].empty()) { set_error("mgb_node_idx_ptr: level %u is not stored (mgb_build_from_level1: level 0 = leaf numbers)", level); return nullptr; }
     return r->node_idx[level].data();
 }
 
 extern "C" int mgb_get_node_idx(const mgb_result* r, uint32_t level, uint32_t* out)
 {
     if (!r || !out || level >= r->node_idx.size()) { set_error("mgb_get_node_idx: bad argument"); return MGB_ERR_INVALID_ARG; }
+    if (r->node_idx[level].empty()) { set_error("mgb_get_node_idx: level %u is not stored (mgb_build_from_level1: level 0 = leaf numbers)", level); return MGB_ERR_INVALID_ARG; }
     memcpy(out, r->node_idx[level].data(), r->node_idx[level].size() * sizeof(uint32_t));
     return MGB_OK;
 }

@@ -53,7 +53,19 @@ struct Mipmap {
     MixtureSet mixtures;
 };
 
-int build_mipmap(const uint32_t* seg, uint64_t X, uint64_t Y, uint64_t Z, int n_threads, Mipmap& out);
+// Levels 0 and 1 classified outside the host builder (mgb_build_from_level1): level 0 is not passed at all.
+struct Level1Front {
+    const uint32_t* leaf_segment_id;   // [n_leaves] sorted distinct segment IDs
+    uint32_t n_leaves;
+    const uint32_t* level1;            // [X_1 Y_1 Z_1] leaf number of a pure parent, 0xFFFFFFFF otherwise
+    const uint32_t* mixed_voxel;       // [n_mixed] level-1 voxel index of every non-pure parent (any order)
+    const uint32_t* mixed_children;    // [n_mixed][8] leaf numbers of its existing children, 0xFFFFFFFF = missing
+    uint64_t n_mixed;
+};
+
+// With `front`, seg is not read and out.level_ids[0] stays empty.
+int build_mipmap(const uint32_t* seg, uint64_t X, uint64_t Y, uint64_t Z, int n_threads, Mipmap& out,
+                 const Level1Front* front = nullptr);
 
 }  // namespace mgb
 

@@ -166,6 +166,52 @@ struct Table {
     }
 };
 
+// The mixture of a parent whose n existing children (handles ch[]) are not all equal: merge them with weight
+// 1/N each (Eq. 4), reduce, hash-cons.  Returns the parent's handle (a leaf number if the merge is pure, else a
+// table handle; 0 with table.failed set on failure) and adds the mixture's non-zeros to nnz.
+uint32_t merge_children(Table& table, const uint32_t* ch, int n, uint32_t l, uint64_t voxel, std::vector<Entry>& buf,
+                        std::vector<Entry>& merged, uint64_t& nnz)
+{
+    // common scale 2^tmax, each child weighs 1/N
+    uint32_t tmax = 0;
+    for (int q = 0; q < n; q++)
+        if (ch[q] & kMixed) tmax = std::max(tmax, table.rec(ch[q]).tlog);
+    buf.clear();
+    for (int q = 0; q < n; q++) {
+        if (ch[q] & kMixed) {
+            const Rec& rc = table.rec(ch[q]);
+            for (uint32_t t = 0; t < rc.k; t++)
+                buf.push_back(Entry{rc.data[t].leaf, 0, rc.data[t].count << (tmax - rc.tlog)});
+        } else {
+            buf.push_back(Entry{ch[q], 0, 1ull << tmax});
+        }
+    }
+    if (buf.size() <= 24) {
+        for (size_t a = 1; a < buf.size(); a++) {
+            Entry e = buf[a];
+            size_t b = a;
+            while (b > 0 && buf[b - 1].leaf > e.leaf) { buf[b] = buf[b - 1]; b--; }
+            buf[b] = e;
+        }
+    } else {
+        std::sort(buf.begin(), buf.end(), [](const Entry& a, const Entry& b) { return a.leaf < b.leaf; });
+    }
+    merged.clear();
+    for (const Entry& e : buf) {
+        if (!merged.empty() && merged.back().leaf == e.leaf) merged.back().count += e.count;
+        else merged.push_back(e);
+    }
+    int tz = 64;
+    for (const Entry& e : merged) tz = std::min(tz, __builtin_ctzll(e.count));
+    for (Entry& e : merged) e.count >>= tz;
+    const uint32_t nlog = (n == 8) ? 3 : (n == 4) ? 2 : (n == 2) ? 1 : 0;   // N is 1, 2, 4 or 8
+    const uint32_t tlog = tmax + nlog - (uint32_t)tz;
+    const uint64_t pos = ((uint64_t)l << 40) | voxel;
+    nnz += merged.size();
+    if (merged.size() == 1) return merged[0].leaf;
+    return table.intern(merged.data(), (uint32_t)merged.size(), tlog, pos);
+}
+
 // Sorted distinct IDs present (every one becomes a leaf, background included: Q14) and ids0 = leaf number.
 int index_leaves(const uint32_t* seg, uint64_t n, std::vector<uint32_t>& ids, std::vector<uint32_t>& ids0)
 {
@@ -211,7 +257,7 @@ int index_leaves(const uint32_t* seg, uint64_t n, std::vector<uint32_t>& ids, st
 
 }  // namespace
 
-int build_mipmap(const uint32_t* seg, uint64_t X, uint64_t Y, uint64_t Z, int n_threads, Mipmap& out)
+int build_mipmap(const uint32_t* seg, uint64_t X, uint64_t Y, uint64_t Z, int n_threads, Mipmap& out, const Level1Front* front)
 {
     if (n_threads > 0) omp_set_num_threads(n_threads);
     // ---- O-1 / L80: dims, ceil-halved down to 1^3
@@ -223,12 +269,56 @@ int build_mipmap(const uint32_t* seg, uint64_t X, uint64_t Y, uint64_t Z, int n_
     }
     const uint32_t n_levels = (uint32_t)(out.dims.size() / 3);
     out.level_ids.assign(n_levels, {});
-    index_leaves(seg, X * Y * Z, out.leaf_segment_id, out.level_ids[0]);   // level 0: H = e_S (Eq. 4, first line)
+    if (!front) index_leaves(seg, X * Y * Z, out.leaf_segment_id, out.level_ids[0]);   // level 0: H = e_S (Eq. 4, first line)
+    else out.leaf_segment_id.assign(front->leaf_segment_id, front->leaf_segment_id + front->n_leaves);
     const uint32_t n_leaves = (uint32_t)out.leaf_segment_id.size();
     uint64_t nnz_total = X * Y * Z;
 
     Table table;
-    for (uint32_t l = 1; l < n_levels; l++) {
+    uint32_t first_level = 1;
+    if (front && n_levels > 1) {
+        // Levels 0 and 1 were classified elsewhere (the device front end): level 0 stays with the caller, the pure
+        // parents of level 1 already hold their leaf, the others come as a list of (voxel, existing children).
+        const uint64_t n1 = out.dims[3] * out.dims[4] * out.dims[5];
+        out.level_ids[1].assign(front->level1, front->level1 + n1);
+        uint32_t* P = out.level_ids[1].data();
+        uint64_t nnz_level = n1 - front->n_mixed, n_marked = 0;
+        for (uint64_t v = 0; v < n1; v++) n_marked += (P[v] == 0xFFFFFFFFu);
+        if (n_marked != front->n_mixed) {
+            set_error("histogram mipmap: level 1 marks %llu parents as not pure, the list has %llu", (unsigned long long)n_marked,
+                      (unsigned long long)front->n_mixed);
+            return MGB_ERR_INVALID_ARG;
+        }
+        bool bad = false;
+#pragma omp parallel reduction(+ : nnz_level)
+        {
+            std::vector<Entry> buf, merged;
+#pragma omp for schedule(dynamic, 1024)
+            for (int64_t q = 0; q < (int64_t)front->n_mixed; q++) {
+                const uint64_t v = front->mixed_voxel[q];
+                uint32_t ch[8];
+                int n = 0;
+                for (int t = 0; t < 8; t++) {
+                    const uint32_t c = front->mixed_children[8 * q + t];
+                    if (c != 0xFFFFFFFFu) ch[n++] = c;
+                }
+                bool ok = v < n1 && P[v] == 0xFFFFFFFFu && (n == 2 || n == 4 || n == 8);
+                for (int t = 0; t < n; t++) ok = ok && ch[t] < n_leaves;
+                if (!ok) { bad = true; continue; }
+                P[v] = merge_children(table, ch, n, 1, v, buf, merged, nnz_level);
+            }
+        }
+        if (bad) { set_error("histogram mipmap: inconsistent level-1 front end (voxel, child count or leaf out of range)"); return MGB_ERR_INVALID_ARG; }
+        if (table.failed) { set_error("histogram mipmap: mixture table full or out of memory at level 1"); return MGB_ERR_LIMIT; }
+        for (uint64_t v = 0; v < n1; v++)
+            if (P[v] == 0xFFFFFFFFu || (!(P[v] & kMixed) && P[v] >= n_leaves)) {
+                set_error("histogram mipmap: level-1 voxel %llu is neither a leaf nor in the mixed list", (unsigned long long)v);
+                return MGB_ERR_INVALID_ARG;
+            }
+        nnz_total += nnz_level;
+        first_level = 2;
+    }
+    for (uint32_t l = first_level; l < n_levels; l++) {
         const uint64_t cx = out.dims[3 * l - 3], cy = out.dims[3 * l - 2], cz = out.dims[3 * l - 1];
         const uint64_t px = out.dims[3 * l], py = out.dims[3 * l + 1], pz = out.dims[3 * l + 2];
         out.level_ids[l].resize(px * py * pz);
@@ -261,46 +351,7 @@ int build_mipmap(const uint32_t* seg, uint64_t X, uint64_t Y, uint64_t Z, int n_
                         nnz_level += (ch[0] & kMixed) ? table.rec(ch[0]).k : 1;
                         continue;
                     }
-                    // merge the children: common scale 2^tmax, each child weighs 1/N
-                    uint32_t tmax = 0;
-                    for (int q = 0; q < n; q++)
-                        if (ch[q] & kMixed) tmax = std::max(tmax, table.rec(ch[q]).tlog);
-                    buf.clear();
-                    for (int q = 0; q < n; q++) {
-                        if (ch[q] & kMixed) {
-                            const Rec& rc = table.rec(ch[q]);
-                            for (uint32_t t = 0; t < rc.k; t++)
-                                buf.push_back(Entry{rc.data[t].leaf, 0, rc.data[t].count << (tmax - rc.tlog)});
-                        } else {
-                            buf.push_back(Entry{ch[q], 0, 1ull << tmax});
-                        }
-                    }
-                    if (buf.size() <= 24) {
-                        for (size_t a = 1; a < buf.size(); a++) {
-                            Entry e = buf[a];
-                            size_t b = a;
-                            while (b > 0 && buf[b - 1].leaf > e.leaf) { buf[b] = buf[b - 1]; b--; }
-                            buf[b] = e;
-                        }
-                    } else {
-                        std::sort(buf.begin(), buf.end(), [](const Entry& a, const Entry& b) { return a.leaf < b.leaf; });
-                    }
-                    merged.clear();
-                    for (const Entry& e : buf) {
-                        if (!merged.empty() && merged.back().leaf == e.leaf) merged.back().count += e.count;
-                        else merged.push_back(e);
-                    }
-                    int tz = 64;
-                    for (const Entry& e : merged) tz = std::min(tz, __builtin_ctzll(e.count));
-                    for (Entry& e : merged) e.count >>= tz;
-                    const uint32_t nlog = (n == 8) ? 3 : (n == 4) ? 2 : (n == 2) ? 1 : 0;   // N is 1, 2, 4 or 8
-                    const uint32_t tlog = tmax + nlog - (uint32_t)tz;
-                    const uint64_t pos = ((uint64_t)l << 40) | ((uint64_t)r * px + i);
-                    uint32_t id;
-                    if (merged.size() == 1) id = merged[0].leaf;
-                    else id = table.intern(merged.data(), (uint32_t)merged.size(), tlog, pos);
-                    P[(uint64_t)r * px + i] = id;
-                    nnz_level += merged.size();
+                    P[(uint64_t)r * px + i] = merge_children(table, ch, n, l, (uint64_t)r * px + i, buf, merged, nnz_level);
                 }
             }
         }

@@ -194,3 +194,60 @@ def test_error_paths():
         builder.build_from_mixtures(2, [[(0, 1), (5, 1)]])          # leaf out of range
     for name in builder.SYMBOLS:
         getattr(builder.lib, name)
+
+
+def _front_end_numpy(seg):
+    """Plain numpy statement of what the device front end computes (levels 0 and 1 of Eq. 4, pure / not pure):
+    leaf numbers of level 0; per level-1 parent the leaf of its existing children if they agree, else 0xFFFFFFFF
+    plus the list (voxel, 8 children with 0xFFFFFFFF for children outside the volume)."""
+    ids, l0 = oracle.leaf_index(seg)
+    Z, Y, X = l0.shape
+    pz, py, px = -(-Z // 2), -(-Y // 2), -(-X // 2)
+    pad = np.full((2 * pz, 2 * py, 2 * px), 0xFFFFFFFF, dtype=np.uint32)
+    pad[:Z, :Y, :X] = l0
+    ch = pad.reshape(pz, 2, py, 2, px, 2).transpose(0, 2, 4, 1, 3, 5).reshape(pz, py, px, 8)
+    exists = ch != 0xFFFFFFFF
+    first = ch[..., 0]                                              # child (0,0,0) always exists
+    pure = ((ch == first[..., None]) | ~exists).all(axis=-1)
+    level1 = np.where(pure, first, 0xFFFFFFFF).astype(np.uint32)
+    mixed = np.flatnonzero(~pure.reshape(-1)).astype(np.uint32)
+    return ids, l0, level1, mixed, ch.reshape(-1, 8)[mixed]
+
+
+@pytest.mark.parametrize("dims,n_seg,bits", [((32, 32, 32), 9, 9), ((37, 29, 23), 12, 9), ((5, 1, 9), 4, 0), ((2, 2, 2), 3, 9)])
+def test_build_from_level1_is_identical_to_build(dims, n_seg, bits):
+    seg = synth.voronoi_volume(dims, synth.voronoi_seeds(dims, n_seg, 61))
+    ids, l0, level1, mixed, children = _front_end_numpy(seg)
+    rng_order = np.argsort(synth.u64(61, 1, np.arange(mixed.size, dtype=np.uint64)))          # any order is allowed
+    a = builder.build(seg, quant_bits=bits)
+    b = builder.build_from_level1(dims, ids, level1, mixed[rng_order], children[rng_order], quant_bits=bits)
+    ga, gb = a.graph(), b.graph()
+    for k in ("child_a", "child_b", "weight", "weight_exact", "weight_sigma", "level_offsets", "leaf_segment_id"):
+        assert np.array_equal(ga[k], gb[k]), k
+    assert a.mip_dims == b.mip_dims
+    for f in ("n_nodes", "n_leaves", "depth", "n_mip_levels", "n_voxels_total", "n_distinct_mixtures", "nnz_total"):
+        assert getattr(a.info, f) == getattr(b.info, f), f
+    assert np.array_equal(a.node_idx(0), l0)                      # level 0 IS the leaf number (what the caller keeps)
+    with pytest.raises(builder.BuilderError):
+        b.node_idx(0)
+    for l in range(1, a.info.n_mip_levels):
+        assert np.array_equal(a.node_idx(l), b.node_idx(l)), l
+
+
+def test_build_from_level1_rejects_inconsistent_input():
+    dims = (8, 8, 8)
+    seg = synth.voronoi_volume(dims, synth.voronoi_seeds(dims, 5, 62))
+    ids, l0, level1, mixed, children = _front_end_numpy(seg)
+    assert mixed.size > 2
+    with pytest.raises(builder.BuilderError):                                    # a mixed parent missing from the list
+        builder.build_from_level1(dims, ids, level1, mixed[1:], children[1:])
+    with pytest.raises(builder.BuilderError):                                    # the same parent twice
+        builder.build_from_level1(dims, ids, level1, np.r_[mixed, mixed[:1]], np.r_[children, children[:1]])
+    bad = children.copy()
+    bad[0, 0] = ids.size                                                         # leaf out of range
+    with pytest.raises(builder.BuilderError):
+        builder.build_from_level1(dims, ids, level1, mixed, bad)
+    with pytest.raises(builder.BuilderError):                                    # IDs not increasing
+        builder.build_from_level1(dims, ids[::-1], level1, mixed, children)
+    with pytest.raises(ValueError):
+        builder.build_from_level1(dims, ids, level1[:-1], mixed, children)
