@@ -48,6 +48,8 @@ def parse_args():
     p.add_argument("--no-cpu-baseline", action="store_true")
     p.add_argument("--no-e2e", action="store_true")
     p.add_argument("--no-attr", action="store_true", help="skip the extra NEXT-1 measurement (multi-attribute propagation)")
+    p.add_argument("--device-mipmap", action="store_true",
+                   help="configs 1-4: classify the two finest mip levels on the device (NEXT-4 front end) instead of on the host")
     p.add_argument("--relabel", action="store_true", help="config 5: load the DAG with MG_RELABEL (levels sorted by children)")
     p.add_argument("--no-query", action="store_true", help="skip the extra NEXT-4 measurement (mixture LUT + range queries)")
     p.add_argument("--no-render", action="store_true", help="skip the extra NEXT-2 measurement (ray-marcher over the paletted mipmap)")
@@ -131,10 +133,11 @@ def oracle_step(w, tf64, plan, chunk: int = 1 << 25):
     """One TF update by the oracle on a sample: (propagate seconds, colourise seconds, threads)."""
     import oracle
     g = w.host_graph
+    levels = [w.host_level(l) for l in range(len(plan))]           # (a download when level 0 only lives on the device)
     t0 = time.perf_counter()
     c, used = oracle.graph_eval_levels(g["child_a"], g["child_b"], g["weight"], g["n_leaves"], tf64, n_threads=0)
     t1 = time.perf_counter()
-    for lvl, n in zip(w.host_idx, plan):
+    for lvl, n in zip(levels, plan):
         flat = lvl.reshape(-1)
         for o in range(0, n, chunk):
             oracle.colourise_rgba8(flat[o:min(n, o + chunk)], c, n_threads=0)
@@ -228,7 +231,7 @@ def run_b200(args) -> dict:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
     from paper_2009_02702_b200 import mg, workload
 
-    w = workload.make(args.config, args.scale, relabel=args.relabel)
+    w = workload.make(args.config, args.scale, relabel=args.relabel, device_mipmap=args.device_mipmap and args.config != 5)
     g = w.graph
     info = g.info
     n_nodes, n_internal = int(info.n_nodes), int(info.n_internal)

@@ -370,6 +370,36 @@ int mg_range_query(mg_mixture_lut *lut, const uint32_t *node_idx_mipmap, const m
                    const uint64_t *boxes, uint32_t n_queries, double *expect, double *err,
                    uint64_t *fetches, uint32_t mode, void *stream);
 
+/* ------------------------------------------------------------------------------------------------
+ * NEXT-4 (second half): device front end of the histogram mipmap (a0; Eq. 4).
+ * The two finest levels hold 98 % of the mipmap's voxels and almost all of them are pure (Table 2);
+ * classifying them is a stream over the volume.  These two calls do that on the device; the host builder
+ * continues from their output (mgb_build_from_level1 of include/mg_builder.h) and produces the same graph and
+ * node indices as mgb_build on the same volume.  Both calls allocate small temporaries and synchronise `stream`.
+ * ------------------------------------------------------------------------------------------------ */
+
+/* Level 0: H(., 0) = e_S (Eq. 4).  The sorted distinct segment IDs present in the volume become the leaves
+ * (reading Q14: background is an ordinary segment).
+ *   seg_device        DEVICE uint32[n_voxels] segment IDs (all < 2^28, else MG_ERR_INVALID_ARG: use mgb_build)
+ *   level0_device     DEVICE uint32[n_voxels] receives the leaf number of every voxel; may be seg_device itself
+ *   leaf_segment_id   HOST uint32[capacity] receives the sorted distinct IDs
+ *   n_leaves          HOST: their number (also set when it exceeds capacity, which is MG_ERR_INVALID_ARG) */
+int mg_mipmap_leaf_index(const uint32_t *seg_device, uint64_t n_voxels, uint32_t *level0_device,
+                         uint32_t *leaf_segment_id, uint32_t capacity, uint32_t *n_leaves, void *stream);
+
+/* Level 1: H(i, j, k, 1) = the average of the existing children (Eq. 4, reading Q2).  A parent whose existing
+ * children are one leaf is that leaf; every other parent is listed with its children for the host builder.
+ *   level0_device          DEVICE uint32[Z][Y][X] leaf numbers (x fastest)
+ *   level1_device          DEVICE uint32[ceil(Z/2)][ceil(Y/2)][ceil(X/2)]: the leaf, or 0xFFFFFFFF for a listed parent
+ *   mixed_voxel_device     DEVICE uint32[capacity]: level-1 voxel index of each listed parent (order unspecified)
+ *   mixed_children_device  DEVICE uint32[capacity][8], 16-byte aligned: its children at [4 dz + 2 dy + dx],
+ *                          0xFFFFFFFF for a child outside the volume
+ *   n_mixed                HOST: number of listed parents; entries beyond `capacity` are dropped, so a caller seeing
+ *                          n_mixed > capacity calls again with larger lists (level1_device is complete either way) */
+int mg_mipmap_front_level1(const uint32_t *level0_device, uint64_t X, uint64_t Y, uint64_t Z,
+                           uint32_t *level1_device, uint32_t *mixed_voxel_device, uint32_t *mixed_children_device,
+                           uint64_t capacity, uint64_t *n_mixed, void *stream);
+
 /* Thread-local description of the last error returned on this thread ("" if none). */
 const char *mg_last_error(void);
 

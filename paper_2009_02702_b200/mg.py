@@ -30,7 +30,8 @@ SYMBOLS = ["mg_load_graph", "mg_free_graph", "mg_graph_info", "mg_level_offsets"
            "mg_last_error", "mg_kernel_launch_count",
            "mg_bits_per_voxel", "mg_packed_stream_bytes", "mg_index_range", "mg_pack_indices", "mg_colorize_packed",
            "mg_propagate_attr", "mg_render",
-           "mg_mixture_lut_build", "mg_mixture_lut_free", "mg_mixture_lut_info", "mg_mixture_lut_export", "mg_range_query"]
+           "mg_mixture_lut_build", "mg_mixture_lut_free", "mg_mixture_lut_info", "mg_mixture_lut_export", "mg_range_query",
+           "mg_mipmap_leaf_index", "mg_mipmap_front_level1"]
 
 
 class MgInfo(C.Structure):
@@ -128,6 +129,13 @@ lib.mg_range_query.argtypes = [_vp, _vp, C.POINTER(MgMipmapDesc), _vp, C.c_uint3
 lib.mg_range_query.restype = C.c_int
 
 
+lib.mg_mipmap_leaf_index.argtypes = [_vp, C.c_uint64, _vp, _vp, C.c_uint32, C.POINTER(C.c_uint32), _vp]
+lib.mg_mipmap_leaf_index.restype = C.c_int
+lib.mg_mipmap_front_level1.argtypes = [_vp, C.c_uint64, C.c_uint64, C.c_uint64, _vp, _vp, _vp, C.c_uint64,
+                                       C.POINTER(C.c_uint64), _vp]
+lib.mg_mipmap_front_level1.restype = C.c_int
+
+
 class MgError(RuntimeError):
     def __init__(self, code: int, where: str):
         self.code = code
@@ -185,6 +193,27 @@ def packed_levels(levels) -> "C.Array":
             l = (l["n_voxels"], l["out_offset"], l["byte_offset"], l["bits"], l["i_min"])
         arr[i] = MgPackedLevel(*[int(x) for x in l])
     return arr
+
+
+def mipmap_leaf_index(seg_device, n_voxels: int, level0_device, capacity: int = 1 << 20, stream: int = 0) -> np.ndarray:
+    """NEXT-4 front end, level 0: writes leaf numbers to level0_device, returns the sorted distinct segment IDs."""
+    ids = np.zeros(int(capacity), dtype=np.uint32)
+    n = C.c_uint32(0)
+    _check(lib.mg_mipmap_leaf_index(_ptr(seg_device), int(n_voxels), _ptr(level0_device), ids.ctypes.data, int(capacity),
+                                    C.byref(n), stream or None), "mg_mipmap_leaf_index")
+    return ids[:n.value].copy()
+
+
+def mipmap_front_level1(level0_device, dims_xyz, level1_device, mixed_voxel_device, mixed_children_device, capacity: int,
+                        stream: int = 0) -> int:
+    """NEXT-4 front end, level 1: fills level1_device and the list of non-pure parents; returns their number
+    (entries beyond ``capacity`` are dropped: call again with larger lists if it is exceeded)."""
+    n = C.c_uint64(0)
+    X, Y, Z = (int(d) for d in dims_xyz)
+    _check(lib.mg_mipmap_front_level1(_ptr(level0_device), X, Y, Z, _ptr(level1_device), _ptr(mixed_voxel_device),
+                                      _ptr(mixed_children_device), int(capacity), C.byref(n), stream or None),
+           "mg_mipmap_front_level1")
+    return int(n.value)
 
 
 def mipmap_desc(level_offsets, level_dims_xyz) -> MgMipmapDesc:

@@ -52,6 +52,13 @@ class Workload:
         return synth.random_tf(self.n_leaves, c.get("seed", 0), update=update,
                                alpha_zero_frac=c.get("alpha_zero_frac", 0.0))
 
+    def host_level(self, l: int) -> np.ndarray:
+        """Node indices of mip level ``l`` on the host, flat uint32 (downloaded when the host never had them)."""
+        if self.host_idx is not None and self.host_idx[l] is not None:
+            return self.host_idx[l].reshape(-1)
+        s = self.level_start[l]
+        return self.d_idx[s:s + self.level_voxels[l]].cpu().numpy().view(np.uint32)
+
     def mip_desc(self) -> "mg.MgMipmapDesc":
         """The mg_mipmap_desc of the concatenated device mipmap (input of mg_render)."""
         return mg.mipmap_desc(self.level_start, self.mip_dims)
@@ -152,6 +159,74 @@ def from_volume(seg: np.ndarray, name: str = "volume", cfg: dict | None = None, 
     return w
 
 
+def from_volume_device(seg_dev, name: str = "volume", cfg: dict | None = None, **builder_params) -> Workload:
+    """The same assembly as ``from_volume`` for a segment-ID volume that is ALREADY ON THE DEVICE (torch int32
+    [Z, Y, X], uint32 values): the two finest mip levels are classified by the device front end
+    (mg_mipmap_leaf_index / mg_mipmap_front_level1, writing level 0's node indices straight into the mipmap
+    buffer), the host builder continues from the list of non-pure level-1 parents (mgb_build_from_level1), and
+    only the levels >= 1 are uploaded.  Same graph and same node indices as ``from_volume`` on the same volume;
+    ``host_idx[0]`` is None (level 0 never exists on the host; ``host_level(0)`` downloads it)."""
+    import torch
+    w = Workload(name)
+    w.cfg = dict(cfg or {})
+    Z, Y, X = (int(d) for d in seg_dev.shape)
+    dims, d = [], (X, Y, Z)
+    while True:
+        dims.append(d)
+        if d == (1, 1, 1):
+            break
+        d = tuple(-(-k // 2) for k in d)
+    w.mip_dims = dims
+    w.level_voxels = [a * b * c for a, b, c in dims]
+    w.level_start, w.n_voxels_padded = _layout(w.level_voxels)
+    w.n_voxels = sum(w.level_voxels)
+    st = torch.cuda.current_stream().cuda_stream
+    t0 = time.perf_counter()
+    w.d_idx = torch.zeros(w.n_voxels_padded, dtype=torch.int32, device="cuda")
+    n0 = w.level_voxels[0]
+    ids = mg.mipmap_leaf_index(seg_dev, n0, w.d_idx[:n0], stream=st)
+    level1 = mixed_voxel = mixed_children = np.zeros(0, np.uint32)
+    if len(dims) > 1:
+        n1, s1 = w.level_voxels[1], w.level_start[1]
+        cap = max(1024, n1 // 16)
+        while True:
+            mv = torch.empty(cap, dtype=torch.int32, device="cuda")
+            mc = torch.empty((cap, 8), dtype=torch.int32, device="cuda")
+            n_mixed = mg.mipmap_front_level1(w.d_idx[:n0], dims[0], w.d_idx[s1:s1 + n1], mv, mc, cap, stream=st)
+            if n_mixed <= cap:
+                break
+            cap = n_mixed
+        level1 = w.d_idx[s1:s1 + n1].cpu().numpy().view(np.uint32)
+        mixed_voxel = mv[:n_mixed].cpu().numpy().view(np.uint32)
+        mixed_children = mc[:n_mixed].cpu().numpy().view(np.uint32)
+        del mv, mc
+    t1 = time.perf_counter()
+    r = builder.build_from_level1(dims[0], ids, level1, mixed_voxel, mixed_children, **builder_params)
+    t2 = time.perf_counter()
+    g = r.graph()
+    w.host_graph = g
+    w.n_leaves = g["n_leaves"]
+    assert r.mip_dims == dims
+    w.graph = mg.Graph(g["child_a"], g["child_b"], g["weight"], g["n_leaves"], level_offsets=g["level_offsets"],
+                       leaf_segment_id=g["leaf_segment_id"])
+    t3 = time.perf_counter()
+    w.host_idx = [None] + [r.node_idx(l, copy=False) for l in range(1, r.info.n_mip_levels)]
+    for s, a in zip(w.level_start[1:], w.host_idx[1:]):
+        w.d_idx[s:s + a.size].copy_(torch.from_numpy(a.reshape(-1).view(np.int32)))
+    torch.cuda.synchronize()
+    t4 = time.perf_counter()
+    i = r.info
+    w.stats = dict(front_end_s=t1 - t0, builder_s=t2 - t1, load_graph_s=t3 - t2, upload_idx_s=t4 - t3, n_nodes=int(i.n_nodes),
+                   n_leaves=int(i.n_leaves), depth=int(i.depth), quant_bits=int(i.quant_bits),
+                   n_distinct_mixtures=int(i.n_distinct_mixtures), nnz_per_voxel=i.nnz_total / max(1, i.n_voxels_total),
+                   n_mip_levels=int(i.n_mip_levels), builder_mipmap_s=i.seconds_mipmap,
+                   builder_factorise_s=i.seconds_factorise, builder_finalise_s=i.seconds_finalise,
+                   n_level1_mixed=int(mixed_voxel.size), device_mipmap=True,
+                   level_sizes=np.diff(g["level_offsets"].astype(np.int64)).tolist())
+    w.build_result = r
+    return w
+
+
 def from_dag(child_a, child_b, weight, level_offsets, n_leaves: int, node_idx: np.ndarray, name: str = "dag",
              cfg: dict | None = None, relabel: bool = False, load: bool = True) -> Workload:
     """A ready-made level-contiguous DAG plus ONE node-index volume (config 5).  ``relabel`` loads it with
@@ -187,7 +262,7 @@ def from_dag(child_a, child_b, weight, level_offsets, n_leaves: int, node_idx: n
 
 
 def make(cfg_id: int, scale: float = 1.0, device_synth: bool = True, keep_seg: bool = False,
-         relabel: bool = False, load: bool = True, **builder_params) -> Workload:
+         relabel: bool = False, load: bool = True, device_mipmap: bool = False, **builder_params) -> Workload:
     """BASELINE.json config ``cfg_id`` (1-5); ``scale`` < 1 gives a geometrically similar smaller
     instance (tests).  Volumes are generated on the GPU (bit-identical to synth.py) unless
     ``device_synth`` is False.  ``keep_seg`` keeps the generated volume in ``Workload.seg``."""
@@ -206,6 +281,19 @@ def make(cfg_id: int, scale: float = 1.0, device_synth: bool = True, keep_seg: b
         return w
     c = synth.scaled_config(cfg_id, scale)
     t0 = time.perf_counter()
+    if device_mipmap:
+        import torch
+        from . import synth_gpu
+        seg_dev = synth_gpu.make_volume(c)
+        torch.cuda.synchronize()
+        t1 = time.perf_counter()
+        w = from_volume_device(seg_dev, name=c["name"], cfg=c, **builder_params)
+        if keep_seg:
+            w.seg = seg_dev.cpu().numpy().view(np.uint32)
+        del seg_dev
+        torch.cuda.empty_cache()
+        w.stats["synth_s"] = t1 - t0
+        return w
     if device_synth:
         import torch
         from . import synth_gpu

@@ -1,0 +1,110 @@
+"""NEXT-4 (second half): the device front end of the histogram mipmap (mg_mipmap_leaf_index,
+mg_mipmap_front_level1) against the oracle's definitions, and the whole device-assisted assembly
+(workload.from_volume_device) against the host builder: bit-exact, everything here is integer work."""
+import numpy as np
+import pytest
+
+import oracle
+from paper_2009_02702_b200 import synth
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+NONE = 0xFFFFFFFF
+
+
+@pytest.fixture(scope="module")
+def libs():
+    if not torch.cuda.is_available():
+        pytest.fail("the gpu-marked tests need a CUDA device (no CPU fallback exists)")
+    from paper_2009_02702_b200 import mg, workload
+    torch.cuda.set_device(0)
+    return mg, workload
+
+
+def _dev(a):
+    return torch.from_numpy(np.ascontiguousarray(a).view(np.int32)).cuda()
+
+
+def _front(mg, seg, capacity=None, in_place=False):
+    Z, Y, X = seg.shape
+    d_seg = _dev(seg)
+    d_l0 = d_seg if in_place else torch.full_like(d_seg, -1)
+    ids = mg.mipmap_leaf_index(d_seg, seg.size, d_l0)
+    pz, py, px = -(-Z // 2), -(-Y // 2), -(-X // 2)
+    n1 = pz * py * px
+    cap = n1 if capacity is None else capacity
+    d_l1 = torch.full((n1,), 7, dtype=torch.int32, device="cuda")
+    mv = torch.full((max(cap, 1),), -1, dtype=torch.int32, device="cuda")
+    mc = torch.full((max(cap, 1), 8), -1, dtype=torch.int32, device="cuda")
+    n_mixed = mg.mipmap_front_level1(d_l0, (X, Y, Z), d_l1, mv, mc, cap)
+    u = lambda t: t.cpu().numpy().view(np.uint32)
+    return ids, u(d_l0).reshape(Z, Y, X), u(d_l1).reshape(pz, py, px), u(mv), u(mc), n_mixed
+
+
+@pytest.mark.parametrize("dims,n_seg", [((32, 32, 32), 9), ((37, 29, 23), 12), ((5, 1, 9), 4), ((1, 1, 1), 1), ((2, 1, 1), 2),
+                                        ((130, 67, 3), 40)])
+def test_front_end_matches_the_definition(libs, dims, n_seg):
+    mg, _ = libs
+    seg = synth.voronoi_volume(dims, synth.voronoi_seeds(dims, n_seg, 71)) * np.uint32(7) + np.uint32(3)    # sparse IDs (Q14)
+    ids, l0, l1, mv, mc, n_mixed = _front(mg, seg)
+    ref_ids, ref_l0 = oracle.leaf_index(seg)
+    assert np.array_equal(ids, ref_ids) and np.array_equal(l0, ref_l0)
+    # level 1 against the oracle's exact histograms (O-2): pure <=> one non-zero count
+    H = oracle.histogram_mipmap(ref_l0, ref_ids.size)
+    if len(H) > 1:
+        h1 = H[1]
+        nnz = (h1 != 0).sum(axis=-1)
+        leaf = h1.argmax(axis=-1).astype(np.uint32)
+        assert np.array_equal(l1 == NONE, nnz > 1)
+        assert np.array_equal(l1[nnz == 1], leaf[nnz == 1])
+        assert n_mixed == int((nnz > 1).sum())
+        order = np.argsort(mv[:n_mixed])
+        assert np.array_equal(mv[:n_mixed][order], np.flatnonzero((nnz > 1).reshape(-1)))        # each listed once
+        Z, Y, X = seg.shape
+        for q in order[:: max(1, n_mixed // 300)]:                                             # children of sampled parents
+            v = int(mv[q])
+            i, j, k = v % l1.shape[2], (v // l1.shape[2]) % l1.shape[1], v // (l1.shape[2] * l1.shape[1])
+            for t in range(8):
+                x, y, z = 2 * i + (t & 1), 2 * j + ((t >> 1) & 1), 2 * k + (t >> 2)
+                want = ref_l0[z, y, x] if (x < X and y < Y and z < Z) else NONE
+                assert mc[q, t] == want
+    else:
+        assert n_mixed == 0
+
+
+def test_front_end_in_place_and_small_capacity(libs):
+    mg, _ = libs
+    dims = (37, 29, 23)
+    seg = synth.voronoi_volume(dims, synth.voronoi_seeds(dims, 12, 72))
+    ids, l0, l1, mv, mc, n_mixed = _front(mg, seg)
+    ids2, l0b, l1b, mv2, mc2, n2 = _front(mg, seg, capacity=5, in_place=True)                 # level0 written over seg
+    assert np.array_equal(ids, ids2) and np.array_equal(l0, l0b) and np.array_equal(l1, l1b)
+    assert n2 == n_mixed > 5                                                                   # the true count is reported
+    assert set(mv2[:5].tolist()) <= set(mv[:n_mixed].tolist())
+    with pytest.raises(mg.MgError):
+        mg.mipmap_leaf_index(_dev(seg), seg.size, torch.zeros(seg.size, dtype=torch.int32, device="cuda"), capacity=3)
+    big = seg.copy()
+    big[0, 0, 0] = 1 << 28
+    with pytest.raises(mg.MgError):
+        mg.mipmap_leaf_index(_dev(big), big.size, torch.zeros(big.size, dtype=torch.int32, device="cuda"))
+
+
+@pytest.mark.parametrize("cfg_id,scale", [(3, 0.08), (2, 0.06), (4, 0.12), (1, 1.0)])
+def test_device_assisted_assembly_equals_the_host_builder(libs, cfg_id, scale):
+    """workload.make(device_mipmap=True) vs the host path: same graph, same device mipmap, same stats."""
+    mg, workload = libs
+    a = workload.make(cfg_id, scale)
+    b = workload.make(cfg_id, scale, device_mipmap=True)
+    try:
+        for k in ("child_a", "child_b", "weight", "weight_sigma", "level_offsets", "leaf_segment_id"):
+            assert np.array_equal(a.host_graph[k], b.host_graph[k]), k
+        assert a.mip_dims == b.mip_dims and a.level_start == b.level_start and a.n_voxels == b.n_voxels
+        assert torch.equal(a.d_idx, b.d_idx)
+        assert b.host_idx[0] is None and np.array_equal(b.host_level(0), a.host_level(0))
+        for k in ("n_nodes", "depth", "n_distinct_mixtures"):
+            assert a.stats[k] == b.stats[k], k
+        assert abs(a.stats["nnz_per_voxel"] - b.stats["nnz_per_voxel"]) < 1e-15
+    finally:
+        a.close()
+        b.close()
