@@ -48,8 +48,9 @@ def parse_args():
     p.add_argument("--no-cpu-baseline", action="store_true")
     p.add_argument("--no-e2e", action="store_true")
     p.add_argument("--no-attr", action="store_true", help="skip the extra NEXT-1 measurement (multi-attribute propagation)")
-    p.add_argument("--device-mipmap", action="store_true",
-                   help="configs 1-4: classify the two finest mip levels on the device (NEXT-4 front end) instead of on the host")
+    p.add_argument("--host-mipmap", action="store_true",
+                   help="configs 1-4: build the whole histogram mipmap on the host (default: the two finest levels are classified "
+                        "on the device, NEXT-4 front end; same graph and node indices either way)")
     p.add_argument("--relabel", action="store_true", help="config 5: load the DAG with MG_RELABEL (levels sorted by children)")
     p.add_argument("--no-query", action="store_true", help="skip the extra NEXT-4 measurement (mixture LUT + range queries)")
     p.add_argument("--no-render", action="store_true", help="skip the extra NEXT-2 measurement (ray-marcher over the paletted mipmap)")
@@ -231,7 +232,7 @@ def run_b200(args) -> dict:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
     from paper_2009_02702_b200 import mg, workload
 
-    w = workload.make(args.config, args.scale, relabel=args.relabel, device_mipmap=args.device_mipmap and args.config != 5)
+    w = workload.make(args.config, args.scale, relabel=args.relabel, device_mipmap=not args.host_mipmap and args.config != 5)
     g = w.graph
     info = g.info
     n_nodes, n_internal = int(info.n_nodes), int(info.n_internal)

@@ -406,3 +406,27 @@ def test_config3_mixture_lut_and_range_queries_full_size(libs):
         lut.close()
     finally:
         w.close()
+
+
+def test_config3_device_mipmap_front_end_full_size(libs):
+    """NEXT-4 (second half) at full size: the device-assisted assembly (bench.py --device-mipmap) yields the host
+    builder's graph and node-index mipmap bit for bit, on all 1,438,087,061 voxels."""
+    mg, workload = libs
+    a = workload.make(3)
+    try:
+        ga = {k: a.host_graph[k].copy() for k in ("child_a", "child_b", "weight", "weight_sigma", "level_offsets", "leaf_segment_id")}
+        ref = a.d_idx.clone()
+        stats_a = dict(a.stats)
+    finally:
+        a.close()
+    b = workload.make(3, device_mipmap=True)
+    try:
+        for k, v in ga.items():
+            assert np.array_equal(v, b.host_graph[k]), k
+        assert torch.equal(ref, b.d_idx)
+        print(f"cfg3 setup: host path synth {stats_a['synth_s']:.2f} + builder {stats_a['builder_s']:.2f} + upload "
+              f"{stats_a['upload_idx_s']:.2f} s; device front end: synth {b.stats['synth_s']:.2f} + front end "
+              f"{b.stats['front_end_s']:.2f} + builder {b.stats['builder_s']:.2f} + upload {b.stats['upload_idx_s']:.2f} s "
+              f"({b.stats['n_level1_mixed']} non-pure level-1 parents)")
+    finally:
+        b.close()

@@ -1,0 +1,57 @@
+"""bench.py's contract line on a GPU box (a down-scaled config 3 so that it runs in seconds): every key the
+driver reads is present and consistent.  The numbers themselves are not judged here."""
+import json
+import os
+import subprocess
+import sys
+
+import pytest
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def _run(*extra):
+    cmd = [sys.executable, os.path.join(ROOT, "bench.py"), "--scale", "0.06", "--steps", "4", "--warmup", "3", *extra]
+    out = subprocess.run(cmd, capture_output=True, text=True, timeout=900)
+    assert out.returncode == 0, out.stderr[-3000:]
+    lines = [l for l in out.stdout.strip().splitlines() if l.startswith("{")]
+    assert len(lines) == 1, out.stdout[-2000:]
+    return json.loads(lines[0])
+
+
+def test_bench_line_has_the_contract_keys():
+    if not torch.cuda.is_available():
+        pytest.fail("the gpu-marked tests need a CUDA device (no CPU fallback exists)")
+    d = _run()
+    for k in ("metric", "value", "unit", "n_gpus", "steps", "warmup", "ms_per_step", "higher_is_better", "scaling",
+              "vs_baseline", "dtype", "data", "config", "roofline", "cpu_baseline", "e2e", "gpu_launches", "clocks"):
+        assert k in d, k
+    assert d["metric"] == "tf_update_latency_ms" and d["unit"] == "ms" and d["higher_is_better"] is False
+    assert d["n_gpus"] == 1 and d["steps"] == 4 and d["warmup"] == 3 and d["vs_baseline"] is None
+    assert d["dtype"] == "f32" and d["data"] == "synthetic" and "workload" in d["config"] and "model" not in d["config"]
+    assert d["value"] > 0 and abs(d["value"] - d["ms_per_step"]) < 1e-9
+    r = d["roofline"]
+    assert r["bound"] == "hbm" and r["unit"] == "GB/s" and r["kernel"] == "k_colorize"
+    assert abs(r["frac"] - r["achieved"] / r["peak"]) < 1e-9 and r["achieved"] > 0
+    c = d["cpu_baseline"]
+    assert c["kind"] == "oracle" and c["cores"] >= 1 and c["value"] > 0 and c["sample"]
+    e = d["e2e"]
+    assert e["value"] > d["value"] and e["h2d_bytes_per_step"] > 0 and e["d2h_bytes_per_step"] > 0
+    per_step = d["gpu_launches"] / d["steps"]
+    assert per_step == int(per_step) and per_step >= 2                       # propagate launches + one colourise
+    assert "sm_mhz" in d["clocks"] and "reasons" in d["clocks"]
+    for k in ("packed", "attr", "render", "query"):                             # the NEXT rows report beside it
+        assert k in d, k
+    assert d["setup_s"].get("front_end_s", 0) > 0                               # device mipmap front end is the default
+
+
+def test_bench_host_mipmap_and_fp16_variants_agree_on_the_workload():
+    a = _run("--host-mipmap", "--no-cpu-baseline", "--no-e2e", "--no-render", "--no-query", "--no-packed", "--no-attr")
+    b = _run("--format", "rgba16f", "--no-cpu-baseline", "--no-e2e", "--no-render", "--no-query", "--no-packed", "--no-attr")
+    for k in ("mip_voxels", "nodes", "leaves", "topo_depth"):
+        assert a["config"][k] == b["config"][k], k
+    assert "front_end_s" not in a["setup_s"] and a["config"]["output"] == "rgba8" and b["config"]["output"] == "rgba16f"
+    assert b["roofline"]["algorithmic_bytes_per_launch"] == 12 * b["config"]["mip_voxels"]
