@@ -283,7 +283,8 @@ int build_mipmap(const uint32_t* seg, uint64_t X, uint64_t Y, uint64_t Z, int n_
         out.level_ids[1].assign(front->level1, front->level1 + n1);
         uint32_t* P = out.level_ids[1].data();
         uint64_t nnz_level = n1 - front->n_mixed, n_marked = 0;
-        for (uint64_t v = 0; v < n1; v++) n_marked += (P[v] == 0xFFFFFFFFu);
+#pragma omp parallel for reduction(+ : n_marked) schedule(static)
+        for (int64_t v = 0; v < (int64_t)n1; v++) n_marked += (P[v] == 0xFFFFFFFFu);
         if (n_marked != front->n_mixed) {
             set_error("histogram mipmap: level 1 marks %llu parents as not pure, the list has %llu", (unsigned long long)n_marked,
                       (unsigned long long)front->n_mixed);
@@ -310,11 +311,17 @@ int build_mipmap(const uint32_t* seg, uint64_t X, uint64_t Y, uint64_t Z, int n_
         }
         if (bad) { set_error("histogram mipmap: inconsistent level-1 front end (voxel, child count or leaf out of range)"); return MGB_ERR_INVALID_ARG; }
         if (table.failed) { set_error("histogram mipmap: mixture table full or out of memory at level 1"); return MGB_ERR_LIMIT; }
-        for (uint64_t v = 0; v < n1; v++)
+        int64_t first_bad = -1;
+#pragma omp parallel for schedule(static)
+        for (int64_t v = 0; v < (int64_t)n1; v++)
             if (P[v] == 0xFFFFFFFFu || (!(P[v] & kMixed) && P[v] >= n_leaves)) {
-                set_error("histogram mipmap: level-1 voxel %llu is neither a leaf nor in the mixed list", (unsigned long long)v);
-                return MGB_ERR_INVALID_ARG;
+#pragma omp critical
+                if (first_bad < 0 || v < first_bad) first_bad = v;
             }
+        if (first_bad >= 0) {
+            set_error("histogram mipmap: level-1 voxel %lld is neither a leaf nor in the mixed list", (long long)first_bad);
+            return MGB_ERR_INVALID_ARG;
+        }
         nnz_total += nnz_level;
         first_level = 2;
     }

@@ -31,7 +31,10 @@ __global__ void k_mark_ids(const uint32_t* __restrict__ seg, uint64_t n, uint8_t
     uint32_t last = kNone;
     for (uint64_t v = (uint64_t)blockIdx.x * kThreads + threadIdx.x; v < n; v += (uint64_t)gridDim.x * kThreads) {
         const uint32_t s = __ldg(seg + v);
-        if (s != last) { present[s] = 1; last = s; }                  // racing stores of the same value
+        if (s != last) {                                              // test first: a handful of hot bytes, mostly already set
+            if (!present[s]) present[s] = 1;                          // (racing stores of the same value)
+            last = s;
+        }
     }
 }
 
