@@ -19,8 +19,12 @@ Function -> passage (PAPER.md line):
   lookup               L221, L267
   to_rgba8 / to_rgba16f  Q13 (defined by this repo; not in the paper)
   bits_per_voxel, index_range, pack_level, unpack_level   NEXT-3: Table 1 (8),(9),(A), Eq. 15-16
-  pixel_ray, sample_lod, render   NEXT-2: ray-marching the paletted mipmap, readings R1-R6 (L265-L271, L414)
-All functions are pinned by tests/test_oracle_pins.py / tests/test_oracle_render.py; none is "parity unpinned".
+  pixel_ray, sample_lod, render, render_pixels   NEXT-2: ray-marching the paletted mipmap, readings R1-R6 (L265-L271, L414)
+  mixture_lut          NEXT-4: mu and dmu per node, Eq. 17-18 L229-L239, L375 (reading Q19)
+  fa_axis, range_query_fa, range_query_naive   NEXT-4: footprint assembly, section 3.6, Table 4 (reading Q20)
+All functions are pinned by tests/test_oracle_pins.py / test_oracle_render.py / test_oracle_query.py; none is "parity
+unpinned".  The weakest pin is Eq. 18 (mixture_lut's dmu): the paper prints no value for it, so it is tied only to a
+hand-worked two-node case, its homogeneity in dw and the zero-sigma case; mu itself is pinned through symbolic_eval.
 """
 from __future__ import annotations
 

@@ -10,7 +10,10 @@
  *
  * Pins (tests/test_oracle_*.py, -m "not gpu"): Table 2 voxel totals (O-1), brute force vs
  * recursion and the textbook box filter (O-2/O-3), Fig. 2 / Fig. 4 worked examples and closed-form
- * chains (O-4), mu . TF == colour and row sums (O-5), known values for the output conversions.
+ * chains (O-4), mu . TF == colour and row sums (O-5), known values for the output conversions;
+ * hand-worked rays / scipy map_coordinates / Beer-Lambert closed forms (ray-marcher, R1-R6); Table 4's fetch
+ * counts, brute-force tilings, np.bincount and the sum-to-volume identity (range queries); a hand-worked
+ * case for Eq. 18 (the only pin it has).
  *
  * Layout conventions: volumes are [Z][Y][X], x fastest; colours are 4 doubles (R,G,B,A) per entry.
  */
