@@ -53,6 +53,11 @@ def parse_args():
                         "on the device, NEXT-4 front end; same graph and node indices either way)")
     p.add_argument("--relabel", action="store_true", help="config 5: load the DAG with MG_RELABEL (levels sorted by children)")
     p.add_argument("--no-query", action="store_true", help="skip the extra NEXT-4 measurement (mixture LUT + range queries)")
+    p.add_argument("--render-empty-background", action="store_true",
+                   help="render section: make the first leaf (config 4: background ID 0) exactly transparent, the case "
+                        "empty-space skipping is for (L271)")
+    p.add_argument("--render-alpha-zero-frac", type=float, default=None,
+                   help="render section: fraction of segments made exactly transparent (default: the config's own)")
     p.add_argument("--no-render", action="store_true", help="skip the extra NEXT-2 measurement (ray-marcher over the paletted mipmap)")
     p.add_argument("--no-packed", action="store_true", help="skip the extra NEXT-3 measurement (bit-packed node IDs)")
     p.add_argument("--cpu-sample-voxels", type=int, default=1 << 31, help="oracle sample size (>= the mipmap = whole workload)")
@@ -333,13 +338,18 @@ def run_b200(args) -> dict:
     if not args.no_render and rank == 0 and len(w.mip_dims) > 1:
         from paper_2009_02702_b200 import synth
         view = synth.render_view(w.cfg)
-        g.propagate(torch.from_numpy(synth.render_tf(w.tf(0))).cuda(), nodes, st)
+        rtf = synth.render_tf(w.tf(0) if args.render_alpha_zero_frac is None else
+                              synth.random_tf(w.n_leaves, w.cfg.get("seed", 0), alpha_zero_frac=args.render_alpha_zero_frac))
+        if args.render_empty_background:
+            rtf[0, 3] = 0.0
+        g.propagate(torch.from_numpy(rtf).cuda(), nodes, st)
         img = torch.empty((view["height"], view["width"], 4), dtype=torch.float32, device="cuda")
         desc = w.mip_desc()
         render = {"what": "NEXT-2 mg_render: pinhole ray-marcher over the node-index mipmap + fp32 palette, per-sample LOD, "
                           "manual trilinear + inter-level blend, opacity correction, hierarchical empty-space skipping "
                           "(PAPER.md L267-L271, L414)", "width": view["width"], "height": view["height"],
-                  "step_voxels": view["step_voxels"], "tf": f"config TF, opacities x {synth.RENDER_ALPHA_SCALE}", "frames": 10}
+                  "step_voxels": view["step_voxels"], "tf": f"config TF, opacities x {synth.RENDER_ALPHA_SCALE}" + (", first leaf transparent" if args.render_empty_background else ""),
+                  "frames": 10}
         for label, thr, fl in (("ess", view["ess_threshold"], view["flags"]), ("no_ess", -1.0, view["flags"]),
                                ("ess_generic_mipmap", view["ess_threshold"], 0), ("no_ess_generic_mipmap", -1.0, 0)):
             v = mg.view_struct(dict(view, ess_threshold=thr, flags=fl))
