@@ -305,7 +305,7 @@ enum {
  *                    [1] += samples skipped by R6, [2] += those of [0] whose coarse level named one leaf
  *                    (MG_VIEW_HISTOGRAM_MIPMAP: fine level not fetched), [3] unused.
  * Errors: MG_ERR_INVALID_ARG (NULL, misalignment, bad sizes, level dims that are not the ceil-halving
- * chain of L80, offsets overlapping), MG_ERR_CUDA.
+ * chain of L80, offsets overlapping, a step so small that a ray would need more than 2^24 of them), MG_ERR_CUDA.
  */
 int mg_render(mg_graph *g, const uint32_t *node_idx_mipmap, const mg_mipmap_desc *mip,
               const float *node_rgba, const mg_view *view, float *out_rgba, uint64_t *stats_device,

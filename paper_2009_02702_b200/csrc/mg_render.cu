@@ -356,6 +356,14 @@ extern "C" int mg_render(mg_graph* g, const uint32_t* node_idx_mipmap, const mg_
     P.W = view->width;
     P.H = view->height;
     const double s_ref = fmin(s[0], fmin(s[1], s[2]));
+    {   // a ray takes at most diagonal / (step_voxels s_ref) steps: refuse views that would march (almost) forever
+        double diag2 = 0.0;
+        for (int a = 0; a < 3; a++) diag2 += (double)mip->level_dim[0][a] * s[a] * (double)mip->level_dim[0][a] * s[a];
+        if (sqrt(diag2) / (view->step_voxels * s_ref) > 16777216.0) {
+            mg::set_error("mg_render: step_voxels = %g needs more than 2^24 steps per ray", view->step_voxels);
+            return MG_ERR_INVALID_ARG;
+        }
+    }
     for (int a = 0; a < 3; a++) {
         P.eye[a] = view->eye[a]; P.right[a] = view->right[a]; P.up[a] = view->up[a]; P.fwd[a] = view->forward[a];
         P.inv_s[a] = 1.0 / s[a];

@@ -221,6 +221,7 @@ def test_render_error_paths(mg):
     cases = [
         (good_mip, dict(view, width=0)),
         (good_mip, dict(view, step_voxels=0.0)),
+        (good_mip, dict(view, step_voxels=1e-8)),                              # would march 3e8 steps per ray
         (good_mip, dict(view, spacing=np.array([1.0, -1.0, 1.0]))),
         (([0, 8], [(2, 2, 2), (2, 1, 1)]), view),                              # not ceil-halving
         (([0, 4], [(2, 2, 2), (1, 1, 1)]), view),                              # level 1 inside level 0
