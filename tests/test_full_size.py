@@ -155,8 +155,7 @@ def test_volume_config_full_size(libs, cfg_id):
                 worst = max(worst, float(np.abs(nodes_host[idx_l[v]] - direct).max()))
         assert worst <= TOL_DIRECT, worst
         print(f"cfg {cfg_id}: {w.stats['n_nodes']} nodes depth {w.stats['depth']}, max |graph - direct| on samples = {worst:.2e}")
-        if cfg_id == 3:
-            _check_render_full_size(mg, w, tf)
+        _check_render_full_size(mg, w, tf)
     finally:
         w.close()
 
@@ -184,7 +183,11 @@ def _check_render_full_size(mg, w, tf):
     got, got_off = img.cpu().numpy().astype(np.float64), img_off.cpu().numpy().astype(np.float64)
     st = stats.cpu().numpy().reshape(3, 4)
     assert np.isfinite(got).all() and got[..., 3].max() > 0.5
-    assert st[0, 1] > 0 and st[1, 1] == 0 and st[0, 0] < st[1, 0] and st[0, 2] > 0 and st[2, 2] == 0
+    assert st[1, 1] == 0 and st[0, 0] <= st[1, 0] and st[2, 2] == 0
+    if w.cfg.get("alpha_zero_frac", 0.0) > 0:                      # configs without a transparent segment have nothing to skip
+        assert st[0, 1] > 0 and st[0, 0] < st[1, 0]
+    if w.cfg.get("zscale", 1) > 1:                                  # lambda > 0 somewhere: the coarse-first shortcut fires
+        assert st[0, 2] > 0
     assert st[0, :2].sum() == st[1, :2].sum() == st[2, :2].sum()
     assert np.abs(got - got_off).max() <= 1e-5                     # skipped samples were (numerically) transparent
     assert np.abs(got - img_plain.cpu().numpy()).max() <= 1e-6     # one-leaf blocks do not change the image
@@ -200,7 +203,7 @@ def _check_render_full_size(mg, w, tf):
     ref, _ = oracle.render_pixels(None, pal, view, ij, flat=(flat, w.level_start, np.array(w.mip_dims)))
     err = np.abs(got[ij[:, 1], ij[:, 0]] - ref).max()
     hit = (ref[:, 3] > 0).mean()
-    print(f"render 1600x1200 cfg3: max|err| on {ij.shape[0]} sampled pixels = {err:.2e} ({hit:.0%} hit the volume); "
+    print(f"render 1600x1200 {w.name}: max|err| on {ij.shape[0]} sampled pixels = {err:.2e} ({hit:.0%} hit the volume); "
           f"samples composited/skipped/from one-leaf blocks: {st[0, :3].tolist()}, without ESS {st[1, :3].tolist()}, "
           f"without the histogram-mipmap flag {st[2, :3].tolist()}")
     assert hit > 0.3 and err <= 5e-6, err
@@ -342,14 +345,15 @@ def _sub_dag(hg, targets):
     return sa, sb, hg["weight"][old].astype(np.float64), hg["weight_sigma"][old].astype(np.float64), n_sub_leaves, old
 
 
-def test_config3_mixture_lut_and_range_queries_full_size(libs):
+@pytest.mark.parametrize("cfg_id", [3, 4])
+def test_mixture_lut_and_range_queries_full_size(libs, cfg_id):
     """NEXT-4 at full size, in bench.py's launch configuration (batches of random cubes, Table 4's sizes).
     The dense oracle cannot hold 1.7 M x 1182 entries, so: sampled rows of the table against the oracle run on
     the sub-DAG below them; every row sums to 1; NAIVE == the plain per-segment voxel count of the generator's
     volume (exact); FA fetch counts == the oracle's decomposition; FA sums to the box volume (L251) and stays
     within 1 % of the volume of the true counts (L251: 'about 0.3 %')."""
     mg, workload = libs
-    w = workload.make(3, keep_seg=True)
+    w = workload.make(cfg_id, keep_seg=True)
     try:
         hg, g = w.host_graph, w.graph
         nl = hg["n_leaves"]
@@ -373,13 +377,13 @@ def test_config3_mixture_lut_and_range_queries_full_size(libs):
             np.testing.assert_allclose(mu[s:e], omu[row, cols], rtol=1e-12)
             np.testing.assert_allclose(dmu[s:e], odmu[row, cols], rtol=1e-12, atol=1e-300)
 
-        dims = synth.CONFIGS[3]["dims"]
+        dims = synth.CONFIGS[cfg_id]["dims"]
         ids, seg_index = _leaf_index_chunked(w.seg)
         desc = w.mip_desc()
         l_max = len(w.mip_dims) - 1
         worst = 0.0
         for side in (16, 64, 256):
-            boxes = synth.query_boxes(dims, side, 24, seed=3)
+            boxes = synth.query_boxes(dims, side, 24, seed=cfg_id)
             nq = len(boxes)
             e_fa = torch.empty((nq, nl), dtype=torch.float64, device="cuda")
             d_fa = torch.empty((nq, nl), dtype=torch.float64, device="cuda")
@@ -400,7 +404,7 @@ def test_config3_mixture_lut_and_range_queries_full_size(libs):
                 assert abs(e_fa[q].sum() - vol) <= 1e-9 * vol
                 assert (e_fa[q] >= 0).all() and (d_fa[q] >= 0).all()
                 worst = max(worst, float(np.abs(e_fa[q] - truth).max()) / vol)
-        print(f"cfg3 range queries: LUT {lut.info.nnz} entries ({lut.info.device_bytes / 1e6:.0f} MB, longest row "
+        print(f"cfg{cfg_id} range queries: LUT {lut.info.nnz} entries ({lut.info.device_bytes / 1e6:.0f} MB, longest row "
               f"{lut.info.max_row_nnz}); max |FA - true count| / volume = {worst:.2e}")
         assert worst < 0.01, worst
         lut.close()
