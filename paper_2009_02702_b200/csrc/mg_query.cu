@@ -42,6 +42,7 @@ namespace {
 
 constexpr int kBuildThreads = 128;
 constexpr int kQueryThreads = 256;
+constexpr int kNaiveUnroll = 4;
 constexpr int kMaxPieces = 2 * MG_MAX_MIP_LEVELS + 2;     // pieces of one axis: at most 2 per level
 
 __global__ void k_lut_leaves(uint32_t n_leaves, const uint64_t* __restrict__ row_ptr, uint32_t* row_len, uint32_t* col,
@@ -334,31 +335,69 @@ k_range_query_fa(const __grid_constant__ QueryParams P)
     if (P.fetches && lane == 0 && n_fetch) atomicAdd(P.fetches + q, n_fetch);
 }
 
-// The naive approach (L377): every level-0 voxel of the box is one sample.
+// The naive approach (L377): every level-0 voxel of the box is one sample.  Warps take rows of the box (lanes
+// along x: coalesced, no divisions in the inner loop).  Level-0 voxels are leaves (L223), so with SMEM their counts
+// go to a per-CTA histogram in shared memory (uint32[n_leaves], grouped per warp by __match_any_sync first) that is
+// flushed once with one fp64 atomic per non-zero bin; any other node, or a table too large for shared memory
+// (SMEM = false), takes the general path of add_sample.
+template <bool SMEM>
 __global__ void __launch_bounds__(kQueryThreads)
 k_range_query_naive(const __grid_constant__ QueryParams P)
 {
+    extern __shared__ uint32_t s_cnt[];
     const uint32_t q = blockIdx.x;
     const uint64_t* box = P.boxes + 6ull * q;
     const uint32_t x0 = (uint32_t)box[0], y0 = (uint32_t)box[1], z0 = (uint32_t)box[2];
     const uint32_t dx = (uint32_t)box[3] - x0, dy = (uint32_t)box[4] - y0, dz = (uint32_t)box[5] - z0;
-    const unsigned long long n_vox = (unsigned long long)dx * dy * dz;
     const int X = P.dim[0][0], Y = P.dim[0][1];
     double* expect = P.expect + (uint64_t)q * P.n_leaves;
     double* var = P.var ? P.var + (uint64_t)q * P.n_leaves : nullptr;
-    const unsigned long long stride = (unsigned long long)gridDim.y * kQueryThreads;
-    const unsigned long long first = (unsigned long long)blockIdx.y * kQueryThreads + threadIdx.x;
-    for (unsigned long long base = first - (threadIdx.x & 31); base < n_vox; base += stride) {   // warp-uniform trip count
-        const unsigned long long v = base + (threadIdx.x & 31);
-        const bool active = v < n_vox;
-        uint32_t node = 0;
-        if (active) {
-            const uint32_t ix = (uint32_t)(v % dx), iy = (uint32_t)((v / dx) % dy), iz = (uint32_t)(v / ((unsigned long long)dx * dy));
-            node = __ldg(P.idx + P.off[0] + ((size_t)(z0 + iz) * Y + (y0 + iy)) * X + (x0 + ix));
-        }
-        add_sample(P, expect, var, active, node, 1.0);
+    if (SMEM) {
+        for (uint32_t i = threadIdx.x; i < P.n_leaves; i += kQueryThreads) s_cnt[i] = 0;
+        __syncthreads();
     }
-    if (P.fetches && blockIdx.y == 0 && threadIdx.x == 0) atomicAdd(P.fetches + q, n_vox);
+    const unsigned lane = threadIdx.x & 31;
+    const unsigned n_warps = gridDim.y * (kQueryThreads / 32), warp = blockIdx.y * (kQueryThreads / 32) + threadIdx.x / 32;
+    const uint32_t n_rows = dy * dz;                                       // < 2^32: level 0 has < 2^40 voxels, dx >= 1
+    for (uint32_t r = warp; r < n_rows; r += n_warps) {
+        const uint32_t iy = r % dy, iz = r / dy;
+        const uint32_t* row = P.idx + P.off[0] + ((size_t)(z0 + iz) * Y + (y0 + iy)) * X + x0;
+        for (uint32_t bx = 0; bx < dx; bx += 32 * kNaiveUnroll) {          // warp-uniform trip count
+            uint32_t node[kNaiveUnroll];
+            bool active[kNaiveUnroll];
+#pragma unroll
+            for (int u = 0; u < kNaiveUnroll; u++) {                       // the loads of the whole group first
+                active[u] = bx + 32 * u + lane < dx;
+                node[u] = active[u] ? __ldg(row + bx + 32 * u + lane) : 0u;
+            }
+#pragma unroll
+            for (int u = 0; u < kNaiveUnroll; u++) {
+                if (bx + 32 * u >= dx) break;                              // (uniform)
+                if (SMEM) {
+                    const bool pure = active[u] && node[u] < P.n_leaves;
+                    const unsigned pm = __ballot_sync(0xffffffffu, pure);
+                    const uint32_t first = __shfl_sync(0xffffffffu, node[u], 0);
+                    if (pm == 0xffffffffu && __all_sync(0xffffffffu, node[u] == first)) {
+                        if (lane == 0) atomicAdd(&s_cnt[first], 32u);      // a run of one segment: the common case
+                    } else {
+                        if (pure) {
+                            const unsigned grp = __match_any_sync(pm, node[u]);
+                            if (lane == (unsigned)(__ffs(grp) - 1)) atomicAdd(&s_cnt[node[u]], (uint32_t)__popc(grp));
+                        }
+                        add_sample(P, expect, var, active[u] && !pure, node[u], 1.0);   // not a leaf: its table row
+                    }
+                } else {
+                    add_sample(P, expect, var, active[u], node[u], 1.0);
+                }
+            }
+        }
+    }
+    if (SMEM) {
+        __syncthreads();
+        for (uint32_t i = threadIdx.x; i < P.n_leaves; i += kQueryThreads)
+            if (s_cnt[i]) atomicAdd(expect + i, (double)s_cnt[i]);
+    }
+    if (P.fetches && blockIdx.y == 0 && threadIdx.x == 0) atomicAdd(P.fetches + q, (unsigned long long)dx * dy * dz);
 }
 
 __global__ void k_query_finish(double* var, uint64_t n)
@@ -439,7 +478,19 @@ extern "C" int mg_range_query(mg_mixture_lut* lut, const uint32_t* node_idx_mipm
     const uint32_t splits = std::max<uint32_t>(1, std::min<uint32_t>(64, (148 * 8 + n_queries - 1) / n_queries));
     const dim3 grid(n_queries, splits);
     if (mode == MG_QUERY_FA) k_range_query_fa<<<grid, kQueryThreads, 0, st>>>(P);
-    else k_range_query_naive<<<grid, kQueryThreads, 0, st>>>(P);
+    else {
+        const size_t smem = (size_t)lut->n_leaves * sizeof(uint32_t);
+        if (smem <= 200 * 1024) {                                          // per-CTA leaf histogram in shared memory
+            static bool attr_set = false;                                  // (per process; the attribute is per function)
+            if (!attr_set) {
+                MG_CUDA(cudaFuncSetAttribute(k_range_query_naive<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
+                attr_set = true;
+            }
+            k_range_query_naive<true><<<grid, kQueryThreads, smem, st>>>(P);
+        } else {
+            k_range_query_naive<false><<<grid, kQueryThreads, 0, st>>>(P);
+        }
+    }
     MG_CUDA(cudaGetLastError());
     mg::count_launch();
     if (err) {
