@@ -339,7 +339,12 @@ typedef struct mg_lut_info {
     uint32_t max_row_nnz;  /* longest row                                                 */
 } mg_lut_info;
 
-enum { MG_QUERY_FA = 0u, MG_QUERY_NAIVE = 1u };
+enum {
+    MG_QUERY_FA = 0u,      /* footprint assembly                                                               */
+    MG_QUERY_NAIVE = 1u,   /* every level-0 voxel                                                              */
+    MG_QUERY_FA_WALK = 2u  /* footprint assembly with the work distribution used for queries of > 4096 boxes   */
+                           /* (every warp walks all boxes); same result, exposed so that it can be tested       */
+};
 
 /* Build the table for a loaded graph.  weight_sigma: HOST float[n_nodes] in the library's numbering
  * (entries of the leaves ignored), or NULL for dw = 0 everywhere.  Allocates device memory and
@@ -362,7 +367,7 @@ int mg_mixture_lut_export(const mg_mixture_lut *lut, uint64_t *row_ptr, uint32_t
  *   expect, err      DEVICE double[n_queries][n_leaves]: expected voxels per leaf and its error
  *                    (err may be NULL).  sum_i expect[q][i] = volume of box q (L251).
  *   fetches          DEVICE uint64[n_queries] or NULL: samples fetched per query (Table 4).
- *   mode             MG_QUERY_FA or MG_QUERY_NAIVE.
+ *   mode             MG_QUERY_FA, MG_QUERY_NAIVE or MG_QUERY_FA_WALK.
  * Enqueue-only apart from the staging copy.  Accumulation uses fp64 atomics: the result is the oracle's
  * up to summation order.
  */

@@ -236,6 +236,7 @@ struct QueryParams {
     double* expect;
     double* var;                     // may be NULL
     unsigned long long* fetches;     // may be NULL
+    int force_walk;                  // MG_QUERY_FA_WALK
 };
 
 // Add one mipmap sample (node, denormalised by `scale` voxels) to query q's dense result.  Called by all
@@ -280,14 +281,54 @@ __device__ int fa_axis(uint32_t lo, uint32_t hi, int max_level, uint32_t* start,
     return n;
 }
 
-// grid = (n_queries, splits); the warps of all CTAs of a query share its boxes: chunk c (32 cubes) of box t
-// goes to warp (t + c) mod n_warps, which spreads both many one-cube boxes and few huge ones.
+// The box t = a + nx (b + ny c) of the footprint's tensor product: its cube level and grid of cubes.
+struct FaBox {
+    int l, ex, ey, ez;                  // cube level; cubes per axis = 2^e
+    uint32_t bx, by, bz;                // first cube, in level-l voxel coordinates
+    unsigned long long n_cubes;
+};
+
+__device__ __forceinline__ FaBox fa_box(const uint32_t (*s_start)[kMaxPieces], const int (*s_level)[kMaxPieces], int a, int b, int c)
+{
+    FaBox B;
+    const int lx = s_level[0][a], ly = s_level[1][b], lz = s_level[2][c];
+    B.l = min(lx, min(ly, lz));                                          // cube side = the shortest extent
+    B.ex = lx - B.l; B.ey = ly - B.l; B.ez = lz - B.l;
+    B.n_cubes = 1ull << (B.ex + B.ey + B.ez);
+    B.bx = s_start[0][a] >> B.l; B.by = s_start[1][b] >> B.l; B.bz = s_start[2][c] >> B.l;
+    return B;
+}
+
+// Chunk ch (32 cubes, one per lane) of a box: one mipmap sample per cube, denormalised by side^3 = 8^l.
+__device__ __forceinline__ unsigned fa_chunk(const QueryParams& P, double* expect, double* var, const FaBox& B, unsigned long long ch)
+{
+    const unsigned lane = threadIdx.x & 31;
+    const unsigned long long k = (ch << 5) + lane;
+    const bool active = k < B.n_cubes;
+    uint32_t node = 0;
+    if (active) {
+        const uint32_t ix = (uint32_t)(k & ((1ull << B.ex) - 1)), iy = (uint32_t)((k >> B.ex) & ((1ull << B.ey) - 1)),
+                       iz = (uint32_t)(k >> (B.ex + B.ey));
+        node = __ldg(P.idx + P.off[B.l] + ((size_t)(B.bz + iz) * P.dim[B.l][1] + (B.by + iy)) * P.dim[B.l][0] + (B.bx + ix));
+    }
+    add_sample(P, expect, var, active, node, __hiloint2double((1023 + 3 * B.l) << 20, 0));
+    return (unsigned)min(32ull, B.n_cubes - (ch << 5));
+}
+
+constexpr int kMaxBoxes = 4096;         // boxes whose chunk prefix fits the CTA's shared memory
+
+// grid = (n_queries, splits); the warps of all CTAs of a query share its chunks (32 cubes of one box).  Every
+// CTA builds the prefix sum of the chunks per box in shared memory (threads over boxes, then a scan), and warp w of
+// the query takes the chunks g = w, w + n_warps, ...: a binary search finds the box.  Queries with more than
+// kMaxBoxes boxes fall back to every warp walking all boxes (chunk c of box t goes to warp (t + c) mod n_warps).
 __global__ void __launch_bounds__(kQueryThreads)
 k_range_query_fa(const __grid_constant__ QueryParams P)
 {
     __shared__ uint32_t s_start[3][kMaxPieces];
     __shared__ int s_level[3][kMaxPieces];
     __shared__ int s_n[3];
+    __shared__ unsigned long long s_pref[kMaxBoxes + 1];
+    __shared__ unsigned long long s_part[kQueryThreads];
     const uint32_t q = blockIdx.x;
     const uint64_t* box = P.boxes + 6ull * q;
     if (threadIdx.x < 3)
@@ -301,35 +342,51 @@ k_range_query_fa(const __grid_constant__ QueryParams P)
     double* var = P.var ? P.var + (uint64_t)q * P.n_leaves : nullptr;
     unsigned long long n_fetch = 0;
     const unsigned n_boxes = (unsigned)(nx * ny * nz);
-    // every warp walks all boxes (a, b, c) = t in x-fastest order; (a, b, c) and t mod n_warps are carried along
-    // incrementally -- no divisions in the walk, most boxes are left after a few instructions
-    int a = -1, b = 0, c = 0;
-    unsigned tm = n_warps - 1;                                           // (t - 1) mod n_warps
-    for (unsigned t = 0; t < n_boxes; t++) {
-        if (++a == nx) { a = 0; if (++b == ny) { b = 0; ++c; } }
-        if (++tm == n_warps) tm = 0;
-        const int lx = s_level[0][a], ly = s_level[1][b], lz = s_level[2][c];
-        const int l = min(lx, min(ly, lz));                              // cube side = the shortest extent
-        const int ex = lx - l, ey = ly - l, ez = lz - l;                 // cubes per axis = 2^e
-        const unsigned long long n_cubes = 1ull << (ex + ey + ez);
-        const unsigned long long n_chunks = (n_cubes + 31) >> 5;
-        const unsigned long long ch0 = warp >= tm ? warp - tm : warp + n_warps - tm;   // (warp - t) mod n_warps
-        if (ch0 >= n_chunks) continue;
-        const double scale = __hiloint2double((1023 + 3 * l) << 20, 0);  // side^3 = 8^l
-        const int X = P.dim[l][0], Y = P.dim[l][1];
-        const uint32_t* lvl = P.idx + P.off[l];
-        const uint32_t bx = s_start[0][a] >> l, by = s_start[1][b] >> l, bz = s_start[2][c] >> l;
-        for (unsigned long long ch = ch0; ch < n_chunks; ch += n_warps) {
-            const unsigned long long k = (ch << 5) + lane;
-            const bool active = k < n_cubes;
-            uint32_t node = 0;
-            if (active) {
-                const uint32_t ix = (uint32_t)(k & ((1ull << ex) - 1)), iy = (uint32_t)((k >> ex) & ((1ull << ey) - 1)),
-                               iz = (uint32_t)(k >> (ex + ey));
-                node = __ldg(lvl + ((size_t)(bz + iz) * Y + (by + iy)) * X + (bx + ix));
+    if (n_boxes <= (unsigned)kMaxBoxes && !P.force_walk) {
+        // chunks per box -> inclusive prefix: each thread a run of boxes, then the runs' totals are scanned
+        const unsigned per = (n_boxes + kQueryThreads - 1) / kQueryThreads;
+        const unsigned t0 = min(threadIdx.x * per, n_boxes), t1 = min(t0 + per, n_boxes);
+        unsigned long long run = 0;
+        for (unsigned t = t0; t < t1; t++) {
+            const FaBox B = fa_box(s_start, s_level, (int)(t % nx), (int)((t / nx) % ny), (int)(t / (nx * ny)));
+            run += (B.n_cubes + 31) >> 5;
+            s_pref[t + 1] = run;
+        }
+        s_part[threadIdx.x] = run;
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            unsigned long long acc = 0;
+            for (int i = 0; i < kQueryThreads; i++) { const unsigned long long v = s_part[i]; s_part[i] = acc; acc += v; }
+            s_pref[0] = 0;
+        }
+        __syncthreads();
+        const unsigned long long base = s_part[threadIdx.x];
+        for (unsigned t = t0; t < t1; t++) s_pref[t + 1] += base;
+        __syncthreads();
+        const unsigned long long total = s_pref[n_boxes];
+        for (unsigned long long g = warp; g < total; g += n_warps) {
+            unsigned lo = 0, hi = n_boxes;                               // largest t with s_pref[t] <= g
+            while (hi - lo > 1) {
+                const unsigned mid = (lo + hi) >> 1;
+                if (s_pref[mid] <= g) lo = mid; else hi = mid;
             }
-            add_sample(P, expect, var, active, node, scale);
-            if (lane == 0) n_fetch += min(32ull, n_cubes - (ch << 5));
+            const FaBox B = fa_box(s_start, s_level, (int)(lo % nx), (int)((lo / nx) % ny), (int)(lo / (nx * ny)));
+            const unsigned f = fa_chunk(P, expect, var, B, g - s_pref[lo]);
+            if (lane == 0) n_fetch += f;
+        }
+    } else {
+        // (a, b, c) and t mod n_warps are carried along incrementally: no divisions in the walk
+        int a = -1, b = 0, c = 0;
+        unsigned tm = n_warps - 1;                                       // (t - 1) mod n_warps
+        for (unsigned t = 0; t < n_boxes; t++) {
+            if (++a == nx) { a = 0; if (++b == ny) { b = 0; ++c; } }
+            if (++tm == n_warps) tm = 0;
+            const FaBox B = fa_box(s_start, s_level, a, b, c);
+            const unsigned long long n_chunks = (B.n_cubes + 31) >> 5;
+            for (unsigned long long ch = warp >= tm ? warp - tm : warp + n_warps - tm; ch < n_chunks; ch += n_warps) {
+                const unsigned f = fa_chunk(P, expect, var, B, ch);
+                if (lane == 0) n_fetch += f;
+            }
         }
     }
     if (P.fetches && lane == 0 && n_fetch) atomicAdd(P.fetches + q, n_fetch);
@@ -416,7 +473,7 @@ extern "C" int mg_range_query(mg_mixture_lut* lut, const uint32_t* node_idx_mipm
         mg::set_error("mg_range_query: NULL argument");
         return MG_ERR_INVALID_ARG;
     }
-    if (mode != MG_QUERY_FA && mode != MG_QUERY_NAIVE) { mg::set_error("mg_range_query: unknown mode %u", mode); return MG_ERR_INVALID_ARG; }
+    if (mode != MG_QUERY_FA && mode != MG_QUERY_NAIVE && mode != MG_QUERY_FA_WALK) { mg::set_error("mg_range_query: unknown mode %u", mode); return MG_ERR_INVALID_ARG; }
     if (((uintptr_t)expect & 7) || ((uintptr_t)err & 7) || ((uintptr_t)fetches & 7) || ((uintptr_t)node_idx_mipmap & 3)) {
         mg::set_error("mg_range_query: misaligned buffer");
         return MG_ERR_INVALID_ARG;
@@ -477,7 +534,8 @@ extern "C" int mg_range_query(mg_mixture_lut* lut, const uint32_t* node_idx_mipm
     // spread a query over enough CTAs to fill the machine when there are few queries (148 SMs x 8 CTAs)
     const uint32_t splits = std::max<uint32_t>(1, std::min<uint32_t>(64, (148 * 8 + n_queries - 1) / n_queries));
     const dim3 grid(n_queries, splits);
-    if (mode == MG_QUERY_FA) k_range_query_fa<<<grid, kQueryThreads, 0, st>>>(P);
+    P.force_walk = (mode == MG_QUERY_FA_WALK);
+    if (mode != MG_QUERY_NAIVE) k_range_query_fa<<<grid, kQueryThreads, 0, st>>>(P);
     else {
         const size_t smem = (size_t)lut->n_leaves * sizeof(uint32_t);
         if (smem <= 200 * 1024) {                                          // per-CTA leaf histogram in shared memory

@@ -116,7 +116,7 @@ class MgLutInfo(C.Structure):
                 ("n_leaves", C.c_uint32), ("max_row_nnz", C.c_uint32)]
 
 
-MG_QUERY_FA, MG_QUERY_NAIVE = 0, 1
+MG_QUERY_FA, MG_QUERY_NAIVE, MG_QUERY_FA_WALK = 0, 1, 2
 lib.mg_mixture_lut_build.argtypes = [_vp, _vp, C.POINTER(_vp), _vp]
 lib.mg_mixture_lut_build.restype = C.c_int
 lib.mg_mixture_lut_free.argtypes = [_vp]

@@ -110,12 +110,16 @@ def test_range_queries_match_oracle(mg, dims, quant_bits):
     e_fa, d_fa, f_fa = _query(lut, d_idx, mip, boxes, nl, mg.MG_QUERY_FA)
     e_nv, d_nv, f_nv = _query(lut, d_idx, mip, boxes, nl, mg.MG_QUERY_NAIVE)
     e_only, _, _ = _query(lut, d_idx, mip, boxes, nl, mg.MG_QUERY_FA, want_err=False)
+    e_walk, d_walk, f_walk = _query(lut, d_idx, mip, boxes, nl, mg.MG_QUERY_FA_WALK)
     for q, box in enumerate(boxes):
         x0, y0, z0, x1, y1, z1 = box
         vol = (x1 - x0) * (y1 - y0) * (z1 - z0)
         re, rd, rf = oracle.range_query_fa(levels, mu, dmu, box)
         np.testing.assert_allclose(e_fa[q], re, rtol=0, atol=1e-9 * vol)
         np.testing.assert_allclose(e_only[q], re, rtol=0, atol=1e-9 * vol)
+        np.testing.assert_allclose(e_walk[q], re, rtol=0, atol=1e-9 * vol)
+        np.testing.assert_allclose(d_walk[q], rd, rtol=1e-9, atol=1e-12 * vol)
+        assert f_walk[q] == rf
         np.testing.assert_allclose(d_fa[q], rd, rtol=1e-9, atol=1e-12 * vol)
         assert f_fa[q] == rf and f_nv[q] == vol
         truth = np.bincount(seg_index[z0:z1, y0:y1, x0:x1].reshape(-1), minlength=nl)
