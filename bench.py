@@ -51,6 +51,9 @@ def parse_args():
     p.add_argument("--host-mipmap", action="store_true",
                    help="configs 1-4: build the whole histogram mipmap on the host (default: the two finest levels are classified "
                         "on the device, NEXT-4 front end; same graph and node indices either way)")
+    p.add_argument("--partition", choices=["replicas", "slab"], default="replicas",
+                   help="N > 1: independent replicas of the whole update (default, weak scaling) or ONE update whose colourise is "
+                        "split into N contiguous voxel slabs with the graph replicated (strong scaling, SURVEY.md 8(e)); no collective either way")
     p.add_argument("--relabel", action="store_true", help="config 5: load the DAG with MG_RELABEL (levels sorted by children)")
     p.add_argument("--no-query", action="store_true", help="skip the extra NEXT-4 measurement (mixture LUT + range queries)")
     p.add_argument("--render-empty-background", action="store_true",
@@ -168,7 +171,9 @@ def workload_config(w, args, n_gpus: int) -> dict:
     s = w.stats
     cfg = {"workload": w.name, "baseline_config": args.config, "mip_voxels": w.n_voxels, "mip_levels": len(w.level_voxels),
            "nodes": s["n_nodes"], "leaves": s["n_leaves"], "topo_depth": s["depth"], "output": args.format,
-           "parallelism": "single GPU" if n_gpus == 1 else f"{n_gpus} independent replicas (no collective)",
+           "parallelism": "single GPU" if n_gpus == 1 else
+                          (f"{n_gpus}-way voxel-slab partition of colourise, graph and propagation replicated (no collective)"
+                           if getattr(args, "partition", "replicas") == "slab" else f"{n_gpus} independent replicas (no collective)"),
            "l2": "inputs larger than L2 (node-index stream %.2f GB per step, L2 126 MB); no explicit flush" % (4e-9 * w.n_voxels)}
     if "quant_bits" in s:
         cfg["quant_bits"] = s["quant_bits"]
@@ -195,6 +200,16 @@ def max_over_ranks(value: float, world: int, device="cpu") -> float:
     t = torch.tensor([value], dtype=torch.float64, device=device)
     dist.all_reduce(t, op=dist.ReduceOp.MAX)
     return float(t.item())
+
+
+def slab_range(n_voxels_padded: int, rank: int, world: int, align: int = 2048):
+    """Voxel range [lo, hi) of rank's slab: the concatenated mipmap cut into `world` contiguous pieces whose
+    boundaries are multiples of `align` voxels (one colourise CTA; keeps every 16-byte vector aligned).  The
+    pieces are disjoint, cover [0, n_voxels_padded) and differ by at most `align` voxels."""
+    blocks = -(-int(n_voxels_padded) // align)
+    lo = (blocks * rank // world) * align
+    hi = (blocks * (rank + 1) // world) * align
+    return min(lo, n_voxels_padded), min(hi, n_voxels_padded)
 
 
 def aggregate_value(ms_per_step: float, world: int) -> float:
@@ -249,10 +264,13 @@ def run_b200(args) -> dict:
     tfs = [torch.from_numpy(w.tf(u)).cuda() for u in range(n_tf)]          # resident in HBM before the timed region
     stream = torch.cuda.current_stream()
     st = stream.cuda_stream
+    slab = args.partition == "slab" and world > 1
+    v_lo, v_hi = slab_range(w.n_voxels_padded, rank, world) if slab else (0, w.n_voxels_padded)
+    idx_part, out_part, n_part = w.d_idx[v_lo:v_hi], out[v_lo * out_bytes:v_hi * out_bytes], v_hi - v_lo
 
     def step(k: int):
         g.propagate(tfs[k % n_tf], nodes, st)
-        g.colorize(w.d_idx, w.n_voxels_padded, nodes, out, fmt=fmt, stream=st)
+        g.colorize(idx_part, n_part, nodes, out_part, fmt=fmt, stream=st)
 
     def barrier():
         if world > 1:
@@ -274,7 +292,7 @@ def run_b200(args) -> dict:
             e[0].record(stream)
             g.propagate(tfs[(args.warmup + k) % n_tf], nodes, st)
             e[1].record(stream)
-            g.colorize(w.d_idx, w.n_voxels_padded, nodes, out, fmt=fmt, stream=st)
+            g.colorize(idx_part, n_part, nodes, out_part, fmt=fmt, stream=st)
             e[2].record(stream)
         t_end.record(stream)
         barrier()
@@ -419,20 +437,20 @@ def run_b200(args) -> dict:
     if not args.no_e2e:
         ke = args.e2e_steps or min(K, 8)
         tf_pinned = [torch.from_numpy(w.tf(u)).pin_memory() for u in range(min(n_tf, ke))]
-        out_host = torch.empty(w.n_voxels_padded * out_bytes, dtype=torch.uint8).pin_memory()
+        out_host = torch.empty(max(n_part, 1) * out_bytes, dtype=torch.uint8).pin_memory()
         for k in range(2):
-            g.tf_update_host(tf_pinned[k % len(tf_pinned)], nodes, w.d_idx, w.n_voxels_padded, out, out_host, fmt=fmt, stream=st)
+            g.tf_update_host(tf_pinned[k % len(tf_pinned)], nodes, idx_part, n_part, out_part, out_host, fmt=fmt, stream=st)
         barrier()
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         e0.record(stream)
         for k in range(ke):
-            g.tf_update_host(tf_pinned[k % len(tf_pinned)], nodes, w.d_idx, w.n_voxels_padded, out, out_host, fmt=fmt, stream=st)
+            g.tf_update_host(tf_pinned[k % len(tf_pinned)], nodes, idx_part, n_part, out_part, out_host, fmt=fmt, stream=st)
         e1.record(stream)
         barrier()
         e2e_ms = e0.elapsed_time(e1)
         e2e_ms = max_over_ranks(e2e_ms, world, "cuda")
-        e2e = {"value": aggregate_value(e2e_ms / ke, world), "unit": UNIT, "h2d_bytes_per_step": int(w.n_leaves * 16),
-               "d2h_bytes_per_step": int(w.n_voxels_padded * out_bytes), "steps": ke,
+        e2e = {"value": e2e_ms / ke if slab else aggregate_value(e2e_ms / ke, world), "unit": UNIT,
+               "h2d_bytes_per_step": int(w.n_leaves * 16), "d2h_bytes_per_step": int(n_part * out_bytes), "steps": ke,
                "what": "mg_tf_update_host: pinned-host TF -> H2D -> propagate -> colourise all levels -> D2H of the whole "
                        "mipmap into pinned host memory (PCIe-bound)"}
         del out_host
@@ -447,15 +465,16 @@ def run_b200(args) -> dict:
     bpv = BYTES_PER_VOXEL[args.format]
     col_avg = float(col_ms.mean())
     prop_avg = float(prop_ms.mean())
-    algo_bytes = float(bpv) * w.n_voxels
+    algo_bytes = float(bpv) * w.n_voxels * (n_part / max(1, w.n_voxels_padded))      # rank 0's share (all of it unless --partition slab)
     achieved = algo_bytes / (col_avg * 1e-3) / 1e9
     kernel = "k_colorize"
     res = {
-        "metric": METRIC, "value": aggregate_value(ms_per_step, world), "unit": UNIT, "n_gpus": world, "steps": K, "warmup": args.warmup,
-        "ms_per_step": ms_per_step, "higher_is_better": False, "scaling": "weak", "vs_baseline": None,
+        "metric": METRIC, "value": ms_per_step if slab else aggregate_value(ms_per_step, world), "unit": UNIT, "n_gpus": world,
+        "steps": K, "warmup": args.warmup,
+        "ms_per_step": ms_per_step, "higher_is_better": False, "scaling": "strong" if slab else "weak", "vs_baseline": None,
         "dtype": "f32", "data": "synthetic", "config": workload_config(w, args, world),
         "propagate_ms": prop_avg, "colorize_ms": col_avg, "propagate_ms_min": float(prop_ms.min()), "colorize_ms_min": float(col_ms.min()),
-        "nodes_per_s": n_internal / (prop_avg * 1e-3), "voxels_per_s": w.n_voxels / (col_avg * 1e-3),
+        "nodes_per_s": n_internal / (prop_avg * 1e-3), "voxels_per_s": w.n_voxels * (n_part / max(1, w.n_voxels_padded)) / (col_avg * 1e-3),
         "hbm_gbs_step": (algo_bytes + BYTES_PER_NODE_L2 * n_internal) / (ms_per_step * 1e-3) / 1e9,
         "frac_of_nominal_8TBs": achieved / NOMINAL_HBM_GBS,
         "roofline": {"bound": "hbm", "kernel": kernel, "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
