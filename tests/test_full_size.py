@@ -1,8 +1,8 @@
 """Full-size parity: BASELINE.json's configs in the launch configuration bench.py times.
 
-The whole workload is assembled exactly as bench.py does (workload.make: GPU volume generator ->
-host builder -> mg_load_graph -> ONE concatenated node-index mipmap, ONE mg_colorize call over all
-levels).  The oracle cannot colourise 1.4 G voxels element by element in seconds, so:
+The whole workload is assembled exactly as bench.py does (workload.make with the device front end of the
+histogram mipmap: GPU volume generator -> mg_mipmap_leaf_index / mg_mipmap_front_level1 -> host builder ->
+mg_load_graph -> ONE concatenated node-index mipmap, ONE mg_colorize call over all levels).  The oracle cannot colourise 1.4 G voxels element by element in seconds, so:
   * node colours: EVERY node against the same-graph oracle (O-4), leaves bit-exact, max-abs <= 1e-5;
   * level 0 (87 % of the voxels): EVERY voxel -- its colour must be the RGBA8 code of TF[S(v)] (I5, L223),
     with S from the input generator (not from the builder) and the 4 x n_leaves codes from the oracle;
@@ -93,10 +93,11 @@ def _sample_positions(n, k, seed, stream):
 @pytest.mark.parametrize("cfg_id", [3, 2, 4])
 def test_volume_config_full_size(libs, cfg_id):
     mg, workload = libs
-    w = workload.make(cfg_id, keep_seg=True)
+    w = workload.make(cfg_id, keep_seg=True, device_mipmap=True)              # the assembly bench.py uses by default
     try:
         c = synth.CONFIGS[cfg_id]
         X, Y, Z = c["dims"]
+        assert w.host_idx[0] is None                                             # level 0 never existed on the host
         assert w.mip_dims == oracle.mip_dims((X, Y, Z))                     # O-1 at full size (Table 2 totals)
         assert w.n_voxels == sum(x * y * z for x, y, z in w.mip_dims)
         tf = w.tf(1)
@@ -126,7 +127,9 @@ def test_volume_config_full_size(libs, cfg_id):
         for l, (s0, nv) in enumerate(zip(w.level_start, w.level_voxels)):
             pos = _sample_positions(nv, 200000, 77 + cfg_id, l)
             got = out4[torch.from_numpy(pos + s0).cuda()].cpu().numpy()
-            idx = w.host_idx[l].reshape(-1)[pos]
+            # node indices the oracle looks up: the builder's for levels >= 1; level 0 = leaf number of S(v), taken
+            # from the generator's volume (never from the device front end that produced the GPU's copy)
+            idx = (seg_index if l == 0 else w.host_idx[l]).reshape(-1)[pos]
             assert _rgba8_close(got, oracle.lookup(idx, ref_nodes)), f"level {l}"
             out_host_levels.append((pos, got))
             pad_end = w.level_start[l + 1] if l + 1 < len(w.level_start) else w.n_voxels_padded
@@ -155,12 +158,12 @@ def test_volume_config_full_size(libs, cfg_id):
                 worst = max(worst, float(np.abs(nodes_host[idx_l[v]] - direct).max()))
         assert worst <= TOL_DIRECT, worst
         print(f"cfg {cfg_id}: {w.stats['n_nodes']} nodes depth {w.stats['depth']}, max |graph - direct| on samples = {worst:.2e}")
-        _check_render_full_size(mg, w, tf)
+        _check_render_full_size(mg, w, tf, seg_index)
     finally:
         w.close()
 
 
-def _check_render_full_size(mg, w, tf):
+def _check_render_full_size(mg, w, tf, seg_index):
     """NEXT-2 in bench.py's launch configuration (synth.render_view: 1600 x 1200, 0.5-voxel steps, ESS 1e-8,
     spacing 1:1:7): sampled pixels + the image corners against the oracle's per-ray march on the same
     pyramid (tolerance: tests/test_gpu_render.py), and the ESS-off image must equal the ESS-on image."""
@@ -198,7 +201,8 @@ def _check_render_full_size(mg, w, tf):
     hg = w.host_graph
     pal = oracle.graph_eval(hg["child_a"], hg["child_b"], hg["weight"], hg["n_leaves"], rtf.astype(np.float64))
     flat = np.zeros(w.n_voxels_padded, dtype=np.uint32)
-    for s0, lv in zip(w.level_start, w.host_idx):
+    for l, s0 in enumerate(w.level_start):                          # level 0 from the generator's volume, not from the device
+        lv = seg_index if l == 0 else w.host_idx[l]
         flat[s0:s0 + lv.size] = lv.reshape(-1)
     ref, _ = oracle.render_pixels(None, pal, view, ij, flat=(flat, w.level_start, np.array(w.mip_dims)))
     err = np.abs(got[ij[:, 1], ij[:, 0]] - ref).max()
