@@ -345,7 +345,7 @@ int build_mipmap(const uint32_t* seg, uint64_t X, uint64_t Y, uint64_t Z, int n_
                 for (uint64_t i = 0; i < px; i++) {
                     const uint64_t x0 = 2 * i;
                     const int nx = (x0 + 1 < cx) ? 2 : 1;
-                    uint32_t ch[8];
+                    uint32_t ch[8] = {0, 0, 0, 0, 0, 0, 0, 0};
                     int n = 0;
                     for (int q = 0; q < n_rows; q++) {
                         ch[n++] = rows[q][x0];

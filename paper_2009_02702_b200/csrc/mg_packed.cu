@@ -37,12 +37,6 @@ struct PackedParams {
     uint32_t n_levels;
 };
 
-__device__ __forceinline__ uint4 ld_cs_u4(const uint4* p)
-{
-    uint4 r;
-    asm volatile("ld.global.cs.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "l"(p));
-    return r;
-}
 __device__ __forceinline__ void st_cs_u4(uint4* p, uint4 v)
 {
     asm volatile("st.global.cs.v4.u32 [%0], {%1,%2,%3,%4};" :: "l"(p), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
