@@ -202,7 +202,7 @@ def max_over_ranks(value: float, world: int, device="cpu") -> float:
     return float(t.item())
 
 
-def slab_range(n_voxels_padded: int, rank: int, world: int, align: int = 2048):
+def slab_range(n_voxels_padded: int, rank: int, world: int, align: int = 4096):
     """Voxel range [lo, hi) of rank's slab: the concatenated mipmap cut into `world` contiguous pieces whose
     boundaries are multiples of `align` voxels (one colourise CTA; keeps every 16-byte vector aligned).  The
     pieces are disjoint, cover [0, n_voxels_padded) and differ by at most `align` voxels."""

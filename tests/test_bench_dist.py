@@ -78,12 +78,12 @@ def test_slab_ranges_partition_the_mipmap():
     """bench.py --partition slab: the ranks' voxel ranges are disjoint, aligned, balanced and cover everything."""
     sys.path.insert(0, ROOT)
     import bench
-    for n in (1438087680, 2048, 2049, 5, 299648):
+    for n in (1438087680, 4096, 4097, 5, 299648):
         for world in (1, 2, 3, 4, 8):
             r = [bench.slab_range(n, k, world) for k in range(world)]
             assert r[0][0] == 0 and r[-1][1] == n
             for (a0, a1), (b0, b1) in zip(r, r[1:]):
                 assert a1 == b0 and a0 <= a1
             sizes = [b - a for a, b in r]
-            assert all(a % 2048 == 0 for a, _ in r)
-            assert max(sizes) - min(sizes) <= 2048 or n < 2048 * world
+            assert all(a % 4096 == 0 for a, _ in r)
+            assert max(sizes) - min(sizes) <= 4096 or n < 4096 * world
