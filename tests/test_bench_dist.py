@@ -87,3 +87,13 @@ def test_slab_ranges_partition_the_mipmap():
             sizes = [b - a for a, b in r]
             assert all(a % 4096 == 0 for a, _ in r)
             assert max(sizes) - min(sizes) <= 4096 or n < 4096 * world
+
+
+def test_committed_traffic_table_is_readable_by_bench():
+    """roofline.traffic comes from profiles/roofline_traffic.csv (ncu dram bytes per launch of the dominant kernel)."""
+    sys.path.insert(0, ROOT)
+    import bench
+    t = bench.ncu_traffic("cfg3_neocortex_shaped", "k_colorize")
+    assert t is not None and 0.9 * 8 * 1438087061 < t < 1.1 * 8 * 1438087061          # about the algorithmic 8 B / voxel
+    assert bench.ncu_traffic("cfg5_dag_stress", "k_colorize") > 8 * 512 ** 3         # random gathers: far above it
+    assert bench.ncu_traffic("no_such_workload", "k_colorize") is None
