@@ -64,24 +64,36 @@ struct Cell {
     float fx, fy, fz;
 };
 
-__device__ __forceinline__ void fetch_cell(const RenderParams& P, int l, double px, double py, double pz, Cell& c)
+// q = floor(p 2^32): the sample position in 32.32 fixed point.  u = p / 2^l - 1/2 becomes U = (q >> l) - 2^31, whose
+// integer part is the voxel index and whose low 32 bits are the interpolation fraction (to 2^-32 of a voxel) -- integer
+// shifts instead of fp64 multiplies, floors and subtractions per level.  SMALL: every level has < 2^32 voxels, so the
+// row offsets are computed in 32 bits.
+template <bool SMALL>
+__device__ __forceinline__ void fetch_cell(const RenderParams& P, int l, long long qx, long long qy, long long qz, Cell& c)
 {
-    const double sc = __hiloint2double((1023 - l) << 20, 0);            // 2^-l
-    const double ux = fma(px, sc, -0.5), uy = fma(py, sc, -0.5), uz = fma(pz, sc, -0.5);
-    const double flx = floor(ux), fly = floor(uy), flz = floor(uz);
-    c.fx = (float)(ux - flx); c.fy = (float)(uy - fly); c.fz = (float)(uz - flz);
+    const long long Ux = (qx >> l) - (1ll << 31), Uy = (qy >> l) - (1ll << 31), Uz = (qz >> l) - (1ll << 31);
+    c.fx = __uint2float_rn((unsigned)Ux) * 2.3283064365386963e-10f;
+    c.fy = __uint2float_rn((unsigned)Uy) * 2.3283064365386963e-10f;
+    c.fz = __uint2float_rn((unsigned)Uz) * 2.3283064365386963e-10f;
     const int X = P.dim[l][0], Y = P.dim[l][1], Z = P.dim[l][2];
-    const int ix = (int)flx, iy = (int)fly, iz = (int)flz;
+    const int ix = (int)(Ux >> 32), iy = (int)(Uy >> 32), iz = (int)(Uz >> 32);
     const int x0 = clampi(ix, X - 1), x1 = clampi(ix + 1, X - 1);
     const int y0 = clampi(iy, Y - 1), y1 = clampi(iy + 1, Y - 1);
     const int z0 = clampi(iz, Z - 1), z1 = clampi(iz + 1, Z - 1);
     const uint32_t* base = P.idx + P.off[l];
-    const uint32_t* r00 = base + ((size_t)z0 * Y + y0) * X;
-    const uint32_t* r01 = base + ((size_t)z0 * Y + y1) * X;
-    const uint32_t* r10 = base + ((size_t)z1 * Y + y0) * X;
-    const uint32_t* r11 = base + ((size_t)z1 * Y + y1) * X;
-    c.n[0] = __ldg(r00 + x0); c.n[1] = __ldg(r00 + x1); c.n[2] = __ldg(r01 + x0); c.n[3] = __ldg(r01 + x1);
-    c.n[4] = __ldg(r10 + x0); c.n[5] = __ldg(r10 + x1); c.n[6] = __ldg(r11 + x0); c.n[7] = __ldg(r11 + x1);
+    if (SMALL) {
+        const unsigned r00 = ((unsigned)z0 * Y + y0) * X, r01 = ((unsigned)z0 * Y + y1) * X;
+        const unsigned r10 = ((unsigned)z1 * Y + y0) * X, r11 = ((unsigned)z1 * Y + y1) * X;
+        c.n[0] = __ldg(base + (r00 + x0)); c.n[1] = __ldg(base + (r00 + x1)); c.n[2] = __ldg(base + (r01 + x0)); c.n[3] = __ldg(base + (r01 + x1));
+        c.n[4] = __ldg(base + (r10 + x0)); c.n[5] = __ldg(base + (r10 + x1)); c.n[6] = __ldg(base + (r11 + x0)); c.n[7] = __ldg(base + (r11 + x1));
+    } else {
+        const uint32_t* r00 = base + ((size_t)z0 * Y + y0) * X;
+        const uint32_t* r01 = base + ((size_t)z0 * Y + y1) * X;
+        const uint32_t* r10 = base + ((size_t)z1 * Y + y0) * X;
+        const uint32_t* r11 = base + ((size_t)z1 * Y + y1) * X;
+        c.n[0] = __ldg(r00 + x0); c.n[1] = __ldg(r00 + x1); c.n[2] = __ldg(r01 + x0); c.n[3] = __ldg(r01 + x1);
+        c.n[4] = __ldg(r10 + x0); c.n[5] = __ldg(r10 + x1); c.n[6] = __ldg(r11 + x0); c.n[7] = __ldg(r11 + x1);
+    }
 }
 
 __device__ __forceinline__ bool one_node(const Cell& c)
@@ -141,6 +153,7 @@ __device__ __forceinline__ bool inside_block(const Block& B, int m2, int hx, int
     return in;
 }
 
+template <bool SMALL>
 __global__ void __launch_bounds__(kTileX * kTileY)
 k_render(const __grid_constant__ RenderParams P)
 {
@@ -201,6 +214,8 @@ k_render(const __grid_constant__ RenderParams P)
                 const double px = fma(ts, d[0], P.eye[0]) * P.inv_s[0];
                 const double py = fma(ts, d[1], P.eye[1]) * P.inv_s[1];
                 const double pz = fma(ts, d[2], P.eye[2]) * P.inv_s[2];
+                const long long qx = __double2ll_rd(px * 4294967296.0), qy = __double2ll_rd(py * 4294967296.0),
+                                qz = __double2ll_rd(pz * 4294967296.0);                    // 32.32 fixed point (see fetch_cell)
                 const float fl = floorf(lambda);
                 const int l0 = (int)fl;
                 const int l1 = min(l0 + 1, l_max);
@@ -210,7 +225,7 @@ k_render(const __grid_constant__ RenderParams P)
                 const int m2 = 1 << l1;                                          // 2 m, m = 2^l1 / 2
                 const bool probe = ess && empty_mode;                            // R6: only where the ray is in empty space
                 if (probe) {                                                     // in half-voxel integers
-                    hx = (int)floor(px + px); hy = (int)floor(py + py); hz = (int)floor(pz + pz);
+                    hx = (int)(qx >> 31); hy = (int)(qy >> 31); hz = (int)(qz >> 31);                 // floor(2 p)
                     if (inside_block(E, m2, hx, hy, hz)) {
                         n_skip++;
                         continue;
@@ -222,7 +237,7 @@ k_render(const __grid_constant__ RenderParams P)
                 // climb of R6 so that the two dependent chains overlap.
                 Cell cell;
                 const bool coarse_first = uni && f != 0.f;                        // frac(lambda) = 0: only level l0 is needed
-                fetch_cell(P, coarse_first ? l1 : l0, px, py, pz, cell);
+                fetch_cell<SMALL>(P, coarse_first ? l1 : l0, qx, qy, qz, cell);
                 if (probe) {
                     // Empty mode and not inside the remembered block: the oracle forgets its block and climbs again
                     // from level l1 + 1.  The climb is a pure
@@ -255,12 +270,12 @@ k_render(const __grid_constant__ RenderParams P)
                     float4 c1 = make_float4(0.f, 0.f, 0.f, 0.f);
                     if (coarse_first) {                                          // cell = coarse level (f != 0, l0 < l1)
                         c1 = shade_cell(P, cell);
-                        fetch_cell(P, l0, px, py, pz, cell);
+                        fetch_cell<SMALL>(P, l0, qx, qy, qz, cell);
                         c = shade_cell(P, cell);
                     } else {                                                     // cell = fine level
                         c = shade_cell(P, cell);
                         if (f != 0.f) {
-                            fetch_cell(P, l1, px, py, pz, cell);
+                            fetch_cell<SMALL>(P, l1, qx, qy, qz, cell);
                             c1 = shade_cell(P, cell);
                         }
                     }
@@ -378,7 +393,11 @@ extern "C" int mg_render(mg_graph* g, const uint32_t* node_idx_mipmap, const mg_
     P.cutoff = view->alpha_cutoff;
     P.n_leaves = (view->flags & MG_VIEW_HISTOGRAM_MIPMAP) ? g->n_leaves : 0u;
     const dim3 grid((P.W + kTileX - 1) / kTileX, (P.H + kTileY - 1) / kTileY);
-    k_render<<<grid, kTileX * kTileY, 0, (cudaStream_t)stream>>>(P);
+    bool small = true;
+    for (uint32_t l = 0; l < mip->n_levels; l++)
+        small = small && (uint64_t)mip->level_dim[l][0] * mip->level_dim[l][1] * mip->level_dim[l][2] < (1ull << 32);
+    if (small) k_render<true><<<grid, kTileX * kTileY, 0, (cudaStream_t)stream>>>(P);
+    else k_render<false><<<grid, kTileX * kTileY, 0, (cudaStream_t)stream>>>(P);
     MG_CUDA(cudaGetLastError());
     mg::count_launch();
     return MG_OK;
