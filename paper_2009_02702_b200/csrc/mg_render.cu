@@ -122,6 +122,30 @@ __device__ __forceinline__ float4 shade_cell(const RenderParams& P, const Cell& 
     return acc;
 }
 
+// R4: alpha' = 1 - (1 - alpha)^e = -expm1(e log1p(-alpha)), accurate to ~1e-7 relative like the libm pair, but the
+// common case of a translucent sample (alpha <= 1/16, |e log1p(-alpha)| < 1/8) costs two short polynomials instead of
+// two libm calls: log1p(-a) = -a (1 + a/2 + ... + a^6/7) (truncation < a^7/8) and expm1(y) = y (1 + y/2 + ... + y^5/720)
+// (truncation < y^7/5040).
+__device__ __forceinline__ float opacity_correct(float alpha, float e)
+{
+    if (alpha <= 0.f) return 0.f;
+    float y;                                                             // e log1p(-alpha) <= 0
+    if (alpha <= 0.0625f) {
+        float p = fmaf(alpha, 1.f / 7.f, 1.f / 6.f);
+        p = fmaf(alpha, p, 0.2f); p = fmaf(alpha, p, 0.25f); p = fmaf(alpha, p, 1.f / 3.f); p = fmaf(alpha, p, 0.5f);
+        p = fmaf(alpha, p, 1.f);
+        y = -e * (alpha * p);
+    } else {
+        y = e * log1pf(-alpha);                                          // alpha = 1: -inf, and the result is 1
+    }
+    if (y > -0.125f) {
+        float p = fmaf(y, 1.f / 720.f, 1.f / 120.f);
+        p = fmaf(y, p, 1.f / 24.f); p = fmaf(y, p, 1.f / 6.f); p = fmaf(y, p, 0.5f); p = fmaf(y, p, 1.f);
+        return -y * p;
+    }
+    return -expm1f(y);
+}
+
 // R6 block: voxel-aligned box in level-0 coordinates, kept in HALF-voxel integers so that the oracle's
 // tests on p become integer tests on h = floor(2 p):  p < lo + m  <=>  h < 2 lo + 2 m  and
 // p >= hi - m  <=>  h >= 2 hi - 2 m  (2 lo, 2 hi, 2 m = 2^l1 are integers).  A face on the volume's
@@ -288,7 +312,7 @@ k_render(const __grid_constant__ RenderParams P)
                 const float alpha = fminf(fmaxf(c.w, 0.f), 1.f);
                 empty_mode = (double)alpha < P.thr;                               // R6
                 const float e = (float)de * P.inv_ref;
-                const float ac = -expm1f(e * log1pf(-alpha));                     // 1 - (1 - alpha)^e
+                const float ac = opacity_correct(alpha, e);                       // 1 - (1 - alpha)^e
                 const double wgt = (1.0 - A) * (double)ac;                        // R5, accumulated in fp64
                 Cr = fma(wgt, (double)c.x, Cr); Cg = fma(wgt, (double)c.y, Cg); Cb = fma(wgt, (double)c.z, Cb);
                 A += wgt;
