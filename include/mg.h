@@ -256,8 +256,9 @@ int mg_propagate_attr(mg_graph *g, const float *leaf_attr, float *node_attr, uin
  *      a sample is fetched, climb from level floor(lambda)+2 upwards while the parent voxel's palette opacity
  *      is < ess_threshold; samples whose whole 2 x 8-voxel footprint lies in the largest such block are not
  *      fetched.  ess_threshold < 0 disables it.
- * Arithmetic: ray geometry (t, step, sample position, trilinear fractions, block tests) in fp64;
- * fractional LOD, interpolation weights, colours, opacity correction and compositing in fp32.
+ * Arithmetic: ray parameter, step and sample position in fp64 (positions then in 32.32 fixed point for the per-level
+ * voxel indices, fractions and block tests); fractional LOD, interpolation weights, colours and opacity correction in
+ * fp32; compositing sums in fp64.
  * ------------------------------------------------------------------------------------------------ */
 #define MG_MAX_MIP_LEVELS 24
 

@@ -20,11 +20,11 @@
 // the 8 coarse voxels name one leaf all 16 taps are that leaf: segment interiors cost 8 index
 // gathers + 1 palette gather instead of 16 + 2.  The block tests of R6 run on floor(2 p) in
 // integers (exactly the oracle's comparisons, see Block).
-// Arithmetic: t, the step, the sample position, the trilinear fractions and the block tests in fp64
-// (the B200's fp64 pipe is half the fp32 rate and the loop is gather-latency-bound, so this is free
-// and keeps sample positions within 1e-12 voxels of the oracle's); the fractional LOD, the weights,
-// colours and opacity correction in fp32; the compositing sums C and A in fp64 (thousands of
-// samples per ray would otherwise add their fp32 rounding errors).
+// Arithmetic: t, the step and the sample position in fp64 (the B200's fp64 pipe is half the fp32 rate); the position
+// is then held in 32.32 fixed point, from which the voxel indices, the trilinear fractions (to 2^-32 voxel) and the
+// block tests of every level follow by integer shifts; the fractional LOD, the weights, colours and opacity correction
+// in fp32; the compositing sums C and A in fp64 (thousands of samples per ray would otherwise add their fp32
+// rounding errors).
 #include <math.h>
 
 #include <cstring>
