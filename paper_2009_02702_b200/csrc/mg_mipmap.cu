@@ -18,34 +18,98 @@ namespace {
 constexpr int kThreads = 256;
 constexpr uint32_t kNone = 0xFFFFFFFFu;
 
-__global__ void k_max_id(const uint32_t* __restrict__ seg, uint64_t n, uint32_t* out)
+// The three leaf-index passes stream the 4-byte volume once each: 16-byte loads, two per thread in flight, the
+// 0-3 elements before the first 16-byte boundary and after the last whole vector taken one by one by block 0.
+struct Span { uint64_t head, nv, tail; };                            // [0,head) | nv uint4 from head | [tail,n)
+__device__ __forceinline__ Span span_of(const void* p, uint64_t n)
 {
+    uint64_t head = ((16 - ((uintptr_t)p & 15)) & 15) / 4;
+    if (head > n) head = n;
+    const uint64_t nv = (n - head) / 4;
+    return {head, nv, head + 4 * nv};
+}
+// index of the i-th ragged element (i < head + n - tail)
+__device__ __forceinline__ uint64_t ragged(const Span& s, uint64_t i) { return i < s.head ? i : s.tail + (i - s.head); }
+
+__global__ void __launch_bounds__(kThreads) k_max_id(const uint32_t* __restrict__ seg, uint64_t n, uint32_t* out)
+{
+    const Span sp = span_of(seg, n);
+    const uint4* v4 = reinterpret_cast<const uint4*>(seg + sp.head);
+    const uint64_t stride = (uint64_t)gridDim.x * kThreads;
     uint32_t m = 0;
-    for (uint64_t v = (uint64_t)blockIdx.x * kThreads + threadIdx.x; v < n; v += (uint64_t)gridDim.x * kThreads) m = max(m, __ldg(seg + v));
+    uint64_t i = (uint64_t)blockIdx.x * kThreads + threadIdx.x;
+    for (; i + stride < sp.nv; i += 2 * stride) {
+        const uint4 a = __ldcs(v4 + i), b = __ldcs(v4 + i + stride);
+        m = max(max(max(a.x, a.y), max(a.z, a.w)), max(m, max(max(b.x, b.y), max(b.z, b.w))));
+    }
+    if (i < sp.nv) {
+        const uint4 a = __ldcs(v4 + i);
+        m = max(m, max(max(a.x, a.y), max(a.z, a.w)));
+    }
+    if (blockIdx.x == 0 && threadIdx.x < sp.head + (n - sp.tail)) m = max(m, seg[ragged(sp, threadIdx.x)]);
     m = __reduce_max_sync(0xffffffffu, m);
-    if ((threadIdx.x & 31) == 0) atomicMax(out, m);
+    if ((threadIdx.x & 31) == 0 && m) atomicMax(out, m);
 }
 
-__global__ void k_mark_ids(const uint32_t* __restrict__ seg, uint64_t n, uint8_t* present)
+// test first: a handful of hot bytes, mostly already set (racing stores of the same value)
+__device__ __forceinline__ void mark(uint8_t* present, uint32_t s, uint32_t& last)
 {
-    uint32_t last = kNone;
-    for (uint64_t v = (uint64_t)blockIdx.x * kThreads + threadIdx.x; v < n; v += (uint64_t)gridDim.x * kThreads) {
-        const uint32_t s = __ldg(seg + v);
-        if (s != last) {                                              // test first: a handful of hot bytes, mostly already set
-            if (!present[s]) present[s] = 1;                          // (racing stores of the same value)
-            last = s;
-        }
+    if (s != last) {
+        if (!present[s]) present[s] = 1;
+        last = s;
     }
 }
 
-// level0[v] = leaf_of[S(v)]; seg and level0 may be the same buffer (element-wise).
-__global__ void k_map_ids(const uint32_t* seg, uint64_t n, const uint32_t* __restrict__ leaf_of, uint32_t* level0)
+__global__ void __launch_bounds__(kThreads) k_mark_ids(const uint32_t* __restrict__ seg, uint64_t n, uint8_t* present)
 {
-    for (uint64_t v = (uint64_t)blockIdx.x * kThreads + threadIdx.x; v < n; v += (uint64_t)gridDim.x * kThreads)
-        level0[v] = __ldg(leaf_of + seg[v]);
+    const Span sp = span_of(seg, n);
+    const uint4* v4 = reinterpret_cast<const uint4*>(seg + sp.head);
+    const uint64_t stride = (uint64_t)gridDim.x * kThreads;
+    uint32_t last = kNone;
+    uint64_t i = (uint64_t)blockIdx.x * kThreads + threadIdx.x;
+    for (; i + stride < sp.nv; i += 2 * stride) {
+        const uint4 a = __ldcs(v4 + i), b = __ldcs(v4 + i + stride);
+        mark(present, a.x, last); mark(present, a.y, last); mark(present, a.z, last); mark(present, a.w, last);
+        mark(present, b.x, last); mark(present, b.y, last); mark(present, b.z, last); mark(present, b.w, last);
+    }
+    if (i < sp.nv) {
+        const uint4 a = __ldcs(v4 + i);
+        mark(present, a.x, last); mark(present, a.y, last); mark(present, a.z, last); mark(present, a.w, last);
+    }
+    if (blockIdx.x == 0 && threadIdx.x < sp.head + (n - sp.tail)) mark(present, seg[ragged(sp, threadIdx.x)], last);
 }
 
-// One thread per level-1 parent (x fastest).  Children t = 4 dz + 2 dy + dx; kNone outside the volume.
+// level0[v] = leaf_of[S(v)]; seg and level0 may be the same buffer (element-wise: every thread reads its elements
+// before it writes them, and nobody else touches them).  VEC needs seg and level0 congruent modulo 16 bytes.
+template <bool VEC>
+__global__ void __launch_bounds__(kThreads) k_map_ids(const uint32_t* seg, uint64_t n, const uint32_t* __restrict__ leaf_of, uint32_t* level0)
+{
+    const uint64_t stride = (uint64_t)gridDim.x * kThreads;
+    uint64_t i = (uint64_t)blockIdx.x * kThreads + threadIdx.x;
+    if (!VEC) {
+        for (; i < n; i += stride) level0[i] = __ldg(leaf_of + seg[i]);
+        return;
+    }
+    const Span sp = span_of(seg, n);
+    const uint4* v4 = reinterpret_cast<const uint4*>(seg + sp.head);
+    uint4* o4 = reinterpret_cast<uint4*>(level0 + sp.head);
+    auto map4 = [&](const uint4 a) { return make_uint4(__ldg(leaf_of + a.x), __ldg(leaf_of + a.y), __ldg(leaf_of + a.z), __ldg(leaf_of + a.w)); };
+    for (; i + stride < sp.nv; i += 2 * stride) {
+        const uint4 a = __ldcs(v4 + i), b = __ldcs(v4 + i + stride);
+        const uint4 ra = map4(a), rb = map4(b);
+        o4[i] = ra;
+        o4[i + stride] = rb;
+    }
+    if (i < sp.nv) o4[i] = map4(__ldcs(v4 + i));
+    if (blockIdx.x == 0 && threadIdx.x < sp.head + (n - sp.tail)) {
+        const uint64_t r = ragged(sp, threadIdx.x);
+        level0[r] = __ldg(leaf_of + seg[r]);
+    }
+}
+
+// One thread per level-1 parent (x fastest; n1 < 2^32).  Children t = 4 dz + 2 dy + dx; kNone outside the volume.
+// PAIR (cx even, l0 8-byte aligned): the two x-children of a row always both exist and come as one 8-byte load.
+template <bool PAIR>
 __global__ void __launch_bounds__(kThreads)
 k_front_level1(const uint32_t* __restrict__ l0, uint32_t cx, uint32_t cy, uint32_t cz, uint32_t px, uint32_t py, uint64_t n1,
                uint32_t* __restrict__ level1, uint32_t* __restrict__ mixed_voxel, uint32_t* __restrict__ mixed_children,
@@ -56,11 +120,18 @@ k_front_level1(const uint32_t* __restrict__ l0, uint32_t cx, uint32_t cy, uint32
     uint32_t ch[8];
     bool pure = true;
     if (live) {
-        const uint32_t i = (uint32_t)(v % px), j = (uint32_t)((v / px) % py), k = (uint32_t)(v / ((uint64_t)px * py));
+        const uint32_t v32 = (uint32_t)v, row = v32 / px, i = v32 - row * px, k = row / py, j = row - k * py;
 #pragma unroll
-        for (int t = 0; t < 8; t++) {
+        for (int t = 0; t < 8; t += PAIR ? 2 : 1) {
             const uint32_t x = 2 * i + (t & 1), y = 2 * j + ((t >> 1) & 1), z = 2 * k + (t >> 2);
-            ch[t] = (x < cx && y < cy && z < cz) ? __ldg(l0 + ((uint64_t)z * cy + y) * cx + x) : kNone;
+            const uint64_t at = ((uint64_t)z * cy + y) * cx + x;
+            if (PAIR) {
+                const uint2 c = (y < cy && z < cz) ? __ldcs(reinterpret_cast<const uint2*>(l0 + at)) : make_uint2(kNone, kNone);
+                ch[t] = c.x;
+                ch[t + 1] = c.y;
+            } else {
+                ch[t] = (x < cx && y < cy && z < cz) ? __ldg(l0 + at) : kNone;
+            }
         }
 #pragma unroll
         for (int t = 1; t < 8; t++) pure = pure && (ch[t] == ch[0] || ch[t] == kNone);   // child 0 always exists
@@ -95,7 +166,7 @@ extern "C" int mg_mipmap_leaf_index(const uint32_t* seg_device, uint64_t n_voxel
     }
     *n_leaves = 0;
     cudaStream_t st = (cudaStream_t)stream;
-    const unsigned grid = (unsigned)std::min<uint64_t>((n_voxels + kThreads - 1) / kThreads, 148ull * 16);
+    const unsigned grid = (unsigned)std::min<uint64_t>((n_voxels / 4 + kThreads) / kThreads, 148ull * 8);   // 2048 threads per SM
     uint32_t* d_max = nullptr;
     uint8_t* d_present = nullptr;
     uint32_t* d_leaf_of = nullptr;
@@ -140,7 +211,10 @@ extern "C" int mg_mipmap_leaf_index(const uint32_t* seg_device, uint64_t n_voxel
     }
     MM_CUDA(cudaMalloc(&d_leaf_of, n_ids * sizeof(uint32_t)));
     MM_CUDA(cudaMemcpyAsync(d_leaf_of, leaf_of.data(), n_ids * sizeof(uint32_t), cudaMemcpyHostToDevice, st));
-    k_map_ids<<<grid, kThreads, 0, st>>>(seg_device, n_voxels, d_leaf_of, level0_device);
+    if ((((uintptr_t)seg_device ^ (uintptr_t)level0_device) & 15) == 0)
+        k_map_ids<true><<<grid, kThreads, 0, st>>>(seg_device, n_voxels, d_leaf_of, level0_device);
+    else
+        k_map_ids<false><<<grid, kThreads, 0, st>>>(seg_device, n_voxels, d_leaf_of, level0_device);
     MM_CUDA(cudaGetLastError());
     mg::count_launch();
     MM_CUDA(cudaStreamSynchronize(st));                                // leaf_of (host) and the temporaries die here
@@ -169,9 +243,13 @@ extern "C" int mg_mipmap_front_level1(const uint32_t* level0_device, uint64_t X,
     MG_CUDA(cudaMalloc(&d_counter, sizeof(unsigned long long)));
     cudaError_t e = cudaMemsetAsync(d_counter, 0, sizeof(unsigned long long), st);
     if (e == cudaSuccess) {
-        k_front_level1<<<(unsigned)((n1 + kThreads - 1) / kThreads), kThreads, 0, st>>>(
-            level0_device, (uint32_t)X, (uint32_t)Y, (uint32_t)Z, (uint32_t)px, (uint32_t)py, n1, level1_device, mixed_voxel_device,
-            mixed_children_device, capacity, d_counter);
+        const unsigned grid = (unsigned)((n1 + kThreads - 1) / kThreads);
+        if (X % 2 == 0 && ((uintptr_t)level0_device & 7) == 0)
+            k_front_level1<true><<<grid, kThreads, 0, st>>>(level0_device, (uint32_t)X, (uint32_t)Y, (uint32_t)Z, (uint32_t)px, (uint32_t)py,
+                                                            n1, level1_device, mixed_voxel_device, mixed_children_device, capacity, d_counter);
+        else
+            k_front_level1<false><<<grid, kThreads, 0, st>>>(level0_device, (uint32_t)X, (uint32_t)Y, (uint32_t)Z, (uint32_t)px, (uint32_t)py,
+                                                             n1, level1_device, mixed_voxel_device, mixed_children_device, capacity, d_counter);
         e = cudaGetLastError();
         mg::count_launch();
     }

@@ -90,6 +90,43 @@ def test_front_end_in_place_and_small_capacity(libs):
         mg.mipmap_leaf_index(_dev(big), big.size, torch.zeros(big.size, dtype=torch.int32, device="cuda"))
 
 
+@pytest.mark.parametrize("dims", [(24, 10, 9), (23, 10, 9), (6, 1, 1)])
+@pytest.mark.parametrize("off_in,off_out", [(0, 0), (1, 1), (2, 2), (3, 3), (1, 0), (0, 3), (2, 1)])
+def test_front_end_at_any_alignment(libs, dims, off_in, off_out):
+    """The kernels take 16-byte (leaf index) and 8-byte (level 1) loads where the pointers allow it: every offset of
+    the volume and of level 0 from a 16-byte boundary, equal or not, even and odd X, gives the aligned result."""
+    mg, _ = libs
+    X, Y, Z = dims
+    seg = synth.voronoi_volume(dims, synth.voronoi_seeds(dims, min(11, X * Y * Z // 2), 73)) * np.uint32(5) + np.uint32(1)
+    ref_ids, ref_l0 = oracle.leaf_index(seg)
+    n = seg.size
+    buf_in = torch.full((n + 8,), -1, dtype=torch.int32, device="cuda")
+    buf_out = torch.full((n + 8,), -2, dtype=torch.int32, device="cuda")
+    buf_in[off_in:off_in + n] = _dev(seg).reshape(-1)
+    d_l0 = buf_out[off_out:off_out + n]
+    ids = mg.mipmap_leaf_index(buf_in[off_in:off_in + n], n, d_l0)
+    assert np.array_equal(ids, ref_ids)
+    out = buf_out.cpu().numpy()
+    assert np.array_equal(out[off_out:off_out + n].view(np.uint32), ref_l0.reshape(-1))
+    assert (out[:off_out] == -2).all() and (out[off_out + n:] == -2).all()                    # nothing outside is written
+    assert (buf_in.cpu().numpy()[:off_in] == -1).all()
+    # level 1 from the (mis)aligned level 0 == level 1 from an aligned copy
+    pz, py, px = -(-Z // 2), -(-Y // 2), -(-X // 2)
+    n1 = pz * py * px
+    res = []
+    for l0 in (d_l0, d_l0.clone()):
+        d_l1 = torch.full((n1,), 7, dtype=torch.int32, device="cuda")
+        mv = torch.full((n1,), -1, dtype=torch.int32, device="cuda")
+        mc = torch.full((n1, 8), -1, dtype=torch.int32, device="cuda")
+        nm = mg.mipmap_front_level1(l0, (X, Y, Z), d_l1, mv, mc, n1)
+        order = torch.argsort(mv[:nm])
+        res.append((nm, d_l1.cpu(), mv[:nm][order].cpu(), mc[:nm][order].cpu()))
+    assert res[0][0] == res[1][0] and all(torch.equal(a, b) for a, b in zip(res[0][1:], res[1][1:]))
+    H = oracle.histogram_mipmap(ref_l0, ref_ids.size)
+    if len(H) > 1:
+        assert np.array_equal(res[0][1].numpy().view(np.uint32).reshape(pz, py, px) == NONE, (H[1] != 0).sum(axis=-1) > 1)
+
+
 @pytest.mark.parametrize("cfg_id,scale", [(3, 0.08), (2, 0.06), (4, 0.12), (1, 1.0)])
 def test_device_assisted_assembly_equals_the_host_builder(libs, cfg_id, scale):
     """workload.make(device_mipmap=True) vs the host path: same graph, same device mipmap, same stats."""
