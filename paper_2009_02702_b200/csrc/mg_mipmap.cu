@@ -107,19 +107,28 @@ __global__ void __launch_bounds__(kThreads) k_map_ids(const uint32_t* seg, uint6
     }
 }
 
-// One thread per level-1 parent (x fastest; n1 < 2^32).  Children t = 4 dz + 2 dy + dx; kNone outside the volume.
-// PAIR (cx even, l0 8-byte aligned): the two x-children of a row always both exist and come as one 8-byte load.
+// kPar level-1 parents per thread (x fastest; n1 < 2^32), kThreads * kPar consecutive parents per CTA.  Children
+// t = 4 dz + 2 dy + dx; kNone outside the volume.  PAIR (cx even, l0 8-byte aligned): the two x-children of a row
+// always both exist and come as one 8-byte load.  The list slots of a CTA's mixed parents come from ONE atomic on the
+// global counter: on the paper-shaped volumes a quarter of all warps hold a mixed parent, and that many value-returning
+// atomics on one address serialise in L2 to longer than the whole stream takes.
+constexpr int kPar = 4;
+
 template <bool PAIR>
 __global__ void __launch_bounds__(kThreads)
 k_front_level1(const uint32_t* __restrict__ l0, uint32_t cx, uint32_t cy, uint32_t cz, uint32_t px, uint32_t py, uint64_t n1,
                uint32_t* __restrict__ level1, uint32_t* __restrict__ mixed_voxel, uint32_t* __restrict__ mixed_children,
                unsigned long long capacity, unsigned long long* counter)
 {
-    const uint64_t v = (uint64_t)blockIdx.x * kThreads + threadIdx.x;
-    const bool live = v < n1;
-    uint32_t ch[8];
-    bool pure = true;
-    if (live) {
+    __shared__ unsigned warp_total[kThreads / 32];
+    __shared__ unsigned long long cta_base;
+    const uint64_t v0 = (uint64_t)blockIdx.x * (kThreads * kPar) + threadIdx.x;
+    uint32_t ch[kPar][8];
+    unsigned mixed = 0;                                               // bit p: parent p of this thread is mixed
+#pragma unroll
+    for (int p = 0; p < kPar; p++) {
+        const uint64_t v = v0 + (uint64_t)p * kThreads;
+        if (v >= n1) continue;
         const uint32_t v32 = (uint32_t)v, row = v32 / px, i = v32 - row * px, k = row / py, j = row - k * py;
 #pragma unroll
         for (int t = 0; t < 8; t += PAIR ? 2 : 1) {
@@ -127,31 +136,54 @@ k_front_level1(const uint32_t* __restrict__ l0, uint32_t cx, uint32_t cy, uint32
             const uint64_t at = ((uint64_t)z * cy + y) * cx + x;
             if (PAIR) {
                 const uint2 c = (y < cy && z < cz) ? __ldcs(reinterpret_cast<const uint2*>(l0 + at)) : make_uint2(kNone, kNone);
-                ch[t] = c.x;
-                ch[t + 1] = c.y;
+                ch[p][t] = c.x;
+                ch[p][t + 1] = c.y;
             } else {
-                ch[t] = (x < cx && y < cy && z < cz) ? __ldg(l0 + at) : kNone;
+                ch[p][t] = (x < cx && y < cy && z < cz) ? __ldg(l0 + at) : kNone;
             }
         }
-#pragma unroll
-        for (int t = 1; t < 8; t++) pure = pure && (ch[t] == ch[0] || ch[t] == kNone);   // child 0 always exists
-        level1[v] = pure ? ch[0] : kNone;
     }
-    // one atomic per warp for the list slots
-    const unsigned m = __ballot_sync(0xffffffffu, live && !pure);
-    if (m == 0) return;
-    const unsigned lane = threadIdx.x & 31, leader = __ffs(m) - 1;
-    unsigned long long base = 0;
-    if (lane == leader) base = atomicAdd(counter, (unsigned long long)__popc(m));
-    base = __shfl_sync(0xffffffffu, base, leader);
-    if (live && !pure) {
-        const unsigned long long slot = base + __popc(m & ((1u << lane) - 1));
+#pragma unroll
+    for (int p = 0; p < kPar; p++) {
+        const uint64_t v = v0 + (uint64_t)p * kThreads;
+        if (v >= n1) continue;
+        bool pure = true;
+#pragma unroll
+        for (int t = 1; t < 8; t++) pure = pure && (ch[p][t] == ch[p][0] || ch[p][t] == kNone);   // child 0 always exists
+        level1[v] = pure ? ch[p][0] : kNone;
+        if (!pure) mixed |= 1u << p;
+    }
+    // exclusive prefix of the mixed counts over the CTA: shuffles inside a warp, shared memory across the warps
+    const unsigned lane = threadIdx.x & 31, warp = threadIdx.x >> 5, cnt = __popc(mixed);
+    unsigned incl = cnt;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+        const unsigned up = __shfl_up_sync(0xffffffffu, incl, d);
+        if (lane >= d) incl += up;
+    }
+    if (lane == 31) warp_total[warp] = incl;
+    __syncthreads();
+    unsigned before = 0, total = 0;
+#pragma unroll
+    for (int w = 0; w < kThreads / 32; w++) {
+        const unsigned c = warp_total[w];
+        if (w < (int)warp) before += c;
+        total += c;
+    }
+    if (total == 0) return;                                           // uniform over the CTA
+    if (threadIdx.x == 0) cta_base = atomicAdd(counter, (unsigned long long)total);
+    __syncthreads();
+    unsigned long long slot = cta_base + before + (incl - cnt);
+#pragma unroll
+    for (int p = 0; p < kPar; p++) {
+        if (!(mixed & (1u << p))) continue;
         if (slot < capacity) {
-            mixed_voxel[slot] = (uint32_t)v;
+            mixed_voxel[slot] = (uint32_t)(v0 + (uint64_t)p * kThreads);
             uint4* dst = reinterpret_cast<uint4*>(mixed_children + 8 * slot);
-            dst[0] = make_uint4(ch[0], ch[1], ch[2], ch[3]);
-            dst[1] = make_uint4(ch[4], ch[5], ch[6], ch[7]);
+            dst[0] = make_uint4(ch[p][0], ch[p][1], ch[p][2], ch[p][3]);
+            dst[1] = make_uint4(ch[p][4], ch[p][5], ch[p][6], ch[p][7]);
         }
+        slot++;
     }
 }
 
@@ -243,7 +275,7 @@ extern "C" int mg_mipmap_front_level1(const uint32_t* level0_device, uint64_t X,
     MG_CUDA(cudaMalloc(&d_counter, sizeof(unsigned long long)));
     cudaError_t e = cudaMemsetAsync(d_counter, 0, sizeof(unsigned long long), st);
     if (e == cudaSuccess) {
-        const unsigned grid = (unsigned)((n1 + kThreads - 1) / kThreads);
+        const unsigned grid = (unsigned)((n1 + kThreads * kPar - 1) / (kThreads * kPar));
         if (X % 2 == 0 && ((uintptr_t)level0_device & 7) == 0)
             k_front_level1<true><<<grid, kThreads, 0, st>>>(level0_device, (uint32_t)X, (uint32_t)Y, (uint32_t)Z, (uint32_t)px, (uint32_t)py,
                                                             n1, level1_device, mixed_voxel_device, mixed_children_device, capacity, d_counter);
