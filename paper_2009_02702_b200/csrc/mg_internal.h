@@ -34,6 +34,21 @@ int relabel_by_level(const uint32_t* child_a, const uint32_t* child_b, uint64_t 
                      uint32_t n_leaves, std::vector<uint32_t>& new_of_old,
                      std::vector<uint64_t>& level_off);
 
+#ifdef __CUDACC__
+// A stream of n 4-byte elements at p, split for 16-byte loads: [0, head) one by one | nv uint4 from p + head |
+// [tail, n) one by one.  head + (n - tail) <= 6.
+struct Span { uint64_t head, nv, tail; };
+__device__ __forceinline__ Span span_of(const void* p, uint64_t n)
+{
+    uint64_t head = ((16 - ((uintptr_t)p & 15)) & 15) / 4;
+    if (head > n) head = n;
+    const uint64_t nv = (n - head) / 4;
+    return {head, nv, head + 4 * nv};
+}
+// index of the i-th ragged element (i < head + n - tail)
+__device__ __forceinline__ uint64_t ragged(const Span& s, uint64_t i) { return i < s.head ? i : s.tail + (i - s.head); }
+#endif
+
 }  // namespace mg
 
 struct mg_graph {

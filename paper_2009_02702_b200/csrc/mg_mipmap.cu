@@ -20,16 +20,9 @@ constexpr uint32_t kNone = 0xFFFFFFFFu;
 
 // The three leaf-index passes stream the 4-byte volume once each: 16-byte loads, two per thread in flight, the
 // 0-3 elements before the first 16-byte boundary and after the last whole vector taken one by one by block 0.
-struct Span { uint64_t head, nv, tail; };                            // [0,head) | nv uint4 from head | [tail,n)
-__device__ __forceinline__ Span span_of(const void* p, uint64_t n)
-{
-    uint64_t head = ((16 - ((uintptr_t)p & 15)) & 15) / 4;
-    if (head > n) head = n;
-    const uint64_t nv = (n - head) / 4;
-    return {head, nv, head + 4 * nv};
-}
-// index of the i-th ragged element (i < head + n - tail)
-__device__ __forceinline__ uint64_t ragged(const Span& s, uint64_t i) { return i < s.head ? i : s.tail + (i - s.head); }
+using mg::Span;
+using mg::span_of;
+using mg::ragged;
 
 __global__ void __launch_bounds__(kThreads) k_max_id(const uint32_t* __restrict__ seg, uint64_t n, uint32_t* out)
 {

@@ -43,36 +43,66 @@ __device__ __forceinline__ void st_cs_u4(uint4* p, uint4 v)
     asm volatile("st.global.cs.v4.u32 [%0], {%1,%2,%3,%4};" :: "l"(p), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
 }
 
+// 16-byte streaming loads, two per thread in flight; one atomic pair per warp at the end (grid-stride: few warps).
 __global__ void __launch_bounds__(256) k_index_range(const uint32_t* __restrict__ idx, uint64_t n, uint32_t* __restrict__ mm)
 {
+    const mg::Span sp = mg::span_of(idx, n);
+    const uint4* v4 = reinterpret_cast<const uint4*>(idx + sp.head);
+    const uint64_t stride = (uint64_t)gridDim.x * blockDim.x;
     uint32_t lo = 0xFFFFFFFFu, hi = 0u;
-    for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (uint64_t)gridDim.x * blockDim.x) {
-        const uint32_t v = idx[i];
+    auto take = [&](const uint4 a) {
+        lo = min(lo, min(min(a.x, a.y), min(a.z, a.w)));
+        hi = max(hi, max(max(a.x, a.y), max(a.z, a.w)));
+    };
+    uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    for (; i + stride < sp.nv; i += 2 * stride) {
+        const uint4 a = __ldcs(v4 + i), b = __ldcs(v4 + i + stride);
+        take(a);
+        take(b);
+    }
+    if (i < sp.nv) take(__ldcs(v4 + i));
+    if (blockIdx.x == 0 && threadIdx.x < sp.head + (n - sp.tail)) {
+        const uint32_t v = idx[mg::ragged(sp, threadIdx.x)];
         lo = min(lo, v); hi = max(hi, v);
     }
     lo = __reduce_min_sync(0xFFFFFFFFu, lo);
     hi = __reduce_max_sync(0xFFFFFFFFu, hi);
-    if ((threadIdx.x & 31) == 0) { atomicMin(mm, lo); atomicMax(mm + 1, hi); }
+    if ((threadIdx.x & 31) == 0 && lo <= hi) { atomicMin(mm, lo); atomicMax(mm + 1, hi); }
 }
 
 // word w of the stream holds stream bits [32 w, 32 w + 32): the voxels that overlap it are
-// floor(32 w / r) .. floor((32 w + 31) / r).
+// floor(32 w / r) .. floor((32 w + 31) / r).  The one 64-bit division (first bit of the CTA's words by r) is taken
+// once per CTA; everything per thread is 32-bit and relative to it.  kPackWords words per thread (a CTA of one word
+// per thread is over before the next one is launched: the kernel then runs at the CTA launch rate, not at HBM's).
+constexpr int kPackWords = 8;
+
 __global__ void __launch_bounds__(256)
 k_pack_bits(const uint32_t* __restrict__ idx, uint64_t n, uint32_t i_min, uint32_t r, uint32_t* __restrict__ words, uint64_t n_words)
 {
-    const uint64_t w = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (w >= n_words) return;
-    uint32_t out = 0;
-    if (r) {
-        const uint64_t b0 = 32 * w, b1 = b0 + 32;
-        uint64_t v = b0 / r;
-        for (; v < n && v * r < b1; v++) {
-            const uint64_t val = (uint64_t)(idx[v] - i_min);
-            const int64_t sh = (int64_t)(v * r) - (int64_t)b0;          // position of the value's bit 0 inside the word
-            out |= (sh >= 0) ? (uint32_t)(val << sh) : (uint32_t)(val >> (-sh));
-        }
+    __shared__ uint64_t s_q;
+    __shared__ uint32_t s_rem;
+    const uint64_t w0 = (uint64_t)blockIdx.x * (256 * kPackWords);        // first word of this CTA
+    if (threadIdx.x == 0 && r) {
+        s_q = (w0 * 32) / r;
+        s_rem = (uint32_t)(w0 * 32 - s_q * r);
     }
-    words[w] = out;
+    __syncthreads();
+#pragma unroll 2
+    for (int k = 0; k < kPackWords; k++) {
+        const uint32_t wl = k * 256 + threadIdx.x;
+        if (w0 + wl >= n_words) return;
+        uint32_t out = 0;
+        if (r) {
+            const uint32_t rel = s_rem + 32u * wl;                        // the word's bit 0, counted from voxel s_q's bit 0
+            const uint32_t vr = rel / r;
+            uint64_t v = s_q + vr;
+            for (int sh = (int)(vr * r) - (int)rel; sh < 32 && v < n; sh += (int)r, v++) {   // sh: the value's bit 0 inside the word
+                const uint64_t val = (uint64_t)(__ldg(idx + v) - i_min);
+                out |= (sh >= 0) ? (uint32_t)(val << sh) : (uint32_t)(val >> (-sh));
+            }
+        }
+        words[w0 + wl] = out;
+    }
 }
 
 // One tile (kTileVox voxels of one level) at the compile-time bitrate R.  A lane handles groups of 4
@@ -187,8 +217,8 @@ extern "C" int mg_index_range(const uint32_t* idx_device, uint64_t n, uint32_t* 
     const uint32_t init[2] = {0xFFFFFFFFu, 0u};
     cudaError_t e = cudaMemcpyAsync(d_mm, init, 8, cudaMemcpyHostToDevice, st);
     if (e == cudaSuccess) {
-        uint64_t blocks = (n + 255) / 256;
-        if (blocks > 148ull * 16) blocks = 148ull * 16;
+        uint64_t blocks = (n / 4 + 256) / 256;
+        if (blocks > 148ull * 8) blocks = 148ull * 8;
         k_index_range<<<(unsigned)blocks, 256, 0, st>>>(idx_device, n, d_mm);
         count_launch();
         uint32_t out[2] = {0, 0};
@@ -207,7 +237,7 @@ extern "C" int mg_pack_indices(const uint32_t* idx_device, uint64_t n, uint32_t 
     if (bits > 32) { set_error("mg_pack_indices: bits must be <= 32"); return MG_ERR_INVALID_ARG; }
     if ((uintptr_t)packed_device & 15) { set_error("mg_pack_indices: the stream must be 16-byte aligned"); return MG_ERR_INVALID_ARG; }
     const uint64_t n_words = mg_packed_stream_bytes(n, bits) / 4;
-    const uint64_t blocks = (n_words + 255) / 256;
+    const uint64_t blocks = (n_words + 256 * kPackWords - 1) / (256 * kPackWords);
     if (blocks > 0x7fffffffull) { set_error("mg_pack_indices: too many voxels for one launch"); return MG_ERR_INVALID_ARG; }
     k_pack_bits<<<(unsigned)blocks, 256, 0, (cudaStream_t)stream>>>(idx_device, n, i_min, bits, (uint32_t*)packed_device, n_words);
     count_launch();

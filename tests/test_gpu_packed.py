@@ -51,6 +51,28 @@ def test_index_range_and_pack_match_oracle(mg, n, i_min, span):
     assert np.array_equal(oracle.unpack_level(got, n, lo, r), ids)
 
 
+@pytest.mark.parametrize("off", [0, 1, 2, 3])
+@pytest.mark.parametrize("n", [1, 2, 3, 6, 9, 1000, 4099])
+def test_index_range_and_pack_at_any_alignment(mg, off, n):
+    """mg_index_range reads 16 bytes at a time between the 16-byte boundaries: the extremes placed in the first and the
+    last element (the ones taken one by one) at every offset of the level from a boundary; the packer from the same view."""
+    ids = _ids(n, 1000, 5000, 32 + off)
+    for first, last in ((7, 900000), (900000, 7)):
+        ids[0], ids[-1] = first, last
+        if n == 1:
+            first = last
+        buf = torch.zeros(n + 8, dtype=torch.int32, device="cuda")                         # zeros outside: must not be read
+        buf[off:off + n] = _dev(ids.view(np.int32))
+        d = buf[off:off + n]
+        lo, hi = mg.index_range(d, n)
+        assert (lo, hi) == oracle.index_range(ids) == (min(first, last), max(first, last))
+        r = mg.bits_per_voxel(lo, hi)
+        packed = torch.zeros(mg.packed_stream_bytes(n, r), dtype=torch.uint8, device="cuda")
+        mg.pack_indices(d, n, lo, r, packed)
+        ref = oracle.pack_level(ids, lo, r)
+        assert np.array_equal(packed.cpu().numpy()[:ref.size], ref)
+
+
 def _graph(mg, sizes, seed):
     a, b, w, off = synth.random_dag_levels(sizes, seed=seed)
     tf = synth.random_tf(sizes[0], seed + 1)
