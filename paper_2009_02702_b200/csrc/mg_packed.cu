@@ -72,33 +72,38 @@ __global__ void __launch_bounds__(256) k_index_range(const uint32_t* __restrict_
 
 // word w of the stream holds stream bits [32 w, 32 w + 32): the voxels that overlap it are
 // floor(32 w / r) .. floor((32 w + 31) / r).  The one 64-bit division (first bit of the CTA's words by r) is taken
-// once per CTA; everything per thread is 32-bit and relative to it.  kPackWords words per thread (a CTA of one word
-// per thread is over before the next one is launched: the kernel then runs at the CTA launch rate, not at HBM's).
+// once per CTA; everything per thread is 32-bit and relative to it (the kernel is issue-bound, not HBM-bound: ncu
+// showed 78 % issue-slot use at 43 % DRAM throughput with a 32-bit division and 64-bit shifts per word).
+// kPackWords words per thread: a CTA of one word per thread is over before the next one is launched, and the kernel
+// then runs at the CTA launch rate.
 constexpr int kPackWords = 8;
 
 __global__ void __launch_bounds__(256)
 k_pack_bits(const uint32_t* __restrict__ idx, uint64_t n, uint32_t i_min, uint32_t r, uint32_t* __restrict__ words, uint64_t n_words)
 {
-    __shared__ uint64_t s_q;
-    __shared__ uint32_t s_rem;
+    __shared__ const uint32_t* s_base;                                    // voxel q = floor(first bit of the CTA / r)
+    __shared__ uint32_t s_rem, s_n;                                       // first bit - q r; voxels from q on (capped)
     const uint64_t w0 = (uint64_t)blockIdx.x * (256 * kPackWords);        // first word of this CTA
     if (threadIdx.x == 0 && r) {
-        s_q = (w0 * 32) / r;
-        s_rem = (uint32_t)(w0 * 32 - s_q * r);
+        const uint64_t q = (w0 * 32) / r;
+        s_base = idx + q;
+        s_rem = (uint32_t)(w0 * 32 - q * r);
+        s_n = q < n ? (uint32_t)min(n - q, (uint64_t)1 << 30) : 0u;
     }
     __syncthreads();
+    const uint32_t magic = r > 1 ? 0xFFFFFFFFu / r + 1u : 0u;            // floor(x / r) = umulhi(x, magic) for x < 2^27, 1 < r <= 32
 #pragma unroll 2
     for (int k = 0; k < kPackWords; k++) {
         const uint32_t wl = k * 256 + threadIdx.x;
         if (w0 + wl >= n_words) return;
         uint32_t out = 0;
         if (r) {
-            const uint32_t rel = s_rem + 32u * wl;                        // the word's bit 0, counted from voxel s_q's bit 0
-            const uint32_t vr = rel / r;
-            uint64_t v = s_q + vr;
-            for (int sh = (int)(vr * r) - (int)rel; sh < 32 && v < n; sh += (int)r, v++) {   // sh: the value's bit 0 inside the word
-                const uint64_t val = (uint64_t)(__ldg(idx + v) - i_min);
-                out |= (sh >= 0) ? (uint32_t)(val << sh) : (uint32_t)(val >> (-sh));
+            const uint32_t* base = s_base;
+            const uint32_t rel = s_rem + 32u * wl, n_rel = s_n;           // the word's bit 0, counted from voxel q's bit 0
+            uint32_t v = r > 1 ? __umulhi(rel, magic) : rel;
+            for (int sh = (int)(v * r) - (int)rel; sh < 32 && v < n_rel; sh += (int)r, v++) {   // sh: the value's bit 0 inside the word
+                const uint32_t val = __ldg(base + v) - i_min;
+                out |= (sh >= 0) ? (val << sh) : (val >> (-sh));
             }
         }
         words[w0 + wl] = out;
