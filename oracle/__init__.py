@@ -11,6 +11,8 @@ Function -> passage (PAPER.md line):
   histogram_mipmap     O-2  Eq. 4 L78-L80 (integer counts scaled to 8^l)
   direct_colour        O-2  L66 (<m, x>)
   brute_force_histogram O-3 Eq. 4 unrolled
+  brute_force_level    O-3 for every voxel of one level in one pass over the finest voxels
+  symbolic_eval_sparse O-5 on a sparse matrix, level by level (full-size graphs; a scipy sparse product per level)
   graph_eval           O-4  L259, L269, L371, Eq. 8
   graph_eval_attr      NEXT-1: any numeric attribute, n_ch channels (L269, L271 (i)-(ii), L277)
   topo_levels          L211
@@ -53,6 +55,8 @@ _lib.mgo_direct_colour.argtypes = [_u64p, _u64, _u32, _u32, _f64p, _f64p]
 _lib.mgo_direct_colour.restype = None
 _lib.mgo_brute_force_histogram.argtypes = [_u32p, _u64, _u64, _u64, _u32, _u32, _u64, _u64, _u64, _f64p]
 _lib.mgo_brute_force_histogram.restype = None
+_lib.mgo_brute_force_level.argtypes = [_u32p, _u64, _u64, _u64, _u32, _u32, _f64p]
+_lib.mgo_brute_force_level.restype = None
 _lib.mgo_graph_eval.argtypes = [_u32p, _u32p, _f64p, _u64, _u64, _f64p, _f64p]
 _lib.mgo_graph_eval.restype = None
 _lib.mgo_graph_eval_attr.argtypes = [_u32p, _u32p, _f64p, _u64, _u64, _u32, _f64p, _f64p]
@@ -152,6 +156,17 @@ def brute_force_histogram(seg_index, n_seg, level, i, j, k):
     return h
 
 
+def brute_force_level(seg_index, n_seg, level):
+    """Normalised histograms of EVERY voxel of ``level`` by the unrolled Eq. 4 (one pass over the finest voxels):
+    fp64 [Z_l, Y_l, X_l, n_seg], every voxel's histogram summing to 1.  Dense: for the coarse levels of big volumes."""
+    seg_index = _c(seg_index, np.uint32)
+    Z, Y, X = seg_index.shape
+    xl, yl, zl = mip_dims((X, Y, Z))[level]
+    h = np.zeros((zl, yl, xl, n_seg), dtype=np.float64)
+    _lib.mgo_brute_force_level(seg_index.reshape(-1), X, Y, Z, n_seg, level, h.reshape(-1))
+    return h
+
+
 def graph_eval(child_a, child_b, weight, n_leaves, tf):
     """c[n] fp64 [n_nodes, 4]: leaves = tf, then (1-w) c[a] + w c[b] in index order (O-4).
     ``weight`` may be fp32 (converted exactly) or fp64."""
@@ -211,6 +226,31 @@ def symbolic_eval(child_a, child_b, weight, n_leaves):
     mu = np.zeros((a.size, n_leaves), dtype=np.float64)
     _lib.mgo_symbolic_eval(a, b, w, a.size, n_leaves, mu.reshape(-1))
     return mu
+
+
+def symbolic_eval_sparse(child_a, child_b, weight, n_leaves):
+    """O-5 for graphs too large for the dense table: mu as a scipy CSR matrix [n_nodes, n_leaves], fp64.
+    Leaves carry unit vectors; the nodes of topological level L (= max + 1, L211) are all
+    mu[n] = (1 - w) mu[a] + w mu[b] of rows of lower levels, i.e. ONE sparse product W_L @ mu_below with two
+    entries (1 - w, w) per row of W_L -- the same recurrence as symbolic_eval, a level at a time."""
+    import scipy.sparse as sp
+    a, b = _c(child_a, np.uint32).astype(np.int64), _c(child_b, np.uint32).astype(np.int64)
+    w = _c(weight, np.float64)
+    n = a.size
+    lev, depth = topo_levels(child_a, child_b, n_leaves)
+    mu = sp.identity(n_leaves, dtype=np.float64, format="csr")
+    mu.resize((n, n_leaves))
+    for L in range(1, depth + 1):                                    # (rows of the levels >= L are still empty)
+        rows = np.flatnonzero(lev == L)
+        k = rows.size
+        W = sp.csr_matrix((np.concatenate([1.0 - w[rows], w[rows]]),
+                           (np.concatenate([np.arange(k), np.arange(k)]), np.concatenate([a[rows], b[rows]]))),
+                          shape=(k, n))
+        level_rows = W @ mu
+        # scatter the new rows into mu (children of later levels read them)
+        sel = sp.csr_matrix((np.ones(k), (rows, np.arange(k))), shape=(n, k))
+        mu = mu + sel @ level_rows
+    return mu.tocsr()
 
 
 def lookup(node_idx, c, n_threads=1):

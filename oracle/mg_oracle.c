@@ -143,6 +143,45 @@ void mgo_brute_force_histogram(const uint32_t *seg_index, uint64_t x0, uint64_t 
     }
 }
 
+/* ---- O-3 for EVERY voxel of level l at once: the same unrolled Eq. 4 as mgo_brute_force_histogram, visited in
+ * the order of the finest voxels instead of once per coarse voxel -- finest voxel (x,y,z) adds
+ * wx(x) wy(y) wz(z) to H(x>>l, y>>l, z>>l, l)[S(x,y,z)].  The three axis weights are tabulated first (axis_weight
+ * of every coordinate), nothing else differs.  hist is dense [Z_l][Y_l][X_l][n_seg], Z_l = ceil-halved l times.
+ * Pins: mgo_brute_force_histogram voxel by voxel, the recursion (O-2) on ragged volumes, count / 8^l on
+ * power-of-two ones (tests/test_oracle_pins.py). */
+void mgo_brute_force_level(const uint32_t *seg_index, uint64_t x0, uint64_t y0, uint64_t z0,
+                           uint32_t n_seg, uint32_t l, double *hist)
+{
+    uint64_t xl = x0, yl = y0, zl = z0;
+    for (uint32_t m = 0; m < l; m++) {
+        xl = (xl + 1) / 2;
+        yl = (yl + 1) / 2;
+        zl = (zl + 1) / 2;
+    }
+    double *wx = (double *)malloc(x0 * sizeof(double));
+    double *wy = (double *)malloc(y0 * sizeof(double));
+    double *wz = (double *)malloc(z0 * sizeof(double));
+    for (uint64_t x = 0; x < x0; x++) wx[x] = axis_weight(x, x0, l);
+    for (uint64_t y = 0; y < y0; y++) wy[y] = axis_weight(y, y0, l);
+    for (uint64_t z = 0; z < z0; z++) wz[z] = axis_weight(z, z0, l);
+    memset(hist, 0, (size_t)(xl * yl * zl) * n_seg * sizeof(double));
+    /* coarse z-slabs are independent: one thread per k, every thread walks its own finest z range in order */
+#pragma omp parallel for schedule(dynamic, 1)
+    for (int64_t k = 0; k < (int64_t)zl; k++) {
+        for (uint64_t z = (uint64_t)k << l; z < z0 && (z >> l) == (uint64_t)k; z++)
+            for (uint64_t y = 0; y < y0; y++) {
+                double *row = hist + (((uint64_t)k * yl + (y >> l)) * xl) * n_seg;
+                const uint32_t *s = seg_index + (z * y0 + y) * x0;
+                double wzy = wz[z] * wy[y];
+                for (uint64_t x = 0; x < x0; x++)
+                    row[(x >> l) * n_seg + s[x]] += wx[x] * wzy;
+            }
+    }
+    free(wx);
+    free(wy);
+    free(wz);
+}
+
 /* ---- O-4: graph evaluation.  "assign colors to the source leaf nodes ... For each node, we
  * fetch data from its children and perform one interpolation" (L371); a triple (i, j, w) denotes
  * (1 - w) s_i + w s_j (L259) -- the weight multiplies the SECOND child; nodes are visited in index

@@ -100,6 +100,32 @@ def test_hist_pow2_is_textbook_box_filter_and_root_is_global_histogram():
     assert (H[4][0, 0, 0] == np.bincount(S.reshape(-1), minlength=n_seg)).all()
 
 
+def test_brute_force_level_is_the_per_voxel_brute_force_and_the_box_filter():
+    """brute_force_level (one pass over the finest voxels, all voxels of a level) against what fixes it: the per-voxel
+    unrolled Eq. 4 and the integer recursion on a ragged volume; numpy's reshape-sum box count / 8^l on a
+    power-of-two one; exact fractions on the 5x1x1 border case."""
+    S = _random_labels((7, 9, 13), 5, 14)
+    H = oracle.histogram_mipmap(S, 5)
+    for l in range(len(H)):
+        lvl = oracle.brute_force_level(S, 5, l)
+        assert lvl.shape == H[l].shape
+        np.testing.assert_allclose(lvl.sum(axis=-1), 1.0, rtol=0, atol=1e-15)
+        np.testing.assert_allclose(lvl, H[l] / 8.0 ** l, rtol=0, atol=1e-15)
+        Z, Y, X, _ = lvl.shape
+        for (i, j, k) in {(0, 0, 0), (X - 1, Y - 1, Z - 1), (X // 2, Y - 1, 0), (X - 1, 0, Z // 2)}:
+            np.testing.assert_allclose(lvl[k, j, i], oracle.brute_force_histogram(S, 5, l, i, j, k), rtol=0, atol=1e-16)
+    n_seg = 6
+    S = _random_labels((16, 16, 16), n_seg, 15)
+    onehot = (S[..., None] == np.arange(n_seg)).astype(np.float64)
+    for l in range(5):
+        b = 1 << l
+        box = onehot.reshape(16 // b, b, 16 // b, b, 16 // b, b, n_seg).sum(axis=(1, 3, 5))
+        assert np.array_equal(oracle.brute_force_level(S, n_seg, l), box / b ** 3)
+    S = np.array([[[0, 1, 2, 3, 4]]], dtype=np.uint32)
+    assert oracle.brute_force_level(S, 5, 3)[0, 0, 0].tolist() == [0.125] * 4 + [0.5]
+    assert oracle.brute_force_level(S, 5, 1)[0, 0].tolist() == [[.5, .5, 0, 0, 0], [0, 0, .5, .5, 0], [0, 0, 0, 0, 1]]
+
+
 def test_level0_is_lossless_unit_vector():
     """L223: the finest level holds exactly one ID per voxel."""
     S = _random_labels((4, 5, 6), 7, 6)
@@ -221,6 +247,24 @@ def test_symbolic_eval_ties_graph_eval_to_matmul():
     np.testing.assert_allclose(mu.sum(axis=1), 1.0, rtol=0, atol=1e-12)
     assert (mu >= 0).all()
     np.testing.assert_allclose(c, mu @ tf, rtol=0, atol=1e-13)
+
+
+def test_symbolic_eval_sparse_fig2_fig4_and_dense(golden_dir):
+    """The sparse level-by-level O-5 (used on full-size graphs) reproduces Fig. 2 / Fig. 4's printed mixtures, equals
+    the dense node-by-node table on a random DAG with shared nodes, and mu . TF is the O-4 colour."""
+    nodes, mix = _load_fig2(golden_dir)
+    a, b, w = _graph_from_fig(nodes, 9)
+    mu = oracle.symbolic_eval_sparse(a, b, w, 4).toarray()
+    np.testing.assert_allclose(mu[4], [1 / 3, 2 / 3, 0, 0], atol=1e-16)
+    np.testing.assert_allclose(mu[6], mix["m"], atol=1e-16)
+    np.testing.assert_allclose(mu[8], mix["mprime"], atol=1e-16)
+    a, b, w, off, nl = _small_dag(seed=23)
+    sp_mu = oracle.symbolic_eval_sparse(a, b, w, nl)
+    assert sp_mu.shape == (a.size, nl)
+    np.testing.assert_allclose(sp_mu.toarray(), oracle.symbolic_eval(a, b, w, nl), rtol=0, atol=1e-15)
+    tf = synth.random_tf(nl, 24).astype(np.float64)
+    np.testing.assert_allclose(sp_mu @ tf, oracle.graph_eval(a, b, w, nl, tf), rtol=0, atol=1e-13)
+    np.testing.assert_allclose(np.asarray(sp_mu.sum(axis=1)).reshape(-1), 1.0, rtol=0, atol=1e-12)
 
 
 def test_constant_tf_and_linearity():
