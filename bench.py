@@ -54,6 +54,13 @@ def parse_args():
     p.add_argument("--partition", choices=["replicas", "slab"], default="replicas",
                    help="N > 1: independent replicas of the whole update (default, weak scaling) or ONE update whose colourise is "
                         "split into N contiguous voxel slabs with the graph replicated (strong scaling, SURVEY.md 8(e)); no collective either way")
+    p.add_argument("--dist-backend", choices=["nccl", "gloo"], default="nccl",
+                   help="N > 1: process-group backend for the barrier and the max-over-ranks timing reduction (the only cross-rank "
+                        "traffic).  gloo lets several ranks share one GPU (rank r uses device r mod device_count): how the N > 1 "
+                        "code path is exercised on a one-GPU box (tests/test_gpu_dist.py); its timings are not scaling numbers")
+    p.add_argument("--dump-dir", default=None,
+                   help="every rank writes rank<r>.npz there: its voxel range and the host copy of its colourised mipmap slab as "
+                        "the last mg_tf_update_host of the e2e leg left it (tests compare the stitched slabs with the oracle)")
     p.add_argument("--relabel", action="store_true", help="config 5: load the DAG with MG_RELABEL (levels sorted by children)")
     p.add_argument("--no-query", action="store_true", help="skip the extra NEXT-4 measurement (mixture LUT + range queries)")
     p.add_argument("--render-empty-background", action="store_true",
@@ -138,18 +145,18 @@ def _sample_plan(w, n_sample: int):
     return [max(1, int(np.ceil(v * frac))) if v else 0 for v in w.level_voxels]
 
 
-def oracle_step(w, tf64, plan, chunk: int = 1 << 25):
-    """One TF update by the oracle on a sample: (propagate seconds, colourise seconds, threads)."""
+def oracle_step(w, tf64, plan, chunk: int = 1 << 25, n_threads: int = 0):
+    """One TF update by the oracle on a sample: (propagate seconds, colourise seconds, threads); n_threads = 0: all cores."""
     import oracle
     g = w.host_graph
     levels = [w.host_level(l) for l in range(len(plan))]           # (a download when level 0 only lives on the device)
     t0 = time.perf_counter()
-    c, used = oracle.graph_eval_levels(g["child_a"], g["child_b"], g["weight"], g["n_leaves"], tf64, n_threads=0)
+    c, used = oracle.graph_eval_levels(g["child_a"], g["child_b"], g["weight"], g["n_leaves"], tf64, n_threads=n_threads)
     t1 = time.perf_counter()
     for lvl, n in zip(levels, plan):
         flat = lvl.reshape(-1)
         for o in range(0, n, chunk):
-            oracle.colourise_rgba8(flat[o:min(n, o + chunk)], c, n_threads=0)
+            oracle.colourise_rgba8(flat[o:min(n, o + chunk)], c, n_threads=n_threads)
     t2 = time.perf_counter()
     return t1 - t0, t2 - t1, int(used)
 
@@ -160,11 +167,20 @@ def cpu_baseline(w, n_sample: int) -> dict:
     tp, tc, used = oracle_step(w, tf64, plan)
     n_s = sum(plan)
     ms = 1e3 * (tp + tc * (w.n_voxels / n_s))
+    # the same oracle on ONE thread (SURVEY.md 8(d) "Oracle timing (i)"; the paper's CPU figures, are multi-core):
+    # full propagation, colourise on an eighth of the sample, scaled
+    plan1 = _sample_plan(w, max(1, n_s // 8))
+    tp1, tc1, used1 = oracle_step(w, tf64, plan1, n_threads=1)
+    n_s1 = sum(plan1)
+    ms1 = 1e3 * (tp1 + tc1 * (w.n_voxels / n_s1))
     return {"value": ms, "unit": UNIT, "cores": used, "kind": "oracle",
             "sample": f"full fp64 level-synchronous propagation of all {w.stats['n_nodes']} nodes ({1e3 * tp:.1f} ms) + "
                       f"fp64 lookup/RGBA8 conversion of the leading {n_s} of {w.n_voxels} voxels (same share of every "
                       f"mip level, {1e3 * tc:.1f} ms), colourise time scaled to the whole mipmap",
-            "propagate_ms": 1e3 * tp, "colorize_sample_ms": 1e3 * tc, "sample_voxels": n_s}
+            "propagate_ms": 1e3 * tp, "colorize_sample_ms": 1e3 * tc, "sample_voxels": n_s,
+            "threads_1_ms": ms1, "threads_1_propagate_ms": 1e3 * tp1, "threads_1_cores": used1,
+            "threads_1_sample": f"one thread: full propagation ({1e3 * tp1:.1f} ms) + the leading {n_s1} voxels "
+                                f"({1e3 * tc1:.1f} ms), colourise time scaled to the whole mipmap"}
 
 
 def workload_config(w, args, n_gpus: int) -> dict:
@@ -212,9 +228,10 @@ def slab_range(n_voxels_padded: int, rank: int, world: int, align: int = 4096):
     return min(lo, n_voxels_padded), min(hi, n_voxels_padded)
 
 
-def aggregate_value(ms_per_step: float, world: int) -> float:
-    """Whole-job milliseconds per TF update: `world` independent replicas finish `world` updates per step."""
-    return ms_per_step / max(1, world)
+def aggregate_updates_per_s(ms_per_step: float, world: int) -> float:
+    """Whole-job THROUGHPUT of a replica run: `world` independent replicas finish `world` updates per step time.
+    (The latency metric itself does not improve with replicas: every update still takes ms_per_step.)"""
+    return max(1, world) / (ms_per_step * 1e-3)
 
 
 def peak_hbm_gbs():
@@ -247,9 +264,15 @@ def run_b200(args) -> dict:
     rank, local_rank, world = dist_env()
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device (the hot path has no CPU fallback)")
-    torch.cuda.set_device(local_rank)
+    device_index = local_rank % torch.cuda.device_count()           # (> 1 rank per GPU only with --dist-backend gloo)
+    torch.cuda.set_device(device_index)
+    red_dev = "cuda"
     if world > 1:
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+        if args.dist_backend == "nccl":
+            dist.init_process_group("nccl", device_id=torch.device("cuda", device_index))
+        else:
+            dist.init_process_group("gloo")
+            red_dev = "cpu"
     from paper_2009_02702_b200 import mg, workload
 
     w = workload.make(args.config, args.scale, relabel=args.relabel, device_mipmap=not args.host_mipmap and args.config != 5)
@@ -270,7 +293,7 @@ def run_b200(args) -> dict:
 
     def step(k: int):
         g.propagate(tfs[k % n_tf], nodes, st)
-        g.colorize(idx_part, n_part, nodes, out_part, fmt=fmt, stream=st)
+        g.colorize(idx_part, n_part, nodes, out_part, fmt=fmt, stream=st, from_last_propagate=True)
 
     def barrier():
         if world > 1:
@@ -284,7 +307,7 @@ def run_b200(args) -> dict:
     ev = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(K)]
     t_begin, t_end = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     launches0 = mg.kernel_launch_count()
-    with ClockSampler(local_rank) as clocks:
+    with ClockSampler(device_index) as clocks:
         barrier()
         t_begin.record(stream)
         for k in range(K):
@@ -292,7 +315,7 @@ def run_b200(args) -> dict:
             e[0].record(stream)
             g.propagate(tfs[(args.warmup + k) % n_tf], nodes, st)
             e[1].record(stream)
-            g.colorize(idx_part, n_part, nodes, out_part, fmt=fmt, stream=st)
+            g.colorize(idx_part, n_part, nodes, out_part, fmt=fmt, stream=st, from_last_propagate=True)
             e[2].record(stream)
         t_end.record(stream)
         barrier()
@@ -300,7 +323,7 @@ def run_b200(args) -> dict:
     total_ms = t_begin.elapsed_time(t_end)
     prop_ms = np.array([e[0].elapsed_time(e[1]) for e in ev])
     col_ms = np.array([e[1].elapsed_time(e[2]) for e in ev])
-    total_ms = max_over_ranks(total_ms, world, "cuda")
+    total_ms = max_over_ranks(total_ms, world, red_dev)
     ms_per_step = total_ms / K
 
     # ---- NEXT-3 variant: the same update with the node IDs bit-packed at r(l) bits per voxel (Table 1)
@@ -310,7 +333,7 @@ def run_b200(args) -> dict:
         lv = w.packed_levels
         for k in range(3):
             g.propagate(tfs[k % n_tf], nodes, st)
-            g.colorize_packed(w.d_packed, lv, nodes, out, fmt=fmt, stream=st)
+            g.colorize_packed(w.d_packed, lv, nodes, out, fmt=fmt, stream=st, from_last_propagate=True)
         torch.cuda.synchronize()
         kp = min(K, 100)
         evp = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(kp)]
@@ -318,7 +341,7 @@ def run_b200(args) -> dict:
             evp[k][0].record(stream)
             g.propagate(tfs[k % n_tf], nodes, st)
             evp[k][1].record(stream)
-            g.colorize_packed(w.d_packed, lv, nodes, out, fmt=fmt, stream=st)
+            g.colorize_packed(w.d_packed, lv, nodes, out, fmt=fmt, stream=st, from_last_propagate=True)
             evp[k][2].record(stream)
         torch.cuda.synchronize()
         pc = float(np.mean([e[1].elapsed_time(e[2]) for e in evp]))
@@ -448,8 +471,12 @@ def run_b200(args) -> dict:
         e1.record(stream)
         barrier()
         e2e_ms = e0.elapsed_time(e1)
-        e2e_ms = max_over_ranks(e2e_ms, world, "cuda")
-        e2e = {"value": e2e_ms / ke if slab else aggregate_value(e2e_ms / ke, world), "unit": UNIT,
+        e2e_ms = max_over_ranks(e2e_ms, world, red_dev)
+        if args.dump_dir:
+            os.makedirs(args.dump_dir, exist_ok=True)
+            np.savez(os.path.join(args.dump_dir, f"rank{rank}.npz"), v_lo=v_lo, v_hi=v_hi, out=out_host.numpy().copy(),
+                     nodes=nodes.cpu().numpy(), tf_update=(ke - 1) % len(tf_pinned), n_voxels_padded=w.n_voxels_padded)
+        e2e = {"value": e2e_ms / ke, "unit": UNIT,
                "h2d_bytes_per_step": int(w.n_leaves * 16), "d2h_bytes_per_step": int(n_part * out_bytes), "steps": ke,
                "what": "mg_tf_update_host: pinned-host TF -> H2D -> propagate -> colourise all levels -> D2H of the whole "
                        "mipmap into pinned host memory (PCIe-bound)"}
@@ -469,7 +496,10 @@ def run_b200(args) -> dict:
     achieved = algo_bytes / (col_avg * 1e-3) / 1e9
     kernel = "k_colorize"
     res = {
-        "metric": METRIC, "value": ms_per_step if slab else aggregate_value(ms_per_step, world), "unit": UNIT, "n_gpus": world,
+        # latency of ONE update: replicas do not shorten it (each rank runs a whole update; max over ranks), a slab
+        # partition does (strong scaling).  The whole-job throughput of a replica run is `updates_per_s`.
+        "metric": METRIC, "value": ms_per_step, "unit": UNIT, "n_gpus": world,
+        "updates_per_s": aggregate_updates_per_s(ms_per_step, 1 if slab else world),
         "steps": K, "warmup": args.warmup,
         "ms_per_step": ms_per_step, "higher_is_better": False, "scaling": "strong" if slab else "weak", "vs_baseline": None,
         "dtype": "f32", "data": "synthetic", "config": workload_config(w, args, world),

@@ -18,6 +18,9 @@
  *     Caller-owned buffers must outlive the enqueued work.
  *   - the library owns only its device copy of the graph (and per-graph scratch: 8-bit / 16-bit
  *     palettes, a TF staging buffer), released by mg_free_graph.
+ *   - a graph handle is not thread-safe: calls on ONE handle must be serialised by the caller
+ *     (different handles are independent).  Every call that launches work checks that the graph's
+ *     device is the current one and fails with MG_ERR_INVALID_ARG otherwise.
  *   - there is no CPU fallback: without a CUDA device every compute call fails with MG_ERR_CUDA.
  */
 #ifndef MG_H_
@@ -41,11 +44,15 @@ enum {
 
 /* mg_load_graph flags */
 enum {
-    MG_RELABEL = 1u /* input is only children-before-parents (Eq. 8), not level-contiguous:
+    MG_RELABEL = 1u, /* input is only children-before-parents (Eq. 8), not level-contiguous:
                        the library computes the topological levels (L211), permutes the nodes so
                        that every level is contiguous (leaves keep their numbers; inside a level
                        nodes are ordered by their children's new numbers for L2 locality) and
                        exposes the permutation through mg_node_permutation.                      */
+    MG_NO_PALETTES = 2u /* mg_propagate writes node_rgba only, not the 8-bit / 16-bit palettes (12 B per
+                           node less traffic for callers that only want the fp32 palette, e.g. for
+                           mg_render); mg_colorize then always derives them itself and rejects
+                           MG_PALETTE_FROM_LAST_PROPAGATE.                                           */
 };
 
 /* mg_colorize output formats (bit mask) */
@@ -53,7 +60,10 @@ enum {
     MG_RGBA8 = 1u,         /* 4 x uint8 per voxel, R in byte 0: round_half_even(clamp(c,0,1)*255)  */
     MG_RGBA16F = 2u,       /* 4 x IEEE fp16 per voxel (round to nearest even)                      */
     MG_BOTH = 3u,          /* both; RGBA8 to out_rgba, fp16 to out_rgba_aux                        */
-    MG_FORCE_CONVERT = 16u /* do not reuse the palettes cached by mg_propagate (see mg_colorize)   */
+    MG_FORCE_CONVERT = 16u, /* derive the palettes from node_rgba: this IS the default since the palette
+                               contract became explicit; the flag is accepted and changes nothing      */
+    MG_PALETTE_FROM_LAST_PROPAGATE = 32u /* gather from the palettes the last mg_propagate derived (see
+                                            mg_colorize): no conversion kernel                         */
 };
 
 typedef struct mg_info {
@@ -83,7 +93,7 @@ typedef struct mg_info {
  *   n_topo_levels     depth + 1 (ignored with MG_RELABEL when level_offsets is NULL).
  *   leaf_segment_id   host uint32[n_leaves] or NULL: the segment ID of each leaf (kept for
  *                     mg_graph_info consumers; strictly increasing if given).
- *   flags             0 or MG_RELABEL.
+ *   flags             0, MG_RELABEL, MG_NO_PALETTES or both.
  *   out               receives the graph handle.
  *
  * All arrays are caller-owned and copied.  Errors: MG_ERR_INVALID_ARG (NULL, n_leaves = 0,
@@ -142,13 +152,25 @@ int mg_propagate_host(mg_graph *g, const float *tf_rgba_host, float *node_rgba, 
  *                    index and output pointers to have the same offset modulo 16 bytes in units of
  *                    voxels (true for any two cudaMalloc'ed buffers indexed at the same voxel).
  *   n_voxels         number of voxels; authoritative.  0 is allowed (no work).
- *   node_rgba        DEVICE float[n_nodes][4] as filled by mg_propagate.  If it is the buffer most
- *                    recently filled by mg_propagate on this graph, the 8/16-bit palettes derived
- *                    there are reused; for any other pointer, or with MG_FORCE_CONVERT, the
- *                    palettes are first re-derived from node_rgba (one extra kernel).
+ *   node_rgba        DEVICE float[n_nodes][4], 16-byte aligned: THE palette ("one vec4 colour entry
+ *                    per node", L267), in the library's numbering.  By default the call first derives
+ *                    the 8-bit / 16-bit palette of the requested format from this buffer (one extra
+ *                    kernel on `stream`, 20-24 B per node), so the output always reflects the buffer
+ *                    as it is on `stream` at this point -- whoever wrote it (mg_propagate,
+ *                    mg_propagate_attr with 4 channels, the caller's own kernels).
  *   out_rgba         DEVICE output, n_voxels * 4 bytes (MG_RGBA8, MG_BOTH) or * 8 (MG_RGBA16F).
  *   out_rgba_aux     DEVICE fp16 output for MG_BOTH, else ignored (may be NULL).
- *   format           MG_RGBA8 | MG_RGBA16F | MG_BOTH, optionally | MG_FORCE_CONVERT.
+ *   format           MG_RGBA8 | MG_RGBA16F | MG_BOTH, optionally | MG_PALETTE_FROM_LAST_PROPAGATE:
+ *                    the caller states that node_rgba is the buffer the most recent mg_propagate /
+ *                    mg_propagate_host on this graph filled, that nothing has written it since, and
+ *                    that this call is ordered after that propagation (same stream, or an event).
+ *                    The palettes that propagation derived are then gathered as they are (no
+ *                    conversion kernel: a TF update is mg_propagate's launches + ONE colourise launch).
+ *                    The library can only check what it sees: the flag is rejected with
+ *                    MG_ERR_INVALID_ARG when node_rgba is not that buffer, when a library call has
+ *                    written into it since (mg_propagate_attr), when an unflagged colourise has
+ *                    re-derived the palettes since, or on a MG_NO_PALETTES graph.  Writes by the
+ *                    caller's own kernels are the caller's to declare -- by NOT passing the flag.
  */
 int mg_colorize(mg_graph *g, uint32_t mip_level, const uint32_t *node_idx_volume,
                 uint64_t n_voxels, const float *node_rgba, void *out_rgba, void *out_rgba_aux,
@@ -196,7 +218,8 @@ uint64_t mg_packed_stream_bytes(uint64_t n_voxels, uint32_t bits);
 int mg_index_range(const uint32_t *idx_device, uint64_t n, uint32_t *i_min, uint32_t *i_max, void *stream);
 
 /* One-off encoder step (Table 1 row (A)): pack DEVICE uint32 indices (every value in
- * [i_min, i_min + 2^bits)) into the DEVICE stream `packed_device` (16-byte aligned,
+ * [i_min, i_min + 2^bits); a value outside is reduced modulo 2^bits and never touches its neighbours'
+ * bits) into the DEVICE stream `packed_device` (16-byte aligned,
  * mg_packed_stream_bytes(n, bits) bytes, fully written incl. zero padding).  Enqueue-only. */
 int mg_pack_indices(const uint32_t *idx_device, uint64_t n, uint32_t i_min, uint32_t bits,
                     void *packed_device, void *stream);
@@ -204,9 +227,10 @@ int mg_pack_indices(const uint32_t *idx_device, uint64_t n, uint32_t i_min, uint
 /* mg_colorize with packed input, ALL levels in one launch: for every level l and voxel v < n_voxels,
  * out[out_offset + v] = convert(c[i_min + bits(v)]).  `levels` is a HOST array of n_levels
  * (<= MG_MAX_PACKED_LEVELS) descriptors, copied at enqueue.  packed_device, out_rgba, out_rgba_aux
- * are DEVICE, 16-byte aligned.  node_rgba must be the buffer most recently filled by mg_propagate
- * on this graph (its derived 8/16-bit palettes are gathered); otherwise MG_ERR_INVALID_ARG.
- * format: MG_RGBA8 | MG_RGBA16F | MG_BOTH.  Enqueue-only. */
+ * are DEVICE, 16-byte aligned.  node_rgba and the palette contract are those of mg_colorize: the palettes
+ * are derived from node_rgba first unless format carries MG_PALETTE_FROM_LAST_PROPAGATE.  Unpacked indices
+ * are clamped to n_nodes - 1 (a stale (i_min, bits) pair cannot gather out of bounds).
+ * format: MG_RGBA8 | MG_RGBA16F | MG_BOTH [| MG_PALETTE_FROM_LAST_PROPAGATE].  Enqueue-only. */
 int mg_colorize_packed(mg_graph *g, const void *packed_device, const mg_packed_level *levels,
                        uint32_t n_levels, const float *node_rgba, void *out_rgba, void *out_rgba_aux,
                        uint32_t format, void *stream);
@@ -225,8 +249,9 @@ int mg_colorize_packed(mg_graph *g, const void *packed_device, const mg_packed_l
  *   n_channels  1 .. MG_MAX_ATTR_CHANNELS.  Both buffers 4-byte aligned; 16-byte (8-byte) aligned
  *               buffers with n_channels % 4 == 0 (% 2 == 0) take the vectorised path.
  *
- * Enqueue-only, no allocation.  Does not touch the 8/16-bit palettes of mg_propagate (mg_colorize on
- * a 4-channel node_attr re-derives them, as for any foreign node_rgba).
+ * Enqueue-only, no allocation.  Does not write the 8/16-bit palettes of mg_propagate; if node_attr
+ * overlaps the node_rgba those palettes mirror, MG_PALETTE_FROM_LAST_PROPAGATE is refused from here on
+ * (mg_colorize on a 4-channel node_attr derives its palettes from it, as for any node_rgba).
  * Errors: MG_ERR_INVALID_ARG (NULL, aliasing, misalignment, n_channels out of range), MG_ERR_CUDA.
  * ------------------------------------------------------------------------------------------------ */
 #define MG_MAX_ATTR_CHANNELS 64

@@ -31,6 +31,34 @@ int cuda_fail(cudaError_t e, const char* what)
 
 void count_launch(unsigned n) { g_launches.fetch_add(n, std::memory_order_relaxed); }
 
+int SmemAttrOnce::ensure(const void* func, int bytes, int device)
+{
+    const uint64_t bit = (device >= 0 && device < 64) ? (1ull << device) : 0;
+    if (bit && (mask.load(std::memory_order_acquire) & bit)) return MG_OK;
+    MG_CUDA(cudaFuncSetAttribute(func, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
+    if (bit) mask.fetch_or(bit, std::memory_order_release);
+    return MG_OK;
+}
+
+int check_device(const mg_graph* g, const char* who)
+{
+    int dev = -1;
+    MG_CUDA(cudaGetDevice(&dev));
+    if (dev != g->device) {
+        set_error("%s: the graph lives on CUDA device %d but device %d is current", who, g->device, dev);
+        return MG_ERR_INVALID_ARG;
+    }
+    return MG_OK;
+}
+
+void invalidate_palettes_if_written(mg_graph* g, const void* p, uint64_t bytes)
+{
+    if (!g->pal_src) return;
+    const uintptr_t a0 = (uintptr_t)p, a1 = a0 + bytes;
+    const uintptr_t b0 = (uintptr_t)g->pal_src, b1 = b0 + g->n_nodes * 16;
+    if (a0 < b1 && b0 < a1) g->pal_src = nullptr;
+}
+
 // Levels >= first_fused_level run inside ONE persistent CTA (k_tail) that works entirely in shared
 // memory: the distinct "external" children (below the tail) are gathered once, then every level is
 // smem gathers + a __syncthreads().  The tail is the longest suffix of levels whose working set fits:
@@ -120,7 +148,7 @@ extern "C" int mg_load_graph(const uint32_t* child_a, const uint32_t* child_b, c
     *out = nullptr;
     if (n_leaves == 0 || n_nodes < n_leaves) { set_error("mg_load_graph: need 0 < n_leaves <= n_nodes"); return MG_ERR_INVALID_ARG; }
     if (n_nodes >= (1ull << 32)) { set_error("mg_load_graph: n_nodes must be < 2^32"); return MG_ERR_INVALID_ARG; }
-    if (flags & ~(uint32_t)MG_RELABEL) { set_error("mg_load_graph: unknown flags 0x%x", flags); return MG_ERR_INVALID_ARG; }
+    if (flags & ~(uint32_t)(MG_RELABEL | MG_NO_PALETTES)) { set_error("mg_load_graph: unknown flags 0x%x", flags); return MG_ERR_INVALID_ARG; }
     if (n_nodes > n_leaves && (!child_a || !child_b || !weight)) { set_error("mg_load_graph: NULL graph array"); return MG_ERR_INVALID_ARG; }
     const bool relabel = (flags & MG_RELABEL) != 0;
     if (!relabel && !level_offsets) { set_error("mg_load_graph: level_offsets is NULL without MG_RELABEL"); return MG_ERR_INVALID_ARG; }
@@ -141,6 +169,7 @@ extern "C" int mg_load_graph(const uint32_t* child_a, const uint32_t* child_b, c
     if (!g) { set_error("mg_load_graph: host allocation failed"); return MG_ERR_OOM; }
     g->n_nodes = n_nodes;
     g->n_leaves = n_leaves;
+    g->no_palettes = (flags & MG_NO_PALETTES) != 0;
     if (leaf_segment_id) g->leaf_segment_id.assign(leaf_segment_id, leaf_segment_id + n_leaves);
 
     std::vector<uint32_t> ha, hb;
@@ -276,6 +305,8 @@ extern "C" int mg_relabel_indices(mg_graph* g, uint32_t* idx_device, uint64_t n,
 {
     if (!g || (!idx_device && n)) { set_error("mg_relabel_indices: NULL argument"); return MG_ERR_INVALID_ARG; }
     if (!g->d_new_of_old || n == 0) return MG_OK;
+    const int rc = check_device(g, "mg_relabel_indices");
+    if (rc != MG_OK) return rc;
     uint64_t blocks = (n + 255) / 256;
     if (blocks > 148ull * 64) blocks = 148ull * 64;
     k_relabel_indices<<<(unsigned)blocks, 256, 0, (cudaStream_t)stream>>>(idx_device, n, g->d_new_of_old);

@@ -154,6 +154,10 @@ extern "C" int mg_propagate_attr(mg_graph* g, const float* leaf_attr, float* nod
     }
     if (((uintptr_t)leaf_attr | (uintptr_t)node_attr) & 3) { mg::set_error("mg_propagate_attr: buffers must be 4-byte aligned"); return MG_ERR_INVALID_ARG; }
     if (leaf_attr == node_attr) { mg::set_error("mg_propagate_attr: leaf_attr and node_attr must not alias"); return MG_ERR_INVALID_ARG; }
+    const int rc = mg::check_device(g, "mg_propagate_attr");
+    if (rc != MG_OK) return rc;
+    // node_attr may be (part of) the node_rgba the 8/16-bit palettes mirror: they stop mirroring it here
+    mg::invalidate_palettes_if_written(g, node_attr, g->n_nodes * (uint64_t)n_channels * 4);
     const uintptr_t al = (uintptr_t)leaf_attr | (uintptr_t)node_attr;
     cudaStream_t st = (cudaStream_t)stream;
     if (n_channels % 4 == 0 && (al & 15) == 0) return propagate_attr<float4>(g, leaf_attr, node_attr, n_channels / 4, st);

@@ -48,14 +48,16 @@ __device__ __forceinline__ uint2 cvt16(float4 c)
     return r;
 }
 
-// Re-derive both palettes from an arbitrary node_rgba (only when mg_propagate's are not reusable).
+// Derive the palette(s) a colourise call gathers from out of node_rgba (the default of mg_colorize; skipped
+// only under MG_PALETTE_FROM_LAST_PROPAGATE).  A normal launch: node_rgba may have been written by anything.
+template <bool W8, bool W16>
 __global__ void __launch_bounds__(256)
 k_convert_palette(const float4* __restrict__ c, uint32_t n, uint32_t* __restrict__ pal8, uint2* __restrict__ pal16)
 {
     for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
         const float4 v = __ldg(c + i);
-        pal8[i] = cvt8(v);
-        pal16[i] = cvt16(v);
+        if (W8) pal8[i] = cvt8(v);
+        if (W16) pal16[i] = cvt16(v);
     }
 }
 
@@ -153,13 +155,42 @@ int launch_colorize(const mg_graph* g, const uint32_t* idx, uint64_t n, uint32_t
 
 using namespace mg;
 
+// The palette contract of mg_colorize / mg_colorize_packed (include/mg.h): by default the palettes of the
+// requested format are derived from node_rgba here, on `st`, so the gather sees exactly the caller's buffer;
+// with MG_PALETTE_FROM_LAST_PROPAGATE the caller states that node_rgba is what the last mg_propagate on this
+// graph filled (and nothing wrote it since) and the palettes that call derived are gathered as they are.
+int mg::prepare_palettes(mg_graph* g, const float* node_rgba, uint32_t format, cudaStream_t st, const char* who)
+{
+    const uint32_t fmt = format & 3u;
+    if (format & MG_PALETTE_FROM_LAST_PROPAGATE) {
+        if (format & MG_FORCE_CONVERT) { set_error("%s: MG_FORCE_CONVERT and MG_PALETTE_FROM_LAST_PROPAGATE exclude each other", who); return MG_ERR_INVALID_ARG; }
+        if (g->no_palettes) { set_error("%s: MG_PALETTE_FROM_LAST_PROPAGATE on a graph loaded with MG_NO_PALETTES", who); return MG_ERR_INVALID_ARG; }
+        if (!g->pal_src || g->pal_src != node_rgba) {
+            set_error("%s: MG_PALETTE_FROM_LAST_PROPAGATE, but node_rgba is not the buffer the last mg_propagate on this graph "
+                      "filled (or a library call wrote it / re-derived the palettes since)", who);
+            return MG_ERR_INVALID_ARG;
+        }
+        return MG_OK;
+    }
+    const uint32_t n = (uint32_t)g->n_nodes;
+    uint32_t blocks = (n + 255) / 256;
+    if (blocks > 148u * 16) blocks = 148u * 16;
+    const float4* c = reinterpret_cast<const float4*>(node_rgba);
+    if (fmt == MG_RGBA8) k_convert_palette<true, false><<<blocks, 256, 0, st>>>(c, n, g->d_pal8, g->d_pal16);
+    else if (fmt == MG_RGBA16F) k_convert_palette<false, true><<<blocks, 256, 0, st>>>(c, n, g->d_pal8, g->d_pal16);
+    else k_convert_palette<true, true><<<blocks, 256, 0, st>>>(c, n, g->d_pal8, g->d_pal16);
+    count_launch();
+    g->pal_src = nullptr;          // the palettes now mirror a buffer the library knows nothing about
+    return MG_OK;
+}
+
 extern "C" int mg_colorize(mg_graph* g, uint32_t mip_level, const uint32_t* node_idx_volume, uint64_t n_voxels,
                            const float* node_rgba, void* out_rgba, void* out_rgba_aux, uint32_t format, void* stream)
 {
     (void)mip_level;
     if (!g || !node_rgba) { set_error("mg_colorize: NULL argument"); return MG_ERR_INVALID_ARG; }
     const uint32_t fmt = format & 3u;
-    if (fmt == 0 || (format & ~(3u | MG_FORCE_CONVERT))) { set_error("mg_colorize: bad format 0x%x", format); return MG_ERR_INVALID_ARG; }
+    if (fmt == 0 || (format & ~(3u | MG_FORCE_CONVERT | MG_PALETTE_FROM_LAST_PROPAGATE))) { set_error("mg_colorize: bad format 0x%x", format); return MG_ERR_INVALID_ARG; }
     if (n_voxels && (!node_idx_volume || !out_rgba)) { set_error("mg_colorize: NULL buffer"); return MG_ERR_INVALID_ARG; }
     if (fmt == MG_BOTH && n_voxels && !out_rgba_aux) { set_error("mg_colorize: MG_BOTH needs out_rgba_aux"); return MG_ERR_INVALID_ARG; }
     if (((uintptr_t)node_idx_volume & 3) || ((uintptr_t)out_rgba & 3) || (fmt == MG_RGBA16F && ((uintptr_t)out_rgba & 7)) ||
@@ -167,15 +198,10 @@ extern "C" int mg_colorize(mg_graph* g, uint32_t mip_level, const uint32_t* node
         set_error("mg_colorize: misaligned buffer"); return MG_ERR_INVALID_ARG;
     }
     cudaStream_t st = (cudaStream_t)stream;
-    if ((format & MG_FORCE_CONVERT) || g->pal_src != node_rgba) {
-        uint32_t n = (uint32_t)g->n_nodes;
-        uint32_t blocks = (n + 255) / 256;
-        if (blocks > 148u * 16) blocks = 148u * 16;
-        k_convert_palette<<<blocks, 256, 0, st>>>(reinterpret_cast<const float4*>(node_rgba), n, g->d_pal8, g->d_pal16);
-        count_launch();
-        g->pal_src = (format & MG_FORCE_CONVERT) ? nullptr : node_rgba;
-    }
-    int rc = MG_OK;
+    int rc = check_device(g, "mg_colorize");
+    if (rc != MG_OK) return rc;
+    rc = prepare_palettes(g, node_rgba, format, st, "mg_colorize");
+    if (rc != MG_OK) return rc;
     if (n_voxels) {
         if (fmt == MG_RGBA8) rc = launch_colorize<true, false>(g, node_idx_volume, n_voxels, (uint32_t*)out_rgba, nullptr, st);
         else if (fmt == MG_RGBA16F) rc = launch_colorize<false, true>(g, node_idx_volume, n_voxels, nullptr, (uint2*)out_rgba, st);
@@ -189,10 +215,12 @@ extern "C" int mg_colorize(mg_graph* g, uint32_t mip_level, const uint32_t* node
 extern "C" int mg_tf_update_host(mg_graph* g, const float* tf_rgba_host, float* node_rgba, const uint32_t* node_idx_volume,
                                  uint64_t n_voxels, void* out_device, void* out_host, uint32_t format, void* stream)
 {
-    if ((format & 3u) == MG_BOTH) { set_error("mg_tf_update_host: MG_BOTH is not accepted"); return MG_ERR_INVALID_ARG; }
+    if ((format & 3u) == MG_BOTH || (format & ~3u)) { set_error("mg_tf_update_host: format must be MG_RGBA8 or MG_RGBA16F"); return MG_ERR_INVALID_ARG; }
     int rc = mg_propagate_host(g, tf_rgba_host, node_rgba, stream);
     if (rc != MG_OK) return rc;
-    rc = mg_colorize(g, 0xFFFFFFFFu, node_idx_volume, n_voxels, node_rgba, out_device, nullptr, format, stream);
+    // this call has just enqueued the propagation that filled node_rgba on this very stream
+    const uint32_t reuse = g->no_palettes ? 0u : (uint32_t)MG_PALETTE_FROM_LAST_PROPAGATE;
+    rc = mg_colorize(g, 0xFFFFFFFFu, node_idx_volume, n_voxels, node_rgba, out_device, nullptr, (format & 3u) | reuse, stream);
     if (rc != MG_OK) return rc;
     if (out_host && n_voxels) {
         const size_t bytes = (size_t)n_voxels * (((format & 3u) == MG_RGBA8) ? 4 : 8);

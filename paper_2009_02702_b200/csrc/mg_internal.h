@@ -4,6 +4,7 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <atomic>
 #include <string>
 #include <vector>
 
@@ -24,6 +25,13 @@ void count_launch(unsigned n = 1);
         cudaError_t e__ = (call);                             \
         if (e__ != cudaSuccess) return mg::cuda_fail(e__, #call); \
     } while (0)
+
+// cudaFuncSetAttribute(MaxDynamicSharedMemorySize) belongs to the function instance in the CURRENT device's
+// context, so it is set once per (function, device): a bit per device id, devices >= 64 set it every time.
+struct SmemAttrOnce {
+    std::atomic<uint64_t> mask{0};
+    int ensure(const void* func, int bytes, int device);
+};
 
 // Host-side relabelling (csrc/relabel.cpp, also linked into the builder library).
 // Input: any children-before-parents graph.  Output: level-contiguous numbering.
@@ -51,6 +59,17 @@ __device__ __forceinline__ uint64_t ragged(const Span& s, uint64_t i) { return i
 
 }  // namespace mg
 
+struct mg_graph;
+namespace mg {
+// API entry guard: g's device must be the current one (include/mg.h, Conventions).
+int check_device(const mg_graph* g, const char* who);
+// A library call is about to write [p, p + bytes): if that overlaps the buffer the palettes mirror, they no
+// longer do.
+void invalidate_palettes_if_written(mg_graph* g, const void* p, uint64_t bytes);
+// mg_colorize.cu: derive the palettes `format` needs from node_rgba on `st`, or check MG_PALETTE_FROM_LAST_PROPAGATE.
+int prepare_palettes(mg_graph* g, const float* node_rgba, uint32_t format, cudaStream_t st, const char* who);
+}  // namespace mg
+
 struct mg_graph {
     int device = 0;
     uint64_t n_nodes = 0;
@@ -69,7 +88,10 @@ struct mg_graph {
     float* d_tf_stage = nullptr;           // [n_leaves][4]
     uint32_t* d_pal8 = nullptr;            // [n_nodes] RGBA8
     uint2* d_pal16 = nullptr;              // [n_nodes] 4 x fp16
-    const float* pal_src = nullptr;        // node_rgba the palettes were last derived from
+    // node_rgba that mg_propagate last filled TOGETHER WITH both palettes, and that no library call has written
+    // since; nullptr otherwise.  Only consulted to reject a wrong MG_PALETTE_FROM_LAST_PROPAGATE (mg_colorize).
+    const float* pal_src = nullptr;
+    bool no_palettes = false;              // MG_NO_PALETTES: mg_propagate does not derive the palettes
     // launch plan: levels >= first_fused_level run in the single-CTA tail kernel (0 = none).  The tail
     // works entirely in shared memory on LOCAL indices: [0, tail_n_ext) = the distinct children that lie
     // below the tail ("external": gathered once), [tail_n_ext, tail_n_ext + tail_n) = the tail's nodes.

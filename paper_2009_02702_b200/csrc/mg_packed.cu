@@ -92,6 +92,7 @@ k_pack_bits(const uint32_t* __restrict__ idx, uint64_t n, uint32_t i_min, uint32
     }
     __syncthreads();
     const uint32_t magic = r > 1 ? 0xFFFFFFFFu / r + 1u : 0u;            // floor(x / r) = umulhi(x, magic) for x < 2^27, 1 < r <= 32
+    const uint32_t vmask = r >= 32 ? 0xFFFFFFFFu : (1u << r) - 1u;        // an index outside [i_min, i_min + 2^r) must not spill into its neighbours' bits
 #pragma unroll 2
     for (int k = 0; k < kPackWords; k++) {
         const uint32_t wl = k * 256 + threadIdx.x;
@@ -102,7 +103,7 @@ k_pack_bits(const uint32_t* __restrict__ idx, uint64_t n, uint32_t i_min, uint32
             const uint32_t rel = s_rem + 32u * wl, n_rel = s_n;           // the word's bit 0, counted from voxel q's bit 0
             uint32_t v = r > 1 ? __umulhi(rel, magic) : rel;
             for (int sh = (int)(v * r) - (int)rel; sh < 32 && v < n_rel; sh += (int)r, v++) {   // sh: the value's bit 0 inside the word
-                const uint32_t val = __ldg(base + v) - i_min;
+                const uint32_t val = (__ldg(base + v) - i_min) & vmask;
                 out |= (sh >= 0) ? (val << sh) : (val >> (-sh));
             }
         }
@@ -116,7 +117,7 @@ k_pack_bits(const uint32_t* __restrict__ idx, uint64_t n, uint32_t i_min, uint32
 // group's bit offset (a runtime funnel shift) and extracts the four values at COMPILE-TIME positions
 // j R -- no shared memory, no barrier, word selection never depends on runtime data.
 template <int R, bool W8, bool W16>
-__device__ __forceinline__ void colorize_tile(const uint32_t* __restrict__ words, uint32_t i_min, uint32_t nv, uint64_t o0,
+__device__ __forceinline__ void colorize_tile(const uint32_t* __restrict__ words, uint32_t i_min, uint32_t id_max, uint32_t nv, uint64_t o0,
                                               const uint32_t* __restrict__ pal8, const uint2* __restrict__ pal16,
                                               uint32_t* __restrict__ out8, uint2* __restrict__ out16)
 {
@@ -148,7 +149,7 @@ __device__ __forceinline__ void colorize_tile(const uint32_t* __restrict__ words
             const int p = j * R;                                        // compile-time after unrolling
             uint32_t v = 0;
             if (R > 0) v = (p & 31) ? __funnelshift_r(w[p >> 5], w[(p >> 5) + 1 <= NW ? (p >> 5) + 1 : NW], p & 31) : w[p >> 5];
-            id[j] = i_min + (v & mask);
+            id[j] = min(i_min + (v & mask), id_max);                   // a stale (i_min, r) pair must not gather out of bounds
         }
         const uint64_t o = o0 + vb;
         if (vb + 4 <= nv) {
@@ -173,7 +174,7 @@ __device__ __forceinline__ void colorize_tile(const uint32_t* __restrict__ words
 template <bool W8, bool W16>
 __global__ void __launch_bounds__(kThreads)
 k_colorize_packed(const __grid_constant__ PackedParams P, const uint32_t* __restrict__ pal8, const uint2* __restrict__ pal16,
-                  uint32_t* __restrict__ out8, uint2* __restrict__ out16)
+                  uint32_t id_max, uint32_t* __restrict__ out8, uint2* __restrict__ out16)
 {
     uint32_t l = 0;
     while (l + 1 < P.n_levels && blockIdx.x >= P.lv[l + 1].tile_begin) l++;
@@ -183,7 +184,7 @@ k_colorize_packed(const __grid_constant__ PackedParams P, const uint32_t* __rest
     const uint32_t nv = (uint32_t)min((uint64_t)kTileVox, L.n_vox - v0);
     const uint32_t* words = L.words + tile * (uint64_t)(kTileVox / 32) * L.bits;   // a tile starts on a word boundary
     const uint64_t o0 = L.out_off + v0;
-#define MG_CASE(R) case R: colorize_tile<R, W8, W16>(words, L.i_min, nv, o0, pal8, pal16, out8, out16); break;
+#define MG_CASE(R) case R: colorize_tile<R, W8, W16>(words, L.i_min, id_max, nv, o0, pal8, pal16, out8, out16); break;
     switch (L.bits) {                                                    // uniform per CTA
         MG_CASE(0) MG_CASE(1) MG_CASE(2) MG_CASE(3) MG_CASE(4) MG_CASE(5) MG_CASE(6) MG_CASE(7) MG_CASE(8)
         MG_CASE(9) MG_CASE(10) MG_CASE(11) MG_CASE(12) MG_CASE(13) MG_CASE(14) MG_CASE(15) MG_CASE(16)
@@ -255,16 +256,14 @@ extern "C" int mg_colorize_packed(mg_graph* g, const void* packed_device, const 
 {
     if (!g || !node_rgba || !levels || !packed_device || !out_rgba) { set_error("mg_colorize_packed: NULL argument"); return MG_ERR_INVALID_ARG; }
     const uint32_t fmt = format & 3u;
-    if (fmt == 0 || (format & ~3u)) { set_error("mg_colorize_packed: bad format 0x%x", format); return MG_ERR_INVALID_ARG; }
+    if (fmt == 0 || (format & ~(3u | MG_FORCE_CONVERT | MG_PALETTE_FROM_LAST_PROPAGATE))) { set_error("mg_colorize_packed: bad format 0x%x", format); return MG_ERR_INVALID_ARG; }
     if (fmt == MG_BOTH && !out_rgba_aux) { set_error("mg_colorize_packed: MG_BOTH needs out_rgba_aux"); return MG_ERR_INVALID_ARG; }
     if (n_levels == 0 || n_levels > (uint32_t)kMaxLevels) { set_error("mg_colorize_packed: n_levels must be 1..%d", kMaxLevels); return MG_ERR_INVALID_ARG; }
     if (((uintptr_t)packed_device & 15) || ((uintptr_t)out_rgba & 15) || (fmt == MG_BOTH && ((uintptr_t)out_rgba_aux & 15)) || ((uintptr_t)node_rgba & 15)) {
         set_error("mg_colorize_packed: buffers must be 16-byte aligned"); return MG_ERR_INVALID_ARG;
     }
-    if (g->pal_src != node_rgba) {
-        set_error("mg_colorize_packed: node_rgba must be the buffer most recently filled by mg_propagate on this graph");
-        return MG_ERR_INVALID_ARG;
-    }
+    int rc = check_device(g, "mg_colorize_packed");
+    if (rc != MG_OK) return rc;
     PackedParams P;
     memset(&P, 0, sizeof(P));
     uint64_t tiles = 0;
@@ -276,6 +275,7 @@ extern "C" int mg_colorize_packed(mg_graph* g, const void* packed_device, const 
             return MG_ERR_INVALID_ARG;
         }
         if (s.n_voxels == 0) continue;
+        if (s.i_min >= g->n_nodes) { set_error("mg_colorize_packed: level %u: i_min = %u is not a node of this graph", l, s.i_min); return MG_ERR_INVALID_ARG; }
         PackedLevel& d = P.lv[m++];
         d.words = reinterpret_cast<const uint32_t*>(static_cast<const char*>(packed_device) + s.byte_offset);
         d.n_vox = s.n_voxels; d.out_off = s.out_offset; d.bits = s.bits; d.i_min = s.i_min;
@@ -284,12 +284,15 @@ extern "C" int mg_colorize_packed(mg_graph* g, const void* packed_device, const 
         if (tiles > 0x7fffffffull) { set_error("mg_colorize_packed: too many voxels for one launch"); return MG_ERR_INVALID_ARG; }
     }
     P.n_levels = m;
-    if (m == 0) return MG_OK;
     cudaStream_t st = (cudaStream_t)stream;
+    rc = prepare_palettes(g, node_rgba, format, st, "mg_colorize_packed");
+    if (rc != MG_OK) return rc;
+    if (m == 0) return MG_OK;
+    const uint32_t id_max = (uint32_t)g->n_nodes - 1;
     // normal launches: the palette gathers use the non-coherent path (see mg_colorize.cu)
-    if (fmt == MG_RGBA8) k_colorize_packed<true, false><<<(unsigned)tiles, kThreads, 0, st>>>(P, g->d_pal8, g->d_pal16, (uint32_t*)out_rgba, nullptr);
-    else if (fmt == MG_RGBA16F) k_colorize_packed<false, true><<<(unsigned)tiles, kThreads, 0, st>>>(P, g->d_pal8, g->d_pal16, nullptr, (uint2*)out_rgba);
-    else k_colorize_packed<true, true><<<(unsigned)tiles, kThreads, 0, st>>>(P, g->d_pal8, g->d_pal16, (uint32_t*)out_rgba, (uint2*)out_rgba_aux);
+    if (fmt == MG_RGBA8) k_colorize_packed<true, false><<<(unsigned)tiles, kThreads, 0, st>>>(P, g->d_pal8, g->d_pal16, id_max, (uint32_t*)out_rgba, nullptr);
+    else if (fmt == MG_RGBA16F) k_colorize_packed<false, true><<<(unsigned)tiles, kThreads, 0, st>>>(P, g->d_pal8, g->d_pal16, id_max, nullptr, (uint2*)out_rgba);
+    else k_colorize_packed<true, true><<<(unsigned)tiles, kThreads, 0, st>>>(P, g->d_pal8, g->d_pal16, id_max, (uint32_t*)out_rgba, (uint2*)out_rgba_aux);
     count_launch();
     MG_CUDA(cudaGetLastError());
     return MG_OK;

@@ -83,12 +83,16 @@ __device__ __forceinline__ uint2 to_rgba16f(float4 c)
     return r;
 }
 
+// PAL: also derive the node's 8-bit / 16-bit palette entries (off for graphs loaded with MG_NO_PALETTES).
+template <bool PAL>
 __device__ __forceinline__ void store_node(float4* c, uint32_t* __restrict__ pal8,
                                            uint2* __restrict__ pal16, uint32_t n, float4 v)
 {
     c[n] = v;
-    pal8[n] = to_rgba8(v);
-    pal16[n] = to_rgba16f(v);
+    if (PAL) {
+        pal8[n] = to_rgba8(v);
+        pal16[n] = to_rgba16f(v);
+    }
 }
 
 // FIRST: the source is the caller's TF (read-only input: non-coherent path); else node colours.
@@ -97,7 +101,7 @@ __device__ __forceinline__ float4 ld_src(const float4* p) { return FIRST ? __ldg
 
 // One level [lo, hi).  Work is cut into groups of 4 nodes aligned to absolute index 4g, so the
 // 16-byte loads of a/b/w are aligned whatever lo is; edge groups fall back to scalar accesses.
-template <bool FIRST>
+template <bool FIRST, bool PAL>
 __global__ void __launch_bounds__(kLevelThreads)
 k_level(const uint32_t* __restrict__ ga, const uint32_t* __restrict__ gb, const float* __restrict__ gw,
         const float4* __restrict__ src,   // FIRST: the TF; else: node colours of the lower levels
@@ -126,16 +130,18 @@ k_level(const uint32_t* __restrict__ ga, const uint32_t* __restrict__ gb, const 
         const float4 r2 = lerp4(ca2, cb2, __uint_as_float(wu.z));
         const float4 r3 = lerp4(ca3, cb3, __uint_as_float(wu.w));
         c[n0] = r0; c[n0 + 1] = r1; c[n0 + 2] = r2; c[n0 + 3] = r3;
-        *reinterpret_cast<uint4*>(pal8 + n0) = make_uint4(to_rgba8(r0), to_rgba8(r1), to_rgba8(r2), to_rgba8(r3));
-        const uint2 h0 = to_rgba16f(r0), h1 = to_rgba16f(r1), h2 = to_rgba16f(r2), h3 = to_rgba16f(r3);
-        *reinterpret_cast<uint4*>(pal16 + n0) = make_uint4(h0.x, h0.y, h1.x, h1.y);
-        *reinterpret_cast<uint4*>(pal16 + n0 + 2) = make_uint4(h2.x, h2.y, h3.x, h3.y);
+        if (PAL) {
+            *reinterpret_cast<uint4*>(pal8 + n0) = make_uint4(to_rgba8(r0), to_rgba8(r1), to_rgba8(r2), to_rgba8(r3));
+            const uint2 h0 = to_rgba16f(r0), h1 = to_rgba16f(r1), h2 = to_rgba16f(r2), h3 = to_rgba16f(r3);
+            *reinterpret_cast<uint4*>(pal16 + n0) = make_uint4(h0.x, h0.y, h1.x, h1.y);
+            *reinterpret_cast<uint4*>(pal16 + n0 + 2) = make_uint4(h2.x, h2.y, h3.x, h3.y);
+        }
     } else if (live) {
 #pragma unroll
         for (uint32_t k = 0; k < 4; k++) {
             const uint32_t n = n0 + k;
             if (n >= lo && n < hi)
-                store_node(c, pal8, pal16, n, lerp4(ld_src<FIRST>(src + ga[n]), ld_src<FIRST>(src + gb[n]), gw[n]));
+                store_node<PAL>(c, pal8, pal16, n, lerp4(ld_src<FIRST>(src + ga[n]), ld_src<FIRST>(src + gb[n]), gw[n]));
         }
     }
     if (FIRST) {
@@ -144,7 +150,7 @@ k_level(const uint32_t* __restrict__ ga, const uint32_t* __restrict__ gb, const 
         const uint32_t spare0 = n_groups;
         const uint32_t n_spare = total - spare0;
         if (t >= spare0)
-            for (uint32_t k = t - spare0; k < n_leaves; k += n_spare) store_node(c, pal8, pal16, k, __ldg(src + k));
+            for (uint32_t k = t - spare0; k < n_leaves; k += n_spare) store_node<PAL>(c, pal8, pal16, k, __ldg(src + k));
     }
 }
 
@@ -152,6 +158,7 @@ k_level(const uint32_t* __restrict__ ga, const uint32_t* __restrict__ gb, const 
 //   s_c[0, n_ext)            colours of the distinct children below the tail (gathered once)
 //   s_c[n_ext, n_ext + T)    colours of the tail's nodes, in index order
 // ta/tb are the tail's children in local indices, gw_tail its weights; off[] the level offsets.
+template <bool PAL>
 __global__ void __launch_bounds__(kTailThreads, 1)
 k_tail(const uint32_t* __restrict__ ta, const uint32_t* __restrict__ tb, const float* __restrict__ gw_tail,
        const uint32_t* __restrict__ ext, const float4* __restrict__ tf, float4* c,
@@ -174,7 +181,7 @@ k_tail(const uint32_t* __restrict__ ta, const uint32_t* __restrict__ tb, const f
     for (int k = 0; k < 4; k++) { const uint32_t e = tid + k * kTailThreads; my_ext[k] = (e < n_ext) ? ext[e] : 0u; }
     griddep_wait();
     if (copy_leaves)
-        for (uint32_t k = tid; k < n_leaves; k += kTailThreads) store_node(c, pal8, pal16, k, ld_colour(tf + k));
+        for (uint32_t k = tid; k < n_leaves; k += kTailThreads) store_node<PAL>(c, pal8, pal16, k, ld_colour(tf + k));
 #pragma unroll
     for (int k = 0; k < 4; k++) {
         const uint32_t e = tid + k * kTailThreads;
@@ -190,7 +197,7 @@ k_tail(const uint32_t* __restrict__ ta, const uint32_t* __restrict__ tb, const f
         for (uint32_t t = lo + tid; t < hi; t += kTailThreads) {
             const float4 r = lerp4(s_c[s_a[t]], s_c[s_b[t]], s_w[t]);
             s_c[n_ext + t] = r;
-            store_node(c, pal8, pal16, base + t, r);
+            store_node<PAL>(c, pal8, pal16, base + t, r);
         }
         __syncthreads();   // the level barrier
     }
@@ -219,6 +226,7 @@ static cudaError_t launch_pdl(bool pdl, void (*kernel)(KArgs...), unsigned grid,
     return cudaLaunchKernelEx(&cfg, kernel, KArgs(args)...);
 }
 
+template <bool PAL>
 static int propagate_impl(mg_graph* g, const float* tf_dev, float* node_rgba, cudaStream_t st)
 {
     const float4* tf4 = reinterpret_cast<const float4*>(tf_dev);
@@ -234,11 +242,11 @@ static int propagate_impl(mg_graph* g, const float* tf_dev, float* node_rgba, cu
             uint32_t want = n_groups + (g->n_leaves + 3) / 4;
             uint32_t blocks = (want + kLevelThreads - 1) / kLevelThreads;
             if ((uint64_t)blocks * kLevelThreads == n_groups) blocks++;
-            MG_CUDA(launch_pdl(false, k_level<true>, blocks, kLevelThreads, 0, st, g->d_a, g->d_b, g->d_w, tf4, c4, g->d_pal8,
+            MG_CUDA(launch_pdl(false, k_level<true, PAL>, blocks, kLevelThreads, 0, st, g->d_a, g->d_b, g->d_w, tf4, c4, g->d_pal8,
                                g->d_pal16, lo, hi, g->n_leaves, n_groups));
         } else {
             uint32_t blocks = (n_groups + kLevelThreads - 1) / kLevelThreads;
-            MG_CUDA(launch_pdl(true, k_level<false>, blocks, kLevelThreads, 0, st, g->d_a, g->d_b, g->d_w, (const float4*)c4, c4,
+            MG_CUDA(launch_pdl(true, k_level<false, PAL>, blocks, kLevelThreads, 0, st, g->d_a, g->d_b, g->d_w, (const float4*)c4, c4,
                                g->d_pal8, g->d_pal16, lo, hi, g->n_leaves, n_groups));
         }
         count_launch();
@@ -248,12 +256,13 @@ static int propagate_impl(mg_graph* g, const float* tf_dev, float* node_rgba, cu
         const uint32_t first = fused ? fused : n_levels;               // n_levels: no internal level at all
         const int copy_leaves = (last_big == 0);
         const size_t smem = (size_t)(g->tail_n_ext + g->tail_n) * sizeof(float4) + (size_t)g->tail_n * 12;
-        MG_CUDA(launch_pdl(last_big != 0, k_tail, 1u, (unsigned)kTailThreads, smem, st, g->d_tail_a, g->d_tail_b,
+        MG_CUDA(launch_pdl(last_big != 0, k_tail<PAL>, 1u, (unsigned)kTailThreads, smem, st, g->d_tail_a, g->d_tail_b,
                            g->d_w + g->tail_base, g->d_tail_ext, tf4, c4, g->d_pal8, g->d_pal16, g->d_level_off, first,
                            n_levels, g->n_leaves, g->tail_base, g->tail_n, g->tail_n_ext, copy_leaves));
         count_launch();
     }
-    g->pal_src = node_rgba;
+    // the palettes now mirror node_rgba: what MG_PALETTE_FROM_LAST_PROPAGATE refers to (mg_colorize)
+    g->pal_src = PAL ? node_rgba : nullptr;
     return MG_OK;
 }
 
@@ -261,17 +270,17 @@ static int check_args(mg_graph* g, const float* tf, float* node_rgba, const char
 {
     if (!g || !tf || !node_rgba) { set_error("%s: NULL argument", who); return MG_ERR_INVALID_ARG; }
     if (((uintptr_t)node_rgba & 15) != 0) { set_error("%s: node_rgba must be 16-byte aligned", who); return MG_ERR_INVALID_ARG; }
-    return MG_OK;
+    int rc = check_device(g, who);
+    if (rc != MG_OK) return rc;
+    // the tail kernel's dynamic shared memory limit: once per (function, device)
+    static SmemAttrOnce once_pal, once_nopal;
+    return g->no_palettes ? once_nopal.ensure((const void*)k_tail<false>, MG_TAIL_SMEM_BYTES, g->device)
+                          : once_pal.ensure((const void*)k_tail<true>, MG_TAIL_SMEM_BYTES, g->device);
 }
 
-static int ensure_tail_smem()
+static int propagate_any(mg_graph* g, const float* tf_dev, float* node_rgba, cudaStream_t st)
 {
-    static bool done = false;   // per process; the attribute is per function (all devices share the setting call)
-    if (!done) {
-        MG_CUDA(cudaFuncSetAttribute(k_tail, cudaFuncAttributeMaxDynamicSharedMemorySize, MG_TAIL_SMEM_BYTES));
-        done = true;
-    }
-    return MG_OK;
+    return g->no_palettes ? propagate_impl<false>(g, tf_dev, node_rgba, st) : propagate_impl<true>(g, tf_dev, node_rgba, st);
 }
 
 extern "C" int mg_propagate(mg_graph* g, const float* tf_rgba, float* node_rgba, void* stream)
@@ -279,17 +288,13 @@ extern "C" int mg_propagate(mg_graph* g, const float* tf_rgba, float* node_rgba,
     int rc = check_args(g, tf_rgba, node_rgba, "mg_propagate");
     if (rc != MG_OK) return rc;
     if (((uintptr_t)tf_rgba & 15) != 0) { set_error("mg_propagate: tf_rgba must be 16-byte aligned"); return MG_ERR_INVALID_ARG; }
-    rc = ensure_tail_smem();
-    if (rc != MG_OK) return rc;
-    return propagate_impl(g, tf_rgba, node_rgba, (cudaStream_t)stream);
+    return propagate_any(g, tf_rgba, node_rgba, (cudaStream_t)stream);
 }
 
 extern "C" int mg_propagate_host(mg_graph* g, const float* tf_rgba_host, float* node_rgba, void* stream)
 {
     int rc = check_args(g, tf_rgba_host, node_rgba, "mg_propagate_host");
     if (rc != MG_OK) return rc;
-    rc = ensure_tail_smem();
-    if (rc != MG_OK) return rc;
     MG_CUDA(cudaMemcpyAsync(g->d_tf_stage, tf_rgba_host, (size_t)g->n_leaves * 16, cudaMemcpyHostToDevice, (cudaStream_t)stream));
-    return propagate_impl(g, g->d_tf_stage, node_rgba, (cudaStream_t)stream);
+    return propagate_any(g, g->d_tf_stage, node_rgba, (cudaStream_t)stream);
 }

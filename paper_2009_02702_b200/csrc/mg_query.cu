@@ -105,6 +105,10 @@ extern "C" int mg_mixture_lut_build(mg_graph* g, const float* weight_sigma, mg_m
 {
     if (!g || !out) { mg::set_error("mg_mixture_lut_build: NULL argument"); return MG_ERR_INVALID_ARG; }
     *out = nullptr;
+    {
+        const int rc = mg::check_device(g, "mg_mixture_lut_build");
+        if (rc != MG_OK) return rc;
+    }
     cudaStream_t st = (cudaStream_t)stream;
     const uint64_t n = g->n_nodes;
     const uint32_t nl = g->n_leaves;
@@ -415,9 +419,9 @@ k_range_query_naive(const __grid_constant__ QueryParams P)
     }
     const unsigned lane = threadIdx.x & 31;
     const unsigned n_warps = gridDim.y * (kQueryThreads / 32), warp = blockIdx.y * (kQueryThreads / 32) + threadIdx.x / 32;
-    const uint32_t n_rows = dy * dz;                                       // < 2^32: level 0 has < 2^40 voxels, dx >= 1
-    for (uint32_t r = warp; r < n_rows; r += n_warps) {
-        const uint32_t iy = r % dy, iz = r / dy;
+    const uint64_t n_rows = (uint64_t)dy * dz;                             // up to 2^40 (2^20 voxels per axis)
+    for (uint64_t r = warp; r < n_rows; r += n_warps) {
+        const uint32_t iy = (uint32_t)(r % dy), iz = (uint32_t)(r / dy);
         const uint32_t* row = P.idx + P.off[0] + ((size_t)(z0 + iz) * Y + (y0 + iy)) * X + x0;
         for (uint32_t bx = 0; bx < dx; bx += 32 * kNaiveUnroll) {          // warp-uniform trip count
             uint32_t node[kNaiveUnroll];
@@ -509,6 +513,11 @@ extern "C" int mg_range_query(mg_mixture_lut* lut, const uint32_t* node_idx_mipm
             }
     }
     if (n_queries == 0) return MG_OK;
+    {
+        int dev = -1;
+        MG_CUDA(cudaGetDevice(&dev));
+        if (dev != lut->device) { mg::set_error("mg_range_query: the table lives on CUDA device %d but device %d is current", lut->device, dev); return MG_ERR_INVALID_ARG; }
+    }
     cudaStream_t st = (cudaStream_t)stream;
     if (n_queries > lut->boxes_cap) {
         MG_CUDA(cudaStreamSynchronize(st));                              // earlier queries may still read the old buffer
@@ -532,18 +541,28 @@ extern "C" int mg_range_query(mg_mixture_lut* lut, const uint32_t* node_idx_mipm
     P.var = err;
     P.fetches = reinterpret_cast<unsigned long long*>(fetches);
     // spread a query over enough CTAs to fill the machine when there are few queries (148 SMs x 8 CTAs)
-    const uint32_t splits = std::max<uint32_t>(1, std::min<uint32_t>(64, (148 * 8 + n_queries - 1) / n_queries));
+    uint32_t splits = std::max<uint32_t>(1, std::min<uint32_t>(64, (148 * 8 + n_queries - 1) / n_queries));
+    if (mode == MG_QUERY_NAIVE) {
+        // the per-CTA leaf histogram counts in uint32: a CTA takes rows round-robin, at most vol / splits + 8 rows'
+        // worth of voxels, so keep vol / splits <= 2^31 (dx <= 2^20 leaves the margin)
+        uint64_t max_vol = 0;
+        for (uint32_t q = 0; q < n_queries; q++) {
+            const uint64_t* b = boxes + 6ull * q;
+            max_vol = std::max(max_vol, (b[3] - b[0]) * (b[4] - b[1]) * (b[5] - b[2]));
+        }
+        const uint64_t need = (max_vol >> 31) + 1;
+        if (need > 65535) { mg::set_error("mg_range_query: MG_QUERY_NAIVE supports boxes of up to 2^46 voxels"); return MG_ERR_INVALID_ARG; }
+        splits = std::max<uint32_t>(splits, (uint32_t)need);
+    }
     const dim3 grid(n_queries, splits);
     P.force_walk = (mode == MG_QUERY_FA_WALK);
     if (mode != MG_QUERY_NAIVE) k_range_query_fa<<<grid, kQueryThreads, 0, st>>>(P);
     else {
         const size_t smem = (size_t)lut->n_leaves * sizeof(uint32_t);
         if (smem <= 200 * 1024) {                                          // per-CTA leaf histogram in shared memory
-            static bool attr_set = false;                                  // (per process; the attribute is per function)
-            if (!attr_set) {
-                MG_CUDA(cudaFuncSetAttribute(k_range_query_naive<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
-                attr_set = true;
-            }
+            static mg::SmemAttrOnce once;                                  // per (function, device)
+            const int rc = once.ensure((const void*)k_range_query_naive<true>, 200 * 1024, lut->device);
+            if (rc != MG_OK) return rc;
             k_range_query_naive<true><<<grid, kQueryThreads, smem, st>>>(P);
         } else {
             k_range_query_naive<false><<<grid, kQueryThreads, 0, st>>>(P);

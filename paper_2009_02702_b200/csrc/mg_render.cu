@@ -367,6 +367,10 @@ extern "C" int mg_render(mg_graph* g, const uint32_t* node_idx_mipmap, const mg_
         mg::set_error("mg_render: spacing, step_voxels, ref_step_voxels and tan_half_fov must be positive and finite");
         return MG_ERR_INVALID_ARG;
     }
+    {
+        const int rc = mg::check_device(g, "mg_render");
+        if (rc != MG_OK) return rc;
+    }
     RenderParams P;
     memset(&P, 0, sizeof(P));
     for (uint32_t l = 0; l < mip->n_levels; l++) {

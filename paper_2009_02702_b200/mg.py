@@ -20,8 +20,8 @@ if not os.path.exists(LIB_PATH):
 lib = C.CDLL(LIB_PATH)
 
 MG_OK, MG_ERR_INVALID_ARG, MG_ERR_INVALID_GRAPH, MG_ERR_CUDA, MG_ERR_OOM = 0, -1, -2, -3, -4
-MG_RELABEL = 1
-MG_RGBA8, MG_RGBA16F, MG_BOTH, MG_FORCE_CONVERT = 1, 2, 3, 16
+MG_RELABEL, MG_NO_PALETTES = 1, 2
+MG_RGBA8, MG_RGBA16F, MG_BOTH, MG_FORCE_CONVERT, MG_PALETTE_FROM_LAST_PROPAGATE = 1, 2, 3, 16, 32
 ALL_LEVELS = 0xFFFFFFFF
 
 # every symbol include/mg.h declares (tests check that the library exports all of them)
@@ -301,16 +301,20 @@ class Graph:
                                      stream or None), "mg_propagate_attr")
 
     def colorize(self, node_idx_device, n_voxels: int, node_rgba_device, out, out_aux=None,
-                 fmt: int = MG_RGBA8, mip_level: int = ALL_LEVELS, stream: int = 0) -> None:
+                 fmt: int = MG_RGBA8, mip_level: int = ALL_LEVELS, stream: int = 0,
+                 from_last_propagate: bool = False) -> None:
+        """``from_last_propagate`` adds MG_PALETTE_FROM_LAST_PROPAGATE to ``fmt`` (see include/mg.h)."""
+        f = int(fmt) | (MG_PALETTE_FROM_LAST_PROPAGATE if from_last_propagate else 0)
         _check(lib.mg_colorize(self._h, int(mip_level), _ptr(node_idx_device), int(n_voxels),
-                               _ptr(node_rgba_device), _ptr(out), _ptr(out_aux), int(fmt), stream or None),
+                               _ptr(node_rgba_device), _ptr(out), _ptr(out_aux), f, stream or None),
                "mg_colorize")
 
     def colorize_packed(self, packed_device, levels, node_rgba_device, out, out_aux=None, fmt: int = MG_RGBA8,
-                        stream: int = 0) -> None:
+                        stream: int = 0, from_last_propagate: bool = False) -> None:
         arr = levels if isinstance(levels, C.Array) else packed_levels(levels)
+        f = int(fmt) | (MG_PALETTE_FROM_LAST_PROPAGATE if from_last_propagate else 0)
         _check(lib.mg_colorize_packed(self._h, _ptr(packed_device), arr, len(arr), _ptr(node_rgba_device), _ptr(out),
-                                      _ptr(out_aux), int(fmt), stream or None), "mg_colorize_packed")
+                                      _ptr(out_aux), f, stream or None), "mg_colorize_packed")
 
     def tf_update_host(self, tf_host, node_rgba_device, node_idx_device, n_voxels: int, out_device,
                        out_host=None, fmt: int = MG_RGBA8, stream: int = 0) -> None:

@@ -28,7 +28,7 @@ def _worker(rank, world, port, q):
     mine = 1.5 + rank                      # rank 1 is the slow replica
     total = bench.max_over_ranks(mine, world, "cpu")
     dist.barrier()
-    q.put((rank, total, bench.aggregate_value(total, world)))
+    q.put((rank, total, bench.aggregate_updates_per_s(total, world)))
     dist.destroy_process_group()
 
 
@@ -45,13 +45,13 @@ def test_max_over_ranks_and_aggregate_world2():
         p.join(timeout=60)
         assert p.exitcode == 0
     assert [r[1] for r in res] == [2.5, 2.5]            # both ranks see the slowest replica's time
-    assert [r[2] for r in res] == [1.25, 1.25]          # 2 replicas -> 2 updates per step time
+    assert [r[2] for r in res] == [800.0, 800.0]        # 2 replicas -> 2 updates per 2.5 ms step: throughput, not latency
 
 
 def test_single_rank_is_identity():
     sys.path.insert(0, ROOT)
     import bench
-    assert bench.max_over_ranks(3.25, 1) == 3.25 and bench.aggregate_value(3.25, 1) == 3.25
+    assert bench.max_over_ranks(3.25, 1) == 3.25 and bench.aggregate_updates_per_s(4.0, 1) == 250.0
     assert bench.dist_env()[2] >= 1
 
 

@@ -67,7 +67,7 @@ def _run_update(mg, w, tf, fmt):
     out = torch.full((w.n_voxels_padded * bpv,), 0xAB, dtype=torch.uint8, device="cuda")
     st = torch.cuda.current_stream().cuda_stream
     g.propagate(torch.from_numpy(tf).cuda(), nodes, st)
-    g.colorize(w.d_idx, w.n_voxels_padded, nodes, out, fmt=fmt, stream=st)
+    g.colorize(w.d_idx, w.n_voxels_padded, nodes, out, fmt=fmt, stream=st, from_last_propagate=True)   # as bench.py does
     torch.cuda.synchronize()
     return nodes, out
 
@@ -245,7 +245,7 @@ def test_packed_mipmap_full_size(libs, cfg_id):
         w.pack()
         out_p = torch.full_like(out, 0xAB)
         st = torch.cuda.current_stream().cuda_stream
-        w.graph.colorize_packed(w.d_packed, w.packed_levels, nodes, out_p, fmt=mg.MG_RGBA8, stream=st)
+        w.graph.colorize_packed(w.d_packed, w.packed_levels, nodes, out_p, fmt=mg.MG_RGBA8, stream=st, from_last_propagate=True)
         torch.cuda.synchronize()
         o4, p4 = out.view(-1, 4), out_p.view(-1, 4)
         for s0, nv in zip(w.level_start, w.level_voxels):                      # every voxel of every level

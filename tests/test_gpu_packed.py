@@ -149,9 +149,42 @@ def test_colorize_packed_error_paths(mg):
     lv = [dict(n_voxels=4, out_offset=0, byte_offset=0, bits=33, i_min=0)]
     with pytest.raises(mg.MgError):
         g.colorize_packed(d, lv, nodes, out)
-    other = torch.zeros_like(nodes)
+    other = torch.rand_like(nodes)
     lv = [dict(n_voxels=4, out_offset=0, byte_offset=0, bits=3, i_min=0)]
-    with pytest.raises(mg.MgError):                                                # not the propagated buffer
-        g.colorize_packed(d, lv, other, out)
-    g.colorize_packed(d, lv, nodes, out)                                           # valid
+    with pytest.raises(mg.MgError):                                                # not the propagated buffer: no reuse
+        g.colorize_packed(d, lv, other, out, from_last_propagate=True)
+    g.colorize_packed(d, lv, nodes, out, from_last_propagate=True)                 # valid: the palettes of mg_propagate
     torch.cuda.synchronize()
+    first = out.cpu().numpy()[:4].copy()
+    g.colorize_packed(d, lv, other, out)                                           # default: derived from what is passed
+    torch.cuda.synchronize()
+    assert np.array_equal(out.cpu().numpy()[:4], oracle.to_rgba8(other.cpu().numpy().astype(np.float64))[[0, 0, 0, 0]])
+    with pytest.raises(mg.MgError):                                                # ... after which reuse is refused
+        g.colorize_packed(d, lv, nodes, out, from_last_propagate=True)
+    g.colorize_packed(d, lv, nodes, out)
+    torch.cuda.synchronize()
+    assert np.array_equal(out.cpu().numpy()[:4], first)
+    lv = [dict(n_voxels=4, out_offset=0, byte_offset=0, bits=3, i_min=10 ** 6)]    # i_min beyond the graph
+    with pytest.raises(mg.MgError):
+        g.colorize_packed(d, lv, nodes, out)
+
+
+def test_stale_index_range_cannot_corrupt_or_overrun(mg):
+    """An (i_min, r) pair that does not cover the data (a stale mg_index_range result): the packer reduces the
+    offending value modulo 2^r instead of spilling into its neighbours' bits, and the colouriser clamps unpacked
+    indices to the last node instead of gathering out of bounds."""
+    g, nodes, ref_nodes = _graph(mg, [8, 100, 10], 36)
+    n_nodes = nodes.shape[0]
+    ids = np.array([5, 6, 7, 5 + 8 + 3, 6, 5, 4, 7], dtype=np.uint32)             # one value >= i_min + 2^r, one < i_min
+    i_min, r = 5, 2
+    d = torch.zeros(mg.packed_stream_bytes(ids.size, r), dtype=torch.uint8, device="cuda")
+    mg.pack_indices(_dev(ids), ids.size, i_min, r, d)
+    torch.cuda.synchronize()
+    want = ((ids.astype(np.int64) - i_min) % (1 << r)).astype(np.uint32)
+    assert np.array_equal(d.cpu().numpy()[:2], oracle.pack_level(want + i_min, i_min, r)[:2])     # 8 values x 2 bits
+    out = torch.zeros((8, 4), dtype=torch.uint8, device="cuda")
+    lv = [dict(n_voxels=8, out_offset=0, byte_offset=0, bits=r, i_min=n_nodes - 2)]   # i_min + 3 > last node
+    g.colorize_packed(d, lv, nodes, out)
+    torch.cuda.synchronize()
+    code = oracle.to_rgba8(nodes.cpu().numpy().astype(np.float64))
+    assert np.array_equal(out.cpu().numpy(), code[np.minimum(n_nodes - 2 + want, n_nodes - 1)])

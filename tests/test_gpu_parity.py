@@ -164,9 +164,10 @@ def _f16_ok(got_f16, ref_c):
     return bool((np.abs(gi - ri) <= 1).all())                # non-negative values: ulp = bit distance
 
 
+@pytest.mark.parametrize("reuse", [False, True], ids=["derive", "from_last_propagate"])
 @pytest.mark.parametrize("n_vox", [0, 1, 3, 5, 2048, 2049, 123457, 1 << 21])
 @pytest.mark.parametrize("fmt_name", ["RGBA8", "RGBA16F", "BOTH"])
-def test_colorize_matches_oracle(mg, n_vox, fmt_name):
+def test_colorize_matches_oracle(mg, n_vox, fmt_name, reuse):
     sizes = PROFILES["big_then_tail"]
     a, b, w, off = synth.random_dag_levels(sizes, seed=5)
     tf = synth.random_tf(sizes[0], 46)
@@ -178,13 +179,16 @@ def test_colorize_matches_oracle(mg, n_vox, fmt_name):
     fmt = getattr(mg, "MG_" + fmt_name)
     out8 = torch.full((max(n_vox, 1), 4), 7, dtype=torch.uint8, device="cuda")
     out16 = torch.full((max(n_vox, 1), 4), 7, dtype=torch.float16, device="cuda")
+    launches0 = mg.kernel_launch_count()
     if fmt_name == "RGBA8":
-        g.colorize(d_idx, n_vox, nodes, out8, fmt=fmt, mip_level=0)
+        g.colorize(d_idx, n_vox, nodes, out8, fmt=fmt, mip_level=0, from_last_propagate=reuse)
     elif fmt_name == "RGBA16F":
-        g.colorize(d_idx, n_vox, nodes, out16, fmt=fmt, mip_level=0)
+        g.colorize(d_idx, n_vox, nodes, out16, fmt=fmt, mip_level=0, from_last_propagate=reuse)
     else:
-        g.colorize(d_idx, n_vox, nodes, out8, out16, fmt=fmt, mip_level=0)
+        g.colorize(d_idx, n_vox, nodes, out8, out16, fmt=fmt, mip_level=0, from_last_propagate=reuse)
     torch.cuda.synchronize()
+    if n_vox and n_vox % 4 == 0:                             # aligned body only: the flag saves exactly the conversion kernel
+        assert mg.kernel_launch_count() - launches0 == (1 if reuse else 2)
     if n_vox == 0:
         return
     if fmt_name in ("RGBA8", "BOTH"):
@@ -214,7 +218,8 @@ def test_colorize_unaligned_views(mg, shift_idx, shift_out):
 
 
 def test_colorize_foreign_palette_and_force_convert(mg):
-    """node_rgba that did not come from mg_propagate (or was edited) is re-converted."""
+    """node_rgba that did not come from mg_propagate (or was edited) is converted by the call itself: that is the
+    default; MG_FORCE_CONVERT (the pre-contract spelling) is still accepted and means the same."""
     sizes = [8, 100, 10]
     a, b, w, off = synth.random_dag_levels(sizes, seed=8)
     g = mg.Graph(a, b, w, 8, level_offsets=off)
@@ -231,10 +236,100 @@ def test_colorize_foreign_palette_and_force_convert(mg):
     assert np.array_equal(out8.cpu().numpy(), ref)
     assert out8.cpu().numpy()[0].tolist() == [0, 255, 0, 128]
     d_pal[5] = 0.25                                           # edit in place, same pointer
-    g.colorize(_dev(idx), 5000, d_pal, out8, fmt=mg.MG_RGBA8 | mg.MG_FORCE_CONVERT)
-    torch.cuda.synchronize()
     pal[5] = 0.25
-    assert np.array_equal(out8.cpu().numpy(), oracle.to_rgba8(pal.astype(np.float64))[idx])
+    for extra in (0, mg.MG_FORCE_CONVERT):
+        out8.zero_()
+        g.colorize(_dev(idx), 5000, d_pal, out8, fmt=mg.MG_RGBA8 | extra)
+        torch.cuda.synchronize()
+        assert np.array_equal(out8.cpu().numpy(), oracle.to_rgba8(pal.astype(np.float64))[idx])
+    with pytest.raises(mg.MgError) as e:                      # never propagated into: nothing to reuse
+        g.colorize(_dev(idx), 5000, d_pal, out8, fmt=mg.MG_RGBA8, from_last_propagate=True)
+    assert e.value.code == mg.MG_ERR_INVALID_ARG
+
+
+def test_palette_contract(mg):
+    """include/mg.h, mg_colorize: the default derives the palettes from node_rgba as it is on the stream; the 8/16-bit
+    palettes of the last mg_propagate are gathered only under MG_PALETTE_FROM_LAST_PROPAGATE, which the library
+    refuses whenever it can see that they no longer mirror node_rgba (the vec4 entry per node is THE
+    palette)."""
+    sizes = PROFILES["big_then_tail"]
+    a, b, w, off = synth.random_dag_levels(sizes, seed=31)
+    nl, n = sizes[0], sum(sizes)
+    g = mg.Graph(a, b, w, nl, level_offsets=off)
+    idx = synth.random_node_idx(40000, n, 70)
+    d_idx = _dev(idx)
+    out8 = torch.zeros((idx.size, 4), dtype=torch.uint8, device="cuda")
+    X = torch.zeros((n, 4), dtype=torch.float32, device="cuda")
+    tf1, tf2 = synth.random_tf(nl, 71), synth.random_tf(nl, 72)
+    ref1 = oracle.graph_eval(a, b, w, nl, tf1.astype(np.float64))
+    ref2 = oracle.graph_eval_attr(a, b, w, nl, tf2.astype(np.float64))
+
+    def col(**kw):
+        out8.zero_()
+        g.colorize(d_idx, idx.size, X, out8, fmt=mg.MG_RGBA8, **kw)
+        torch.cuda.synchronize()
+        return out8.cpu().numpy()
+
+    # (1) propagate(X) -> propagate_attr(X, C = 4) -> colorize(X): the colours of the SECOND call
+    g.propagate(_dev(tf1), X)
+    assert _rgba8_ok(col(from_last_propagate=True), oracle.lookup(idx, ref1))
+    g.propagate_attr(_dev(tf2), X, 4)
+    assert _rgba8_ok(col(), oracle.lookup(idx, ref2))
+    with pytest.raises(mg.MgError) as e:                      # the library saw the write: reuse refused
+        col(from_last_propagate=True)
+    assert e.value.code == mg.MG_ERR_INVALID_ARG
+    # (2) an attr write that only overlaps the palette buffer (other base pointer) is seen too
+    g.propagate(_dev(tf1), X)
+    g.propagate_attr(_dev(tf2[:, :1].copy()), X.view(-1)[8:8 + n], 1)
+    with pytest.raises(mg.MgError):
+        col(from_last_propagate=True)
+    # (3) an unflagged colourise re-derives the palettes from whatever it is given: reuse refused afterwards
+    g.propagate(_dev(tf1), X)
+    other = _dev(np.ascontiguousarray(ref2, dtype=np.float32))
+    out8.zero_()
+    g.colorize(d_idx, idx.size, other, out8, fmt=mg.MG_RGBA8)
+    torch.cuda.synchronize()
+    assert _rgba8_ok(out8.cpu().numpy(), oracle.lookup(idx, ref2))
+    with pytest.raises(mg.MgError):
+        col(from_last_propagate=True)
+    # (4) a foreign pointer is refused; so is the flag together with MG_FORCE_CONVERT
+    g.propagate(_dev(tf1), X)
+    with pytest.raises(mg.MgError):
+        g.colorize(d_idx, idx.size, other, out8, fmt=mg.MG_RGBA8, from_last_propagate=True)
+    with pytest.raises(mg.MgError):
+        g.colorize(d_idx, idx.size, X, out8, fmt=mg.MG_RGBA8 | mg.MG_FORCE_CONVERT, from_last_propagate=True)
+    # (5) the caller's own in-place edit: the default shows it; the flag is the caller's statement that there
+    # was none, so it shows the propagated colours (documented behaviour, not an error the library can detect)
+    g.propagate(_dev(tf1), X)
+    X[idx[0]] = torch.tensor([1.0, 0.0, 1.0, 0.0], device="cuda")
+    assert col()[0].tolist() == [255, 0, 255, 0]
+    g.propagate(_dev(tf1), X)
+    X[idx[0]] = torch.tensor([1.0, 0.0, 1.0, 0.0], device="cuda")
+    assert _rgba8_ok(col(from_last_propagate=True), oracle.lookup(idx, ref1))
+    g.close()
+
+
+def test_no_palettes_graph(mg):
+    """MG_NO_PALETTES: mg_propagate writes node_rgba only; colourise derives its palettes; the reuse flag is refused."""
+    sizes = PROFILES["big_then_tail"]
+    a, b, w, off = synth.random_dag_levels(sizes, seed=32)
+    tf = synth.random_tf(sizes[0], 73)
+    g, nodes = _propagate(mg, a, b, w, off, sizes[0], tf, flags=mg.MG_NO_PALETTES)
+    ref = _check_nodes(nodes, a, b, w, sizes[0], tf)
+    idx = synth.random_node_idx(30001, a.size, 74)
+    out8 = torch.zeros((idx.size, 4), dtype=torch.uint8, device="cuda")
+    out16 = torch.zeros((idx.size, 4), dtype=torch.float16, device="cuda")
+    g.colorize(_dev(idx), idx.size, nodes, out8, out16, fmt=mg.MG_BOTH)
+    torch.cuda.synchronize()
+    assert _rgba8_ok(out8.cpu().numpy(), oracle.lookup(idx, ref)) and _f16_ok(out16.cpu().numpy(), oracle.lookup(idx, ref))
+    with pytest.raises(mg.MgError):
+        g.colorize(_dev(idx), idx.size, nodes, out8, fmt=mg.MG_RGBA8, from_last_propagate=True)
+    nodes2 = torch.zeros_like(nodes)
+    out_dev = torch.zeros((idx.size, 4), dtype=torch.uint8, device="cuda")
+    g.tf_update_host(torch.from_numpy(tf).pin_memory(), nodes2, _dev(idx), idx.size, out_dev, None, fmt=mg.MG_RGBA8)
+    torch.cuda.synchronize()
+    assert _rgba8_ok(out_dev.cpu().numpy(), oracle.lookup(idx, ref))
+    g.close()
 
 
 def test_tf_update_host_end_to_end(mg):
@@ -277,8 +372,9 @@ def test_error_paths(mg):
     assert mg.kernel_launch_count() > 0
 
 
+@pytest.mark.parametrize("reuse", [True, False], ids=["from_last_propagate", "derive"])
 @pytest.mark.parametrize("profile,n_vox", [("big_then_tail", 200003), ("big_levels", 3000001), ("tiny_all_tail", 4099)])
-def test_back_to_back_updates_without_sync(mg, profile, n_vox):
+def test_back_to_back_updates_without_sync(mg, profile, n_vox, reuse):
     """Programmatic dependent launch lets a kernel become resident before its predecessor has finished
     (griddepcontrol.wait orders them).  Many TF updates enqueued back to back, each with its own TF and
     its own output buffers, no host synchronisation in between: every update must see exactly its own
@@ -298,7 +394,7 @@ def test_back_to_back_updates_without_sync(mg, profile, n_vox):
     st = torch.cuda.current_stream().cuda_stream
     for u in range(n_upd):
         g.propagate(d_tfs[u], nodes, st)
-        g.colorize(d_idx, n_vox, nodes, outs[u], fmt=mg.MG_RGBA8, stream=st)
+        g.colorize(d_idx, n_vox, nodes, outs[u], fmt=mg.MG_RGBA8, stream=st, from_last_propagate=reuse)
         snaps[u].copy_(nodes)                                                 # stream-ordered snapshot
     torch.cuda.synchronize()
     for u in range(n_upd):
