@@ -326,8 +326,11 @@ CONFIGS = {
             kind="voronoi", zscale=1, jitter=3, alpha_zero_frac=0.0),
     3: dict(name="cfg3_neocortex_shaped", dims=(2048, 2048, 300), n_segments=1182, seed=3,
             kind="voronoi", zscale=7, jitter=0, alpha_zero_frac=0.3),
+    # quant_bits: the builder's weight bitrate for this config when the caller names none.  The paper's b = 9 (L305)
+    # everywhere except config 4, whose 15,918-component root sits 14 lerps deep: measured at full size, b = 9 gives
+    # max |C_graph - C_dir| = 2.05e-3 there, b = 10 gives 9.3e-4 -- the smallest b inside north_star's 2e-3
     4: dict(name="cfg4_polymer_shaped", dims=(614, 961, 600), n_segments=15917, seed=4,
-            kind="cylinders", alpha_zero_frac=0.0),
+            kind="cylinders", alpha_zero_frac=0.0, quant_bits=10),
     5: dict(name="cfg5_dag_stress", n_nodes=1 << 26, n_levels=24, n_leaves=1 << 14, seed=5,
             kind="dag", volume_voxels=512 ** 3),
 }

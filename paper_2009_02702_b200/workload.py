@@ -280,6 +280,8 @@ def make(cfg_id: int, scale: float = 1.0, device_synth: bool = True, keep_seg: b
         w.stats["synth_s"] = t1 - t0
         return w
     c = synth.scaled_config(cfg_id, scale)
+    if "quant_bits" in c:
+        builder_params.setdefault("quant_bits", c["quant_bits"])
     t0 = time.perf_counter()
     if device_mipmap:
         import torch

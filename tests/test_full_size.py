@@ -8,9 +8,15 @@ mg_load_graph -> ONE concatenated node-index mipmap, ONE mg_colorize call over a
     with S from the input generator (not from the builder) and the 4 x n_leaves codes from the oracle;
   * every other level: seeded random samples + the first/last voxels of the level against the oracle's
     lookup/conversion on the same graph, and padding voxels against node 0;
-  * quantised-graph colour vs the DIRECT histogram (O-3 brute force on the generator's volume) on
-    sampled mixed voxels of levels 1-7: max-abs <= 2e-3 (north_star).
+  * quantised-graph colour vs the DIRECT histogram (O-3 brute force on the generator's volume): EVERY voxel of
+    every level whose dense histogram table fits 2 GB (levels >= 5 or 6: where the mixtures have hundreds of
+    components and the quantisation error peaks, Table 2), >= 1000 mixed voxels of each finer level:
+    max-abs <= 2e-3 (north_star); max ||mu - H||_1 (I11) and the bound I12 on the same voxels.  The per-level
+    maxima go to $MG_PARITY_REPORT_DIR/direct_parity_cfg<N>.json when that is set (DESIGN.md section 9 quotes them).
 """
+import json
+import os
+
 import numpy as np
 import pytest
 
@@ -137,28 +143,84 @@ def test_volume_config_full_size(libs, cfg_id):
                 padv = out4[s0 + nv:pad_end].cpu().numpy()
                 assert _rgba8_close(padv, np.broadcast_to(ref_nodes[0], padv.shape).copy())
 
-        # ---- quantised graph vs the DIRECT histogram on sampled mixed voxels (levels 1-7)
-        nl = ids.size
-        tf64 = tf.astype(np.float64)
-        nodes_host = nodes.cpu().numpy().astype(np.float64)
-        worst = 0.0
-        for l in range(1, min(8, len(w.mip_dims))):
-            xl, yl, zl = w.mip_dims[l]
-            idx_l = w.host_idx[l].reshape(-1)
+        # ---- quantised graph vs the DIRECT histogram (north_star's second tolerance; I11 / I12)
+        _check_direct_histogram(w, cfg_id, tf, nodes.cpu().numpy().astype(np.float64), seg_index, ids.size)
+        _check_render_full_size(mg, w, tf, seg_index)
+    finally:
+        w.close()
+
+
+def _check_direct_histogram(w, cfg_id, tf, nodes_host, seg_index, nl, dense_bytes=2 << 30, n_sample=1000, tol=TOL_DIRECT,
+                            first_level=1, tag=""):
+    """GPU node colours (fp32, quantised graph) against C_dir = sum_s H_s TF[s] with H by brute force from the
+    generator's volume (O-3), and the graph's symbolic mixtures mu (O-5) against H."""
+    hg = w.host_graph
+    tf64 = tf.astype(np.float64)
+    mu = oracle.symbolic_eval_sparse(hg["child_a"], hg["child_b"], hg["weight"], nl)
+    span = float(tf64.max() - tf64.min())
+    report = {"config": cfg_id, "quant_bits": int(w.stats["quant_bits"]), "n_nodes": int(w.stats["n_nodes"]),
+              "depth": int(w.stats["depth"]), "tolerance": TOL_DIRECT, "levels": []}
+    worst_c = worst_l1 = 0.0
+    for l in range(first_level, len(w.mip_dims)):
+        xl, yl, zl = w.mip_dims[l]
+        idx_l = w.host_idx[l].reshape(-1)
+        nv = idx_l.size
+        if nv * nl * 8 <= dense_bytes:                                     # every voxel of the level
+            H = oracle.brute_force_level(seg_index, nl, l).reshape(nv, nl)
+            vox = np.arange(nv)
+        else:                                                              # >= n_sample mixed voxels (a pure voxel is a leaf: exact)
             mixed = np.flatnonzero(idx_l >= nl)
             if mixed.size == 0:
                 continue
-            pick = mixed[(synth.u64(5, 300 + l, np.arange(6, dtype=np.uint64)) % np.uint64(mixed.size)).astype(np.int64)]
-            for v in pick:
-                k, rem = divmod(int(v), xl * yl)
-                j, i = divmod(rem, xl)
-                h = oracle.brute_force_histogram(seg_index, nl, l, i, j, k)
-                assert abs(h.sum() - 1.0) < 1e-12
-                direct = h @ tf64
-                worst = max(worst, float(np.abs(nodes_host[idx_l[v]] - direct).max()))
-        assert worst <= TOL_DIRECT, worst
-        print(f"cfg {cfg_id}: {w.stats['n_nodes']} nodes depth {w.stats['depth']}, max |graph - direct| on samples = {worst:.2e}")
-        _check_render_full_size(mg, w, tf, seg_index)
+            if mixed.size <= 2 * n_sample:
+                vox = mixed
+            else:                                                          # draws with replacement: a third more than needed
+                k = n_sample + n_sample // 3
+                vox = np.unique(mixed[(synth.u64(5, 300 + l, np.arange(k, dtype=np.uint64)) % np.uint64(mixed.size)).astype(np.int64)])
+                assert vox.size >= n_sample
+            H = np.stack([oracle.brute_force_histogram(seg_index, nl, l, int(v % xl), int((v // xl) % yl), int(v // (xl * yl)))
+                          for v in vox])
+        assert np.abs(H.sum(axis=1) - 1.0).max() < 1e-12
+        node = idx_l[vox].astype(np.int64)
+        err_c = np.abs(nodes_host[node] - H @ tf64).max(axis=1)
+        l1 = np.abs(mu[node].toarray() - H).sum(axis=1)
+        assert (err_c <= 0.5 * l1 * span + 2e-6).all(), f"I12 violated on level {l}"
+        report["levels"].append({"level": l, "voxels": int(nv), "checked": int(vox.size), "every_voxel": bool(vox.size == nv),
+                                 "max_abs_colour": float(err_c.max()), "max_l1_mixture": float(l1.max())})
+        worst_c, worst_l1 = max(worst_c, float(err_c.max())), max(worst_l1, float(l1.max()))
+    report["max_abs_colour"], report["max_l1_mixture"] = worst_c, worst_l1
+    print(f"cfg {cfg_id} (b = {report['quant_bits']}, {report['n_nodes']} nodes, depth {report['depth']}): max |C_graph - C_dir| = "
+          f"{worst_c:.3e}, max ||mu - H||_1 = {worst_l1:.3e}; per level: " +
+          ", ".join(f"l{r['level']}:{r['max_abs_colour']:.1e}/{r['max_l1_mixture']:.1e}({r['checked']})" for r in report["levels"]))
+    out_dir = os.environ.get("MG_PARITY_REPORT_DIR")
+    if out_dir:
+        os.makedirs(out_dir, exist_ok=True)
+        with open(os.path.join(out_dir, f"direct_parity_cfg{cfg_id}{tag}.json"), "w") as f:
+            json.dump(report, f, indent=1)
+    assert worst_c <= tol, worst_c
+    return report
+
+
+def test_config4_at_the_papers_bitrate_is_reported(libs):
+    """Config 4 at the paper's b = 9 (L305), which its synthetic stand-in does NOT carry inside north_star's 2e-3
+    (SURVEY.md Q7 expected as much: Table 2's max error 0.005 in l1 allows 2.5e-3 in colour): the same check as above
+    on every voxel of the levels >= 5 (where the error peaks), asserted only against I12 and 3e-3, and written to
+    the report as direct_parity_cfg4_b9.json.  The config itself is built at b = 10, the smallest bitrate that meets
+    the tolerance (synth.CONFIGS[4])."""
+    mg, workload = libs
+    w = workload.make(4, keep_seg=True, quant_bits=9)
+    try:
+        assert w.stats["quant_bits"] == 9
+        tf = w.tf(1)
+        g = w.graph
+        nodes = torch.empty((g.info.n_nodes, 4), dtype=torch.float32, device="cuda")
+        g.propagate(torch.from_numpy(tf).cuda(), nodes)
+        torch.cuda.synchronize()
+        _check_nodes(w, nodes, tf)
+        ids, seg_index = _leaf_index_chunked(w.seg)
+        r = _check_direct_histogram(w, 4, tf, nodes.cpu().numpy().astype(np.float64), seg_index, ids.size, tol=3e-3,
+                                    first_level=5, tag="_b9")
+        assert r["max_abs_colour"] > 0.5 * TOL_DIRECT                   # (it is the tolerance's order of magnitude)
     finally:
         w.close()
 
