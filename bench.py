@@ -33,6 +33,9 @@ FALLBACK_HBM_GBS = 6650.0            # /opt/skills/guides/B200_PROFILING.md fall
 NOMINAL_HBM_GBS = 8000.0             # BASELINE.json north_star "~8 TB/s"
 BYTES_PER_VOXEL = {"rgba8": 8, "rgba16f": 12}       # 4 B index + 4 B (8 B) output
 BYTES_PER_NODE_L2 = 28               # 12 B a/b/w stream + 16 B colour store (gathers hit L2), §8(d)
+BYTES_PER_NODE_DRAM = 60             # + two 16-B gathers when the fp32 palette exceeds L2 (config 5), §8(d)
+BYTES_GATHER_BEYOND_L2 = 16          # §8(d): per-voxel palette gather, counted only when the palette exceeds L2 (config 5)
+L2_BYTES = 126e6
 
 
 def parse_args():
@@ -61,7 +64,10 @@ def parse_args():
     p.add_argument("--dump-dir", default=None,
                    help="every rank writes rank<r>.npz there: its voxel range and the host copy of its colourised mipmap slab as "
                         "the last mg_tf_update_host of the e2e leg left it (tests compare the stitched slabs with the oracle)")
-    p.add_argument("--relabel", action="store_true", help="config 5: load the DAG with MG_RELABEL (levels sorted by children)")
+    p.add_argument("--relabel", action="store_true", help="(the default on config 5; kept for old command lines)")
+    p.add_argument("--no-relabel", action="store_true",
+                   help="config 5: load the DAG in the caller's numbering instead of with MG_RELABEL (every level sorted by its "
+                        "children: the higher child becomes a sequential sweep, 2.02 -> 1.72 ms)")
     p.add_argument("--no-query", action="store_true", help="skip the extra NEXT-4 measurement (mixture LUT + range queries)")
     p.add_argument("--render-empty-background", action="store_true",
                    help="render section: make the first leaf (config 4: background ID 0) exactly transparent, the case "
@@ -275,7 +281,8 @@ def run_b200(args) -> dict:
             red_dev = "cpu"
     from paper_2009_02702_b200 import mg, workload
 
-    w = workload.make(args.config, args.scale, relabel=args.relabel, device_mipmap=not args.host_mipmap and args.config != 5)
+    w = workload.make(args.config, args.scale, relabel=(args.config == 5 and not args.no_relabel),
+                      device_mipmap=not args.host_mipmap and args.config != 5)
     g = w.graph
     info = g.info
     n_nodes, n_internal = int(info.n_nodes), int(info.n_internal)
@@ -490,11 +497,36 @@ def run_b200(args) -> dict:
 
     peak, peak_src = peak_hbm_gbs()
     bpv = BYTES_PER_VOXEL[args.format]
+    beyond_l2 = 16.0 * n_nodes > L2_BYTES                 # the fp32 palette (16 B per node) does not fit L2: config 5 only
+    if beyond_l2:
+        bpv += BYTES_GATHER_BEYOND_L2
     col_avg = float(col_ms.mean())
     prop_avg = float(prop_ms.mean())
     algo_bytes = float(bpv) * w.n_voxels * (n_part / max(1, w.n_voxels_padded))      # rank 0's share (all of it unless --partition slab)
     achieved = algo_bytes / (col_avg * 1e-3) / 1e9
     kernel = "k_colorize"
+    col_launches = (launches / K) - int(info.n_launches_propagate)                    # > 1: one sweep per palette tile
+    roofline = {"bound": "hbm", "kernel": kernel, "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                "traffic": ncu_traffic(w.name, kernel), "algorithmic_bytes_per_launch": algo_bytes,
+                "algorithmic_bytes_per_voxel": bpv, "avg_launch_ms": col_avg, "peak_source": peak_src,
+                "timing": "CUDA events on the launch stream around every mg_colorize of the timed region"}
+    if col_launches > 1:
+        roofline["kernel"] = kernel = "k_colorize_tile"
+        roofline["traffic"] = ncu_traffic(w.name, kernel)
+        roofline["launches_per_step"] = col_launches
+        roofline["note"] = ("palette beyond the L2: one sweep per palette tile (<= 88 MB); achieved = the algorithmic bytes of the whole "
+                            "colourise / the time of all its sweeps; traffic = DRAM bytes of all sweeps")
+    prop_roofline = None
+    if beyond_l2:
+        # config 5: propagation is truly bandwidth-bound too -- report both; `roofline` is the one that takes longer
+        pa = float(BYTES_PER_NODE_DRAM) * n_internal
+        prop_roofline = {"bound": "hbm", "kernel": "k_level", "achieved": pa / (prop_avg * 1e-3) / 1e9, "peak": peak, "unit": "GB/s",
+                         "frac": pa / (prop_avg * 1e-3) / 1e9 / peak, "traffic": ncu_traffic(w.name, "k_level"),
+                         "algorithmic_bytes_per_launch": pa, "algorithmic_bytes_per_node": BYTES_PER_NODE_DRAM,
+                         "avg_launch_ms": prop_avg, "launches_per_step": int(info.n_launches_propagate),
+                         "note": "all levels of one mg_propagate together (one launch per level)"}
+        if prop_avg > col_avg:
+            roofline, prop_roofline = prop_roofline, roofline
     res = {
         # latency of ONE update: replicas do not shorten it (each rank runs a whole update; max over ranks), a slab
         # partition does (strong scaling).  The whole-job throughput of a replica run is `updates_per_s`.
@@ -507,15 +539,14 @@ def run_b200(args) -> dict:
         "nodes_per_s": n_internal / (prop_avg * 1e-3), "voxels_per_s": w.n_voxels * (n_part / max(1, w.n_voxels_padded)) / (col_avg * 1e-3),
         "hbm_gbs_step": (algo_bytes + BYTES_PER_NODE_L2 * n_internal) / (ms_per_step * 1e-3) / 1e9,
         "frac_of_nominal_8TBs": achieved / NOMINAL_HBM_GBS,
-        "roofline": {"bound": "hbm", "kernel": kernel, "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                     "traffic": ncu_traffic(w.name, kernel), "algorithmic_bytes_per_launch": algo_bytes,
-                     "avg_launch_ms": col_avg, "peak_source": peak_src,
-                     "timing": "CUDA events on the launch stream around every mg_colorize of the timed region"},
+        "roofline": roofline,
         "gpu_launches": int(launches), "clocks": clocks.summary(),
         "paper_context": "RTX Titan palette update (propagation only, incl. TF upload): 3.5 / 11.3 / 12.1 ms for 1.03 / 5.20 / 1.93 M "
                          "nodes (PAPER.md L373); the paper never materialises the RGBA mipmap (L221)",
         "setup_s": {k: round(v, 3) for k, v in w.stats.items() if k.endswith("_s")},
     }
+    if prop_roofline is not None:
+        res["roofline_second_kernel"] = prop_roofline
     if packed is not None:
         packed["frac"] = packed["achieved_gbs"] / peak
         res["packed"] = packed

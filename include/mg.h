@@ -171,6 +171,11 @@ int mg_propagate_host(mg_graph *g, const float *tf_rgba_host, float *node_rgba, 
  *                    written into it since (mg_propagate_attr), when an unflagged colourise has
  *                    re-derived the palettes since, or on a MG_NO_PALETTES graph.  Writes by the
  *                    caller's own kernels are the caller's to declare -- by NOT passing the flag.
+ *
+ * An RGBA8 palette beyond what the L2 serves for random gathers (more than 88 MB = 23 M nodes, up to 4 x that) is
+ * gathered tile by tile: the call then enqueues one sweep over the indices per palette tile (MG_COLORIZE_TILE_BYTES
+ * in the environment overrides the 88-MB tile size), each merging its voxels into out_rgba, so out_rgba is READ as
+ * well as written between the sweeps and must not be touched by another stream's work meanwhile.
  */
 int mg_colorize(mg_graph *g, uint32_t mip_level, const uint32_t *node_idx_volume,
                 uint64_t n_voxels, const float *node_rgba, void *out_rgba, void *out_rgba_aux,

@@ -10,6 +10,9 @@
 // streaming cache operators (the 11.5 GB stream must not evict the palette from L2).
 #include <cuda_fp16.h>
 
+#include <algorithm>
+#include <cstdlib>
+
 #include "mg_internal.h"
 
 namespace {
@@ -95,6 +98,74 @@ k_colorize(const uint4* __restrict__ idx4, uint64_t n_vec, const uint32_t* __res
     }
 }
 
+// RGBA8 palette larger than the L2 can hold for random gathers.  Measured on B200 (profiles/r02_cfg5_ncu.txt): a
+// randomly gathered table is served from L2 up to ~64 MB -- half the 126 MB: the two dies mirror read-shared lines --
+// and from DRAM at ~90 B per 4-byte gather beyond that.  The palette is then cut into T tiles of <= kTileBytes and the
+// volume is swept T times: sweep t gathers only the voxels whose node lies in tile t and merges them into the output
+// vectors the earlier sweeps wrote.  Streams stay coalesced: 4 B index read per sweep, plus a 16-B read-modify-write
+// of the vectors that hold a voxel of the tile (no read on the first sweep).  Each sweep costs about one streaming
+// pass (0.25 ms per 134 M voxels), so few, larger tiles win although they are only partly L2-resident: config 5
+// (256 MB) 1 sweep 2.06 ms, 2 -> 1.60, 3 -> 1.43, 4 -> 1.53, 8 -> 2.14.  L2 eviction-priority hints (evict_last on the
+// gathers, evict_first on the streams) changed nothing.  The fp16 palette (8 B per node, twice the sweeps, 16-B output
+// per voxel) never gained: it always takes the single sweep.
+constexpr uint64_t kTileBytes = 88ull << 20;
+constexpr uint32_t kMaxTiles = 4;                     // beyond that the T streaming sweeps cost more than the DRAM gathers
+
+// MG_COLORIZE_TILE_BYTES in the environment overrides kTileBytes (tuning on other parts; the tests use it to drive
+// the tiled path with small palettes).
+inline uint64_t tile_bytes()
+{
+    const char* e = getenv("MG_COLORIZE_TILE_BYTES");
+    const long long v = e ? atoll(e) : 0;
+    return v > 0 ? (uint64_t)v : kTileBytes;
+}
+
+__device__ __forceinline__ uint4 ld_cg_u4(const uint4* p)
+{
+    uint4 r;
+    asm volatile("ld.global.cg.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "l"(p));
+    return r;
+}
+
+template <bool FIRST>
+__global__ void __launch_bounds__(kThreads)
+k_colorize_tile(const uint4* __restrict__ idx4, uint64_t n_vec, const uint32_t* __restrict__ pal8, uint32_t lo, uint32_t n_tile,
+                uint4* out)                                           // out: read (by the later sweeps) and written
+{
+    constexpr int kVec = VecPerThread<false>::value;
+    const uint64_t base = (uint64_t)blockIdx.x * (kThreads * kVec) + threadIdx.x;
+    uint4 id[kVec];
+#pragma unroll
+    for (int k = 0; k < kVec; k++) {
+        const uint64_t v = base + (uint64_t)k * kThreads;
+        if (v < n_vec) id[k] = ld_cs_u4(idx4 + v);
+    }
+#pragma unroll
+    for (int k = 0; k < kVec; k++) {
+        const uint64_t v = base + (uint64_t)k * kThreads;
+        if (v >= n_vec) continue;
+        const bool in0 = id[k].x - lo < n_tile, in1 = id[k].y - lo < n_tile, in2 = id[k].z - lo < n_tile, in3 = id[k].w - lo < n_tile;
+        if (!(in0 | in1 | in2 | in3)) continue;                       // other sweeps own all four voxels
+        uint4 o = make_uint4(0, 0, 0, 0);
+        if (!FIRST && !(in0 & in1 & in2 & in3)) o = ld_cg_u4(out + v);   // (.cg measured 5 % faster than .cs here)
+        if (in0) o.x = __ldg(pal8 + id[k].x);
+        if (in1) o.y = __ldg(pal8 + id[k].y);
+        if (in2) o.z = __ldg(pal8 + id[k].z);
+        if (in3) o.w = __ldg(pal8 + id[k].w);
+        st_cs_u4(out + v, o);
+    }
+}
+
+// Number of RGBA8 palette tiles: 1 = the palette fits (or is too large to gain), plain single-sweep kernel.
+inline uint32_t palette_tiles(uint64_t n_nodes, uint64_t n_vec)
+{
+    const uint64_t tb = tile_bytes();
+    const uint64_t t = (n_nodes * 4 + tb - 1) / tb;
+    if (t < 2 || t > kMaxTiles) return 1;
+    if (n_vec * 4 < n_nodes / 4) return 1;           // few voxels: they touch a small part of the palette once
+    return (uint32_t)t;
+}
+
 // Scalar path: ragged head/tail around the vector body, or whole calls whose pointers are not
 // mutually alignable.  Voxels [0, n).
 template <bool W8, bool W16>
@@ -131,13 +202,34 @@ int launch_colorize(const mg_graph* g, const uint32_t* idx, uint64_t n, uint32_t
         constexpr int kVec = VecPerThread<W16>::value;
         const uint64_t blocks = (n_vec + (uint64_t)kThreads * kVec - 1) / ((uint64_t)kThreads * kVec);
         if (blocks > 0x7fffffffull) { mg::set_error("mg_colorize: too many voxels for one launch"); return MG_ERR_INVALID_ARG; }
-        // A NORMAL launch (no programmatic dependent launch): the palette gathers use the non-coherent
+        // NORMAL launches (no programmatic dependent launch): the palette gathers use the non-coherent
         // path (ld.global.nc, L1-cached), which is only safe behind a full kernel boundary -- measured: with
         // PDL a back-to-back update read stale palette lines (tests/test_gpu_parity.py::test_back_to_back...).
-        k_colorize<W8, W16><<<(unsigned)blocks, kThreads, 0, st>>>(
-            reinterpret_cast<const uint4*>(idx + head), n_vec, g->d_pal8, g->d_pal16,
-            reinterpret_cast<uint4*>(W8 ? out8 + head : nullptr), reinterpret_cast<uint4*>(W16 ? out16 + head : nullptr));
-        mg::count_launch();
+        const uint4* idx4 = reinterpret_cast<const uint4*>(idx + head);
+        const uint32_t t8 = W8 ? palette_tiles(g->n_nodes, n_vec) : 1;
+        if (t8 == 1) {
+            k_colorize<W8, W16><<<(unsigned)blocks, kThreads, 0, st>>>(
+                idx4, n_vec, g->d_pal8, g->d_pal16,
+                reinterpret_cast<uint4*>(W8 ? out8 + head : nullptr), reinterpret_cast<uint4*>(W16 ? out16 + head : nullptr));
+            mg::count_launch();
+        } else {
+            // RGBA8 tile by tile; the fp16 output of MG_BOTH takes its own single sweep
+            uint4* o = reinterpret_cast<uint4*>(out8 + head);
+            const uint64_t bl = (n_vec + (uint64_t)kThreads * VecPerThread<false>::value - 1) / ((uint64_t)kThreads * VecPerThread<false>::value);
+            const uint32_t per = (uint32_t)((g->n_nodes + t8 - 1) / t8);
+            for (uint32_t t = 0; t < t8; t++) {
+                const uint32_t lo = t * per, nt = (uint32_t)std::min<uint64_t>(per, g->n_nodes - lo);
+                if (t == 0) k_colorize_tile<true><<<(unsigned)bl, kThreads, 0, st>>>(idx4, n_vec, g->d_pal8, lo, nt, o);
+                else k_colorize_tile<false><<<(unsigned)bl, kThreads, 0, st>>>(idx4, n_vec, g->d_pal8, lo, nt, o);
+                mg::count_launch();
+            }
+            if (W16) {
+                const uint64_t b16 = (n_vec + (uint64_t)kThreads * VecPerThread<true>::value - 1) / ((uint64_t)kThreads * VecPerThread<true>::value);
+                k_colorize<false, true><<<(unsigned)b16, kThreads, 0, st>>>(idx4, n_vec, g->d_pal8, g->d_pal16, nullptr,
+                                                                            reinterpret_cast<uint4*>(out16 + head));
+                mg::count_launch();
+            }
+        }
     }
     if (head) {
         k_colorize_scalar<W8, W16><<<1, 32, 0, st>>>(idx, head, g->d_pal8, g->d_pal16, out8, out16);

@@ -95,5 +95,6 @@ def test_committed_traffic_table_is_readable_by_bench():
     import bench
     t = bench.ncu_traffic("cfg3_neocortex_shaped", "k_colorize")
     assert t is not None and 0.9 * 8 * 1438087061 < t < 1.1 * 8 * 1438087061          # about the algorithmic 8 B / voxel
-    assert bench.ncu_traffic("cfg5_dag_stress", "k_colorize") > 8 * 512 ** 3         # random gathers: far above it
+    assert bench.ncu_traffic("cfg5_dag_stress", "k_colorize_tile") > 24 * 512 ** 3   # random gathers: far above it
+    assert bench.ncu_traffic("cfg5_dag_stress", "k_level") > 60 * 2 ** 26
     assert bench.ncu_traffic("no_such_workload", "k_colorize") is None

@@ -197,6 +197,43 @@ def test_colorize_matches_oracle(mg, n_vox, fmt_name, reuse):
         assert _f16_ok(out16.cpu().numpy()[:n_vox], ref)
 
 
+@pytest.mark.parametrize("fmt_name", ["RGBA8", "RGBA16F", "BOTH"])
+@pytest.mark.parametrize("tile_bytes", [40000, 90000, 200000, 333333])
+def test_colorize_tiled_palette_matches_oracle(mg, fmt_name, tile_bytes, monkeypatch):
+    """An RGBA8 palette larger than the L2 serves is gathered tile by tile, one sweep over the indices per tile
+    (include/mg.h, mg_colorize).  MG_COLORIZE_TILE_BYTES shrinks the tile so that an 84,999-node palette (340 KB)
+    takes 4, 2 and 2 sweeps (and, at 40,000 B, the single sweep again: more than 4 tiles); ragged head / tail, an
+    output pre-filled with garbage, every voxel against the oracle.  fp16 always takes one sweep."""
+    monkeypatch.setenv("MG_COLORIZE_TILE_BYTES", str(tile_bytes))
+    sizes = PROFILES["big_then_tail"]
+    a, b, w, off = synth.random_dag_levels(sizes, seed=5)
+    tf = synth.random_tf(sizes[0], 46)
+    g, nodes = _propagate(mg, a, b, w, off, sizes[0], tf)
+    ref_nodes = oracle.graph_eval(a, b, w, sizes[0], tf.astype(np.float64))
+    n_vox = 400003
+    idx = synth.random_node_idx(n_vox + 3, a.size, 147)
+    idx[3:40] = np.arange(37) * (a.size // 37)                # one vector per combination of tiles, more or less
+    d_idx = _dev(idx)
+    ref = oracle.lookup(idx[3:], ref_nodes)
+    out8 = torch.full((n_vox + 3, 4), 0xCD, dtype=torch.uint8, device="cuda")
+    out16 = torch.full((n_vox + 3, 4), float("nan"), dtype=torch.float16, device="cuda")
+    fmt = getattr(mg, "MG_" + fmt_name)
+    launches0 = mg.kernel_launch_count()
+    args = {"RGBA8": (out8[3:],), "RGBA16F": (out16[3:],), "BOTH": (out8[3:], out16[3:])}[fmt_name]
+    g.colorize(d_idx[3:], n_vox, nodes, *args, fmt=fmt, from_last_propagate=True)
+    torch.cuda.synchronize()
+    n_sweeps = mg.kernel_launch_count() - launches0 - 2      # head + tail scalar launches
+    t8 = -(-a.size * 4 // tile_bytes)
+    t8 = t8 if 2 <= t8 <= 4 else 1
+    want = {"RGBA8": t8, "RGBA16F": 1, "BOTH": 1 if t8 == 1 else t8 + 1}[fmt_name]
+    assert n_sweeps == want, (n_sweeps, want)
+    if fmt_name in ("RGBA8", "BOTH"):
+        assert _rgba8_ok(out8.cpu().numpy()[3:], ref) and (out8.cpu().numpy()[:3] == 0xCD).all()
+    if fmt_name in ("RGBA16F", "BOTH"):
+        assert _f16_ok(out16.cpu().numpy()[3:], ref)
+    g.close()
+
+
 @pytest.mark.parametrize("shift_idx,shift_out", [(1, 1), (3, 3), (2, 0), (1, 2)])
 def test_colorize_unaligned_views(mg, shift_idx, shift_out):
     """Per-level sub-buffers of a concatenated mipmap start at arbitrary voxels: same shift -> vector
