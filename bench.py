@@ -398,24 +398,43 @@ def run_b200(args) -> dict:
                           "(PAPER.md L267-L271, L414)", "width": view["width"], "height": view["height"],
                   "step_voxels": view["step_voxels"], "tf": f"config TF, opacities x {synth.RENDER_ALPHA_SCALE}" + (", first leaf transparent" if args.render_empty_background else ""),
                   "frames": 10}
-        for label, thr, fl in (("ess", view["ess_threshold"], view["flags"]), ("no_ess", -1.0, view["flags"]),
-                               ("ess_generic_mipmap", view["ess_threshold"], 0), ("no_ess_generic_mipmap", -1.0, 0)):
+        # the empty-space mask of mg_ess_mask_build (rebuilt per TF update: timed on its own) turns R6's climb into one load
+        mask = None
+        if 3 <= len(w.mip_dims) <= 18:
+            mask = torch.empty(w.level_voxels[2], dtype=torch.int16, device="cuda")
+            for _ in range(2):
+                g.ess_mask_build(w.d_idx, desc, nodes, view["ess_threshold"], mask, st)
+            m0, m1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            m0.record(stream)
+            for _ in range(10):
+                g.ess_mask_build(w.d_idx, desc, nodes, view["ess_threshold"], mask, st)
+            m1.record(stream)
+            torch.cuda.synchronize()
+            render["ess_mask_build_ms"] = m0.elapsed_time(m1) / 10
+            render["ess_mask_mbytes"] = 2e-6 * w.level_voxels[2]
+        for label, thr, fl, use_mask in (("ess", view["ess_threshold"], view["flags"], True), ("no_ess", -1.0, view["flags"], False),
+                                         ("ess_climb", view["ess_threshold"], view["flags"], False),
+                                         ("ess_generic_mipmap", view["ess_threshold"], 0, True), ("no_ess_generic_mipmap", -1.0, 0, False)):
             v = mg.view_struct(dict(view, ess_threshold=thr, flags=fl))
+            mk = mask if use_mask else None
             stats = torch.zeros(4, dtype=torch.int64, device="cuda")
             for _ in range(2):
-                g.render(w.d_idx, desc, nodes, v, img, None, st)
+                g.render(w.d_idx, desc, nodes, v, img, None, st, ess_mask_device=mk)
             torch.cuda.synchronize()
             r0, r1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
             r0.record(stream)
             for _ in range(render["frames"]):
-                g.render(w.d_idx, desc, nodes, v, img, None, st)
+                g.render(w.d_idx, desc, nodes, v, img, None, st, ess_mask_device=mk)
             r1.record(stream)
-            g.render(w.d_idx, desc, nodes, v, img, stats, st)
+            g.render(w.d_idx, desc, nodes, v, img, stats, st, ess_mask_device=mk)
             torch.cuda.synchronize()
             ms = r0.elapsed_time(r1) / render["frames"]
             ev_, sk_, un_, _ = (int(x) for x in stats.cpu().numpy())
             render[label] = {"ms_per_frame": ms, "fps": 1e3 / ms, "samples_composited": ev_, "samples_skipped": sk_,
-                             "samples_one_leaf_shortcut": un_, "samples_per_s": (ev_ + sk_) / (ms * 1e-3)}
+                             "samples_one_leaf_shortcut": un_, "samples_per_s": (ev_ + sk_) / (ms * 1e-3),
+                             "ess_mask": bool(use_mask and mask is not None)}
+        render["ess_speedup"] = render["no_ess"]["ms_per_frame"] / render["ess"]["ms_per_frame"]
+        del mask
         render["histogram_mipmap_flag_speedup"] = render["no_ess_generic_mipmap"]["ms_per_frame"] / render["no_ess"]["ms_per_frame"]
         render["coverage"] = float((img[..., 3] > 0).float().mean().item())
         del img

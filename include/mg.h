@@ -342,6 +342,33 @@ int mg_render(mg_graph *g, const uint32_t *node_idx_mipmap, const mg_mipmap_desc
               const float *node_rgba, const mg_view *view, float *out_rgba, uint64_t *stats_device,
               void *stream);
 
+/*
+ * Hierarchical empty-space skipping without the per-probe climb (R6; PAPER.md L271 (i)-(iii)).  The climb of R6
+ * reads, per probe, the palette opacity of the parent voxels from level floor(lambda) + 2 upwards -- a chain of
+ * dependent gathers.  Those comparisons depend only on the voxel, the palette and the threshold, so they can be
+ * made once per TF update: mg_ess_mask_build writes, for every voxel of mip level 2, a 16-bit mask whose bit k says
+ * "the ancestor of this voxel on level 2 + k has opacity < ess_threshold" (bit 0: the voxel itself).  A probe of
+ * mg_render_ex is then ONE 2-byte load: the run of set bits from level floor(lambda) + 2 on is exactly the climb.
+ * Same blocks, same skipped samples, same image as mg_render.
+ *   ess_mask        DEVICE uint16[X_2 Y_2 Z_2] (level 2 of `mip`, x fastest), caller-allocated
+ *   ess_threshold   the mg_view.ess_threshold the mask will be used with
+ * Needs 3 <= n_levels <= 18.  Must be rebuilt after every change of node_rgba or of the threshold (the library
+ * cannot see a stale mask: with one, skipped samples are no longer provably transparent).  Enqueue-only, one launch.
+ */
+int mg_ess_mask_build(mg_graph *g, const uint32_t *node_idx_mipmap, const mg_mipmap_desc *mip,
+                      const float *node_rgba, double ess_threshold, uint16_t *ess_mask, void *stream);
+
+/* Optional acceleration data of mg_render_ex; every pointer may be NULL (then the plain path of mg_render is taken). */
+typedef struct mg_render_aux {
+    const uint16_t *ess_mask;   /* DEVICE, from mg_ess_mask_build on THIS mipmap, palette and view->ess_threshold */
+    const void *reserved;       /* NULL */
+} mg_render_aux;
+
+/* mg_render with acceleration data (aux may be NULL: identical to mg_render). */
+int mg_render_ex(mg_graph *g, const uint32_t *node_idx_mipmap, const mg_mipmap_desc *mip,
+                 const float *node_rgba, const mg_view *view, const mg_render_aux *aux, float *out_rgba,
+                 uint64_t *stats_device, void *stream);
+
 /* ------------------------------------------------------------------------------------------------
  * NEXT-4: mixture lookup table with error propagation and sub-volume (range) queries
  * (section 3.5 Eq. 17-18, section 3.6, Table 4).

@@ -29,7 +29,7 @@ SYMBOLS = ["mg_load_graph", "mg_free_graph", "mg_graph_info", "mg_level_offsets"
            "mg_relabel_indices", "mg_propagate", "mg_propagate_host", "mg_colorize", "mg_tf_update_host",
            "mg_last_error", "mg_kernel_launch_count",
            "mg_bits_per_voxel", "mg_packed_stream_bytes", "mg_index_range", "mg_pack_indices", "mg_colorize_packed",
-           "mg_propagate_attr", "mg_render",
+           "mg_propagate_attr", "mg_render", "mg_render_ex", "mg_ess_mask_build",
            "mg_mixture_lut_build", "mg_mixture_lut_free", "mg_mixture_lut_info", "mg_mixture_lut_export", "mg_range_query",
            "mg_mipmap_leaf_index", "mg_mipmap_front_level1"]
 
@@ -109,6 +109,16 @@ class MgView(C.Structure):
 
 lib.mg_render.argtypes = [_vp, _vp, C.POINTER(MgMipmapDesc), _vp, C.POINTER(MgView), _vp, _vp, _vp]
 lib.mg_render.restype = C.c_int
+
+
+class MgRenderAux(C.Structure):
+    _fields_ = [("ess_mask", _vp), ("reserved", _vp)]
+
+
+lib.mg_render_ex.argtypes = [_vp, _vp, C.POINTER(MgMipmapDesc), _vp, C.POINTER(MgView), C.POINTER(MgRenderAux), _vp, _vp, _vp]
+lib.mg_render_ex.restype = C.c_int
+lib.mg_ess_mask_build.argtypes = [_vp, _vp, C.POINTER(MgMipmapDesc), _vp, C.c_double, _vp, _vp]
+lib.mg_ess_mask_build.restype = C.c_int
 
 
 class MgLutInfo(C.Structure):
@@ -323,11 +333,24 @@ class Graph:
                "mg_tf_update_host")
 
     def render(self, node_idx_device, mip, node_rgba_device, view, out_rgba_device, stats_device=None,
-               stream: int = 0) -> None:
+               stream: int = 0, ess_mask_device=None) -> None:
+        """mg_render, or mg_render_ex when ``ess_mask_device`` (from ess_mask_build) is given."""
         m = mip if isinstance(mip, MgMipmapDesc) else mipmap_desc(*mip)
         v = view if isinstance(view, MgView) else view_struct(view)
-        _check(lib.mg_render(self._h, _ptr(node_idx_device), C.byref(m), _ptr(node_rgba_device), C.byref(v),
-                             _ptr(out_rgba_device), _ptr(stats_device), stream or None), "mg_render")
+        if ess_mask_device is None:
+            _check(lib.mg_render(self._h, _ptr(node_idx_device), C.byref(m), _ptr(node_rgba_device), C.byref(v),
+                                 _ptr(out_rgba_device), _ptr(stats_device), stream or None), "mg_render")
+        else:
+            aux = MgRenderAux(_ptr(ess_mask_device), None)
+            _check(lib.mg_render_ex(self._h, _ptr(node_idx_device), C.byref(m), _ptr(node_rgba_device), C.byref(v),
+                                    C.byref(aux), _ptr(out_rgba_device), _ptr(stats_device), stream or None), "mg_render_ex")
+
+    def ess_mask_build(self, node_idx_device, mip, node_rgba_device, ess_threshold: float, ess_mask_device,
+                       stream: int = 0) -> None:
+        """Fill ``ess_mask_device`` (uint16 per voxel of mip level 2) for mg_render_ex."""
+        m = mip if isinstance(mip, MgMipmapDesc) else mipmap_desc(*mip)
+        _check(lib.mg_ess_mask_build(self._h, _ptr(node_idx_device), C.byref(m), _ptr(node_rgba_device),
+                                     float(ess_threshold), _ptr(ess_mask_device), stream or None), "mg_ess_mask_build")
 
     def mixture_lut(self, weight_sigma=None, stream: int = 0) -> "MixtureLut":
         """NEXT-4: build the mixture lookup table (mu, dmu per node) of this graph on the device."""

@@ -244,7 +244,15 @@ def _check_render_full_size(mg, w, tf, seg_index):
     g.render(w.d_idx, desc, nodes, view, img, stats[0:4])
     g.render(w.d_idx, desc, nodes, dict(view, ess_threshold=-1.0), img_off, stats[4:8])
     g.render(w.d_idx, desc, nodes, dict(view, flags=0), img_plain, stats[8:12])
+    # mg_render_ex with the empty-space mask (what bench.py times as "ess"): same image, same counters as the climb
+    mask = torch.empty(w.level_voxels[2], dtype=torch.int16, device="cuda")
+    g.ess_mask_build(w.d_idx, desc, nodes, view["ess_threshold"], mask)
+    img_mask = torch.full((H, W, 4), float("nan"), dtype=torch.float32, device="cuda")
+    stats_mask = torch.zeros(4, dtype=torch.int64, device="cuda")
+    g.render(w.d_idx, desc, nodes, view, img_mask, stats_mask, ess_mask_device=mask)
     torch.cuda.synchronize()
+    assert torch.equal(img, img_mask) and torch.equal(stats[0:4], stats_mask)
+    del mask, img_mask
     got, got_off = img.cpu().numpy().astype(np.float64), img_off.cpu().numpy().astype(np.float64)
     st = stats.cpu().numpy().reshape(3, 4)
     assert np.isfinite(got).all() and got[..., 3].max() > 0.5

@@ -59,6 +59,16 @@ def _gpu_render(mg, g, levels, pal32_dev, view, align=1):
     stats = torch.zeros(4, dtype=torch.int64, device="cuda")
     g.render(d_idx, (offs, dims), pal32_dev, view, out, stats)
     torch.cuda.synchronize()
+    if view["ess_threshold"] >= 0 and 3 <= len(levels) <= 18:
+        # the same image through mg_render_ex with the empty-space mask of mg_ess_mask_build: the mask holds exactly the
+        # comparisons of R6's climb, so image AND counters must be bit-identical
+        mask = torch.full((levels[2].size,), -1, dtype=torch.int16, device="cuda")
+        g.ess_mask_build(d_idx, (offs, dims), pal32_dev, view["ess_threshold"], mask)
+        out_m = torch.full((H, W, 4), float("nan"), dtype=torch.float32, device="cuda")
+        stats_m = torch.zeros(4, dtype=torch.int64, device="cuda")
+        g.render(d_idx, (offs, dims), pal32_dev, view, out_m, stats_m, ess_mask_device=mask)
+        torch.cuda.synchronize()
+        assert torch.equal(out, out_m) and torch.equal(stats, stats_m), (stats.tolist(), stats_m.tolist())
     s = stats.cpu().numpy()
     assert s[2] <= s[0] and s[3] == 0 and (s[2] == 0 or view.get("flags", 0))
     return out.cpu().numpy().astype(np.float64), (int(s[0]), int(s[1]), int(s[2]))
