@@ -54,6 +54,10 @@ def parse_args():
     p.add_argument("--host-mipmap", action="store_true",
                    help="configs 1-4: build the whole histogram mipmap on the host (default: the two finest levels are classified "
                         "on the device, NEXT-4 front end; same graph and node indices either way)")
+    p.add_argument("--device-levels", action="store_true",
+                   help="configs 1-4: build the levels >= 1 of the histogram mipmap on the device too (mg_mipmap_levels_build: merge + "
+                        "hash-cons per level; the host continues above the last level whose mixtures a warp can merge); same graph "
+                        "and node indices, shorter setup")
     p.add_argument("--partition", choices=["replicas", "slab"], default="replicas",
                    help="N > 1: independent replicas of the whole update (default, weak scaling) or ONE update whose colourise is "
                         "split into N contiguous voxel slabs with the graph replicated (strong scaling, SURVEY.md 8(e)); no collective either way")
@@ -282,7 +286,7 @@ def run_b200(args) -> dict:
     from paper_2009_02702_b200 import mg, workload
 
     w = workload.make(args.config, args.scale, relabel=(args.config == 5 and not args.no_relabel),
-                      device_mipmap=not args.host_mipmap and args.config != 5)
+                      device_mipmap=("levels" if args.device_levels else True) if (not args.host_mipmap and args.config != 5) else False)
     g = w.graph
     info = g.info
     n_nodes, n_internal = int(info.n_nodes), int(info.n_internal)
@@ -562,7 +566,8 @@ def run_b200(args) -> dict:
         "gpu_launches": int(launches), "clocks": clocks.summary(),
         "paper_context": "RTX Titan palette update (propagation only, incl. TF upload): 3.5 / 11.3 / 12.1 ms for 1.03 / 5.20 / 1.93 M "
                          "nodes (PAPER.md L373); the paper never materialises the RGBA mipmap (L221)",
-        "setup_s": {k: round(v, 3) for k, v in w.stats.items() if k.endswith("_s")},
+        "setup_s": dict({k: round(v, 3) for k, v in w.stats.items() if k.endswith("_s")},
+                        **({"device_levels_done": w.stats["device_levels_done"]} if "device_levels_done" in w.stats else {})),
     }
     if prop_roofline is not None:
         res["roofline_second_kernel"] = prop_roofline

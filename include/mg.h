@@ -463,6 +463,51 @@ int mg_mipmap_front_level1(const uint32_t *level0_device, uint64_t X, uint64_t Y
                            uint32_t *level1_device, uint32_t *mixed_voxel_device, uint32_t *mixed_children_device,
                            uint64_t capacity, uint64_t *n_mixed, void *stream);
 
+/*
+ * The levels >= 1 on the device (second half of NEXT-4, continued; Eq. 4: only DISTINCT mixtures
+ * reach the factorisation).  For l = 1, 2, ...: a parent whose existing children carry one mixture inherits it; every
+ * other parent merges its children's sparse integer mixtures (each child weighing 1/N, reading Q2), divides by the common
+ * power of two and hash-conses the result (64-bit hash, contents verified).  A HANDLE is a leaf number (< 2^31) or
+ * 0x80000000 | mixture number (numbers in creation order: arbitrary).  A level in which one parent's children hold more
+ * than 256 entries in total is left to the host together with the levels above it (the few thousand voxels whose
+ * mixtures hold hundreds of segments): mgb_build_from_levels (include/mg_builder.h) continues from the last finished
+ * level and yields the same graph and node indices as mgb_build on the same volume.
+ *   level0_device   DEVICE uint32[Z][Y][X] leaf numbers (mg_mipmap_leaf_index)
+ *   levels_device   DEVICE uint32 buffer; level l >= 1 is written at levels_device + level_offset[l] (handles, x fastest)
+ *   level_offset    HOST uint64[n_levels] in voxels ([0] is not used); n_levels = length of the ceil-halving chain (L80)
+ *   out             the mixture store (device memory owned by the table; mg_mixture_table_free)
+ * Allocates (stores sized from the number of level-1 merges: MG_ERR_OOM if a later level overflows them) and
+ * synchronises `stream` several times per level.  Errors: MG_ERR_INVALID_ARG (NULL, dims / n_levels mismatch, level 1
+ * with >= 2^32 voxels, a 64-bit hash collision between different mixtures), MG_ERR_OOM, MG_ERR_CUDA.
+ */
+typedef struct mg_mixture_table mg_mixture_table;
+
+typedef struct mg_mixture_table_info_t {
+    uint64_t n_mixtures;    /* distinct mixtures with >= 2 non-zeros                                     */
+    uint64_t n_entries;     /* their (leaf, count) entries                                              */
+    uint64_t nnz_levels;    /* non-zeros summed over every voxel of the finished levels 1 .. levels_done */
+    uint64_t device_bytes;  /* device memory owned by the table                                         */
+    uint32_t levels_done;   /* last level built on the device (0: none)                                  */
+    uint32_t n_leaves;
+} mg_mixture_table_info_t;
+
+int mg_mipmap_levels_build(const uint32_t *level0_device, uint64_t X, uint64_t Y, uint64_t Z, uint32_t n_leaves,
+                           uint32_t *levels_device, const uint64_t *level_offset, uint32_t n_levels,
+                           mg_mixture_table **out, void *stream);
+void mg_mixture_table_free(mg_mixture_table *t);
+int mg_mixture_table_info(const mg_mixture_table *t, mg_mixture_table_info_t *info);
+
+/* Copy the store to the HOST: per mixture its first entry (offset), non-zeros k, tlog (the reduced counts sum to
+ * 2^tlog) and first occurrence (level << 40 | voxel: the scanline order of L257); then the entries (leaf ascending
+ * inside a mixture, count).  Any pointer may be NULL.  Synchronises. */
+int mg_mixture_table_export(const mg_mixture_table *t, uint64_t *offset, uint32_t *k, uint32_t *tlog,
+                            uint64_t *first_pos, uint32_t *leaf, uint64_t *count);
+
+/* handles[i] = node_of_mixture[id] for every handle 0x80000000 | id (leaf handles are node numbers already): turns the
+ * device-built levels into node-index volumes once the host has numbered the mixtures' nodes.  DEVICE buffers.  Enqueue-only. */
+int mg_mipmap_remap_handles(uint32_t *handles_device, uint64_t n, const uint32_t *node_of_mixture_device,
+                            uint32_t n_mixtures, void *stream);
+
 /* Thread-local description of the last error returned on this thread ("" if none). */
 const char *mg_last_error(void);
 

@@ -98,6 +98,30 @@ int mgb_build_from_level1(uint64_t X, uint64_t Y, uint64_t Z, const uint32_t *le
                           const uint32_t *level1, const uint32_t *mixed_voxel, const uint32_t *mixed_children,
                           uint64_t n_mixed, const mgb_params *params, mgb_result **out);
 
+/*
+ * mgb_build_from_levels -- mgb_build for a volume whose levels 0 .. level_done of the histogram mipmap were built
+ * elsewhere (mg_mipmap_leaf_index + mg_mipmap_levels_build of include/mg.h).  The caller lists the distinct mixtures
+ * found there and passes the handles of the last finished level; the host continues with Eq. 4 from level_done + 1,
+ * then factorises.  Same graph, same node numbering as mgb_build on the same volume.  The node indices of the levels
+ * 0 .. level_done - 1 are not stored (mgb_get_node_idx fails for them): they follow from the caller's handles through
+ * mgb_get_front_mixture_nodes (mg_mipmap_remap_handles applies it on the device).
+ *   level_done      1 .. l_max
+ *   handles         uint32[voxels of level_done]: a leaf number, or 0x80000000 | q for the q-th listed mixture
+ *   mix_offset/k/tlog/first_pos   per listed mixture: first entry, non-zeros (>= 2), log2 of the sum of its counts,
+ *                   first occurrence level << 40 | voxel (the scanline order the canonical numbering sorts by, L257)
+ *   leaf, count     entries (leaves ascending inside a mixture; counts reduced: not all even)
+ *   nnz_levels      non-zeros summed over every voxel of the levels 1 .. level_done (statistics only)
+ * Errors: MGB_ERR_INVALID_ARG for malformed mixtures or handles.
+ */
+int mgb_build_from_levels(uint64_t X, uint64_t Y, uint64_t Z, const uint32_t *leaf_segment_id, uint32_t n_leaves,
+                          uint32_t level_done, const uint32_t *handles, uint64_t n_mixtures, const uint64_t *mix_offset,
+                          const uint32_t *mix_k, const uint32_t *mix_tlog, const uint64_t *mix_first_pos,
+                          const uint32_t *leaf, const uint64_t *count, uint64_t n_entries, uint64_t nnz_levels,
+                          const mgb_params *params, mgb_result **out);
+
+/* node_of_mixture[q] = node (final numbering) of the q-th mixture listed to mgb_build_from_levels. */
+int mgb_get_front_mixture_nodes(const mgb_result *r, uint32_t *node_of_mixture);
+
 /* Build from explicit mixtures instead of a volume (tests, Fig. 2): mixture m has entries
  * [offsets[m], offsets[m+1]) of (leaf[], count[]) with strictly increasing leaf numbers < n_leaves
  * and positive integer counts (any scale).  The result has one "mip level" holding n_mixtures

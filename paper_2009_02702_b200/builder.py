@@ -19,7 +19,8 @@ lib = C.CDLL(LIB_PATH)
 MGB_OK = 0
 PICK_SMALLEST_INDEX, PICK_SMALLEST_MASS = 0, 1
 
-SYMBOLS = ["mgb_default_params", "mgb_build", "mgb_build_from_level1", "mgb_build_from_mixtures", "mgb_free", "mgb_get_info",
+SYMBOLS = ["mgb_default_params", "mgb_build", "mgb_build_from_level1", "mgb_build_from_levels", "mgb_get_front_mixture_nodes",
+           "mgb_build_from_mixtures", "mgb_free", "mgb_get_info",
            "mgb_mip_dims", "mgb_get_graph", "mgb_node_idx_ptr", "mgb_get_node_idx", "mgb_get_codebook",
            "mgb_get_weight_sigma", "mgb_last_error"]
 
@@ -62,6 +63,11 @@ lib.mgb_get_node_idx.restype = C.c_int
 lib.mgb_build_from_level1.argtypes = [C.c_uint64, C.c_uint64, C.c_uint64, _vp, C.c_uint32, _vp, _vp, _vp, C.c_uint64,
                                       C.POINTER(Params), C.POINTER(_vp)]
 lib.mgb_build_from_level1.restype = C.c_int
+lib.mgb_build_from_levels.argtypes = [C.c_uint64, C.c_uint64, C.c_uint64, _vp, C.c_uint32, C.c_uint32, _vp, C.c_uint64, _vp, _vp, _vp, _vp,
+                                      _vp, _vp, C.c_uint64, C.c_uint64, C.POINTER(Params), C.POINTER(_vp)]
+lib.mgb_build_from_levels.restype = C.c_int
+lib.mgb_get_front_mixture_nodes.argtypes = [_vp, _vp]
+lib.mgb_get_front_mixture_nodes.restype = C.c_int
 lib.mgb_get_weight_sigma.argtypes = [_vp, _vp]
 lib.mgb_get_weight_sigma.restype = C.c_int
 lib.mgb_get_codebook.argtypes = [_vp, _vp, _vp, _vp]
@@ -185,6 +191,27 @@ def build_from_level1(dims_xyz, leaf_segment_id, level1, mixed_voxel, mixed_chil
                                      mv.ctypes.data if mv.size else None, mc.ctypes.data if mv.size else None, mv.size,
                                      C.byref(p), C.byref(h)), "mgb_build_from_level1")
     return Result(h)
+
+
+def build_from_levels(dims_xyz, leaf_segment_id, level_done: int, handles, mixtures: dict, nnz_levels: int,
+                      params: Params | None = None, **overrides):
+    """Build from the levels 0 .. ``level_done`` of the histogram mipmap built elsewhere (mg.MixtureTable):
+    ``handles`` uint32 of level ``level_done``, ``mixtures`` = MixtureTable.export().  Returns (Result, node_of_mixture
+    uint32 [n listed mixtures])."""
+    p = params if params is not None else default_params(**overrides)
+    ids = np.ascontiguousarray(leaf_segment_id, dtype=np.uint32)
+    h = np.ascontiguousarray(handles, dtype=np.uint32).reshape(-1)
+    m = {k: np.ascontiguousarray(v) for k, v in mixtures.items()}
+    X, Y, Z = (int(d) for d in dims_xyz)
+    out = _vp()
+    _check(lib.mgb_build_from_levels(X, Y, Z, ids.ctypes.data, ids.size, int(level_done), h.ctypes.data, m["k"].size,
+                                     m["offset"].ctypes.data, m["k"].ctypes.data, m["tlog"].ctypes.data, m["first_pos"].ctypes.data,
+                                     m["leaf"].ctypes.data, m["count"].ctypes.data, m["leaf"].size, int(nnz_levels), C.byref(p),
+                                     C.byref(out)), "mgb_build_from_levels")
+    r = Result(out)
+    nodes = np.zeros(m["k"].size, dtype=np.uint32)
+    _check(lib.mgb_get_front_mixture_nodes(out, nodes.ctypes.data), "mgb_get_front_mixture_nodes")
+    return r, nodes
 
 
 def build_from_mixtures(n_leaves: int, mixtures, params: Params | None = None, **overrides) -> Result:

@@ -171,12 +171,12 @@ extern "C" void mgb_free(mgb_result* r) { delete r; }
 
 // a0 - a2 for a volume: from the segment IDs (front == nullptr), or from levels 0 / 1 classified by a front end.
 static int build_volume(const uint32_t* seg, uint64_t X, uint64_t Y, uint64_t Z, const Level1Front* front,
-                        const mgb_params* params, mgb_result** out)
+                        const mgb_params* params, mgb_result** out, const LevelsFront* levels = nullptr)
 {
     g_err[0] = 0;
     if (!out) { set_error("mgb_build: out is NULL"); return MGB_ERR_INVALID_ARG; }
     *out = nullptr;
-    if ((!seg && !front) || X == 0 || Y == 0 || Z == 0) { set_error("mgb_build: NULL volume or zero dimension"); return MGB_ERR_INVALID_ARG; }
+    if ((!seg && !front && !levels) || X == 0 || Y == 0 || Z == 0) { set_error("mgb_build: NULL volume or zero dimension"); return MGB_ERR_INVALID_ARG; }
     if (X > 0x7fffffffull || Y > 0x7fffffffull || Z > 0x7fffffffull || X * Y * Z >= (1ull << 40)) {
         set_error("mgb_build: volume too large"); return MGB_ERR_INVALID_ARG;
     }
@@ -188,7 +188,7 @@ static int build_volume(const uint32_t* seg, uint64_t X, uint64_t Y, uint64_t Z,
         R = new mgb_result();
         const double t0 = now_s();
         Mipmap mm;
-        rc = build_mipmap(seg, X, Y, Z, (int)p.n_threads, mm, front);
+        rc = build_mipmap(seg, X, Y, Z, (int)p.n_threads, mm, front, levels);
         if (rc != MGB_OK) { delete R; return rc; }
         const double t1 = now_s();
         Factorised F;
@@ -206,7 +206,8 @@ static int build_volume(const uint32_t* seg, uint64_t X, uint64_t Y, uint64_t Z,
         for (uint32_t l = 0; l < n_mip; l++) {
             std::vector<uint32_t>& ids = mm.level_ids[l];
             const int64_t nv = (int64_t)ids.size();
-            n_vox_total += (l == 0 && front) ? X * Y * Z : (uint64_t)nv;      // with a front end level 0 stays with the caller
+            // with a front end the levels it classified stay with the caller: count their voxels all the same
+            n_vox_total += (ids.empty() && (front || levels)) ? mm.dims[3 * l] * mm.dims[3 * l + 1] * mm.dims[3 * l + 2] : (uint64_t)nv;
             uint32_t* P = ids.data();
             const uint32_t* nom = F.node_of_mix.data();
             const uint32_t* perm = new_of_old.data();
@@ -216,6 +217,10 @@ static int build_volume(const uint32_t* seg, uint64_t X, uint64_t Y, uint64_t Z,
                 P[v] = perm[id < n_leaves ? id : nom[id - n_leaves]];
             }
             R->node_idx[l].swap(ids);
+        }
+        if (levels) {                                                  // node of every mixture the caller listed
+            R->front_mixture_node.resize(mm.front_mixture.size());
+            for (size_t q = 0; q < mm.front_mixture.size(); q++) R->front_mixture_node[q] = new_of_old[F.node_of_mix[mm.front_mixture[q]]];
         }
         R->dims = mm.dims;
         R->leaf_segment_id = mm.leaf_segment_id;
@@ -273,6 +278,35 @@ extern "C" int mgb_build_from_level1(uint64_t X, uint64_t Y, uint64_t Z, const u
         }
     Level1Front front{leaf_segment_id, n_leaves, level1, mixed_voxel, mixed_children, n_mixed};
     return build_volume(nullptr, X, Y, Z, &front, params, out);
+}
+
+extern "C" int mgb_build_from_levels(uint64_t X, uint64_t Y, uint64_t Z, const uint32_t* leaf_segment_id, uint32_t n_leaves,
+                                     uint32_t level_done, const uint32_t* handles, uint64_t n_mixtures, const uint64_t* mix_offset,
+                                     const uint32_t* mix_k, const uint32_t* mix_tlog, const uint64_t* mix_first_pos, const uint32_t* leaf,
+                                     const uint64_t* count, uint64_t n_entries, uint64_t nnz_levels, const mgb_params* params,
+                                     mgb_result** out)
+{
+    g_err[0] = 0;
+    if (out) *out = nullptr;
+    if (!leaf_segment_id || n_leaves == 0 || !handles || (n_mixtures && (!mix_offset || !mix_k || !mix_tlog || !mix_first_pos || !leaf || !count))) {
+        set_error("mgb_build_from_levels: NULL argument or no leaves");
+        return MGB_ERR_INVALID_ARG;
+    }
+    for (uint32_t k = 1; k < n_leaves; k++)
+        if (leaf_segment_id[k] <= leaf_segment_id[k - 1]) {
+            set_error("mgb_build_from_levels: leaf_segment_id must be strictly increasing");
+            return MGB_ERR_INVALID_ARG;
+        }
+    LevelsFront lf{leaf_segment_id, n_leaves, level_done, handles, n_mixtures, mix_offset, mix_k, mix_tlog, mix_first_pos, leaf, count,
+                   n_entries, nnz_levels};
+    return build_volume(nullptr, X, Y, Z, nullptr, params, out, &lf);
+}
+
+extern "C" int mgb_get_front_mixture_nodes(const mgb_result* r, uint32_t* node_of_mixture)
+{
+    if (!r || (!node_of_mixture && !r->front_mixture_node.empty())) { set_error("mgb_get_front_mixture_nodes: NULL argument"); return MGB_ERR_INVALID_ARG; }
+    if (!r->front_mixture_node.empty()) memcpy(node_of_mixture, r->front_mixture_node.data(), r->front_mixture_node.size() * sizeof(uint32_t));
+    return MGB_OK;
 }
 
 extern "C" int mgb_build_from_mixtures(uint32_t n_leaves, uint64_t n_mixtures, const uint64_t* offsets,
@@ -388,14 +422,14 @@ extern "C" int mgb_get_graph(const mgb_result* r, uint32_t* child_a, uint32_t* c
 extern "C" const uint32_t* mgb_node_idx_ptr(const mgb_result* r, uint32_t level)
 {
     if (!r || level >= r->node_idx.size()) { set_error("mgb_node_idx_ptr: bad level"); return nullptr; }
-    if (r->node_idx[level].empty()) { set_error("mgb_node_idx_ptr: level %u is not stored (mgb_build_from_level1: level 0 = leaf numbers)", level); return nullptr; }
+    if (r->node_idx[level].empty()) { set_error("mgb_node_idx_ptr: level %u is not stored (it was classified by the caller's front end)", level); return nullptr; }
     return r->node_idx[level].data();
 }
 
 extern "C" int mgb_get_node_idx(const mgb_result* r, uint32_t level, uint32_t* out)
 {
     if (!r || !out || level >= r->node_idx.size()) { set_error("mgb_get_node_idx: bad argument"); return MGB_ERR_INVALID_ARG; }
-    if (r->node_idx[level].empty()) { set_error("mgb_get_node_idx: level %u is not stored (mgb_build_from_level1: level 0 = leaf numbers)", level); return MGB_ERR_INVALID_ARG; }
+    if (r->node_idx[level].empty()) { set_error("mgb_get_node_idx: level %u is not stored (it was classified by the caller's front end)", level); return MGB_ERR_INVALID_ARG; }
     memcpy(out, r->node_idx[level].data(), r->node_idx[level].size() * sizeof(uint32_t));
     return MGB_OK;
 }

@@ -51,6 +51,7 @@ struct Mipmap {
     std::vector<uint32_t> leaf_segment_id;         // sorted distinct IDs present (Q14)
     uint64_t nnz_total = 0;
     MixtureSet mixtures;
+    std::vector<uint32_t> front_mixture;           // LevelsFront only: canonical number of every listed mixture
 };
 
 // Levels 0 and 1 classified outside the host builder (mgb_build_from_level1): level 0 is not passed at all.
@@ -63,9 +64,28 @@ struct Level1Front {
     uint64_t n_mixed;
 };
 
-// With `front`, seg is not read and out.level_ids[0] stays empty.
+// Levels 1 .. level_done built outside the host builder (mg_mipmap_levels_build of include/mg.h): the distinct mixtures
+// found so far with their first occurrence, and the handles of the last finished level.
+struct LevelsFront {
+    const uint32_t* leaf_segment_id;   // [n_leaves] sorted distinct segment IDs
+    uint32_t n_leaves;
+    uint32_t level_done;               // >= 1
+    const uint32_t* handles;           // [voxels of level_done] leaf number, or 0x80000000 | number of a listed mixture
+    uint64_t n_mix;
+    const uint64_t* mix_offset;        // [n_mix] first entry
+    const uint32_t* mix_k;             // [n_mix] non-zeros (>= 2)
+    const uint32_t* mix_tlog;          // [n_mix] the counts sum to 2^tlog
+    const uint64_t* mix_first_pos;     // [n_mix] level << 40 | voxel of the first occurrence
+    const uint32_t* leaf;              // entries: leaves ascending inside a mixture
+    const uint64_t* count;
+    uint64_t n_entries;
+    uint64_t nnz_levels;               // non-zeros summed over every voxel of the levels 1 .. level_done
+};
+
+// With `front`, seg is not read and out.level_ids[0] stays empty.  With `levels`, neither are the levels
+// 1 .. level_done - 1, and out.front_mixture[q] = canonical number of the q-th listed mixture.
 int build_mipmap(const uint32_t* seg, uint64_t X, uint64_t Y, uint64_t Z, int n_threads, Mipmap& out,
-                 const Level1Front* front = nullptr);
+                 const Level1Front* front = nullptr, const LevelsFront* levels = nullptr);
 
 }  // namespace mgb
 
@@ -81,4 +101,5 @@ struct mgb_result {
     std::vector<std::vector<uint32_t>> node_idx;   // per mip level, final numbering
     std::vector<float> codeword, sigma;
     std::vector<uint64_t> bin_count;
+    std::vector<uint32_t> front_mixture_node;      // mgb_build_from_levels: node of every mixture the caller listed
 };

@@ -257,7 +257,8 @@ int index_leaves(const uint32_t* seg, uint64_t n, std::vector<uint32_t>& ids, st
 
 }  // namespace
 
-int build_mipmap(const uint32_t* seg, uint64_t X, uint64_t Y, uint64_t Z, int n_threads, Mipmap& out, const Level1Front* front)
+int build_mipmap(const uint32_t* seg, uint64_t X, uint64_t Y, uint64_t Z, int n_threads, Mipmap& out, const Level1Front* front,
+                 const LevelsFront* levels)
 {
     if (n_threads > 0) omp_set_num_threads(n_threads);
     // ---- O-1 / L80: dims, ceil-halved down to 1^3
@@ -269,7 +270,8 @@ int build_mipmap(const uint32_t* seg, uint64_t X, uint64_t Y, uint64_t Z, int n_
     }
     const uint32_t n_levels = (uint32_t)(out.dims.size() / 3);
     out.level_ids.assign(n_levels, {});
-    if (!front) index_leaves(seg, X * Y * Z, out.leaf_segment_id, out.level_ids[0]);   // level 0: H = e_S (Eq. 4, first line)
+    if (levels) out.leaf_segment_id.assign(levels->leaf_segment_id, levels->leaf_segment_id + levels->n_leaves);
+    else if (!front) index_leaves(seg, X * Y * Z, out.leaf_segment_id, out.level_ids[0]);   // level 0: H = e_S (Eq. 4, first line)
     else out.leaf_segment_id.assign(front->leaf_segment_id, front->leaf_segment_id + front->n_leaves);
     const uint32_t n_leaves = (uint32_t)out.leaf_segment_id.size();
     uint64_t nnz_total = X * Y * Z;
@@ -324,6 +326,56 @@ int build_mipmap(const uint32_t* seg, uint64_t X, uint64_t Y, uint64_t Z, int n_
         }
         nnz_total += nnz_level;
         first_level = 2;
+    }
+    std::vector<uint32_t> front_handle;                // LevelsFront: table handle of every listed mixture
+    if (levels) {
+        // Levels 1 .. level_done were built elsewhere (the device): take over the distinct mixtures found there, each
+        // with its first occurrence, and the handles of the last finished level; continue above it.
+        const uint32_t Ld = levels->level_done;
+        if (Ld == 0 || Ld >= n_levels) { set_error("histogram mipmap: level_done = %u is not a level 1 .. %u", Ld, n_levels - 1); return MGB_ERR_INVALID_ARG; }
+        front_handle.assign(levels->n_mix, 0);
+        bool bad = false;
+#pragma omp parallel
+        {
+            std::vector<Entry> e;
+#pragma omp for schedule(dynamic, 1024)
+            for (int64_t q = 0; q < (int64_t)levels->n_mix; q++) {
+                const uint64_t o = levels->mix_offset[q];
+                const uint32_t k = levels->mix_k[q];
+                bool ok = k >= 2 && o + k <= levels->n_entries && (levels->mix_first_pos[q] >> 40) >= 1 && (levels->mix_first_pos[q] >> 40) <= Ld;
+                uint64_t total = 0;
+                e.resize(k);
+                for (uint32_t t = 0; ok && t < k; t++) {
+                    e[t] = Entry{levels->leaf[o + t], 0, levels->count[o + t]};
+                    ok = e[t].leaf < n_leaves && e[t].count > 0 && (t == 0 || e[t].leaf > e[t - 1].leaf);
+                    total += e[t].count;
+                }
+                ok = ok && total == (1ull << levels->mix_tlog[q]);
+                if (!ok) { bad = true; continue; }
+                front_handle[q] = table.intern(e.data(), k, levels->mix_tlog[q], levels->mix_first_pos[q]);
+            }
+        }
+        if (bad) { set_error("histogram mipmap: a listed mixture is malformed (entries, total or first occurrence)"); return MGB_ERR_INVALID_ARG; }
+        if (table.failed) { set_error("histogram mipmap: mixture table full or out of memory while taking over the listed mixtures"); return MGB_ERR_LIMIT; }
+        const uint64_t nd = out.dims[3 * Ld] * out.dims[3 * Ld + 1] * out.dims[3 * Ld + 2];
+        out.level_ids[Ld].resize(nd);
+        uint32_t* P = out.level_ids[Ld].data();
+        bool bad_handle = false;
+#pragma omp parallel for schedule(static)
+        for (int64_t v = 0; v < (int64_t)nd; v++) {
+            const uint32_t h = levels->handles[v];
+            if (h & kMixed) {
+                const uint32_t q = h & ~kMixed;
+                if (q >= levels->n_mix) { bad_handle = true; continue; }
+                P[v] = front_handle[q];
+            } else {
+                if (h >= n_leaves) { bad_handle = true; continue; }
+                P[v] = h;
+            }
+        }
+        if (bad_handle) { set_error("histogram mipmap: a handle of level %u names no leaf and no listed mixture", Ld); return MGB_ERR_INVALID_ARG; }
+        nnz_total += levels->nnz_levels;
+        first_level = Ld + 1;
     }
     for (uint32_t l = first_level; l < n_levels; l++) {
         const uint64_t cx = out.dims[3 * l - 3], cy = out.dims[3 * l - 2], cz = out.dims[3 * l - 1];
@@ -394,6 +446,13 @@ int build_mipmap(const uint32_t* seg, uint64_t X, uint64_t Y, uint64_t Z, int n_
         for (uint32_t t = 0; t < rc.k; t++) {
             ms.leaf[ms.off[q] + t] = rc.data[t].leaf;
             ms.count[ms.off[q] + t] = rc.data[t].count;
+        }
+    }
+    if (levels) {
+        out.front_mixture.resize(levels->n_mix);
+        for (uint64_t q = 0; q < levels->n_mix; q++) {
+            const uint32_t h = front_handle[q];
+            out.front_mixture[q] = canon[(h >> kLocalBits) & (kShards - 1)][h & ((1u << kLocalBits) - 1)];
         }
     }
     for (uint32_t l = 1; l < n_levels; l++) {

@@ -31,7 +31,8 @@ SYMBOLS = ["mg_load_graph", "mg_free_graph", "mg_graph_info", "mg_level_offsets"
            "mg_bits_per_voxel", "mg_packed_stream_bytes", "mg_index_range", "mg_pack_indices", "mg_colorize_packed",
            "mg_propagate_attr", "mg_render", "mg_render_ex", "mg_ess_mask_build",
            "mg_mixture_lut_build", "mg_mixture_lut_free", "mg_mixture_lut_info", "mg_mixture_lut_export", "mg_range_query",
-           "mg_mipmap_leaf_index", "mg_mipmap_front_level1"]
+           "mg_mipmap_leaf_index", "mg_mipmap_front_level1", "mg_mipmap_levels_build", "mg_mixture_table_free",
+           "mg_mixture_table_info", "mg_mixture_table_export", "mg_mipmap_remap_handles"]
 
 
 class MgInfo(C.Structure):
@@ -146,6 +147,23 @@ lib.mg_mipmap_front_level1.argtypes = [_vp, C.c_uint64, C.c_uint64, C.c_uint64, 
 lib.mg_mipmap_front_level1.restype = C.c_int
 
 
+class MgMixtureTableInfo(C.Structure):
+    _fields_ = [("n_mixtures", C.c_uint64), ("n_entries", C.c_uint64), ("nnz_levels", C.c_uint64), ("device_bytes", C.c_uint64),
+                ("levels_done", C.c_uint32), ("n_leaves", C.c_uint32)]
+
+
+lib.mg_mipmap_levels_build.argtypes = [_vp, C.c_uint64, C.c_uint64, C.c_uint64, C.c_uint32, _vp, _vp, C.c_uint32, C.POINTER(_vp), _vp]
+lib.mg_mipmap_levels_build.restype = C.c_int
+lib.mg_mixture_table_free.argtypes = [_vp]
+lib.mg_mixture_table_free.restype = None
+lib.mg_mixture_table_info.argtypes = [_vp, C.POINTER(MgMixtureTableInfo)]
+lib.mg_mixture_table_info.restype = C.c_int
+lib.mg_mixture_table_export.argtypes = [_vp, _vp, _vp, _vp, _vp, _vp, _vp]
+lib.mg_mixture_table_export.restype = C.c_int
+lib.mg_mipmap_remap_handles.argtypes = [_vp, C.c_uint64, _vp, C.c_uint32, _vp]
+lib.mg_mipmap_remap_handles.restype = C.c_int
+
+
 class MgError(RuntimeError):
     def __init__(self, code: int, where: str):
         self.code = code
@@ -224,6 +242,46 @@ def mipmap_front_level1(level0_device, dims_xyz, level1_device, mixed_voxel_devi
                                       _ptr(mixed_children_device), int(capacity), C.byref(n), stream or None),
            "mg_mipmap_front_level1")
     return int(n.value)
+
+
+class MixtureTable:
+    """Device mixture store of mg_mipmap_levels_build (the levels >= 1 of the histogram mipmap built on the device)."""
+
+    def __init__(self, level0_device, dims_xyz, n_leaves: int, levels_device, level_offsets, stream: int = 0):
+        X, Y, Z = (int(d) for d in dims_xyz)
+        off = np.ascontiguousarray(level_offsets, dtype=np.uint64)
+        h = _vp()
+        self._h = None
+        _check(lib.mg_mipmap_levels_build(_ptr(level0_device), X, Y, Z, int(n_leaves), _ptr(levels_device), off.ctypes.data,
+                                          int(off.size), C.byref(h), stream or None), "mg_mipmap_levels_build")
+        self._h = h
+        self.info = MgMixtureTableInfo()
+        _check(lib.mg_mixture_table_info(self._h, C.byref(self.info)), "mg_mixture_table_info")
+
+    def export(self) -> dict:
+        """Host copy: offset u64, k u32, tlog u32, first_pos u64 per mixture; leaf u32, count u64 per entry."""
+        n, e = int(self.info.n_mixtures), int(self.info.n_entries)
+        out = dict(offset=np.zeros(n, np.uint64), k=np.zeros(n, np.uint32), tlog=np.zeros(n, np.uint32),
+                   first_pos=np.zeros(n, np.uint64), leaf=np.zeros(e, np.uint32), count=np.zeros(e, np.uint64))
+        _check(lib.mg_mixture_table_export(self._h, *(out[k].ctypes.data for k in ("offset", "k", "tlog", "first_pos", "leaf", "count"))),
+               "mg_mixture_table_export")
+        return out
+
+    def close(self) -> None:
+        if getattr(self, "_h", None):
+            lib.mg_mixture_table_free(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+def mipmap_remap_handles(handles_device, n: int, node_of_mixture_device, n_mixtures: int, stream: int = 0) -> None:
+    _check(lib.mg_mipmap_remap_handles(_ptr(handles_device), int(n), _ptr(node_of_mixture_device), int(n_mixtures), stream or None),
+           "mg_mipmap_remap_handles")
 
 
 def mipmap_desc(level_offsets, level_dims_xyz) -> MgMipmapDesc:

@@ -159,6 +159,74 @@ def from_volume(seg: np.ndarray, name: str = "volume", cfg: dict | None = None, 
     return w
 
 
+def from_volume_device_levels(seg_dev, name: str = "volume", cfg: dict | None = None, **builder_params) -> Workload:
+    """``from_volume_device`` with the levels >= 1 of the histogram mipmap built on the device too
+    (mg_mipmap_levels_build: merge + hash-cons per level, as far up as the mixtures stay small), the host builder
+    continuing above the last finished level (mgb_build_from_levels) and the device-built levels turned into node
+    indices in place (mg_mipmap_remap_handles).  Same graph and node indices as ``from_volume``; ``host_idx[l]`` is None
+    for the levels below the last device-built one."""
+    import torch
+    w = Workload(name)
+    w.cfg = dict(cfg or {})
+    Z, Y, X = (int(d) for d in seg_dev.shape)
+    dims, d = [], (X, Y, Z)
+    while True:
+        dims.append(d)
+        if d == (1, 1, 1):
+            break
+        d = tuple(-(-k // 2) for k in d)
+    w.mip_dims = dims
+    w.level_voxels = [a * b * c for a, b, c in dims]
+    w.level_start, w.n_voxels_padded = _layout(w.level_voxels)
+    w.n_voxels = sum(w.level_voxels)
+    st = torch.cuda.current_stream().cuda_stream
+    t0 = time.perf_counter()
+    w.d_idx = torch.zeros(w.n_voxels_padded, dtype=torch.int32, device="cuda")
+    n0 = w.level_voxels[0]
+    ids = mg.mipmap_leaf_index(seg_dev, n0, w.d_idx[:n0], stream=st)
+    table = mg.MixtureTable(w.d_idx, dims[0], ids.size, w.d_idx, w.level_start, stream=st) if len(dims) > 1 else None
+    Ld = int(table.info.levels_done) if table is not None else 0
+    if Ld == 0:                                    # nothing for the device to do (1 x 1 x 1, or huge mixtures at level 1)
+        if table is not None:
+            table.close()
+        w.d_idx = None
+        return from_volume_device(seg_dev, name=name, cfg=cfg, **builder_params)
+    mix = table.export()
+    s_d, n_d = w.level_start[Ld], w.level_voxels[Ld]
+    handles = w.d_idx[s_d:s_d + n_d].cpu().numpy().view(np.uint32)
+    nnz_levels, n_dev_mix = int(table.info.nnz_levels), int(table.info.n_mixtures)
+    table.close()
+    t1 = time.perf_counter()
+    r, nodes = builder.build_from_levels(dims[0], ids, Ld, handles, mix, nnz_levels, **builder_params)
+    t2 = time.perf_counter()
+    g = r.graph()
+    w.host_graph = g
+    w.n_leaves = g["n_leaves"]
+    assert r.mip_dims == dims
+    w.graph = mg.Graph(g["child_a"], g["child_b"], g["weight"], g["n_leaves"], level_offsets=g["level_offsets"],
+                       leaf_segment_id=g["leaf_segment_id"])
+    t3 = time.perf_counter()
+    d_nodes = torch.from_numpy(nodes.view(np.int32)).cuda() if nodes.size else torch.zeros(1, dtype=torch.int32, device="cuda")
+    s1 = w.level_start[1]
+    mg.mipmap_remap_handles(w.d_idx[s1:], s_d + n_d - s1, d_nodes, nodes.size, st)       # levels 1 .. Ld are contiguous but for padding zeros
+    w.host_idx = [None] * Ld + [r.node_idx(l, copy=False) for l in range(Ld, r.info.n_mip_levels)]
+    for l in range(Ld + 1, len(dims)):
+        a = w.host_idx[l]
+        w.d_idx[w.level_start[l]:w.level_start[l] + a.size].copy_(torch.from_numpy(a.reshape(-1).view(np.int32)))
+    torch.cuda.synchronize()
+    t4 = time.perf_counter()
+    i = r.info
+    w.stats = dict(front_end_s=t1 - t0, builder_s=t2 - t1, load_graph_s=t3 - t2, upload_idx_s=t4 - t3, n_nodes=int(i.n_nodes),
+                   n_leaves=int(i.n_leaves), depth=int(i.depth), quant_bits=int(i.quant_bits),
+                   n_distinct_mixtures=int(i.n_distinct_mixtures), nnz_per_voxel=i.nnz_total / max(1, i.n_voxels_total),
+                   n_mip_levels=int(i.n_mip_levels), builder_mipmap_s=i.seconds_mipmap,
+                   builder_factorise_s=i.seconds_factorise, builder_finalise_s=i.seconds_finalise,
+                   device_mipmap=True, device_levels_done=Ld, n_device_mixtures=n_dev_mix,
+                   level_sizes=np.diff(g["level_offsets"].astype(np.int64)).tolist())
+    w.build_result = r
+    return w
+
+
 def from_volume_device(seg_dev, name: str = "volume", cfg: dict | None = None, **builder_params) -> Workload:
     """The same assembly as ``from_volume`` for a segment-ID volume that is ALREADY ON THE DEVICE (torch int32
     [Z, Y, X], uint32 values): the two finest mip levels are classified by the device front end
@@ -262,7 +330,7 @@ def from_dag(child_a, child_b, weight, level_offsets, n_leaves: int, node_idx: n
 
 
 def make(cfg_id: int, scale: float = 1.0, device_synth: bool = True, keep_seg: bool = False,
-         relabel: bool = False, load: bool = True, device_mipmap: bool = False, **builder_params) -> Workload:
+         relabel: bool = False, load: bool = True, device_mipmap: bool | str = False, **builder_params) -> Workload:
     """BASELINE.json config ``cfg_id`` (1-5); ``scale`` < 1 gives a geometrically similar smaller
     instance (tests).  Volumes are generated on the GPU (bit-identical to synth.py) unless
     ``device_synth`` is False.  ``keep_seg`` keeps the generated volume in ``Workload.seg``."""
@@ -289,7 +357,8 @@ def make(cfg_id: int, scale: float = 1.0, device_synth: bool = True, keep_seg: b
         seg_dev = synth_gpu.make_volume(c)
         torch.cuda.synchronize()
         t1 = time.perf_counter()
-        w = from_volume_device(seg_dev, name=c["name"], cfg=c, **builder_params)
+        assemble = from_volume_device_levels if device_mipmap == "levels" else from_volume_device
+        w = assemble(seg_dev, name=c["name"], cfg=c, **builder_params)
         if keep_seg:
             w.seg = seg_dev.cpu().numpy().view(np.uint32)
         del seg_dev

@@ -251,3 +251,91 @@ def test_build_from_level1_rejects_inconsistent_input():
         builder.build_from_level1(dims, ids[::-1], level1, mixed, children)
     with pytest.raises(ValueError):
         builder.build_from_level1(dims, ids, level1[:-1], mixed, children)
+
+
+def _levels_front_numpy(seg, level_done):
+    """Plain numpy / oracle statement of what mg_mipmap_levels_build hands to the host: the distinct reduced mixtures of
+    the levels 1 .. level_done (the oracle's exact integer histograms divided by their common power of two) in a
+    scrambled order, each with its first occurrence level << 40 | voxel, the handles of every level and the non-zeros."""
+    ids, l0 = oracle.leaf_index(seg)
+    H = oracle.histogram_mipmap(l0, ids.size)
+    table, first, handles, nnz = {}, [], [], 0
+    for l in range(1, level_done + 1):
+        flat = H[l].reshape(-1, ids.size)
+        hl = np.zeros(flat.shape[0], dtype=np.uint32)
+        for v, row in enumerate(flat):
+            leaves = np.flatnonzero(row)
+            nnz += leaves.size
+            if leaves.size == 1:
+                hl[v] = leaves[0]
+                continue
+            counts = row[leaves].astype(np.uint64)
+            tz = min(int(c & -c).bit_length() - 1 for c in counts.tolist())
+            key = (tuple(leaves.tolist()), tuple((counts >> np.uint64(tz)).tolist()), 3 * l - tz)
+            if key not in table:
+                table[key] = len(first)
+                first.append((l << 40) | v)
+            hl[v] = 0x80000000 | table[key]
+        handles.append(hl)
+    keys = list(table)
+    order = np.argsort(synth.u64(63, 2, np.arange(len(keys), dtype=np.uint64)))      # creation order on the device is arbitrary
+    new_of_old = np.empty(len(keys), dtype=np.int64)
+    new_of_old[order] = np.arange(len(keys))
+    mix = dict(offset=[], k=[], tlog=[], first_pos=[], leaf=[], count=[])
+    for q in order:
+        leaves, counts, tlog = keys[q]
+        mix["offset"].append(len(mix["leaf"])); mix["k"].append(len(leaves)); mix["tlog"].append(tlog); mix["first_pos"].append(first[q])
+        mix["leaf"] += leaves; mix["count"] += counts
+    dt = dict(offset=np.uint64, k=np.uint32, tlog=np.uint32, first_pos=np.uint64, leaf=np.uint32, count=np.uint64)
+    mix = {k: np.array(v, dtype=dt[k]) for k, v in mix.items()}
+    for hl in handles:
+        m = hl >= 0x80000000
+        hl[m] = (0x80000000 | new_of_old[hl[m] & 0x7FFFFFFF]).astype(np.uint32)
+    return ids, l0, handles, mix, nnz
+
+
+@pytest.mark.parametrize("dims,n_seg,bits", [((16, 16, 16), 7, 9), ((13, 11, 9), 6, 9), ((5, 1, 9), 4, 0)])
+def test_build_from_levels_is_identical_to_build(dims, n_seg, bits):
+    """mgb_build_from_levels continues Eq. 4 above ANY finished level and reproduces mgb_build: same graph, same node of
+    every listed mixture, same node indices from the finished level on."""
+    seg = synth.voronoi_volume(dims, synth.voronoi_seeds(dims, n_seg, 64))
+    a = builder.build(seg, quant_bits=bits)
+    ga = a.graph()
+    n_lv = a.info.n_mip_levels
+    for level_done in sorted({1, 2, n_lv - 1}):
+        ids, l0, handles, mix, nnz = _levels_front_numpy(seg, level_done)
+        b, nodes = builder.build_from_levels(dims, ids, level_done, handles[-1], mix, nnz, quant_bits=bits)
+        gb = b.graph()
+        for k in ("child_a", "child_b", "weight", "weight_exact", "weight_sigma", "level_offsets", "leaf_segment_id"):
+            assert np.array_equal(ga[k], gb[k]), (level_done, k)
+        for f in ("n_nodes", "n_leaves", "depth", "n_mip_levels", "n_voxels_total", "n_distinct_mixtures", "nnz_total"):
+            assert getattr(a.info, f) == getattr(b.info, f), (level_done, f)
+        for l in range(1, n_lv):
+            want = a.node_idx(l).reshape(-1)
+            if l < level_done:                                     # not stored: they follow from the caller's handles
+                with pytest.raises(builder.BuilderError):
+                    b.node_idx(l)
+            else:
+                assert np.array_equal(b.node_idx(l).reshape(-1), want), (level_done, l)
+            if l <= level_done:
+                h = handles[l - 1]
+                got = np.where(h >= 0x80000000, nodes[h & 0x7FFFFFFF] if nodes.size else 0, h)
+                assert np.array_equal(got, want), (level_done, l)
+        b.close()
+    a.close()
+
+
+def test_build_from_levels_rejects_malformed_input():
+    dims = (8, 8, 8)
+    seg = synth.voronoi_volume(dims, synth.voronoi_seeds(dims, 5, 65))
+    ids, l0, handles, mix, nnz = _levels_front_numpy(seg, 1)
+    assert mix["k"].size > 2
+    bad = dict(mix, count=mix["count"] * np.uint64(2))                             # totals are no longer 2^tlog
+    with pytest.raises(builder.BuilderError):
+        builder.build_from_levels(dims, ids, 1, handles[0], bad, nnz)
+    h = handles[0].copy()
+    h[np.flatnonzero(h >= 0x80000000)[0]] = 0x80000000 | mix["k"].size              # names no listed mixture
+    with pytest.raises(builder.BuilderError):
+        builder.build_from_levels(dims, ids, 1, h, mix, nnz)
+    with pytest.raises(builder.BuilderError):                                      # level_done beyond the chain
+        builder.build_from_levels(dims, ids, 9, handles[0], mix, nnz)

@@ -508,3 +508,30 @@ def test_config3_device_mipmap_front_end_full_size(libs):
               f"({b.stats['n_level1_mixed']} non-pure level-1 parents)")
     finally:
         b.close()
+
+
+@pytest.mark.parametrize("cfg_id", [3, 4])
+def test_device_levels_full_size(libs, cfg_id):
+    """NEXT-4 (second half) at full size: the levels >= 1 of the histogram mipmap merged and hash-consed on the device
+    (bench.py --device-levels) yield the graph and the node-index mipmap of the level-1 front-end path bit for bit."""
+    mg, workload = libs
+    a = workload.make(cfg_id, device_mipmap=True)
+    try:
+        ga = {k: a.host_graph[k].copy() for k in ("child_a", "child_b", "weight", "weight_sigma", "level_offsets", "leaf_segment_id")}
+        ref = a.d_idx.clone()
+        stats_a = dict(a.stats)
+    finally:
+        a.close()
+    b = workload.make(cfg_id, device_mipmap="levels")
+    try:
+        for k, v in ga.items():
+            assert np.array_equal(v, b.host_graph[k]), k
+        assert torch.equal(ref, b.d_idx)
+        assert b.stats["n_distinct_mixtures"] == stats_a["n_distinct_mixtures"] and b.stats["nnz_per_voxel"] == stats_a["nnz_per_voxel"]
+        print(f"cfg{cfg_id} setup, level-1 front end: front {stats_a['front_end_s']:.2f} + builder {stats_a['builder_s']:.2f} "
+              f"(mipmap {stats_a['builder_mipmap_s']:.2f}) + upload {stats_a['upload_idx_s']:.2f} s; device levels 1 .. "
+              f"{b.stats['device_levels_done']}: front {b.stats['front_end_s']:.2f} + builder {b.stats['builder_s']:.2f} "
+              f"(mipmap {b.stats['builder_mipmap_s']:.2f}) + upload {b.stats['upload_idx_s']:.2f} s; "
+              f"{b.stats['n_device_mixtures']} of {b.stats['n_distinct_mixtures']} distinct mixtures found on the device")
+    finally:
+        b.close()

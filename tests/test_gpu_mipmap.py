@@ -145,3 +145,92 @@ def test_device_assisted_assembly_equals_the_host_builder(libs, cfg_id, scale):
     finally:
         a.close()
         b.close()
+
+
+def _same_assembly(a, b):
+    for k in ("child_a", "child_b", "weight", "weight_sigma", "level_offsets", "leaf_segment_id"):
+        assert np.array_equal(a.host_graph[k], b.host_graph[k]), k
+    assert a.mip_dims == b.mip_dims and a.level_start == b.level_start and a.n_voxels == b.n_voxels
+    assert torch.equal(a.d_idx, b.d_idx)                              # the node index of every voxel of every level
+    for k in ("n_nodes", "depth", "n_distinct_mixtures"):
+        assert a.stats[k] == b.stats[k], k
+    assert abs(a.stats["nnz_per_voxel"] - b.stats["nnz_per_voxel"]) < 1e-15
+
+
+@pytest.mark.parametrize("cfg_id,scale", [(3, 0.08), (2, 0.06), (4, 0.12), (1, 1.0)])
+def test_device_levels_assembly_equals_the_host_builder(libs, cfg_id, scale):
+    """workload.make(device_mipmap="levels"): the levels >= 1 merged and hash-consed on the device
+    (mg_mipmap_levels_build), the host continuing above (mgb_build_from_levels): same graph, same device mipmap."""
+    mg, workload = libs
+    a = workload.make(cfg_id, scale)
+    b = workload.make(cfg_id, scale, device_mipmap="levels")
+    try:
+        _same_assembly(a, b)
+        assert b.stats["device_levels_done"] >= 1 and b.host_idx[0] is None
+        print(f"cfg{cfg_id} x{scale}: device built levels 1 .. {b.stats['device_levels_done']} of {len(b.mip_dims) - 1}, "
+              f"{b.stats['n_device_mixtures']} of {b.stats['n_distinct_mixtures']} distinct mixtures")
+    finally:
+        a.close()
+        b.close()
+
+
+@pytest.mark.parametrize("dims,n_seg", [((24, 24, 24), 400), ((37, 29, 23), 12), ((9, 1, 5), 4), ((2, 2, 2), 3), ((64, 48, 3), 900)])
+def test_device_levels_ragged_and_crowded_volumes(libs, dims, n_seg):
+    """Ragged ceil-halving chains (N = 1, 2, 4 children at the borders, Q2) and label noise with hundreds of segments, where
+    the mixtures outgrow the 256 entries a warp merges and the device hands the upper levels to the host early."""
+    mg, workload = libs
+    X, Y, Z = dims
+    seg = (synth.u64(71, 3, np.arange(X * Y * Z, dtype=np.uint64)) % np.uint64(n_seg)).astype(np.uint32).reshape(Z, Y, X) * 3 + 5
+    a = workload.from_volume(seg, name="noise")
+    b = workload.from_volume_device_levels(_dev(seg).view(Z, Y, X), name="noise")
+    try:
+        _same_assembly(a, b)
+        if n_seg >= 400:
+            assert 1 <= b.stats["device_levels_done"] < len(b.mip_dims) - 1     # abandoned before the top
+    finally:
+        a.close()
+        b.close()
+
+
+def test_mixture_table_matches_the_oracle_histograms(libs):
+    """mg_mipmap_levels_build against the definition, not against the host builder: every handle of every finished level
+    expands to the oracle's exact integer histogram of that voxel (Eq. 4, O-2) divided by its common power of two; equal
+    mixtures share one number; first occurrences are the scanline minimum."""
+    mg, workload = libs
+    dims = (21, 18, 14)
+    X, Y, Z = dims
+    seg = synth.voronoi_volume(dims, synth.voronoi_seeds(dims, 9, 72))
+    ids, l0 = oracle.leaf_index(seg)
+    H = oracle.histogram_mipmap(l0, ids.size)
+    sizes = [h.shape[0] * h.shape[1] * h.shape[2] for h in H]
+    start = np.concatenate([[0], np.cumsum(sizes)[:-1]]).astype(np.uint64)
+    buf = torch.zeros(int(sum(sizes)), dtype=torch.int32, device="cuda")
+    buf[:sizes[0]] = _dev(l0.reshape(-1))
+    t = mg.MixtureTable(buf, dims, ids.size, buf, start)
+    assert t.info.levels_done == len(H) - 1 and t.info.n_leaves == ids.size
+    m = t.export()
+    hb = buf.cpu().numpy().view(np.uint32)
+    seen, nnz = {}, 0
+    for l in range(1, len(H)):
+        flat = H[l].reshape(-1, ids.size)
+        for v in range(flat.shape[0]):
+            h = int(hb[int(start[l]) + v])
+            leaves = np.flatnonzero(flat[v])
+            nnz += leaves.size
+            if leaves.size == 1:
+                assert h == leaves[0]
+                continue
+            assert h & 0x80000000
+            q = h & 0x7FFFFFFF
+            o, k = int(m["offset"][q]), int(m["k"][q])
+            counts = flat[v][leaves]
+            tz = min(int(c & -c).bit_length() - 1 for c in counts.tolist())
+            assert np.array_equal(m["leaf"][o:o + k], leaves) and np.array_equal(m["count"][o:o + k], counts >> np.uint64(tz))
+            assert int(m["tlog"][q]) == 3 * l - tz
+            seen.setdefault(q, (l << 40) | v)
+    assert len(seen) == t.info.n_mixtures and nnz == t.info.nnz_levels
+    for q, pos in seen.items():
+        assert int(m["first_pos"][q]) == pos
+    keys = {(tuple(m["leaf"][int(o):int(o) + int(k)]), tuple(m["count"][int(o):int(o) + int(k)])) for o, k in zip(m["offset"], m["k"])}
+    assert len(keys) == t.info.n_mixtures                            # hash-consed: no mixture twice
+    t.close()
