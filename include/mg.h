@@ -417,16 +417,18 @@ int mg_mixture_lut_info(const mg_mixture_lut *lut, mg_lut_info *info);
 int mg_mixture_lut_export(const mg_mixture_lut *lut, uint64_t *row_ptr, uint32_t *leaf, double *mu, double *dmu);
 
 /*
- * mg_range_query -- n_queries boxes in one launch sequence (zero, accumulate, finish).
+ * mg_range_query -- n_queries boxes in two launches: one zeroes the results, the other accumulates and -- in the last
+ * CTA of every query to finish -- takes the square roots of Eq. 17 (no memsets, no separate finishing kernel).
  *   node_idx_mipmap  DEVICE uint32, all levels as `mip` describes (MG_QUERY_NAIVE reads level 0 only).
  *   boxes            HOST uint64[n_queries][6] = x0, y0, z0, x1, y1, z1, half-open, non-empty, inside
- *                    level 0 (validated); copied into a table-owned staging buffer at enqueue (the
- *                    buffer grows, i.e. allocates, when n_queries exceeds every earlier call's).
+ *                    level 0 (validated).  Up to 64 boxes travel in the kernel parameters; larger batches are
+ *                    copied into a table-owned staging buffer at enqueue (it grows, i.e. allocates, when
+ *                    n_queries exceeds every earlier call's).
  *   expect, err      DEVICE double[n_queries][n_leaves]: expected voxels per leaf and its error
  *                    (err may be NULL).  sum_i expect[q][i] = volume of box q (L251).
  *   fetches          DEVICE uint64[n_queries] or NULL: samples fetched per query (Table 4).
  *   mode             MG_QUERY_FA, MG_QUERY_NAIVE or MG_QUERY_FA_WALK.
- * Enqueue-only apart from the staging copy.  Accumulation uses fp64 atomics: the result is the oracle's
+ * Enqueue-only apart from the staging copy of large batches.  Accumulation uses fp64 atomics: the result is the oracle's
  * up to summation order.
  */
 int mg_range_query(mg_mixture_lut *lut, const uint32_t *node_idx_mipmap, const mg_mipmap_desc *mip,

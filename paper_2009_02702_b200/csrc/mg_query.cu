@@ -33,7 +33,8 @@ struct mg_mixture_lut {
     uint32_t* d_col = nullptr;        // [capacity] leaf index, ascending inside a row
     double* d_mu = nullptr;           // [capacity]
     double* d_dmu = nullptr;          // [capacity]
-    uint64_t* d_boxes = nullptr;      // staging for mg_range_query
+    uint64_t* d_boxes = nullptr;      // staging for mg_range_query (batches of more than kInlineQueries boxes)
+    uint32_t* d_done = nullptr;       // [boxes_cap] per-query completion counters
     uint32_t boxes_cap = 0;
     uint64_t device_bytes = 0;
 };
@@ -44,6 +45,7 @@ constexpr int kBuildThreads = 128;
 constexpr int kQueryThreads = 256;
 constexpr int kNaiveUnroll = 4;
 constexpr int kMaxPieces = 2 * MG_MAX_MIP_LEVELS + 2;     // pieces of one axis: at most 2 per level
+constexpr int kInlineQueries = 64;                        // batches up to this size carry their boxes in the kernel parameters
 
 __global__ void k_lut_leaves(uint32_t n_leaves, const uint64_t* __restrict__ row_ptr, uint32_t* row_len, uint32_t* col,
                              double* mu, double* dmu)
@@ -55,6 +57,91 @@ __global__ void k_lut_leaves(uint32_t n_leaves, const uint64_t* __restrict__ row
     col[r] = n;
     mu[r] = 1.0;          // e_i ...
     dmu[r] = 0.0;         // ... "with variance 0" (L375)
+}
+
+// Row capacities on the device, one topological level at a time: cap(n) = min(n_leaves, cap(a) + cap(b)), leaves 1.
+__global__ void __launch_bounds__(256)
+k_lut_cap_level(const uint32_t* __restrict__ ga, const uint32_t* __restrict__ gb, uint32_t lo, uint32_t hi, uint32_t n_leaves, uint32_t* cap)
+{
+    const uint32_t n = lo + blockIdx.x * 256 + threadIdx.x;
+    if (n >= hi) return;
+    if (n < n_leaves) { cap[n] = 1; return; }
+    const uint64_t c = (uint64_t)cap[ga[n]] + cap[gb[n]];
+    cap[n] = (uint32_t)(c < n_leaves ? c : n_leaves);
+}
+
+// Exclusive prefix sum of n uint32 values into uint64 (row starts), two levels: tiles of kScanTile values per CTA.
+constexpr int kScanTile = 2048;     // 256 threads x 8 values
+
+__global__ void __launch_bounds__(256) k_scan_tile_sums(const uint32_t* __restrict__ v, uint64_t n, uint64_t* __restrict__ tile_sum)
+{
+    __shared__ unsigned long long warp_sum[8];
+    const uint64_t base = (uint64_t)blockIdx.x * kScanTile;
+    unsigned long long s = 0;
+    for (int k = 0; k < 8; k++) {
+        const uint64_t i = base + (uint64_t)k * 256 + threadIdx.x;
+        if (i < n) s += v[i];
+    }
+    for (int d = 16; d > 0; d >>= 1) s += __shfl_xor_sync(0xffffffffu, s, d);
+    if ((threadIdx.x & 31) == 0) warp_sum[threadIdx.x >> 5] = s;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        unsigned long long t = 0;
+        for (int w = 0; w < 8; w++) t += warp_sum[w];
+        tile_sum[blockIdx.x] = t;
+    }
+}
+
+// one CTA: exclusive scan of the tile sums in place; total to tile_sum[n_tiles]
+__global__ void __launch_bounds__(1024) k_scan_tiles(uint64_t* tile_sum, uint32_t n_tiles)
+{
+    __shared__ unsigned long long part[1024];
+    const uint32_t per = (n_tiles + 1023) / 1024;
+    const uint32_t t0 = min(threadIdx.x * per, n_tiles), t1 = min(t0 + per, n_tiles);
+    unsigned long long s = 0;
+    for (uint32_t t = t0; t < t1; t++) s += tile_sum[t];
+    part[threadIdx.x] = s;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        unsigned long long acc = 0;
+        for (int i = 0; i < 1024; i++) { const unsigned long long x = part[i]; part[i] = acc; acc += x; }
+        tile_sum[n_tiles] = acc;
+    }
+    __syncthreads();
+    unsigned long long acc = part[threadIdx.x];
+    for (uint32_t t = t0; t < t1; t++) { const unsigned long long x = tile_sum[t]; tile_sum[t] = acc; acc += x; }
+}
+
+__global__ void __launch_bounds__(256)
+k_scan_finish(const uint32_t* __restrict__ v, uint64_t n, const uint64_t* __restrict__ tile_sum, uint64_t* __restrict__ out)
+{
+    __shared__ unsigned long long warp_sum[8];
+    // thread t owns the 8 consecutive values base + 8 t .. base + 8 t + 7
+    const uint64_t i0 = (uint64_t)blockIdx.x * kScanTile + 8ull * threadIdx.x;
+    uint32_t x[8];
+    unsigned long long s = 0;
+    for (int k = 0; k < 8; k++) { x[k] = (i0 + k < n) ? v[i0 + k] : 0u; s += x[k]; }
+    unsigned long long incl = s;
+    const unsigned lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    for (int d = 1; d < 32; d <<= 1) { const unsigned long long up = __shfl_up_sync(0xffffffffu, incl, d); if (lane >= d) incl += up; }
+    if (lane == 31) warp_sum[w] = incl;
+    __syncthreads();
+    unsigned long long before = tile_sum[blockIdx.x];
+    for (unsigned q = 0; q < w; q++) before += warp_sum[q];
+    unsigned long long acc = before + incl - s;
+    for (int k = 0; k < 8; k++) { if (i0 + k < n) out[i0 + k] = acc; acc += x[k]; }
+    if (blockIdx.x == gridDim.x - 1 && threadIdx.x == 255) out[n] = tile_sum[gridDim.x];   // (tile_sum[n_tiles] = the total)
+}
+
+// nnz and the longest row of the finished table: stats[0] += sum, stats[1] = max
+__global__ void __launch_bounds__(256) k_lut_stats(const uint32_t* __restrict__ row_len, uint64_t n, unsigned long long* stats)
+{
+    unsigned long long s = 0;
+    unsigned m = 0;
+    for (uint64_t i = (uint64_t)blockIdx.x * 256 + threadIdx.x; i < n; i += (uint64_t)gridDim.x * 256) { const uint32_t l = row_len[i]; s += l; m = max(m, l); }
+    for (int d = 16; d > 0; d >>= 1) s += __shfl_xor_sync(0xffffffffu, s, d);
+    m = __reduce_max_sync(0xffffffffu, m);
+    if ((threadIdx.x & 31) == 0) { atomicAdd(stats, s); atomicMax(stats + 1, (unsigned long long)m); }
 }
 
 // One topological level [lo, hi): thread per node, a two-way merge of the children's sorted rows.
@@ -97,7 +184,7 @@ extern "C" void mg_mixture_lut_free(mg_mixture_lut* lut)
 {
     if (!lut) return;
     cudaFree(lut->d_row_ptr); cudaFree(lut->d_row_len); cudaFree(lut->d_col);
-    cudaFree(lut->d_mu); cudaFree(lut->d_dmu); cudaFree(lut->d_boxes);
+    cudaFree(lut->d_mu); cudaFree(lut->d_dmu); cudaFree(lut->d_boxes); cudaFree(lut->d_done);
     delete lut;
 }
 
@@ -112,51 +199,70 @@ extern "C" int mg_mixture_lut_build(mg_graph* g, const float* weight_sigma, mg_m
     cudaStream_t st = (cudaStream_t)stream;
     const uint64_t n = g->n_nodes;
     const uint32_t nl = g->n_leaves;
-    // row capacities on the host: cap(n) = min(n_leaves, cap(a) + cap(b))
-    std::vector<uint32_t> ha(n), hb(n);
-    if (n > nl) {
-        MG_CUDA(cudaMemcpyAsync(ha.data(), g->d_a, n * sizeof(uint32_t), cudaMemcpyDeviceToHost, st));
-        MG_CUDA(cudaMemcpyAsync(hb.data(), g->d_b, n * sizeof(uint32_t), cudaMemcpyDeviceToHost, st));
+    // Row capacities cap(n) = min(n_leaves, cap(a) + cap(b)) and the row starts (their exclusive prefix sum) on the
+    // device: one small kernel per topological level + a two-level scan.  (Round 1 did this pass on the host: 14 MB of
+    // graph down, 14 MB of row starts up, 7 MB of row lengths down -- 10 of the 10.7 ms of a build on cfg 3.)
+    uint32_t* d_cap = nullptr;
+    uint64_t* d_row_ptr = nullptr;
+    uint64_t* d_tiles = nullptr;
+    unsigned long long* d_stats = nullptr;
+    const uint32_t n_tiles = (uint32_t)((n + kScanTile - 1) / kScanTile);
+    auto fail0 = [&](int rc) { cudaFree(d_cap); cudaFree(d_row_ptr); cudaFree(d_tiles); cudaFree(d_stats); return rc; };
+#define LUT0_CUDA(call)                                                             \
+    do {                                                                            \
+        cudaError_t e__ = (call);                                                   \
+        if (e__ != cudaSuccess) return fail0(mg::cuda_fail(e__, #call));            \
+    } while (0)
+    LUT0_CUDA(cudaMalloc(&d_cap, n * sizeof(uint32_t)));
+    LUT0_CUDA(cudaMalloc(&d_row_ptr, (n + 1) * sizeof(uint64_t)));
+    LUT0_CUDA(cudaMalloc(&d_tiles, ((size_t)n_tiles + 1) * sizeof(uint64_t)));
+    LUT0_CUDA(cudaMalloc(&d_stats, 2 * sizeof(unsigned long long)));
+    LUT0_CUDA(cudaMemsetAsync(d_stats, 0, 2 * sizeof(unsigned long long), st));
+    for (uint32_t L = 0; L < g->n_levels; L++) {
+        const uint32_t lo = (uint32_t)g->level_off[L], hi = (uint32_t)g->level_off[L + 1];
+        if (hi == lo) continue;
+        k_lut_cap_level<<<(hi - lo + 255) / 256, 256, 0, st>>>(g->d_a, g->d_b, lo, hi, nl, d_cap);
+        mg::count_launch();
     }
-    MG_CUDA(cudaStreamSynchronize(st));
-    std::vector<uint32_t> cap(n);
-    std::vector<uint64_t> row_ptr(n + 1);
+    k_scan_tile_sums<<<n_tiles, 256, 0, st>>>(d_cap, n, d_tiles);
+    k_scan_tiles<<<1, 1024, 0, st>>>(d_tiles, n_tiles);
+    k_scan_finish<<<n_tiles, 256, 0, st>>>(d_cap, n, d_tiles, d_row_ptr);
+    mg::count_launch(3);
+    LUT0_CUDA(cudaGetLastError());
     uint64_t total = 0;
-    for (uint64_t i = 0; i < n; i++) {
-        const uint64_t c = i < nl ? 1 : std::min<uint64_t>(nl, (uint64_t)cap[ha[i]] + cap[hb[i]]);
-        cap[i] = (uint32_t)c;
-        row_ptr[i] = total;
-        total += c;
-    }
-    row_ptr[n] = total;
+    LUT0_CUDA(cudaMemcpyAsync(&total, d_row_ptr + n, sizeof(uint64_t), cudaMemcpyDeviceToHost, st));
+    LUT0_CUDA(cudaStreamSynchronize(st));
+    cudaFree(d_cap);
+    cudaFree(d_tiles);
+    d_cap = nullptr; d_tiles = nullptr;
     size_t free_b = 0, total_b = 0;
-    MG_CUDA(cudaMemGetInfo(&free_b, &total_b));
-    const uint64_t need = total * 20 + (n + 1) * 8 + n * 4 + (weight_sigma ? n * 4 : 0);
+    LUT0_CUDA(cudaMemGetInfo(&free_b, &total_b));
+    const uint64_t need = total * 20 + n * 4 + (weight_sigma ? n * 4 : 0);
     if (need > free_b) {
         mg::set_error("mg_mixture_lut_build: the table needs %llu entries (%.1f GB), %.1f GB are free",
                       (unsigned long long)total, need / 1e9, free_b / 1e9);
-        return MG_ERR_OOM;
+        return fail0(MG_ERR_OOM);
     }
+#undef LUT0_CUDA
     mg_mixture_lut* lut = new (std::nothrow) mg_mixture_lut;
-    if (!lut) { mg::set_error("mg_mixture_lut_build: out of host memory"); return MG_ERR_OOM; }
+    if (!lut) { mg::set_error("mg_mixture_lut_build: out of host memory"); return fail0(MG_ERR_OOM); }
+    lut->d_row_ptr = d_row_ptr;                                          // owned by the table from here on
     lut->device = g->device;
     lut->n_nodes = n;
     lut->n_leaves = nl;
     lut->capacity = total;
     float* d_sig = nullptr;
-    auto fail = [&](int rc) { cudaFree(d_sig); mg_mixture_lut_free(lut); return rc; };
+    auto fail = [&](int rc) { cudaFree(d_sig); cudaFree(d_stats); mg_mixture_lut_free(lut); return rc; };
 #define LUT_CUDA(call)                                                              \
     do {                                                                            \
         cudaError_t e__ = (call);                                                   \
         if (e__ != cudaSuccess) return fail(mg::cuda_fail(e__, #call));             \
     } while (0)
-    LUT_CUDA(cudaMalloc(&lut->d_row_ptr, (n + 1) * sizeof(uint64_t)));
     LUT_CUDA(cudaMalloc(&lut->d_row_len, n * sizeof(uint32_t)));
     LUT_CUDA(cudaMalloc(&lut->d_col, std::max<uint64_t>(total, 1) * sizeof(uint32_t)));
     LUT_CUDA(cudaMalloc(&lut->d_mu, std::max<uint64_t>(total, 1) * sizeof(double)));
     LUT_CUDA(cudaMalloc(&lut->d_dmu, std::max<uint64_t>(total, 1) * sizeof(double)));
     lut->device_bytes = (n + 1) * 8 + n * 4 + total * 20;
-    LUT_CUDA(cudaMemcpyAsync(lut->d_row_ptr, row_ptr.data(), (n + 1) * sizeof(uint64_t), cudaMemcpyHostToDevice, st));
     if (weight_sigma) {
         LUT_CUDA(cudaMalloc(&d_sig, n * sizeof(float)));
         LUT_CUDA(cudaMemcpyAsync(d_sig, weight_sigma, n * sizeof(float), cudaMemcpyHostToDevice, st));
@@ -172,15 +278,17 @@ extern "C" int mg_mixture_lut_build(mg_graph* g, const float* weight_sigma, mg_m
         LUT_CUDA(cudaGetLastError());
         mg::count_launch();
     }
-    std::vector<uint32_t> len(n);
-    LUT_CUDA(cudaMemcpyAsync(len.data(), lut->d_row_len, n * sizeof(uint32_t), cudaMemcpyDeviceToHost, st));
+    k_lut_stats<<<(unsigned)std::min<uint64_t>((n + 255) / 256, 148 * 8), 256, 0, st>>>(lut->d_row_len, n, d_stats);
+    LUT_CUDA(cudaGetLastError());
+    mg::count_launch();
+    unsigned long long stats[2] = {0, 0};
+    LUT_CUDA(cudaMemcpyAsync(stats, d_stats, sizeof(stats), cudaMemcpyDeviceToHost, st));
     LUT_CUDA(cudaStreamSynchronize(st));
 #undef LUT_CUDA
     cudaFree(d_sig);
-    for (uint64_t i = 0; i < n; i++) {
-        lut->nnz += len[i];
-        lut->max_row = std::max(lut->max_row, len[i]);
-    }
+    cudaFree(d_stats);
+    lut->nnz = stats[0];
+    lut->max_row = (uint32_t)stats[1];
     *out = lut;
     return MG_OK;
 }
@@ -236,7 +344,9 @@ struct QueryParams {
     const uint32_t* col;
     const double* mu;
     const double* dmu;
-    const uint64_t* boxes;
+    const uint64_t* boxes;           // [n_queries][6] staged on the device, or NULL: the boxes travel in `inline_box`
+    uint32_t inline_box[kInlineQueries][6];
+    uint32_t* done;                  // [n_queries] CTAs of the query that have finished (zeroed by k_query_prologue)
     double* expect;
     double* var;                     // may be NULL
     unsigned long long* fetches;     // may be NULL
@@ -267,6 +377,45 @@ __device__ __forceinline__ void add_sample(const QueryParams& P, double* expect,
             }
         }
     }
+}
+
+__device__ __forceinline__ void load_box(const QueryParams& P, uint32_t q, uint32_t* b)
+{
+#pragma unroll
+    for (int a = 0; a < 6; a++) b[a] = P.boxes ? (uint32_t)P.boxes[6ull * q + a] : P.inline_box[q][a];
+}
+
+__device__ __forceinline__ void griddep_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+__device__ __forceinline__ void griddep_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+
+// One launch instead of three memsets: the dense results, the fetch counters and the per-query completion counters.
+__global__ void __launch_bounds__(256)
+k_query_prologue(double* expect, double* var, unsigned long long* fetches, uint32_t* done, uint64_t n_out, uint32_t n_queries)
+{
+    griddep_launch_dependents();                                          // the query kernel may set up while this one zeroes
+    const uint64_t stride = (uint64_t)gridDim.x * 256;
+    for (uint64_t i = (uint64_t)blockIdx.x * 256 + threadIdx.x; i < n_out; i += stride) {
+        expect[i] = 0.0;
+        if (var) var[i] = 0.0;
+    }
+    for (uint64_t i = (uint64_t)blockIdx.x * 256 + threadIdx.x; i < n_queries; i += stride) {
+        if (fetches) fetches[i] = 0ull;
+        done[i] = 0u;
+    }
+}
+
+// Eq. 17: errors add in quadrature -- the LAST CTA of a query to finish takes the square roots of its variances
+// (every CTA fences its atomics, then counts itself done; no separate finishing kernel).
+__device__ __forceinline__ void finish_query(const QueryParams& P, uint32_t q, double* var)
+{
+    __shared__ bool s_last;
+    __threadfence();
+    __syncthreads();
+    if (threadIdx.x == 0) s_last = atomicAdd(P.done + q, 1u) == gridDim.y - 1;
+    __syncthreads();
+    if (!s_last || !var) return;
+    __threadfence();
+    for (uint32_t i = threadIdx.x; i < P.n_leaves; i += blockDim.x) var[i] = sqrt(__ldcg(var + i));
 }
 
 // Section 3.6, one axis: [lo, hi) cut left to right into the largest aligned power-of-two pieces.
@@ -334,11 +483,13 @@ k_range_query_fa(const __grid_constant__ QueryParams P)
     __shared__ unsigned long long s_pref[kMaxBoxes + 1];
     __shared__ unsigned long long s_part[kQueryThreads];
     const uint32_t q = blockIdx.x;
-    const uint64_t* box = P.boxes + 6ull * q;
+    uint32_t box[6];
+    load_box(P, q, box);
     if (threadIdx.x < 3)
-        s_n[threadIdx.x] = fa_axis((uint32_t)box[threadIdx.x], (uint32_t)box[3 + threadIdx.x], P.n_levels - 1,
+        s_n[threadIdx.x] = fa_axis(box[threadIdx.x], box[3 + threadIdx.x], P.n_levels - 1,
                                    s_start[threadIdx.x], s_level[threadIdx.x]);
     __syncthreads();
+    griddep_wait();                                                       // k_query_prologue has zeroed the results
     const int nx = s_n[0], ny = s_n[1], nz = s_n[2];
     const unsigned lane = threadIdx.x & 31;
     const unsigned n_warps = gridDim.y * (kQueryThreads / 32), warp = blockIdx.y * (kQueryThreads / 32) + threadIdx.x / 32;
@@ -394,6 +545,7 @@ k_range_query_fa(const __grid_constant__ QueryParams P)
         }
     }
     if (P.fetches && lane == 0 && n_fetch) atomicAdd(P.fetches + q, n_fetch);
+    finish_query(P, q, var);
 }
 
 // The naive approach (L377): every level-0 voxel of the box is one sample.  Warps take rows of the box (lanes
@@ -407,9 +559,11 @@ k_range_query_naive(const __grid_constant__ QueryParams P)
 {
     extern __shared__ uint32_t s_cnt[];
     const uint32_t q = blockIdx.x;
-    const uint64_t* box = P.boxes + 6ull * q;
-    const uint32_t x0 = (uint32_t)box[0], y0 = (uint32_t)box[1], z0 = (uint32_t)box[2];
-    const uint32_t dx = (uint32_t)box[3] - x0, dy = (uint32_t)box[4] - y0, dz = (uint32_t)box[5] - z0;
+    uint32_t box[6];
+    load_box(P, q, box);
+    const uint32_t x0 = box[0], y0 = box[1], z0 = box[2];
+    const uint32_t dx = box[3] - x0, dy = box[4] - y0, dz = box[5] - z0;
+    griddep_wait();                                                       // k_query_prologue has zeroed the results
     const int X = P.dim[0][0], Y = P.dim[0][1];
     double* expect = P.expect + (uint64_t)q * P.n_leaves;
     double* var = P.var ? P.var + (uint64_t)q * P.n_leaves : nullptr;
@@ -459,12 +613,7 @@ k_range_query_naive(const __grid_constant__ QueryParams P)
             if (s_cnt[i]) atomicAdd(expect + i, (double)s_cnt[i]);
     }
     if (P.fetches && blockIdx.y == 0 && threadIdx.x == 0) atomicAdd(P.fetches + q, (unsigned long long)dx * dy * dz);
-}
-
-__global__ void k_query_finish(double* var, uint64_t n)
-{
-    const uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i < n) var[i] = sqrt(var[i]);                                    // Eq. 17: errors add in quadrature
+    finish_query(P, q, var);
 }
 
 }  // namespace
@@ -520,23 +669,37 @@ extern "C" int mg_range_query(mg_mixture_lut* lut, const uint32_t* node_idx_mipm
     }
     cudaStream_t st = (cudaStream_t)stream;
     if (n_queries > lut->boxes_cap) {
-        MG_CUDA(cudaStreamSynchronize(st));                              // earlier queries may still read the old buffer
+        MG_CUDA(cudaStreamSynchronize(st));                              // earlier queries may still read the old buffers
         cudaFree(lut->d_boxes);
+        cudaFree(lut->d_done);
         lut->d_boxes = nullptr;
+        lut->d_done = nullptr;
         lut->boxes_cap = 0;
-        MG_CUDA(cudaMalloc(&lut->d_boxes, (size_t)n_queries * 6 * sizeof(uint64_t)));
-        lut->boxes_cap = n_queries;
+        const uint32_t cap = std::max<uint32_t>(n_queries, kInlineQueries);
+        MG_CUDA(cudaMalloc(&lut->d_boxes, (size_t)cap * 6 * sizeof(uint64_t)));
+        MG_CUDA(cudaMalloc(&lut->d_done, (size_t)cap * sizeof(uint32_t)));
+        lut->boxes_cap = cap;
     }
-    MG_CUDA(cudaMemcpyAsync(lut->d_boxes, boxes, (size_t)n_queries * 6 * sizeof(uint64_t), cudaMemcpyHostToDevice, st));
     const uint64_t n_out = (uint64_t)n_queries * lut->n_leaves;
-    MG_CUDA(cudaMemsetAsync(expect, 0, n_out * sizeof(double), st));
-    if (err) MG_CUDA(cudaMemsetAsync(err, 0, n_out * sizeof(double), st));
-    if (fetches) MG_CUDA(cudaMemsetAsync(fetches, 0, (size_t)n_queries * sizeof(uint64_t), st));
+    if (n_queries <= (uint32_t)kInlineQueries) {                          // small batch: the boxes ride in the kernel parameters
+        P.boxes = nullptr;
+        for (uint32_t q = 0; q < n_queries; q++)
+            for (int a = 0; a < 6; a++) P.inline_box[q][a] = (uint32_t)boxes[6ull * q + a];
+    } else {
+        MG_CUDA(cudaMemcpyAsync(lut->d_boxes, boxes, (size_t)n_queries * 6 * sizeof(uint64_t), cudaMemcpyHostToDevice, st));
+        P.boxes = lut->d_boxes;
+    }
+    P.done = lut->d_done;
+    {
+        const unsigned blocks = (unsigned)std::min<uint64_t>((std::max<uint64_t>(n_out, n_queries) + 255) / 256, 148ull * 8);
+        k_query_prologue<<<blocks, 256, 0, st>>>(expect, err, reinterpret_cast<unsigned long long*>(fetches), lut->d_done, n_out, n_queries);
+        MG_CUDA(cudaGetLastError());
+        mg::count_launch();
+    }
     P.idx = node_idx_mipmap;
     P.n_levels = (int)mip->n_levels;
     P.n_leaves = lut->n_leaves;
     P.row_ptr = lut->d_row_ptr; P.row_len = lut->d_row_len; P.col = lut->d_col; P.mu = lut->d_mu; P.dmu = lut->d_dmu;
-    P.boxes = lut->d_boxes;
     P.expect = expect;
     P.var = err;
     P.fetches = reinterpret_cast<unsigned long long*>(fetches);
@@ -556,24 +719,31 @@ extern "C" int mg_range_query(mg_mixture_lut* lut, const uint32_t* node_idx_mipm
     }
     const dim3 grid(n_queries, splits);
     P.force_walk = (mode == MG_QUERY_FA_WALK);
-    if (mode != MG_QUERY_NAIVE) k_range_query_fa<<<grid, kQueryThreads, 0, st>>>(P);
-    else {
+    // launched with programmatic stream serialisation: the decomposition of the boxes overlaps the prologue's zeroing; every
+    // kernel executes griddepcontrol.wait before its first atomic
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid;
+    cfg.blockDim = dim3(kQueryThreads);
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    if (mode != MG_QUERY_NAIVE) {
+        MG_CUDA(cudaLaunchKernelEx(&cfg, k_range_query_fa, P));
+    } else {
         const size_t smem = (size_t)lut->n_leaves * sizeof(uint32_t);
         if (smem <= 200 * 1024) {                                          // per-CTA leaf histogram in shared memory
             static mg::SmemAttrOnce once;                                  // per (function, device)
             const int rc = once.ensure((const void*)k_range_query_naive<true>, 200 * 1024, lut->device);
             if (rc != MG_OK) return rc;
-            k_range_query_naive<true><<<grid, kQueryThreads, smem, st>>>(P);
+            cfg.dynamicSmemBytes = smem;
+            MG_CUDA(cudaLaunchKernelEx(&cfg, k_range_query_naive<true>, P));
         } else {
-            k_range_query_naive<false><<<grid, kQueryThreads, 0, st>>>(P);
+            MG_CUDA(cudaLaunchKernelEx(&cfg, k_range_query_naive<false>, P));
         }
     }
-    MG_CUDA(cudaGetLastError());
     mg::count_launch();
-    if (err) {
-        k_query_finish<<<(unsigned)((n_out + 255) / 256), 256, 0, st>>>(err, n_out);
-        MG_CUDA(cudaGetLastError());
-        mg::count_launch();
-    }
     return MG_OK;
 }
