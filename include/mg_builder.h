@@ -136,6 +136,11 @@ int mgb_get_info(const mgb_result *r, mgb_info *info);
 /* dims_out: uint64[3 * n_mip_levels] = X_l, Y_l, Z_l per level. */
 int mgb_mip_dims(const mgb_result *r, uint64_t *dims_out);
 
+/* The ceil-halving chain of L80 for a volume that has not been built yet: "we round up the resolution of each
+ * subsequent level ... until we reach l = l_max with a resolution of 1^3 voxels".  Writes X_l, Y_l, Z_l of at most
+ * max_levels levels and returns the number of levels l_max + 1 (0 for a zero dimension).  Host only. */
+uint32_t mgb_mip_chain(uint64_t X, uint64_t Y, uint64_t Z, uint64_t *dims_out, uint32_t max_levels);
+
 /* Copy the graph out.  child_a/child_b/weight/weight_exact have n_nodes entries (leaves' entries 0),
  * level_offsets depth + 2, leaf_segment_id n_leaves.  weight = fp32 codeword (or fp32 of the exact
  * ratio when unquantised), weight_exact = mean of the exact ratios merged into the node (fp64),

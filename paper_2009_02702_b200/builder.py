@@ -21,7 +21,7 @@ PICK_SMALLEST_INDEX, PICK_SMALLEST_MASS = 0, 1
 
 SYMBOLS = ["mgb_default_params", "mgb_build", "mgb_build_from_level1", "mgb_build_from_levels", "mgb_get_front_mixture_nodes",
            "mgb_build_from_mixtures", "mgb_free", "mgb_get_info",
-           "mgb_mip_dims", "mgb_get_graph", "mgb_node_idx_ptr", "mgb_get_node_idx", "mgb_get_codebook",
+           "mgb_mip_dims", "mgb_mip_chain", "mgb_get_graph", "mgb_node_idx_ptr", "mgb_get_node_idx", "mgb_get_codebook",
            "mgb_get_weight_sigma", "mgb_last_error"]
 
 
@@ -54,6 +54,8 @@ lib.mgb_get_info.argtypes = [_vp, C.POINTER(Info)]
 lib.mgb_get_info.restype = C.c_int
 lib.mgb_mip_dims.argtypes = [_vp, _vp]
 lib.mgb_mip_dims.restype = C.c_int
+lib.mgb_mip_chain.argtypes = [C.c_uint64, C.c_uint64, C.c_uint64, _vp, C.c_uint32]
+lib.mgb_mip_chain.restype = C.c_uint32
 lib.mgb_get_graph.argtypes = [_vp, _vp, _vp, _vp, _vp, _vp, _vp]
 lib.mgb_get_graph.restype = C.c_int
 lib.mgb_node_idx_ptr.argtypes = [_vp, C.c_uint32]
@@ -85,6 +87,13 @@ class BuilderError(RuntimeError):
 def _check(rc: int, where: str) -> None:
     if rc != MGB_OK:
         raise BuilderError(rc, where)
+
+
+def mip_chain(dims_xyz) -> list:
+    """[(X_l, Y_l, Z_l)] of the mipmap of a volume that has not been built yet (mgb_mip_chain: the rule of L80)."""
+    d = np.zeros(3 * 64, dtype=np.uint64)
+    n = int(lib.mgb_mip_chain(int(dims_xyz[0]), int(dims_xyz[1]), int(dims_xyz[2]), d.ctypes.data, 64))
+    return [tuple(int(v) for v in d[3 * l:3 * l + 3]) for l in range(n)]
 
 
 def default_params(**overrides) -> Params:

@@ -169,6 +169,18 @@ extern "C" void mgb_default_params(mgb_params* p)
 
 extern "C" void mgb_free(mgb_result* r) { delete r; }
 
+extern "C" uint32_t mgb_mip_chain(uint64_t X, uint64_t Y, uint64_t Z, uint64_t* dims_out, uint32_t max_levels)
+{
+    if (X == 0 || Y == 0 || Z == 0) return 0;
+    uint32_t l = 0;
+    for (uint64_t x = X, y = Y, z = Z;;) {
+        if (dims_out && l < max_levels) { dims_out[3 * l] = x; dims_out[3 * l + 1] = y; dims_out[3 * l + 2] = z; }
+        l++;
+        if (x == 1 && y == 1 && z == 1) return l;
+        x = (x + 1) / 2; y = (y + 1) / 2; z = (z + 1) / 2;
+    }
+}
+
 // a0 - a2 for a volume: from the segment IDs (front == nullptr), or from levels 0 / 1 classified by a front end.
 static int build_volume(const uint32_t* seg, uint64_t X, uint64_t Y, uint64_t Z, const Level1Front* front,
                         const mgb_params* params, mgb_result** out, const LevelsFront* levels = nullptr)

@@ -169,12 +169,7 @@ def from_volume_device_levels(seg_dev, name: str = "volume", cfg: dict | None = 
     w = Workload(name)
     w.cfg = dict(cfg or {})
     Z, Y, X = (int(d) for d in seg_dev.shape)
-    dims, d = [], (X, Y, Z)
-    while True:
-        dims.append(d)
-        if d == (1, 1, 1):
-            break
-        d = tuple(-(-k // 2) for k in d)
+    dims = builder.mip_chain((X, Y, Z))                 # the library's statement of L80, not a Python restatement
     w.mip_dims = dims
     w.level_voxels = [a * b * c for a, b, c in dims]
     w.level_start, w.n_voxels_padded = _layout(w.level_voxels)
@@ -238,12 +233,7 @@ def from_volume_device(seg_dev, name: str = "volume", cfg: dict | None = None, *
     w = Workload(name)
     w.cfg = dict(cfg or {})
     Z, Y, X = (int(d) for d in seg_dev.shape)
-    dims, d = [], (X, Y, Z)
-    while True:
-        dims.append(d)
-        if d == (1, 1, 1):
-            break
-        d = tuple(-(-k // 2) for k in d)
+    dims = builder.mip_chain((X, Y, Z))                 # the library's statement of L80, not a Python restatement
     w.mip_dims = dims
     w.level_voxels = [a * b * c for a, b, c in dims]
     w.level_start, w.n_voxels_padded = _layout(w.level_voxels)

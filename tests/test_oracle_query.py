@@ -6,7 +6,7 @@ import numpy as np
 import pytest
 
 import oracle
-from paper_2009_02702_b200 import builder, synth
+from paper_2009_02702_b200 import synth
 
 
 # ------------------------------------------------------------------------------ 1D decomposition
@@ -80,12 +80,40 @@ def test_mixture_lut_mu_is_symbolic_eval_and_zero_sigma_gives_zero_error():
 
 
 # ------------------------------------------------------------------------------ range queries
-def _case(dims, n_seg, seed, **bp):
+def _case(dims, n_seg, seed, quant_bits=9):
+    """A volume, a Mixture Graph of its histogram mipmap and the per-level node indices, made HERE from the oracle's
+    exact integer histograms (no product code): every distinct mixture (m_1 .. m_k on leaves i_1 < .. < i_k) becomes the
+    chain n_1 = leaf i_1, n_j = (1 - w_j) n_{j-1} + w_j leaf i_j with w_j = m_j / (m_1 + .. + m_j) (Eq. 5-7 applied
+    k - 1 times), nodes shared through a dictionary (L144).  quant_bits > 0: w is replaced by the mid-point of its
+    2^b-bin and every node carries that bin's sigma = 2^-b / sqrt(12) (L176)."""
     seg = synth.voronoi_volume(dims, synth.voronoi_seeds(dims, n_seg, seed))
-    r = builder.build(seg, **bp)
-    g = r.graph()
-    levels = [r.node_idx(l) for l in range(r.info.n_mip_levels)]
     ids, seg_index = oracle.leaf_index(seg)
+    nl = ids.size
+    a, b, w, wq = [0] * nl, [0] * nl, [0.0] * nl, [0.0] * nl
+    node_of, levels = {}, []
+    for H in oracle.histogram_mipmap(seg_index, nl):
+        flat = H.reshape(-1, nl)
+        idx = np.zeros(flat.shape[0], dtype=np.uint32)
+        for v, row in enumerate(flat):
+            leaves = np.flatnonzero(row)
+            node, mass = int(leaves[0]), int(row[leaves[0]])
+            for j in leaves[1:]:
+                mass += int(row[j])
+                ratio = int(row[j]) / mass
+                q = (min((1 << quant_bits) - 1, int(ratio * (1 << quant_bits))) + 0.5) / (1 << quant_bits) if quant_bits else ratio
+                key = (node, int(j), q)
+                if key not in node_of:
+                    node_of[key] = len(a)
+                    a.append(node); b.append(int(j)); w.append(ratio); wq.append(q)
+                node = node_of[key]
+            idx[v] = node
+        levels.append(idx.reshape(H.shape[:3]))
+    n = len(a)
+    sigma = np.zeros(n)
+    if quant_bits:
+        sigma[nl:] = 2.0 ** -quant_bits / np.sqrt(12.0)
+    g = dict(child_a=np.array(a, np.uint32), child_b=np.array(b, np.uint32), weight_exact=np.array(w), n_leaves=nl,
+             weight=np.array(wq, np.float32), weight_sigma=sigma)
     return seg_index, g, levels
 
 
