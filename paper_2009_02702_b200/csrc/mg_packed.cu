@@ -7,7 +7,7 @@
 // This cuts the colourise input from 32 bits per voxel to r(l) (11 bits on level 0 of config 3).
 //
 //   k_index_range      min / max of a node-index volume (i_min, i_max of Eq. 15)
-//   k_pack_bits        one thread = one 32-bit word of the stream (no atomics)
+//   k_pack_bits<R>     one thread = 32 voxels = R words of the stream, staged through shared memory (no atomics)
 //   k_colorize_packed  one CTA = one tile of 4096 voxels of ONE level (uniform switch on the level's
 //                      bitrate into a compile-time-R body, see colorize_tile).  All levels of a mipmap
 //                      go in ONE launch: the per-level table travels as a __grid_constant__ parameter.
@@ -70,45 +70,80 @@ __global__ void __launch_bounds__(256) k_index_range(const uint32_t* __restrict_
     if ((threadIdx.x & 31) == 0 && lo <= hi) { atomicMin(mm, lo); atomicMax(mm + 1, hi); }
 }
 
-// word w of the stream holds stream bits [32 w, 32 w + 32): the voxels that overlap it are
-// floor(32 w / r) .. floor((32 w + 31) / r).  The one 64-bit division (first bit of the CTA's words by r) is taken
-// once per CTA; everything per thread is 32-bit and relative to it (the kernel is issue-bound, not HBM-bound: ncu
-// showed 78 % issue-slot use at 43 % DRAM throughput with a 32-bit division and 64-bit shifts per word).
-// kPackWords words per thread: a CTA of one word per thread is over before the next one is launched, and the kernel
-// then runs at the CTA launch rate.
-constexpr int kPackWords = 8;
+// The encoder, at the compile-time bitrate R: 32 consecutive voxels fill exactly R words, so a thread that owns 32
+// voxels packs them with shifts known at compile time and touches nobody else's words (no atomics, no division).
+// A CTA takes kPackTile = 256 x 32 voxels: coalesced 16-byte loads into shared memory (row stride 33 words: the 32
+// threads of a warp then read 32 different banks), R words per thread packed in registers, written back to shared
+// memory and stored with coalesced 4-byte stores -- the kernel is a stream (round 1's one-thread-per-word encoder ran
+// a variable-length loop per word and was issue-bound: 78 % issue slots at 43 % DRAM throughput, 1.59 ms on level 0 of
+// config 3 against 1.04 ms at the copy peak).  Words past the data (the stream's zero padding) are written as zeros.
+constexpr int kPackThreads = 256;
+constexpr int kPackTile = kPackThreads * 32;
 
-__global__ void __launch_bounds__(256)
-k_pack_bits(const uint32_t* __restrict__ idx, uint64_t n, uint32_t i_min, uint32_t r, uint32_t* __restrict__ words, uint64_t n_words)
+template <int R>
+__device__ __forceinline__ void pack_tile(const uint32_t* __restrict__ idx, uint64_t n, uint32_t i_min, uint32_t* __restrict__ words,
+                                          uint64_t n_words, uint32_t* smem)
 {
-    __shared__ const uint32_t* s_base;                                    // voxel q = floor(first bit of the CTA / r)
-    __shared__ uint32_t s_rem, s_n;                                       // first bit - q r; voxels from q on (capped)
-    const uint64_t w0 = (uint64_t)blockIdx.x * (256 * kPackWords);        // first word of this CTA
-    if (threadIdx.x == 0 && r) {
-        const uint64_t q = (w0 * 32) / r;
-        s_base = idx + q;
-        s_rem = (uint32_t)(w0 * 32 - q * r);
-        s_n = q < n ? (uint32_t)min(n - q, (uint64_t)1 << 30) : 0u;
+    constexpr uint32_t vmask = R >= 32 ? 0xFFFFFFFFu : ((1u << R) - 1u);  // a value outside [i_min, i_min + 2^R) must not spill
+    const uint64_t v0 = (uint64_t)blockIdx.x * kPackTile;                 // first voxel of the tile
+    const uint32_t t = threadIdx.x;
+    // ---- load: voxel v0 + e lands at smem[e + e / 32]
+    const uint64_t left = v0 < n ? n - v0 : 0;
+    const uint32_t nv = (uint32_t)(left < (uint64_t)kPackTile ? left : (uint64_t)kPackTile);
+    if ((((uintptr_t)(idx + v0)) & 15) == 0) {
+        const uint4* src = reinterpret_cast<const uint4*>(idx + v0);
+#pragma unroll
+        for (int k = 0; k < 8; k++) {
+            const uint32_t e = 4u * (t + k * kPackThreads);
+            uint4 x = make_uint4(i_min, i_min, i_min, i_min);
+            if (e + 4 <= nv) x = __ldcs(src + (e >> 2));
+            else if (e < nv) { x.x = idx[v0 + e]; if (e + 1 < nv) x.y = idx[v0 + e + 1]; if (e + 2 < nv) x.z = idx[v0 + e + 2]; }
+            uint32_t* d = smem + e + (e >> 5);                            // 4 consecutive elements never cross a row of 32
+            d[0] = x.x; d[1] = x.y; d[2] = x.z; d[3] = x.w;
+        }
+    } else {
+#pragma unroll 8
+        for (int k = 0; k < 32; k++) {
+            const uint32_t e = t + k * kPackThreads;
+            smem[e + (e >> 5)] = e < nv ? __ldcs(idx + v0 + e) : i_min;
+        }
     }
     __syncthreads();
-    const uint32_t magic = r > 1 ? 0xFFFFFFFFu / r + 1u : 0u;            // floor(x / r) = umulhi(x, magic) for x < 2^27, 1 < r <= 32
-    const uint32_t vmask = r >= 32 ? 0xFFFFFFFFu : (1u << r) - 1u;        // an index outside [i_min, i_min + 2^r) must not spill into its neighbours' bits
-#pragma unroll 2
-    for (int k = 0; k < kPackWords; k++) {
-        const uint32_t wl = k * 256 + threadIdx.x;
-        if (w0 + wl >= n_words) return;
-        uint32_t out = 0;
-        if (r) {
-            const uint32_t* base = s_base;
-            const uint32_t rel = s_rem + 32u * wl, n_rel = s_n;           // the word's bit 0, counted from voxel q's bit 0
-            uint32_t v = r > 1 ? __umulhi(rel, magic) : rel;
-            for (int sh = (int)(v * r) - (int)rel; sh < 32 && v < n_rel; sh += (int)r, v++) {   // sh: the value's bit 0 inside the word
-                const uint32_t val = (__ldg(base + v) - i_min) & vmask;
-                out |= (sh >= 0) ? (val << sh) : (val >> (-sh));
-            }
-        }
-        words[w0 + wl] = out;
+    // ---- pack the thread's 32 voxels (row t) into R words
+    uint32_t out[R > 0 ? R : 1];
+#pragma unroll
+    for (int q = 0; q < (R > 0 ? R : 1); q++) out[q] = 0u;
+#pragma unroll
+    for (int i = 0; i < 32; i++) {
+        const uint32_t val = (smem[t * 33 + i] - i_min) & vmask;
+        constexpr int dummy = 0; (void)dummy;
+        const int bit = i * R, wq = bit >> 5, sh = bit & 31;              // compile-time after unrolling
+        out[wq] |= val << sh;
+        if (sh + R > 32) out[wq + 1] |= val >> (32 - sh);
     }
+    __syncthreads();
+    constexpr bool kSkew = (R % 2) == 0;                                   // word i of the tile at smem[i] for odd R (stride R: 32 banks),
+#pragma unroll
+    for (int q = 0; q < R; q++) {                                          // at smem[i + i / 32] for even R (the skew restores 32 banks)
+        const uint32_t wi = t * R + q;
+        smem[kSkew ? wi + (wi >> 5) : wi] = out[q];
+    }
+    __syncthreads();
+    // ---- store: the tile's kPackThreads * R words are contiguous in the stream
+    const uint64_t w0 = (uint64_t)blockIdx.x * (kPackThreads * R);
+#pragma unroll 4
+    for (int q = 0; q < R; q++) {
+        const uint32_t wl = t + q * kPackThreads;
+        if (w0 + wl < n_words) words[w0 + wl] = smem[kSkew ? wl + (wl >> 5) : wl];
+    }
+}
+
+template <int R>
+__global__ void __launch_bounds__(kPackThreads)
+k_pack_bits(const uint32_t* __restrict__ idx, uint64_t n, uint32_t i_min, uint32_t* __restrict__ words, uint64_t n_words)
+{
+    __shared__ uint32_t smem[kPackThreads * 33];
+    pack_tile<R>(idx, n, i_min, words, n_words, smem);
 }
 
 // One tile (kTileVox voxels of one level) at the compile-time bitrate R.  A lane handles groups of 4
@@ -243,9 +278,24 @@ extern "C" int mg_pack_indices(const uint32_t* idx_device, uint64_t n, uint32_t 
     if (bits > 32) { set_error("mg_pack_indices: bits must be <= 32"); return MG_ERR_INVALID_ARG; }
     if ((uintptr_t)packed_device & 15) { set_error("mg_pack_indices: the stream must be 16-byte aligned"); return MG_ERR_INVALID_ARG; }
     const uint64_t n_words = mg_packed_stream_bytes(n, bits) / 4;
-    const uint64_t blocks = (n_words + 256 * kPackWords - 1) / (256 * kPackWords);
+    cudaStream_t st = (cudaStream_t)stream;
+    if (bits == 0) {                                                      // every voxel is node i_min: the stream is its padding
+        MG_CUDA(cudaMemsetAsync(packed_device, 0, n_words * 4, st));
+        return MG_OK;
+    }
+    // tiles of 8192 voxels = 256 R words; enough of them to cover the padding words behind the data too
+    const uint64_t blocks = (n_words + (uint64_t)kPackThreads * bits - 1) / ((uint64_t)kPackThreads * bits);
     if (blocks > 0x7fffffffull) { set_error("mg_pack_indices: too many voxels for one launch"); return MG_ERR_INVALID_ARG; }
-    k_pack_bits<<<(unsigned)blocks, 256, 0, (cudaStream_t)stream>>>(idx_device, n, i_min, bits, (uint32_t*)packed_device, n_words);
+    uint32_t* words = (uint32_t*)packed_device;
+#define MG_CASE(R) case R: k_pack_bits<R><<<(unsigned)blocks, kPackThreads, 0, st>>>(idx_device, n, i_min, words, n_words); break;
+    switch (bits) {
+        MG_CASE(1) MG_CASE(2) MG_CASE(3) MG_CASE(4) MG_CASE(5) MG_CASE(6) MG_CASE(7) MG_CASE(8)
+        MG_CASE(9) MG_CASE(10) MG_CASE(11) MG_CASE(12) MG_CASE(13) MG_CASE(14) MG_CASE(15) MG_CASE(16)
+        MG_CASE(17) MG_CASE(18) MG_CASE(19) MG_CASE(20) MG_CASE(21) MG_CASE(22) MG_CASE(23) MG_CASE(24)
+        MG_CASE(25) MG_CASE(26) MG_CASE(27) MG_CASE(28) MG_CASE(29) MG_CASE(30) MG_CASE(31) MG_CASE(32)
+        default: break;
+    }
+#undef MG_CASE
     count_launch();
     MG_CUDA(cudaGetLastError());
     return MG_OK;
