@@ -181,6 +181,13 @@ int mg_colorize(mg_graph *g, uint32_t mip_level, const uint32_t *node_idx_volume
                 uint64_t n_voxels, const float *node_rgba, void *out_rgba, void *out_rgba_aux,
                 uint32_t format, void *stream);
 
+/* Count the entries of a DEVICE node-index volume that name no node of g (>= n_nodes): mg_colorize, mg_render and
+ * mg_range_query gather through the indices unchecked, so a caller that did not build them with this library's
+ * builder can validate them once (compute-sanitizer being unavailable on some pools, this is the bounds check a
+ * memcheck run would make).  *n_bad_host receives the count; synchronises `stream`. */
+int mg_check_indices(const mg_graph *g, const uint32_t *node_idx_device, uint64_t n, uint64_t *n_bad_host,
+                     void *stream);
+
 /*
  * mg_tf_update_host -- the whole per-update path with HOST buffers at both ends:
  * H2D of the TF, mg_propagate, mg_colorize over n_voxels (typically every mip level,

@@ -301,6 +301,40 @@ __global__ void __launch_bounds__(256) k_relabel_indices(uint32_t* __restrict__ 
         idx[i] = __ldg(new_of_old + idx[i]);
 }
 
+__global__ void __launch_bounds__(256) k_check_indices(const uint32_t* __restrict__ idx, uint64_t n, uint32_t n_nodes, unsigned long long* bad)
+{
+    unsigned c = 0;
+    for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (uint64_t)gridDim.x * blockDim.x) c += __ldcs(idx + i) >= n_nodes;
+    c = __reduce_add_sync(0xffffffffu, c);
+    if ((threadIdx.x & 31) == 0 && c) atomicAdd(bad, (unsigned long long)c);
+}
+
+extern "C" int mg_check_indices(const mg_graph* g, const uint32_t* node_idx_device, uint64_t n, uint64_t* n_bad_host, void* stream)
+{
+    if (!g || !n_bad_host || (!node_idx_device && n)) { set_error("mg_check_indices: NULL argument"); return MG_ERR_INVALID_ARG; }
+    *n_bad_host = 0;
+    if (n == 0) return MG_OK;
+    const int rc = check_device(g, "mg_check_indices");
+    if (rc != MG_OK) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    unsigned long long* d_bad = nullptr;
+    MG_CUDA(cudaMalloc((void**)&d_bad, sizeof(unsigned long long)));
+    cudaError_t e = cudaMemsetAsync(d_bad, 0, sizeof(unsigned long long), st);
+    unsigned long long bad = 0;
+    if (e == cudaSuccess) {
+        const unsigned blocks = (unsigned)std::min<uint64_t>((n + 255) / 256, 148ull * 16);
+        k_check_indices<<<blocks, 256, 0, st>>>(node_idx_device, n, (uint32_t)g->n_nodes, d_bad);
+        count_launch();
+        e = cudaGetLastError();
+    }
+    if (e == cudaSuccess) e = cudaMemcpyAsync(&bad, d_bad, sizeof(bad), cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    cudaFree(d_bad);
+    if (e != cudaSuccess) return cuda_fail(e, "mg_check_indices");
+    *n_bad_host = bad;
+    return MG_OK;
+}
+
 extern "C" int mg_relabel_indices(mg_graph* g, uint32_t* idx_device, uint64_t n, void* stream)
 {
     if (!g || (!idx_device && n)) { set_error("mg_relabel_indices: NULL argument"); return MG_ERR_INVALID_ARG; }

@@ -26,7 +26,7 @@ ALL_LEVELS = 0xFFFFFFFF
 
 # every symbol include/mg.h declares (tests check that the library exports all of them)
 SYMBOLS = ["mg_load_graph", "mg_free_graph", "mg_graph_info", "mg_level_offsets", "mg_node_permutation",
-           "mg_relabel_indices", "mg_propagate", "mg_propagate_host", "mg_colorize", "mg_tf_update_host",
+           "mg_relabel_indices", "mg_check_indices", "mg_propagate", "mg_propagate_host", "mg_colorize", "mg_tf_update_host",
            "mg_last_error", "mg_kernel_launch_count",
            "mg_bits_per_voxel", "mg_packed_stream_bytes", "mg_index_range", "mg_pack_indices", "mg_colorize_packed",
            "mg_propagate_attr", "mg_render", "mg_render_ex", "mg_ess_mask_build",
@@ -60,6 +60,8 @@ lib.mg_node_permutation.argtypes = [_vp, _vp]
 lib.mg_node_permutation.restype = C.c_int
 lib.mg_relabel_indices.argtypes = [_vp, _vp, C.c_uint64, _vp]
 lib.mg_relabel_indices.restype = C.c_int
+lib.mg_check_indices.argtypes = [_vp, _vp, C.c_uint64, C.POINTER(C.c_uint64), _vp]
+lib.mg_check_indices.restype = C.c_int
 lib.mg_propagate.argtypes = [_vp, _vp, _vp, _vp]
 lib.mg_propagate.restype = C.c_int
 lib.mg_propagate_host.argtypes = [_vp, _vp, _vp, _vp]
@@ -356,6 +358,12 @@ class Graph:
 
     def relabel_indices(self, idx_device, n: int, stream: int = 0) -> None:
         _check(lib.mg_relabel_indices(self._h, _ptr(idx_device), int(n), stream or None), "mg_relabel_indices")
+
+    def check_indices(self, node_idx_device, n: int, stream: int = 0) -> int:
+        """Number of entries of a device index volume that name no node of this graph (mg_check_indices)."""
+        bad = C.c_uint64(0)
+        _check(lib.mg_check_indices(self._h, _ptr(node_idx_device), int(n), C.byref(bad), stream or None), "mg_check_indices")
+        return int(bad.value)
 
     def propagate(self, tf_device, node_rgba_device, stream: int = 0) -> None:
         _check(lib.mg_propagate(self._h, _ptr(tf_device), _ptr(node_rgba_device), stream or None), "mg_propagate")

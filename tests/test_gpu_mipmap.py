@@ -234,3 +234,19 @@ def test_mixture_table_matches_the_oracle_histograms(libs):
     keys = {(tuple(m["leaf"][int(o):int(o) + int(k)]), tuple(m["count"][int(o):int(o) + int(k)])) for o, k in zip(m["offset"], m["k"])}
     assert len(keys) == t.info.n_mixtures                            # hash-consed: no mixture twice
     t.close()
+
+
+def test_levels_build_error_paths(libs):
+    mg, workload = libs
+    l0 = _dev(np.zeros(8 * 8 * 8, np.uint32))
+    buf = torch.zeros(8 * 8 * 8 + 64 + 8 + 1, dtype=torch.int32, device="cuda")
+    start = np.array([0, 512, 576, 584], dtype=np.uint64)
+    with pytest.raises(mg.MgError):                                   # 8^3 has 4 levels, not 3
+        mg.MixtureTable(l0, (8, 8, 8), 1, buf, start[:3])
+    with pytest.raises(mg.MgError):                                   # no leaves
+        mg.MixtureTable(l0, (8, 8, 8), 0, buf, start)
+    t = mg.MixtureTable(l0, (8, 8, 8), 1, buf, start)                 # one segment: every level pure, no mixture at all
+    assert t.info.levels_done == 3 and t.info.n_mixtures == 0 and t.info.nnz_levels == 64 + 8 + 1
+    assert not buf.cpu().numpy().any()
+    assert all(v.size == 0 for v in t.export().values())
+    t.close()

@@ -389,6 +389,16 @@ def test_tf_update_host_end_to_end(mg):
     assert np.array_equal(out_host.numpy(), out_dev.cpu().numpy())
 
 
+def test_check_indices_counts_out_of_range_entries(mg):
+    a, b, w, off = synth.random_dag_levels([4, 6, 2], seed=12)
+    g = mg.Graph(a, b, w, 4, level_offsets=off)
+    idx = synth.random_node_idx(100003, 12, 81)
+    assert g.check_indices(_dev(idx), idx.size) == 0
+    idx[[0, 5, 100002]] = [12, 0xFFFFFFFF, 4000]
+    assert g.check_indices(_dev(idx), idx.size) == 3
+    assert g.check_indices(_dev(idx)[1:], idx.size - 1) == 2 and g.check_indices(_dev(idx), 0) == 0
+
+
 def test_error_paths(mg):
     a, b, w, off = synth.random_dag_levels([4, 6, 2], seed=11)
     g = mg.Graph(a, b, w, 4, level_offsets=off)

@@ -246,3 +246,25 @@ def test_render_error_paths(mg):
     with pytest.raises(mg.MgError):
         g.render(None, good_mip, pal, view, out)
     g.close()
+
+
+def test_ess_mask_error_paths(mg):
+    """mg_ess_mask_build needs a level 2 (3 .. 18 mip levels); mg_render_ex refuses a mask on a mipmap without one;
+    with empty-space skipping off the mask is ignored."""
+    g = _trivial_graph(mg, 4)
+    pal = _dev(synth.random_tf(4, 90))
+    two = [np.zeros((2, 2, 2), np.uint32), np.zeros((1, 1, 1), np.uint32)]
+    d_idx = _dev(np.zeros(9, np.int32))
+    mask = torch.zeros(8, dtype=torch.int16, device="cuda")
+    desc = ([0, 8], [(2, 2, 2), (1, 1, 1)])
+    with pytest.raises(mg.MgError):
+        g.ess_mask_build(d_idx, desc, pal, 1e-8, mask)
+    view = synth.orbit_view((2, 2, 2), width=8, height=8)
+    img = torch.zeros((8, 8, 4), dtype=torch.float32, device="cuda")
+    with pytest.raises(mg.MgError):
+        g.render(d_idx, desc, pal, view, img, ess_mask_device=mask)
+    g.render(d_idx, desc, pal, dict(view, ess_threshold=-1.0), img, ess_mask_device=mask)      # ESS off: not consulted
+    torch.cuda.synchronize()
+    with pytest.raises(mg.MgError):                                                            # NaN threshold
+        g.ess_mask_build(d_idx, ([0, 64, 72, 73], [(4, 4, 4), (2, 2, 2), (1, 1, 1)]), pal, float("nan"), mask)
+    g.close()
