@@ -7,6 +7,8 @@
 // mixtures (sorted (leaf, count) lists on a common power-of-two scale, each child weighing 1/N), divides by the common
 // power of two and HASH-CONSES the result, so that only distinct mixtures reach the factoriser (L88-L98).  Per level:
 //   k_classify   one thread per parent: gather the <= 8 child handles; all equal -> inherit, else append to a list
+//                (level 1, 98 % of the parents: the streaming classifier of mg_mipmap_front_level1, which lists the
+//                parents together with their <= 8 leaves, and k_merge_leaves, one THREAD per listed parent)
 //   k_merge      one warp per listed parent: rank-merge the children's sorted lists in shared memory, combine equal
 //                leaves, reduce, hash (64 bit), park the result in a per-level scratch arena
 //   k_claim      find-or-claim the hash in an open-addressing table; atomicMin of the parent's position
@@ -256,6 +258,69 @@ k_merge(const uint32_t* __restrict__ C, const LevelGeom G, uint32_t* __restrict_
     if (lane == 0) { Q.off[q] = so; Q.k[q] = kk; Q.tlog[q] = tmax + nlog - (uint32_t)tz; Q.hash[q] = h; }
 }
 
+// Level 1: the children are leaves, at most 8 of them -- one THREAD per listed parent sorts them in registers, run-length
+// encodes, reduces and hashes (same hash as k_merge); scratch space comes from one warp-aggregated atomic.
+// children: [n][8] leaf numbers, kNone for a child outside the volume (the list of mg_mipmap_front_level1).
+__global__ void __launch_bounds__(kThreads)
+k_merge_leaves(const uint32_t* __restrict__ children, const Pending Q, uint32_t n_pending, uint32_t* __restrict__ s_leaf,
+               uint64_t* __restrict__ s_cnt, unsigned long long* ctr)
+{
+    const uint32_t q = blockIdx.x * kThreads + threadIdx.x;
+    const bool live = q < n_pending;
+    uint32_t c[8];
+    uint32_t kk = 0, n = 0;
+    uint32_t lf[8], cn[8];
+    if (live) {
+        const uint4 lo = __ldg(reinterpret_cast<const uint4*>(children + 8ull * q)), hi = __ldg(reinterpret_cast<const uint4*>(children + 8ull * q) + 1);
+        c[0] = lo.x; c[1] = lo.y; c[2] = lo.z; c[3] = lo.w; c[4] = hi.x; c[5] = hi.y; c[6] = hi.z; c[7] = hi.w;
+        // sorting network for 8 keys (19 compare-exchanges); kNone sorts last
+#define MG_CX(i, j) { const uint32_t a_ = min(c[i], c[j]), b_ = max(c[i], c[j]); c[i] = a_; c[j] = b_; }
+        MG_CX(0, 1) MG_CX(2, 3) MG_CX(4, 5) MG_CX(6, 7)
+        MG_CX(0, 2) MG_CX(1, 3) MG_CX(4, 6) MG_CX(5, 7)
+        MG_CX(1, 2) MG_CX(5, 6) MG_CX(0, 4) MG_CX(3, 7)
+        MG_CX(1, 5) MG_CX(2, 6)
+        MG_CX(1, 4) MG_CX(3, 6)
+        MG_CX(2, 4) MG_CX(3, 5)
+        MG_CX(3, 4)
+#undef MG_CX
+#pragma unroll
+        for (int t = 0; t < 8; t++) {
+            if (c[t] == kNone) continue;
+            n++;
+            if (kk && lf[kk - 1] == c[t]) cn[kk - 1]++;
+            else { lf[kk] = c[t]; cn[kk] = 1; kk++; }
+        }
+    }
+    // scratch: one atomic per warp
+    const unsigned lane = threadIdx.x & 31;
+    uint32_t incl = kk;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) { const uint32_t up = __shfl_up_sync(0xffffffffu, incl, d); if (lane >= (unsigned)d) incl += up; }
+    const uint32_t tot = __shfl_sync(0xffffffffu, incl, 31);
+    unsigned long long base = 0;
+    if (lane == 0 && tot) { base = atomicAdd(ctr + kScratch, (unsigned long long)tot); atomicAdd(ctr + kNnz, (unsigned long long)tot); }
+    base = __shfl_sync(0xffffffffu, base, 0);
+    if (!live) return;
+    int tz = 32;
+#pragma unroll
+    for (int j = 0; j < 8; j++)
+        if ((uint32_t)j < kk) tz = min(tz, __ffs((int)cn[j]) - 1);
+    uint64_t h = 0;
+    const uint64_t so = base + (incl - kk);
+#pragma unroll
+    for (int j = 0; j < 8; j++) {
+        if ((uint32_t)j >= kk) continue;
+        const uint64_t cnt = cn[j] >> tz;
+        h += mix64((((uint64_t)lf[j] << 32) | (uint32_t)(j + 1)) * 0x9E3779B97F4A7C15ull + cnt);
+        s_leaf[so + j] = lf[j];
+        s_cnt[so + j] = cnt;
+    }
+    h = mix64(h ^ kk);
+    if (h == 0) h = 1;
+    const uint32_t nlog = (n == 8) ? 3u : (n == 4) ? 2u : (n == 2) ? 1u : 0u;
+    Q.off[q] = so; Q.k[q] = kk; Q.tlog[q] = nlog - (uint32_t)tz; Q.hash[q] = h;     // (kk >= 2: the list holds non-pure parents only)
+}
+
 __global__ void __launch_bounds__(kThreads)
 k_claim(const Pending Q, uint32_t n_pending, uint32_t level, uint64_t* hash, uint64_t* hfirst, uint64_t mask, unsigned long long* ctr)
 {
@@ -373,7 +438,10 @@ extern "C" int mg_mipmap_levels_build(const uint32_t* level0_device, uint64_t X,
     Pending Q = {};
     uint32_t* d_sleaf = nullptr;
     uint64_t* d_scnt = nullptr;
+    uint32_t* d_children = nullptr;                                       // level 1 only: the <= 8 leaves of every listed parent
     auto drop_level = [&]() {
+        cudaFree(d_children);
+        d_children = nullptr;
         cudaFree(d_list); cudaFree(Q.off); cudaFree(Q.k); cudaFree(Q.tlog); cudaFree(Q.hash); cudaFree(Q.slot); cudaFree(d_sleaf); cudaFree(d_scnt);
         d_list = nullptr; Q = Pending{}; d_sleaf = nullptr; d_scnt = nullptr;
     };
@@ -401,18 +469,35 @@ extern "C" int mg_mipmap_levels_build(const uint32_t* level0_device, uint64_t X,
             MT_CUDA(cudaMemcpyAsync(&nnz_before, T->d_ctr + kNnz, sizeof(nnz_before), cudaMemcpyDeviceToHost, st));
             MT_CUDA(cudaStreamSynchronize(st));
         }
-        uint32_t list_cap = std::max<uint32_t>(1024, n_par / 8);
+        uint32_t list_cap = std::max<uint32_t>(1024, l == 1 ? n_par / 12 : n_par / 3);
         uint32_t n_pending = 0;
         for (;;) {
             MT_CUDA(cudaMalloc((void**)&d_list, (size_t)list_cap * 4));
-            MT_CUDA(cudaMemsetAsync(T->d_ctr + kNPending, 0, sizeof(unsigned long long), st));
-            MT_CUDA(cudaMemcpyAsync(T->d_ctr + kNnz, &nnz_before, sizeof(nnz_before), cudaMemcpyHostToDevice, st));
-            k_classify<<<(n_par + kThreads - 1) / kThreads, kThreads, 0, st>>>(C, G, n_par, P, d_list, list_cap, T->d_k, T->d_ctr);
-            mg::count_launch();
-            MT_CUDA(cudaGetLastError());
-            MT_CUDA(cudaMemcpyAsync(ctr, T->d_ctr, sizeof(ctr), cudaMemcpyDeviceToHost, st));
-            MT_CUDA(cudaStreamSynchronize(st));
-            if (ctr[kNPending] <= list_cap) { n_pending = (uint32_t)ctr[kNPending]; break; }
+            if (l == 1) {
+                // level 1 is 98 % of the work and its children are leaves: the streaming classifier of the front end
+                // (16-byte / 8-byte loads, four parents per thread, one list atomic per CTA) lists the parents WITH their children
+                cudaError_t e = cudaMalloc((void**)&d_children, (size_t)list_cap * 32);
+                if (e != cudaSuccess) return fail(mg::cuda_fail(e, "cudaMalloc(children list)"));
+                uint64_t n_mixed = 0;
+                const int rc = mg_mipmap_front_level1(level0_device, X, Y, Z, P, d_list, d_children, list_cap, &n_mixed, stream);
+                if (rc != MG_OK) return fail(rc);
+                ctr[kNPending] = n_mixed;
+                ctr[kNnz] = nnz_before + (n_par - n_mixed);               // every other parent is one leaf
+                MT_CUDA(cudaMemcpyAsync(T->d_ctr + kNnz, &ctr[kNnz], sizeof(unsigned long long), cudaMemcpyHostToDevice, st));
+                MT_CUDA(cudaStreamSynchronize(st));                       // (ctr is a stack array that is rewritten below)
+                if (n_mixed <= list_cap) { n_pending = (uint32_t)n_mixed; break; }
+                cudaFree(d_children);
+                d_children = nullptr;
+            } else {
+                MT_CUDA(cudaMemsetAsync(T->d_ctr + kNPending, 0, sizeof(unsigned long long), st));
+                MT_CUDA(cudaMemcpyAsync(T->d_ctr + kNnz, &nnz_before, sizeof(nnz_before), cudaMemcpyHostToDevice, st));
+                k_classify<<<(n_par + kThreads - 1) / kThreads, kThreads, 0, st>>>(C, G, n_par, P, d_list, list_cap, T->d_k, T->d_ctr);
+                mg::count_launch();
+                MT_CUDA(cudaGetLastError());
+                MT_CUDA(cudaMemcpyAsync(ctr, T->d_ctr, sizeof(ctr), cudaMemcpyDeviceToHost, st));
+                MT_CUDA(cudaStreamSynchronize(st));
+                if (ctr[kNPending] <= list_cap) { n_pending = (uint32_t)ctr[kNPending]; break; }
+            }
             cudaFree(d_list);
             d_list = nullptr;
             list_cap = (uint32_t)ctr[kNPending];
@@ -444,8 +529,11 @@ extern "C" int mg_mipmap_levels_build(const uint32_t* level0_device, uint64_t X,
                 MT_CUDA(cudaMemsetAsync(T->d_ctr + kScratch, 0, sizeof(unsigned long long), st));
                 MT_CUDA(cudaMemsetAsync(T->d_ctr + kFlags, 0, sizeof(unsigned long long), st));
                 MT_CUDA(cudaMemcpyAsync(T->d_ctr + kNnz, &nnz_classified, sizeof(nnz_classified), cudaMemcpyHostToDevice, st));
-                k_merge<<<(n_pending + kMergeWarps - 1) / kMergeWarps, kMergeWarps * 32, 0, st>>>(
-                    C, G, P, Q, n_pending, T->d_off, T->d_k, T->d_tlog, T->d_leaf, T->d_cnt, d_sleaf, d_scnt, scratch_cap, T->d_ctr);
+                if (l == 1)
+                    k_merge_leaves<<<(n_pending + kThreads - 1) / kThreads, kThreads, 0, st>>>(d_children, Q, n_pending, d_sleaf, d_scnt, T->d_ctr);
+                else
+                    k_merge<<<(n_pending + kMergeWarps - 1) / kMergeWarps, kMergeWarps * 32, 0, st>>>(
+                        C, G, P, Q, n_pending, T->d_off, T->d_k, T->d_tlog, T->d_leaf, T->d_cnt, d_sleaf, d_scnt, scratch_cap, T->d_ctr);
                 mg::count_launch();
                 MT_CUDA(cudaGetLastError());
                 MT_CUDA(cudaMemcpyAsync(ctr, T->d_ctr, sizeof(ctr), cudaMemcpyDeviceToHost, st));
