@@ -171,6 +171,17 @@ def oracle_step(w, tf64, plan, chunk: int = 1 << 25, n_threads: int = 0):
     return t1 - t0, t2 - t1, int(used)
 
 
+def cpu_model() -> str:
+    try:
+        with open("/proc/cpuinfo") as f:
+            for line in f:
+                if line.lower().startswith("model name"):
+                    return line.split(":", 1)[1].strip()
+    except OSError:
+        pass
+    return "unknown"
+
+
 def cpu_baseline(w, n_sample: int) -> dict:
     plan = _sample_plan(w, n_sample)
     tf64 = w.tf(0).astype(np.float64)
@@ -183,7 +194,7 @@ def cpu_baseline(w, n_sample: int) -> dict:
     tp1, tc1, used1 = oracle_step(w, tf64, plan1, n_threads=1)
     n_s1 = sum(plan1)
     ms1 = 1e3 * (tp1 + tc1 * (w.n_voxels / n_s1))
-    return {"value": ms, "unit": UNIT, "cores": used, "kind": "oracle",
+    return {"value": ms, "unit": UNIT, "cores": used, "kind": "oracle", "cpu_model": cpu_model(), "host_cores": os.cpu_count(),
             "sample": f"full fp64 level-synchronous propagation of all {w.stats['n_nodes']} nodes ({1e3 * tp:.1f} ms) + "
                       f"fp64 lookup/RGBA8 conversion of the leading {n_s} of {w.n_voxels} voxels (same share of every "
                       f"mip level, {1e3 * tc:.1f} ms), colourise time scaled to the whole mipmap",
@@ -559,6 +570,8 @@ def run_b200(args) -> dict:
         "ms_per_step": ms_per_step, "higher_is_better": False, "scaling": "strong" if slab else "weak", "vs_baseline": None,
         "dtype": "f32", "data": "synthetic", "config": workload_config(w, args, world),
         "propagate_ms": prop_avg, "colorize_ms": col_avg, "propagate_ms_min": float(prop_ms.min()), "colorize_ms_min": float(col_ms.min()),
+        "propagate_ms_median": float(np.median(prop_ms)), "colorize_ms_median": float(np.median(col_ms)),
+        "update_ms_median": float(np.median(prop_ms + col_ms)), "update_ms_min": float((prop_ms + col_ms).min()),
         "nodes_per_s": n_internal / (prop_avg * 1e-3), "voxels_per_s": w.n_voxels * (n_part / max(1, w.n_voxels_padded)) / (col_avg * 1e-3),
         "hbm_gbs_step": (algo_bytes + BYTES_PER_NODE_L2 * n_internal) / (ms_per_step * 1e-3) / 1e9,
         "frac_of_nominal_8TBs": achieved / NOMINAL_HBM_GBS,
@@ -633,7 +646,8 @@ def run_reference(args) -> dict:
     return {"impl": "reference", "metric": METRIC, "value": ms, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": 1e3 * wall / max(1, args.steps), "higher_is_better": False, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic", "config": cfg,
-            "cpu_baseline": {"value": ms, "unit": UNIT, "cores": used, "kind": "oracle", "sample": sample},
+            "cpu_baseline": {"value": ms, "unit": UNIT, "cores": used, "kind": "oracle", "sample": sample, "cpu_model": cpu_model(),
+                             "host_cores": os.cpu_count()},
             "e2e": {"value": ms, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0, "propagate_ms": 1e3 * tp, "colorize_sample_ms": 1e3 * tc,
             "note": "no reference implementation exists for this paper; this arm is the repo's CPU fp64 oracle (test "
