@@ -348,6 +348,21 @@ def run_b200(args) -> dict:
     total_ms = max_over_ranks(total_ms, world, red_dev)
     ms_per_step = total_ms / K
 
+    # ---- the same colourise WITHOUT the reuse flag: mg_colorize's default first derives the palette from node_rgba
+    derive = None
+    if rank == 0:
+        kd = min(K, 20)
+        evd = [[torch.cuda.Event(enable_timing=True) for _ in range(2)] for _ in range(kd)]
+        g.propagate(tfs[0], nodes, st)
+        for _ in range(2):
+            g.colorize(idx_part, n_part, nodes, out_part, fmt=fmt, stream=st)
+        for k in range(kd):
+            evd[k][0].record(stream)
+            g.colorize(idx_part, n_part, nodes, out_part, fmt=fmt, stream=st)
+            evd[k][1].record(stream)
+        torch.cuda.synchronize()
+        derive = float(np.mean([e[0].elapsed_time(e[1]) for e in evd]))
+
     # ---- NEXT-3 variant: the same update with the node IDs bit-packed at r(l) bits per voxel (Table 1)
     packed = None
     if not args.no_packed and rank == 0:
@@ -582,6 +597,8 @@ def run_b200(args) -> dict:
         "setup_s": dict({k: round(v, 3) for k, v in w.stats.items() if k.endswith("_s")},
                         **({"device_levels_done": w.stats["device_levels_done"]} if "device_levels_done" in w.stats else {})),
     }
+    if derive is not None:
+        res["colorize_deriving_palette_ms"] = derive      # mg_colorize's default (no MG_PALETTE_FROM_LAST_PROPAGATE): + k_convert_palette
     if prop_roofline is not None:
         res["roofline_second_kernel"] = prop_roofline
     if packed is not None:
