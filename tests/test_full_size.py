@@ -510,7 +510,7 @@ def test_config3_device_mipmap_front_end_full_size(libs):
         b.close()
 
 
-@pytest.mark.parametrize("cfg_id", [3, 4])
+@pytest.mark.parametrize("cfg_id", [3, 4, 2])
 def test_device_levels_full_size(libs, cfg_id):
     """NEXT-4 (second half) at full size: the levels >= 1 of the histogram mipmap merged and hash-consed on the device
     (bench.py --device-levels) yield the graph and the node-index mipmap of the level-1 front-end path bit for bit."""

@@ -55,3 +55,19 @@ def test_bench_host_mipmap_and_fp16_variants_agree_on_the_workload():
         assert a["config"][k] == b["config"][k], k
     assert "front_end_s" not in a["setup_s"] and a["config"]["output"] == "rgba8" and b["config"]["output"] == "rgba16f"
     assert b["roofline"]["algorithmic_bytes_per_launch"] == 12 * b["config"]["mip_voxels"]
+
+
+def test_bench_config5_reports_both_bandwidth_bound_kernels():
+    """Config 5 (scaled to 10 M nodes: a 161 MB palette, beyond the L2): loaded with MG_RELABEL by default, both kernels carry a roofline object, the one that takes
+    longer is `roofline`; --device-levels changes the setup only."""
+    cmd = [sys.executable, os.path.join(ROOT, "bench.py"), "--config", "5", "--scale", "0.15", "--steps", "4", "--warmup", "3",
+           "--no-cpu-baseline", "--no-e2e", "--no-packed", "--no-attr"]
+    out = subprocess.run(cmd, capture_output=True, text=True, timeout=900)
+    assert out.returncode == 0, out.stderr[-3000:]
+    d = json.loads([l for l in out.stdout.strip().splitlines() if l.startswith("{")][-1])
+    assert d["config"]["workload"].startswith("cfg5") and d["value"] > 0
+    names = {d["roofline"]["kernel"], d["roofline_second_kernel"]["kernel"]}
+    assert "k_level" in names and len(names) == 2
+    assert d["roofline"]["avg_launch_ms"] >= d["roofline_second_kernel"]["avg_launch_ms"]
+    a = _run("--device-levels", "--no-cpu-baseline", "--no-e2e", "--no-render", "--no-query", "--no-packed", "--no-attr")
+    assert a["setup_s"]["device_levels_done"] >= 1 and a["value"] > 0
