@@ -6,8 +6,8 @@ mg_load_graph -> ONE concatenated node-index mipmap, ONE mg_colorize call over a
   * node colours: EVERY node against the same-graph oracle (O-4), leaves bit-exact, max-abs <= 1e-5;
   * level 0 (87 % of the voxels): EVERY voxel -- its colour must be the RGBA8 code of TF[S(v)] (I5, L223),
     with S from the input generator (not from the builder) and the 4 x n_leaves codes from the oracle;
-  * every other level: seeded random samples + the first/last voxels of the level against the oracle's
-    lookup/conversion on the same graph, and padding voxels against node 0;
+  * every other level: EVERY voxel against the oracle's lookup/conversion on the same graph (host-built node
+    indices), and padding voxels against node 0;
   * quantised-graph colour vs the DIRECT histogram (O-3 brute force on the generator's volume): EVERY voxel of
     every level whose dense histogram table fits 2 GB (levels >= 5 or 6: where the mixtures have hundreds of
     components and the quantisation error peaks, Table 2), >= 1000 mixed voxels of each finer level:
@@ -128,16 +128,21 @@ def test_volume_config_full_size(libs, cfg_id):
             bad += int((got != exp).sum().item())
         assert bad == 0, f"{bad} level-0 voxels differ from code(TF[S(v)])"
 
-        # ---- every level: samples + edges against the oracle's lookup on the same graph
-        out_host_levels = []
+        # ---- every level >= 1, EVERY voxel (chunked): the oracle's lookup + conversion on the same graph, with the node
+        # indices the host builder produced; level 0 additionally on samples through the oracle's lookup (its every-voxel
+        # check is the TF-code comparison above); padding voxels against node 0
         for l, (s0, nv) in enumerate(zip(w.level_start, w.level_voxels)):
-            pos = _sample_positions(nv, 200000, 77 + cfg_id, l)
-            got = out4[torch.from_numpy(pos + s0).cuda()].cpu().numpy()
-            # node indices the oracle looks up: the builder's for levels >= 1; level 0 = leaf number of S(v), taken
-            # from the generator's volume (never from the device front end that produced the GPU's copy)
-            idx = (seg_index if l == 0 else w.host_idx[l]).reshape(-1)[pos]
-            assert _rgba8_close(got, oracle.lookup(idx, ref_nodes)), f"level {l}"
-            out_host_levels.append((pos, got))
+            if l == 0:
+                pos = _sample_positions(nv, 200000, 77 + cfg_id, l)
+                got = out4[torch.from_numpy(pos + s0).cuda()].cpu().numpy()
+                assert _rgba8_close(got, oracle.lookup(seg_index.reshape(-1)[pos], ref_nodes)), "level 0"
+            else:
+                idx_l = w.host_idx[l].reshape(-1)
+                chunk = 1 << 23
+                for o in range(0, nv, chunk):
+                    e = min(nv, o + chunk)
+                    got = out4[s0 + o:s0 + e].cpu().numpy()
+                    assert _rgba8_close(got, oracle.lookup(idx_l[o:e], ref_nodes)), f"level {l}, voxels {o}..{e}"
             pad_end = w.level_start[l + 1] if l + 1 < len(w.level_start) else w.n_voxels_padded
             if pad_end > s0 + nv:                                            # padding voxels: node 0
                 padv = out4[s0 + nv:pad_end].cpu().numpy()
