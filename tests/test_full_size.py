@@ -342,19 +342,30 @@ def test_packed_mipmap_full_size(libs, cfg_id):
         w.close()
 
 
-def test_config5_dag_stress_full_size(libs):
-    """2^26 nodes, 24 levels, 2^14 leaves, random children; 512^3 random node-index volume."""
+@pytest.mark.parametrize("relabel", [True, False], ids=["relabelled_as_bench_does", "callers_numbering"])
+def test_config5_dag_stress_full_size(libs, relabel):
+    """2^26 nodes, 24 levels, 2^14 leaves, random children; 512^3 random node-index volume: every node and every voxel.
+    bench.py loads this config with MG_RELABEL: the library's numbering is then a permutation of the caller's."""
     mg, workload = libs
-    w = workload.make(5)
+    w = workload.make(5, relabel=relabel)
     try:
         assert w.graph.info.n_nodes == 1 << 26 and w.graph.info.depth == 23 and w.n_voxels == 512 ** 3
+        assert (w.perm is not None) == relabel
         tf = w.tf(0)
         nodes, out = _run_update(mg, w, tf, mg.MG_RGBA8)
-        ref_nodes = _check_nodes(w, nodes, tf)                               # every one of the 2^26 nodes
+        hg = w.host_graph
+        ref_nodes = oracle.graph_eval(hg["child_a"], hg["child_b"], hg["weight"], hg["n_leaves"], tf.astype(np.float64))
+        got = nodes.cpu().numpy()
+        if relabel:
+            got = got[w.perm]                                                # caller's node n lives at perm[n]
+        assert np.array_equal(got[:hg["n_leaves"]].view(np.uint32), tf.view(np.uint32)), "leaves not bit-exact"
+        assert float(np.abs(got - ref_nodes).max()) <= TOL                   # every one of the 2^26 nodes
+        del got
         out4 = out.view(-1, 4)
-        pos = _sample_positions(w.n_voxels, 2000000, 93, 0)
-        got = out4[torch.from_numpy(pos).cuda()].cpu().numpy()
-        assert _rgba8_close(got, oracle.lookup(w.host_idx[0][pos], ref_nodes))
+        chunk = 1 << 23                                                      # every one of the 512^3 voxels, chunked
+        for o in range(0, w.n_voxels, chunk):
+            e = min(w.n_voxels, o + chunk)
+            assert _rgba8_close(out4[o:e].cpu().numpy(), oracle.lookup(w.host_idx[0][o:e], ref_nodes)), (o, e)
     finally:
         w.close()
 
