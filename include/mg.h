@@ -229,6 +229,37 @@ uint64_t mg_packed_stream_bytes(uint64_t n_voxels, uint32_t bits);
  * this call synchronises `stream`. */
 int mg_index_range(const uint32_t *idx_device, uint64_t n, uint32_t *i_min, uint32_t *i_max, void *stream);
 
+/*
+ * mg_index_ranges_static -- i_min(l) / i_max(l) of Eq. 15 for EVERY level of a mipmap in one call that allocates
+ * nothing (no cudaMalloc, no cudaFree, no allocating library routine).
+ *
+ * Who needs it: mg_index_range gets its scratch words from cudaMalloc and returns them with cudaFree on each call.
+ * A host application that has given the device's whole memory to an arena of its own (a renderer's resource pool, a
+ * framework's caching allocator) may find the driver has nothing left to give, and a frame loop cannot take
+ * cudaFree's wait on all of the device's streams between a TF update and the next frame.  Here the scratch -- one
+ * (min, max) pair per level -- is a fixed 256-byte array inside the library image instead; every GPU that loads
+ * libmg.so holds it until the process exits.
+ *
+ *   idx_device          DEVICE uint32 indices, the levels back to back or with gaps, 4-byte aligned.
+ *   level_offsets_host  HOST uint64[n_levels + 1], non-decreasing: level l is idx_device[off[l] .. off[l + 1]).
+ *   n_levels            1 .. MG_INDEX_RANGES_STATIC_MAX_LEVELS; more is refused with MG_ERR_INVALID_ARG (the array
+ *                       has no room: call mg_index_range per level instead).
+ *   i_min_host, i_max_host  HOST uint32[n_levels], caller-owned: receive the ranges, the same values
+ *                       mg_index_range returns level by level.  An empty level reports i_min = 0xFFFFFFFF, i_max = 0.
+ *
+ * Enqueues two kernels and an 8 n_levels-byte copy to the host on `stream`, then synchronises `stream` (like
+ * mg_index_range, it returns values to the host).  The first call on each device also asks the runtime for the
+ * device address of the array (cudaGetSymbolAddress, with that device current; at most 64 devices): make that
+ * first call before any stream capture begins.  All calls on a device share the one array, which keeps whatever the
+ * previous call left; each call resets the pairs it uses first, so calls one after another are independent, but
+ * two calls whose kernels overlap on the same GPU (from two host threads or two streams) race on it and must be
+ * serialised by the caller.  Errors: MG_ERR_INVALID_ARG (NULL, n_levels out of range, decreasing offsets, device
+ * ordinal >= 64), MG_ERR_CUDA.
+ */
+#define MG_INDEX_RANGES_STATIC_MAX_LEVELS 32
+int mg_index_ranges_static(const uint32_t *idx_device, const uint64_t *level_offsets_host, uint32_t n_levels,
+                           uint32_t *i_min_host, uint32_t *i_max_host, void *stream);
+
 /* One-off encoder step (Table 1 row (A)): pack DEVICE uint32 indices (every value in
  * [i_min, i_min + 2^bits); a value outside is reduced modulo 2^bits and never touches its neighbours'
  * bits) into the DEVICE stream `packed_device` (16-byte aligned,

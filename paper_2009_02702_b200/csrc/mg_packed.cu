@@ -347,3 +347,127 @@ extern "C" int mg_colorize_packed(mg_graph* g, const void* packed_device, const 
     MG_CUDA(cudaGetLastError());
     return MG_OK;
 }
+
+// ------------------------------------------------------------------------------------------------
+// mg_index_ranges_static -- Eq. 15's (i_min, i_max) of EVERY level of a mipmap without allocating.
+//
+// mg_index_range above takes its 8 bytes of scratch (the two words the warps' atomicMin / atomicMax
+// meet in) from cudaMalloc and gives them back with cudaFree on every call.  Some callers cannot do
+// that: a renderer or a training process whose own arena already owns all of the device's memory (the
+// driver then has nothing left to hand out, or hands it out from the fragments the arena wanted
+// back), and a frame loop that cannot afford cudaFree's wait for every stream of the device between
+// a TF update and the next frame.  For them the scratch lives in the library image: one
+// (min, max) pair per level in a file-scope __device__ array, MG_INDEX_RANGES_STATIC_MAX_LEVELS
+// pairs = 256 bytes, resident on every GPU that loads libmg.so until the process exits.
+//
+// In host code `g_range_scratch` is only the symbol's host-side shadow, not a device address, so the
+// address the range kernel gets comes from cudaGetSymbolAddress, looked up once per device with that
+// device current (range_scratch_of_current_device).  The reset kernel is device code of this file and
+// names the array directly.  The array is shared by every call and keeps the previous call's pairs:
+// each call resets the pairs it will use before it reduces into them, and two calls whose kernels
+// overlap on one GPU (different host threads, different streams) would reduce into the same pairs.
+// ------------------------------------------------------------------------------------------------
+namespace {
+
+constexpr uint32_t kStaticLevels = MG_INDEX_RANGES_STATIC_MAX_LEVELS;
+constexpr int kStaticMaxDevices = 64;
+
+static __device__ __align__(256) uint32_t g_range_scratch[2 * kStaticLevels];
+
+struct RangeLevels {
+    uint64_t off[kStaticLevels + 1];   // level l = elements [off[l], off[l + 1]) of the index buffer
+    uint32_t n_levels;
+};
+
+// pair l starts at (UINT32_MAX, 0): the neutral elements of min and max
+__global__ void k_range_scratch_reset(uint32_t n_levels)
+{
+    const uint32_t l = threadIdx.x;
+    if (l < n_levels) { g_range_scratch[2 * l] = 0xFFFFFFFFu; g_range_scratch[2 * l + 1] = 0u; }
+}
+
+// k_index_range over several levels in one launch: every CTA walks the levels in turn and takes its grid-stride
+// share of each (16-byte streaming loads between the level's 16-byte boundaries, the ragged ends by CTA 0), then
+// one atomic pair per warp into the level's pair of `mm`.
+__global__ void __launch_bounds__(256) k_index_range_levels(const uint32_t* __restrict__ idx, const __grid_constant__ RangeLevels L,
+                                                            uint32_t* __restrict__ mm)
+{
+    const uint64_t stride = (uint64_t)gridDim.x * blockDim.x;
+    for (uint32_t l = 0; l < L.n_levels; l++) {
+        const uint64_t n = L.off[l + 1] - L.off[l];
+        if (n == 0) continue;                                             // uniform over the grid
+        const uint32_t* p = idx + L.off[l];
+        const mg::Span sp = mg::span_of(p, n);
+        const uint4* v4 = reinterpret_cast<const uint4*>(p + sp.head);
+        uint32_t lo = 0xFFFFFFFFu, hi = 0u;
+        for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < sp.nv; i += stride) {
+            const uint4 a = __ldcs(v4 + i);
+            lo = min(lo, min(min(a.x, a.y), min(a.z, a.w)));
+            hi = max(hi, max(max(a.x, a.y), max(a.z, a.w)));
+        }
+        if (blockIdx.x == 0 && threadIdx.x < sp.head + (n - sp.tail)) {
+            const uint32_t v = p[mg::ragged(sp, threadIdx.x)];
+            lo = min(lo, v); hi = max(hi, v);
+        }
+        lo = __reduce_min_sync(0xFFFFFFFFu, lo);
+        hi = __reduce_max_sync(0xFFFFFFFFu, hi);
+        if ((threadIdx.x & 31) == 0 && lo <= hi) { atomicMin(mm + 2 * l, lo); atomicMax(mm + 2 * l + 1, hi); }
+    }
+}
+
+std::atomic<uint32_t*> g_range_scratch_addr[kStaticMaxDevices];           // device address of g_range_scratch, per device
+
+// Set-up, once per device: ask the runtime where this device's instance of the array lives.
+int range_scratch_of_current_device(uint32_t** out)
+{
+    int dev = -1;
+    MG_CUDA(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= kStaticMaxDevices) {
+        mg::set_error("mg_index_ranges_static: device ordinal %d is beyond the %d this entry point keeps an address for", dev, kStaticMaxDevices);
+        return MG_ERR_INVALID_ARG;
+    }
+    uint32_t* p = g_range_scratch_addr[dev].load(std::memory_order_acquire);
+    if (!p) {
+        MG_CUDA(cudaGetSymbolAddress((void**)&p, g_range_scratch));      // the same answer from every thread: no lock needed
+        g_range_scratch_addr[dev].store(p, std::memory_order_release);
+    }
+    *out = p;
+    return MG_OK;
+}
+
+}  // namespace
+
+extern "C" int mg_index_ranges_static(const uint32_t* idx_device, const uint64_t* level_offsets_host, uint32_t n_levels,
+                                      uint32_t* i_min_host, uint32_t* i_max_host, void* stream)
+{
+    if (!idx_device || !level_offsets_host || !i_min_host || !i_max_host) { set_error("mg_index_ranges_static: NULL argument"); return MG_ERR_INVALID_ARG; }
+    if (n_levels == 0 || n_levels > kStaticLevels) {
+        set_error("mg_index_ranges_static: n_levels = %u, but the built-in scratch holds 1..%u levels (MG_INDEX_RANGES_STATIC_MAX_LEVELS); "
+                  "use mg_index_range per level beyond that", n_levels, kStaticLevels);
+        return MG_ERR_INVALID_ARG;
+    }
+    RangeLevels L;
+    memset(&L, 0, sizeof(L));
+    uint64_t longest = 0;
+    for (uint32_t l = 0; l <= n_levels; l++) {
+        L.off[l] = level_offsets_host[l];
+        if (l && L.off[l] < L.off[l - 1]) { set_error("mg_index_ranges_static: level_offsets must not decrease (level %u)", l - 1); return MG_ERR_INVALID_ARG; }
+        if (l && L.off[l] - L.off[l - 1] > longest) longest = L.off[l] - L.off[l - 1];
+    }
+    L.n_levels = n_levels;
+    uint32_t* d_mm = nullptr;
+    const int rc = range_scratch_of_current_device(&d_mm);
+    if (rc != MG_OK) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    k_range_scratch_reset<<<1, kStaticLevels, 0, st>>>(n_levels);
+    uint64_t blocks = (longest / 4 + 256) / 256;
+    if (blocks > 148ull * 8) blocks = 148ull * 8;
+    k_index_range_levels<<<(unsigned)blocks, 256, 0, st>>>(idx_device, L, d_mm);
+    count_launch(2);
+    MG_CUDA(cudaGetLastError());
+    uint32_t out[2 * kStaticLevels];
+    MG_CUDA(cudaMemcpyAsync(out, d_mm, 2 * sizeof(uint32_t) * n_levels, cudaMemcpyDeviceToHost, st));
+    MG_CUDA(cudaStreamSynchronize(st));
+    for (uint32_t l = 0; l < n_levels; l++) { i_min_host[l] = out[2 * l]; i_max_host[l] = out[2 * l + 1]; }
+    return MG_OK;
+}

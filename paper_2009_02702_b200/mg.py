@@ -28,7 +28,8 @@ ALL_LEVELS = 0xFFFFFFFF
 SYMBOLS = ["mg_load_graph", "mg_free_graph", "mg_graph_info", "mg_level_offsets", "mg_node_permutation",
            "mg_relabel_indices", "mg_check_indices", "mg_propagate", "mg_propagate_host", "mg_colorize", "mg_tf_update_host",
            "mg_last_error", "mg_kernel_launch_count",
-           "mg_bits_per_voxel", "mg_packed_stream_bytes", "mg_index_range", "mg_pack_indices", "mg_colorize_packed",
+           "mg_bits_per_voxel", "mg_packed_stream_bytes", "mg_index_range", "mg_index_ranges_static", "mg_pack_indices",
+           "mg_colorize_packed",
            "mg_propagate_attr", "mg_render", "mg_render_ex", "mg_ess_mask_build",
            "mg_mixture_lut_build", "mg_mixture_lut_free", "mg_mixture_lut_info", "mg_mixture_lut_export", "mg_range_query",
            "mg_mipmap_leaf_index", "mg_mipmap_front_level1", "mg_mipmap_levels_build", "mg_mixture_table_free",
@@ -82,6 +83,9 @@ lib.mg_packed_stream_bytes.argtypes = [C.c_uint64, C.c_uint32]
 lib.mg_packed_stream_bytes.restype = C.c_uint64
 lib.mg_index_range.argtypes = [_vp, C.c_uint64, C.POINTER(C.c_uint32), C.POINTER(C.c_uint32), _vp]
 lib.mg_index_range.restype = C.c_int
+MG_INDEX_RANGES_STATIC_MAX_LEVELS = 32
+lib.mg_index_ranges_static.argtypes = [_vp, _vp, C.c_uint32, _vp, _vp, _vp]
+lib.mg_index_ranges_static.restype = C.c_int
 lib.mg_pack_indices.argtypes = [_vp, C.c_uint64, C.c_uint32, C.c_uint32, _vp, _vp]
 lib.mg_pack_indices.restype = C.c_int
 lib.mg_colorize_packed.argtypes = [_vp, _vp, C.POINTER(MgPackedLevel), C.c_uint32, _vp, _vp, _vp, C.c_uint32, _vp]
@@ -208,6 +212,19 @@ def index_range(idx_device, n: int, stream: int = 0):
     lo, hi = C.c_uint32(), C.c_uint32()
     _check(lib.mg_index_range(_ptr(idx_device), int(n), C.byref(lo), C.byref(hi), stream or None), "mg_index_range")
     return int(lo.value), int(hi.value)
+
+
+def index_ranges_static(idx_device, level_offsets, stream: int = 0):
+    """(i_min[l], i_max[l]) of every level of a device index buffer through mg_index_ranges_static, the entry point for
+    callers that must not allocate device memory (their own arena owns it all, or a cudaFree stall is not affordable):
+    its scratch is a fixed array inside libmg.so, good for up to MG_INDEX_RANGES_STATIC_MAX_LEVELS levels.
+    ``level_offsets`` has one more entry than there are levels.  Synchronises ``stream``."""
+    off = np.ascontiguousarray(level_offsets, dtype=np.uint64)
+    n_levels = off.size - 1
+    lo, hi = np.empty(max(n_levels, 1), np.uint32), np.empty(max(n_levels, 1), np.uint32)
+    _check(lib.mg_index_ranges_static(_ptr(idx_device), off.ctypes.data, n_levels, lo.ctypes.data, hi.ctypes.data,
+                                      stream or None), "mg_index_ranges_static")
+    return lo[:n_levels], hi[:n_levels]
 
 
 def pack_indices(idx_device, n: int, i_min: int, bits: int, packed_device, stream: int = 0) -> None:
