@@ -34,7 +34,9 @@ NOMINAL_HBM_GBS = 8000.0             # BASELINE.json north_star "~8 TB/s"
 BYTES_PER_VOXEL = {"rgba8": 8, "rgba16f": 12}       # 4 B index + 4 B (8 B) output
 BYTES_PER_NODE_L2 = 28               # 12 B a/b/w stream + 16 B colour store (gathers hit L2), §8(d)
 BYTES_PER_NODE_DRAM = 60             # + two 16-B gathers when the fp32 palette exceeds L2 (config 5), §8(d)
-BYTES_GATHER_BEYOND_L2 = 16          # §8(d): per-voxel palette gather, counted only when the palette exceeds L2 (config 5)
+BYTES_GATHER_BEYOND_L2 = {"rgba8": 4, "rgba16f": 8}    # per-voxel palette gather, counted only when the palette exceeds L2 (config 5):
+                                                        # the entry the kernel really reads (RGBA8 / 4 x fp16 palette), not the 16-B
+BYTES_GATHER_SURVEY = 16                                # fp32 entry SURVEY.md §8(d) counts (kept beside it as *_survey)
 L2_BYTES = 126e6
 
 
@@ -464,6 +466,12 @@ def run_b200(args) -> dict:
                              "samples_one_leaf_shortcut": un_, "samples_per_s": (ev_ + sk_) / (ms * 1e-3),
                              "ess_mask": bool(use_mask and mask is not None)}
         render["ess_speedup"] = render["no_ess"]["ms_per_frame"] / render["ess"]["ms_per_frame"]
+        # ESS only pays where most samples can be skipped: report the fraction it skipped in this view next to the ratio, and
+        # which of the two kernels a caller should run here (the faster one; both produce the same image)
+        e_ = render["ess"]
+        render["ess_skippable_fraction"] = e_["samples_skipped"] / max(1, e_["samples_skipped"] + e_["samples_composited"])
+        render["ess_pays_in_this_view"] = bool(render["ess_speedup"] > 1.0)
+        render["best_ms_per_frame"] = min(render["ess"]["ms_per_frame"], render["no_ess"]["ms_per_frame"])
         del mask
         render["histogram_mipmap_flag_speedup"] = render["no_ess_generic_mipmap"]["ms_per_frame"] / render["no_ess"]["ms_per_frame"]
         render["coverage"] = float((img[..., 3] > 0).float().mean().item())
@@ -547,8 +555,9 @@ def run_b200(args) -> dict:
     peak, peak_src = peak_hbm_gbs()
     bpv = BYTES_PER_VOXEL[args.format]
     beyond_l2 = 16.0 * n_nodes > L2_BYTES                 # the fp32 palette (16 B per node) does not fit L2: config 5 only
+    bpv_survey = bpv + BYTES_GATHER_SURVEY
     if beyond_l2:
-        bpv += BYTES_GATHER_BEYOND_L2
+        bpv += BYTES_GATHER_BEYOND_L2[args.format]
     col_avg = float(col_ms.mean())
     prop_avg = float(prop_ms.mean())
     algo_bytes = float(bpv) * w.n_voxels * (n_part / max(1, w.n_voxels_padded))      # rank 0's share (all of it unless --partition slab)
@@ -563,6 +572,9 @@ def run_b200(args) -> dict:
         roofline["kernel"] = kernel = "k_colorize_tile"
         roofline["traffic"] = ncu_traffic(w.name, kernel)
         roofline["launches_per_step"] = col_launches
+    if beyond_l2:
+        roofline["algorithmic_bytes_per_voxel_survey"] = bpv_survey
+        roofline["achieved_at_survey_bytes"] = achieved * bpv_survey / bpv
         roofline["note"] = ("palette beyond the L2: one sweep per palette tile (<= 88 MB); achieved = the algorithmic bytes of the whole "
                             "colourise / the time of all its sweeps; traffic = DRAM bytes of all sweeps")
     prop_roofline = None

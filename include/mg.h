@@ -174,7 +174,8 @@ int mg_propagate_host(mg_graph *g, const float *tf_rgba_host, float *node_rgba, 
  *
  * An RGBA8 palette beyond what the L2 serves for random gathers (more than 88 MB = 23 M nodes, up to 4 x that) is
  * gathered tile by tile: the call then enqueues one sweep over the indices per palette tile (MG_COLORIZE_TILE_BYTES
- * in the environment overrides the 88-MB tile size), each merging its voxels into out_rgba, so out_rgba is READ as
+ * in the environment of mg_load_graph overrides the 88-MB tile size for that graph; it is not consulted afterwards),
+ * each merging its voxels into out_rgba, so out_rgba is READ as
  * well as written between the sweeps and must not be touched by another stream's work meanwhile.
  */
 int mg_colorize(mg_graph *g, uint32_t mip_level, const uint32_t *node_idx_volume,
@@ -516,9 +517,18 @@ int mg_mipmap_front_level1(const uint32_t *level0_device, uint64_t X, uint64_t Y
  *   levels_device   DEVICE uint32 buffer; level l >= 1 is written at levels_device + level_offset[l] (handles, x fastest)
  *   level_offset    HOST uint64[n_levels] in voxels ([0] is not used); n_levels = length of the ceil-halving chain (L80)
  *   out             the mixture store (device memory owned by the table; mg_mixture_table_free)
- * Allocates (stores sized from the number of level-1 merges: MG_ERR_OOM if a later level overflows them) and
- * synchronises `stream` several times per level.  Errors: MG_ERR_INVALID_ARG (NULL, dims / n_levels mismatch, level 1
- * with >= 2^32 voxels, a 64-bit hash collision between different mixtures), MG_ERR_OOM, MG_ERR_CUDA.
+ * Allocates (stores sized once, from the number of level-1 merges: 1.5 merges + 2^20 mixtures, 12 per merge + 2^22
+ * entries) and synchronises `stream` several times per level.  A level whose mixtures do not fit the stores is not an
+ * error: like a level with oversized mixtures it is left to the host together with the levels above it (a
+ * nearest-neighbour-upsampled volume, whose level 1 is pure and whose level 2 holds all the merges, is such a case).
+ * Everything in levels_device at or above level levels_done + 1 is scratch on return (half-written handles).
+ * Errors: MG_ERR_INVALID_ARG (NULL, dims / n_levels mismatch, level 1 with >= 2^32 voxels, a 64-bit hash collision
+ * between different mixtures), MG_ERR_OOM (a device allocation failed), MG_ERR_CUDA.
+ *
+ * mg_mipmap_levels_build_ex is the same call with the store capacities stated by the caller (cap_mixtures distinct
+ * mixtures, cap_entries (leaf, count) entries; 0 = the default sizing above) -- to reserve more for data whose upper
+ * levels are known to keep merging, or to bound the device memory the table may take (24 B per mixture + 40 B per
+ * hash slot, 2 .. 4 slots per mixture; 12 B per entry).
  */
 typedef struct mg_mixture_table mg_mixture_table;
 
@@ -534,6 +544,9 @@ typedef struct mg_mixture_table_info_t {
 int mg_mipmap_levels_build(const uint32_t *level0_device, uint64_t X, uint64_t Y, uint64_t Z, uint32_t n_leaves,
                            uint32_t *levels_device, const uint64_t *level_offset, uint32_t n_levels,
                            mg_mixture_table **out, void *stream);
+int mg_mipmap_levels_build_ex(const uint32_t *level0_device, uint64_t X, uint64_t Y, uint64_t Z, uint32_t n_leaves,
+                              uint32_t *levels_device, const uint64_t *level_offset, uint32_t n_levels,
+                              uint64_t cap_mixtures, uint64_t cap_entries, mg_mixture_table **out, void *stream);
 void mg_mixture_table_free(mg_mixture_table *t);
 int mg_mixture_table_info(const mg_mixture_table *t, mg_mixture_table_info_t *info);
 

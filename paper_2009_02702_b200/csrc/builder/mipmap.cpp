@@ -293,7 +293,7 @@ int build_mipmap(const uint32_t* seg, uint64_t X, uint64_t Y, uint64_t Z, int n_
             return MGB_ERR_INVALID_ARG;
         }
         bool bad = false;
-#pragma omp parallel reduction(+ : nnz_level)
+#pragma omp parallel reduction(+ : nnz_level) reduction(|| : bad)
         {
             std::vector<Entry> buf, merged;
 #pragma omp for schedule(dynamic, 1024)
@@ -335,19 +335,22 @@ int build_mipmap(const uint32_t* seg, uint64_t X, uint64_t Y, uint64_t Z, int n_
         if (Ld == 0 || Ld >= n_levels) { set_error("histogram mipmap: level_done = %u is not a level 1 .. %u", Ld, n_levels - 1); return MGB_ERR_INVALID_ARG; }
         front_handle.assign(levels->n_mix, 0);
         bool bad = false;
-#pragma omp parallel
+#pragma omp parallel reduction(|| : bad)
         {
             std::vector<Entry> e;
 #pragma omp for schedule(dynamic, 1024)
             for (int64_t q = 0; q < (int64_t)levels->n_mix; q++) {
                 const uint64_t o = levels->mix_offset[q];
                 const uint32_t k = levels->mix_k[q];
-                bool ok = k >= 2 && o + k <= levels->n_entries && (levels->mix_first_pos[q] >> 40) >= 1 && (levels->mix_first_pos[q] >> 40) <= Ld;
+                // the caller's arrays are checked before anything is sized or shifted by them
+                bool ok = k >= 2 && k <= levels->n_entries && o <= levels->n_entries - k && levels->mix_tlog[q] < 64 &&
+                          (levels->mix_first_pos[q] >> 40) >= 1 && (levels->mix_first_pos[q] >> 40) <= Ld;
+                if (!ok) { bad = true; continue; }
                 uint64_t total = 0;
                 e.resize(k);
                 for (uint32_t t = 0; ok && t < k; t++) {
                     e[t] = Entry{levels->leaf[o + t], 0, levels->count[o + t]};
-                    ok = e[t].leaf < n_leaves && e[t].count > 0 && (t == 0 || e[t].leaf > e[t - 1].leaf);
+                    ok = e[t].leaf < n_leaves && e[t].count > 0 && (t == 0 || e[t].leaf > e[t - 1].leaf) && total + e[t].count >= total;
                     total += e[t].count;
                 }
                 ok = ok && total == (1ull << levels->mix_tlog[q]);
@@ -361,7 +364,7 @@ int build_mipmap(const uint32_t* seg, uint64_t X, uint64_t Y, uint64_t Z, int n_
         out.level_ids[Ld].resize(nd);
         uint32_t* P = out.level_ids[Ld].data();
         bool bad_handle = false;
-#pragma omp parallel for schedule(static)
+#pragma omp parallel for schedule(static) reduction(|| : bad_handle)
         for (int64_t v = 0; v < (int64_t)nd; v++) {
             const uint32_t h = levels->handles[v];
             if (h & kMixed) {

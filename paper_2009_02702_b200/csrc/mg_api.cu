@@ -4,6 +4,7 @@
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 
@@ -170,6 +171,10 @@ extern "C" int mg_load_graph(const uint32_t* child_a, const uint32_t* child_b, c
     g->n_nodes = n_nodes;
     g->n_leaves = n_leaves;
     g->no_palettes = (flags & MG_NO_PALETTES) != 0;
+    if (const char* e = getenv("MG_COLORIZE_TILE_BYTES")) {               // read here, once per graph: never on the update path
+        const long long v = atoll(e);
+        if (v > 0) g->pal_tile_bytes = (uint64_t)v;
+    }
     if (leaf_segment_id) g->leaf_segment_id.assign(leaf_segment_id, leaf_segment_id + n_leaves);
 
     std::vector<uint32_t> ha, hb;

@@ -108,17 +108,9 @@ k_colorize(const uint4* __restrict__ idx4, uint64_t n_vec, const uint32_t* __res
 // (256 MB) 1 sweep 2.06 ms, 2 -> 1.60, 3 -> 1.43, 4 -> 1.53, 8 -> 2.14.  L2 eviction-priority hints (evict_last on the
 // gathers, evict_first on the streams) changed nothing.  The fp16 palette (8 B per node, twice the sweeps, 16-B output
 // per voxel) never gained: it always takes the single sweep.
-constexpr uint64_t kTileBytes = 88ull << 20;
+// The tile size is a property of the graph object (mg_graph::pal_tile_bytes = MG_DEFAULT_PAL_TILE_BYTES, 88 MB, unless
+// MG_COLORIZE_TILE_BYTES was set in the environment when mg_load_graph ran): nothing is looked up per call.
 constexpr uint32_t kMaxTiles = 4;                     // beyond that the T streaming sweeps cost more than the DRAM gathers
-
-// MG_COLORIZE_TILE_BYTES in the environment overrides kTileBytes (tuning on other parts; the tests use it to drive
-// the tiled path with small palettes).
-inline uint64_t tile_bytes()
-{
-    const char* e = getenv("MG_COLORIZE_TILE_BYTES");
-    const long long v = e ? atoll(e) : 0;
-    return v > 0 ? (uint64_t)v : kTileBytes;
-}
 
 __device__ __forceinline__ uint4 ld_cg_u4(const uint4* p)
 {
@@ -157,9 +149,8 @@ k_colorize_tile(const uint4* __restrict__ idx4, uint64_t n_vec, const uint32_t* 
 }
 
 // Number of RGBA8 palette tiles: 1 = the palette fits (or is too large to gain), plain single-sweep kernel.
-inline uint32_t palette_tiles(uint64_t n_nodes, uint64_t n_vec)
+inline uint32_t palette_tiles(uint64_t tb, uint64_t n_nodes, uint64_t n_vec)
 {
-    const uint64_t tb = tile_bytes();
     const uint64_t t = (n_nodes * 4 + tb - 1) / tb;
     if (t < 2 || t > kMaxTiles) return 1;
     if (n_vec * 4 < n_nodes / 4) return 1;           // few voxels: they touch a small part of the palette once
@@ -206,7 +197,7 @@ int launch_colorize(const mg_graph* g, const uint32_t* idx, uint64_t n, uint32_t
         // path (ld.global.nc, L1-cached), which is only safe behind a full kernel boundary -- measured: with
         // PDL a back-to-back update read stale palette lines (tests/test_gpu_parity.py::test_back_to_back...).
         const uint4* idx4 = reinterpret_cast<const uint4*>(idx + head);
-        const uint32_t t8 = W8 ? palette_tiles(g->n_nodes, n_vec) : 1;
+        const uint32_t t8 = W8 ? palette_tiles(g->pal_tile_bytes, g->n_nodes, n_vec) : 1;
         if (t8 == 1) {
             k_colorize<W8, W16><<<(unsigned)blocks, kThreads, 0, st>>>(
                 idx4, n_vec, g->d_pal8, g->d_pal16,

@@ -13,6 +13,8 @@
 // Single-CTA tail kernel limits (mg_api.cu plans against them, mg_propagate.cu sizes its buffers with them).
 #define MG_TAIL_SMEM_BYTES (224 * 1024)
 #define MG_TAIL_MAX_LEVELS 128
+// RGBA8 palette tile of the tiled colourise (mg_colorize.cu): what the L2 serves for random gathers
+#define MG_DEFAULT_PAL_TILE_BYTES (88ull << 20)
 
 namespace mg {
 
@@ -92,6 +94,7 @@ struct mg_graph {
     // since; nullptr otherwise.  Only consulted to reject a wrong MG_PALETTE_FROM_LAST_PROPAGATE (mg_colorize).
     const float* pal_src = nullptr;
     bool no_palettes = false;              // MG_NO_PALETTES: mg_propagate does not derive the palettes
+    uint64_t pal_tile_bytes = MG_DEFAULT_PAL_TILE_BYTES;   // fixed at mg_load_graph (MG_COLORIZE_TILE_BYTES in its environment)
     // launch plan: levels >= first_fused_level run in the single-CTA tail kernel (0 = none).  The tail
     // works entirely in shared memory on LOCAL indices: [0, tail_n_ext) = the distinct children that lie
     // below the tail ("external": gathered once), [tail_n_ext, tail_n_ext + tail_n) = the tail's nodes.

@@ -407,9 +407,9 @@ extern "C" void mg_mixture_table_free(mg_mixture_table* t)
     delete t;
 }
 
-extern "C" int mg_mipmap_levels_build(const uint32_t* level0_device, uint64_t X, uint64_t Y, uint64_t Z, uint32_t n_leaves,
-                                      uint32_t* levels_device, const uint64_t* level_offset, uint32_t n_levels,
-                                      mg_mixture_table** out, void* stream)
+extern "C" int mg_mipmap_levels_build_ex(const uint32_t* level0_device, uint64_t X, uint64_t Y, uint64_t Z, uint32_t n_leaves,
+                                         uint32_t* levels_device, const uint64_t* level_offset, uint32_t n_levels,
+                                         uint64_t cap_mixtures, uint64_t cap_entries, mg_mixture_table** out, void* stream)
 {
     if (!out) { mg::set_error("mg_mipmap_levels_build: out is NULL"); return MG_ERR_INVALID_ARG; }
     *out = nullptr;
@@ -454,7 +454,7 @@ extern "C" int mg_mipmap_levels_build(const uint32_t* level0_device, uint64_t X,
     MT_CUDA(cudaGetDevice(&T->device));
     MT_CUDA(dalloc(T, &T->d_ctr, (uint64_t)kNCtr));
     MT_CUDA(cudaMemsetAsync(T->d_ctr, 0, kNCtr * sizeof(unsigned long long), st));
-    unsigned long long ctr[kNCtr];
+    unsigned long long ctr[kNCtr] = {};                                   // (level 1 fills only two of them on the host)
     for (uint32_t l = 1; l < n_levels; l++) {
         LevelGeom G;
         G.cx = (uint32_t)dims[3 * l - 3]; G.cy = (uint32_t)dims[3 * l - 2]; G.cz = (uint32_t)dims[3 * l - 1];
@@ -503,9 +503,10 @@ extern "C" int mg_mipmap_levels_build(const uint32_t* level0_device, uint64_t X,
             list_cap = (uint32_t)ctr[kNPending];
         }
         if (l == 1) {
-            // the stores are sized once, from the number of level-1 merges (later levels add little: 1/8 of the voxels each)
-            T->cap_m = (uint64_t)n_pending + n_pending / 2 + (1u << 20);
-            T->cap_e = 12ull * n_pending + (1u << 22);
+            // the stores are sized once: by the caller, or from the number of level-1 merges (on segmentations with coherent
+            // regions later levels add little: 1/8 of the voxels each).  A level that does not fit is the host's (below).
+            T->cap_m = cap_mixtures ? cap_mixtures : (uint64_t)n_pending + n_pending / 2 + (1u << 20);
+            T->cap_e = cap_entries ? cap_entries : 12ull * n_pending + (1u << 22);
             T->cap_h = 1;
             while (T->cap_h < 2 * T->cap_m) T->cap_h <<= 1;
             MT_CUDA(dalloc(T, &T->d_off, T->cap_m)); MT_CUDA(dalloc(T, &T->d_k, T->cap_m)); MT_CUDA(dalloc(T, &T->d_tlog, T->cap_m));
@@ -558,8 +559,13 @@ extern "C" int mg_mipmap_levels_build(const uint32_t* level0_device, uint64_t X,
             MT_CUDA(cudaMemcpyAsync(ctr, T->d_ctr, sizeof(ctr), cudaMemcpyDeviceToHost, st));
             MT_CUDA(cudaStreamSynchronize(st));
             if (ctr[kFlags] & (kStoreFull | kTableFull)) {
-                mg::set_error("mg_mipmap_levels_build: mixture store full at level %u (%llu mixtures, %llu entries)", l, ctr[kNMix], ctr[kNEnt]);
-                return fail(MG_ERR_OOM);
+                // The level's mixtures do not fit the stores.  What it published sits beyond n_mix / n_ent of the finished
+                // levels and is never exported; its handles are scratch.  Like a kTooBig level, it and the levels above it
+                // go to the host (mgb_build_from_levels continues from levels_done = l - 1).
+                MT_CUDA(cudaMemcpyAsync(T->d_ctr + kNnz, &nnz_before, sizeof(nnz_before), cudaMemcpyHostToDevice, st));
+                MT_CUDA(cudaStreamSynchronize(st));                       // (nnz_before is a local of this iteration)
+                drop_level();
+                break;
             }
             if (ctr[kFlags] & kCollision) {
                 mg::set_error("mg_mipmap_levels_build: two different mixtures share a 64-bit hash at level %u: use the host builder", l);
@@ -575,6 +581,13 @@ extern "C" int mg_mipmap_levels_build(const uint32_t* level0_device, uint64_t X,
 #undef MT_CUDA
     *out = T;
     return MG_OK;
+}
+
+extern "C" int mg_mipmap_levels_build(const uint32_t* level0_device, uint64_t X, uint64_t Y, uint64_t Z, uint32_t n_leaves,
+                                      uint32_t* levels_device, const uint64_t* level_offset, uint32_t n_levels,
+                                      mg_mixture_table** out, void* stream)
+{
+    return mg_mipmap_levels_build_ex(level0_device, X, Y, Z, n_leaves, levels_device, level_offset, n_levels, 0, 0, out, stream);
 }
 
 extern "C" int mg_mixture_table_info(const mg_mixture_table* t, mg_mixture_table_info_t* info)

@@ -32,7 +32,8 @@ SYMBOLS = ["mg_load_graph", "mg_free_graph", "mg_graph_info", "mg_level_offsets"
            "mg_colorize_packed",
            "mg_propagate_attr", "mg_render", "mg_render_ex", "mg_ess_mask_build",
            "mg_mixture_lut_build", "mg_mixture_lut_free", "mg_mixture_lut_info", "mg_mixture_lut_export", "mg_range_query",
-           "mg_mipmap_leaf_index", "mg_mipmap_front_level1", "mg_mipmap_levels_build", "mg_mixture_table_free",
+           "mg_mipmap_leaf_index", "mg_mipmap_front_level1", "mg_mipmap_levels_build", "mg_mipmap_levels_build_ex",
+           "mg_mixture_table_free",
            "mg_mixture_table_info", "mg_mixture_table_export", "mg_mipmap_remap_handles"]
 
 
@@ -160,6 +161,9 @@ class MgMixtureTableInfo(C.Structure):
 
 lib.mg_mipmap_levels_build.argtypes = [_vp, C.c_uint64, C.c_uint64, C.c_uint64, C.c_uint32, _vp, _vp, C.c_uint32, C.POINTER(_vp), _vp]
 lib.mg_mipmap_levels_build.restype = C.c_int
+lib.mg_mipmap_levels_build_ex.argtypes = [_vp, C.c_uint64, C.c_uint64, C.c_uint64, C.c_uint32, _vp, _vp, C.c_uint32, C.c_uint64, C.c_uint64,
+                                          C.POINTER(_vp), _vp]
+lib.mg_mipmap_levels_build_ex.restype = C.c_int
 lib.mg_mixture_table_free.argtypes = [_vp]
 lib.mg_mixture_table_free.restype = None
 lib.mg_mixture_table_info.argtypes = [_vp, C.POINTER(MgMixtureTableInfo)]
@@ -266,13 +270,19 @@ def mipmap_front_level1(level0_device, dims_xyz, level1_device, mixed_voxel_devi
 class MixtureTable:
     """Device mixture store of mg_mipmap_levels_build (the levels >= 1 of the histogram mipmap built on the device)."""
 
-    def __init__(self, level0_device, dims_xyz, n_leaves: int, levels_device, level_offsets, stream: int = 0):
+    def __init__(self, level0_device, dims_xyz, n_leaves: int, levels_device, level_offsets, stream: int = 0,
+                 cap_mixtures: int = 0, cap_entries: int = 0):
         X, Y, Z = (int(d) for d in dims_xyz)
         off = np.ascontiguousarray(level_offsets, dtype=np.uint64)
         h = _vp()
         self._h = None
-        _check(lib.mg_mipmap_levels_build(_ptr(level0_device), X, Y, Z, int(n_leaves), _ptr(levels_device), off.ctypes.data,
-                                          int(off.size), C.byref(h), stream or None), "mg_mipmap_levels_build")
+        if cap_mixtures or cap_entries:
+            _check(lib.mg_mipmap_levels_build_ex(_ptr(level0_device), X, Y, Z, int(n_leaves), _ptr(levels_device), off.ctypes.data,
+                                                 int(off.size), int(cap_mixtures), int(cap_entries), C.byref(h), stream or None),
+                   "mg_mipmap_levels_build_ex")
+        else:
+            _check(lib.mg_mipmap_levels_build(_ptr(level0_device), X, Y, Z, int(n_leaves), _ptr(levels_device), off.ctypes.data,
+                                              int(off.size), C.byref(h), stream or None), "mg_mipmap_levels_build")
         self._h = h
         self.info = MgMixtureTableInfo()
         _check(lib.mg_mixture_table_info(self._h, C.byref(self.info)), "mg_mixture_table_info")

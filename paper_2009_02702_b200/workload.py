@@ -159,12 +159,14 @@ def from_volume(seg: np.ndarray, name: str = "volume", cfg: dict | None = None, 
     return w
 
 
-def from_volume_device_levels(seg_dev, name: str = "volume", cfg: dict | None = None, **builder_params) -> Workload:
+def from_volume_device_levels(seg_dev, name: str = "volume", cfg: dict | None = None, store_capacity=(0, 0),
+                              **builder_params) -> Workload:
     """``from_volume_device`` with the levels >= 1 of the histogram mipmap built on the device too
     (mg_mipmap_levels_build: merge + hash-cons per level, as far up as the mixtures stay small), the host builder
     continuing above the last finished level (mgb_build_from_levels) and the device-built levels turned into node
     indices in place (mg_mipmap_remap_handles).  Same graph and node indices as ``from_volume``; ``host_idx[l]`` is None
-    for the levels below the last device-built one."""
+    for the levels below the last device-built one.  ``store_capacity`` = (mixtures, entries) of the device store
+    (mg_mipmap_levels_build_ex; 0 = the library's sizing): a level that does not fit is continued on the host."""
     import torch
     w = Workload(name)
     w.cfg = dict(cfg or {})
@@ -179,7 +181,8 @@ def from_volume_device_levels(seg_dev, name: str = "volume", cfg: dict | None = 
     w.d_idx = torch.zeros(w.n_voxels_padded, dtype=torch.int32, device="cuda")
     n0 = w.level_voxels[0]
     ids = mg.mipmap_leaf_index(seg_dev, n0, w.d_idx[:n0], stream=st)
-    table = mg.MixtureTable(w.d_idx, dims[0], ids.size, w.d_idx, w.level_start, stream=st) if len(dims) > 1 else None
+    table = mg.MixtureTable(w.d_idx, dims[0], ids.size, w.d_idx, w.level_start, stream=st, cap_mixtures=store_capacity[0],
+                            cap_entries=store_capacity[1]) if len(dims) > 1 else None
     Ld = int(table.info.levels_done) if table is not None else 0
     if Ld == 0:                                    # nothing for the device to do (1 x 1 x 1, or huge mixtures at level 1)
         if table is not None:

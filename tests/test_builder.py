@@ -339,3 +339,18 @@ def test_build_from_levels_rejects_malformed_input():
         builder.build_from_levels(dims, ids, 1, h, mix, nnz)
     with pytest.raises(builder.BuilderError):                                      # level_done beyond the chain
         builder.build_from_levels(dims, ids, 9, handles[0], mix, nnz)
+    # corrupt descriptors must be refused before they size or shift anything
+    def with_(key, q, value):
+        m = {k: v.copy() for k, v in mix.items()}
+        m[key][q] = value
+        return m
+    for bad in (with_("tlog", 1, 64), with_("tlog", 0, 0xFFFFFFFF),                # a shift by >= 64 bits
+                with_("k", 1, 0xFFFFFFF0),                                         # 4 G entries for one mixture
+                with_("offset", 2, mix["leaf"].size),                              # starts behind the entries
+                with_("offset", 0, 2 ** 64 - 1),                                   # offset + k wraps around
+                with_("k", 0, 1), with_("first_pos", 0, 5), with_("first_pos", 1, (2 << 40) | 1)):   # k < 2; level 0 / 2 of a level-1 front
+        with pytest.raises(builder.BuilderError) as ei:
+            builder.build_from_levels(dims, ids, 1, handles[0], bad, nnz)
+        assert "malformed" in str(ei.value)
+    b, _ = builder.build_from_levels(dims, ids, 1, handles[0], mix, nnz)           # (the untouched input is accepted)
+    b.close()

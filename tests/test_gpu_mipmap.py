@@ -192,6 +192,31 @@ def test_device_levels_ragged_and_crowded_volumes(libs, dims, n_seg):
         b.close()
 
 
+@pytest.mark.parametrize("upsampled,cap,done", [(True, (100, 800), 1), (True, (0, 300), 1), (False, (64, 0), 0)])
+def test_device_levels_store_overflow_goes_to_the_host(libs, upsampled, cap, done):
+    """A level whose mixtures do not fit the device store is handed to the host with the levels above it, not reported as
+    an error.  The case that reaches this with the default sizing is a nearest-neighbour 2x-upsampled volume: level 1 is
+    pure throughout (no merge to size the stores from) and level 2 holds every merge; small explicit capacities
+    (mg_mipmap_levels_build_ex) bring it to a size a test can afford -- too few mixtures, too few entries, and a noise
+    volume whose level 1 already overflows (nothing built on the device).  Same graph and indices as the host builder."""
+    mg, workload = libs
+    n = 20
+    small = (synth.u64(72, 3, np.arange(n ** 3, dtype=np.uint64)) % np.uint64(150)).astype(np.uint32).reshape(n, n, n) * 2 + 1
+    seg = np.repeat(np.repeat(np.repeat(small, 2, 0), 2, 1), 2, 2) if upsampled else small
+    if upsampled:
+        ids, l0 = oracle.leaf_index(seg)
+        H = oracle.histogram_mipmap(l0, ids.size)
+        assert ((H[1] != 0).sum(axis=-1) == 1).all() and ((H[2] != 0).sum(axis=-1) > 1).mean() > 0.99
+    a = workload.from_volume(seg, name="overflow")
+    b = workload.from_volume_device_levels(_dev(seg).view(*seg.shape), name="overflow", store_capacity=cap)
+    try:
+        _same_assembly(a, b)
+        assert b.stats.get("device_levels_done", 0) == done
+    finally:
+        a.close()
+        b.close()
+
+
 def test_mixture_table_matches_the_oracle_histograms(libs):
     """mg_mipmap_levels_build against the definition, not against the host builder: every handle of every finished level
     expands to the oracle's exact integer histogram of that voxel (Eq. 4, O-2) divided by its common power of two; equal
@@ -249,4 +274,10 @@ def test_levels_build_error_paths(libs):
     assert t.info.levels_done == 3 and t.info.n_mixtures == 0 and t.info.nnz_levels == 64 + 8 + 1
     assert not buf.cpu().numpy().any()
     assert all(v.size == 0 for v in t.export().values())
+    t.close()
+    # a pure 2 x 2 x 2 volume: two levels, so no level ever reads the device counters back -- the table is still empty
+    buf2 = torch.full((8 + 1,), 5, dtype=torch.int32, device="cuda")
+    t = mg.MixtureTable(l0, (2, 2, 2), 1, buf2, np.array([0, 8], dtype=np.uint64))
+    assert t.info.levels_done == 1 and t.info.n_mixtures == 0 and t.info.n_entries == 0 and t.info.nnz_levels == 1
+    assert int(buf2[8]) == 0 and all(v.size == 0 for v in t.export().values())
     t.close()
