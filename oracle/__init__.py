@@ -10,6 +10,7 @@ Function -> passage (PAPER.md line):
   leaf_index           Q14  L76, L130 (sources = the segment IDs present)
   histogram_mipmap     O-2  Eq. 4 L78-L80 (integer counts scaled to 8^l)
   direct_colour        O-2  L66 (<m, x>)
+  direct_colour_level  O-3c L66 with Eq. 4 unrolled: every voxel of a level, no histogram table
   brute_force_histogram O-3 Eq. 4 unrolled
   brute_force_level    O-3 for every voxel of one level in one pass over the finest voxels
   symbolic_eval_sparse O-5 on a sparse matrix, level by level (full-size graphs; a scipy sparse product per level)
@@ -57,6 +58,8 @@ _lib.mgo_brute_force_histogram.argtypes = [_u32p, _u64, _u64, _u64, _u32, _u32, 
 _lib.mgo_brute_force_histogram.restype = None
 _lib.mgo_brute_force_level.argtypes = [_u32p, _u64, _u64, _u64, _u32, _u32, _f64p]
 _lib.mgo_brute_force_level.restype = None
+_lib.mgo_direct_colour_level.argtypes = [_u32p, _u64, _u64, _u64, _f64p, _u32, _u64, _u64, _f64p]
+_lib.mgo_direct_colour_level.restype = None
 _lib.mgo_graph_eval.argtypes = [_u32p, _u32p, _f64p, _u64, _u64, _f64p, _f64p]
 _lib.mgo_graph_eval.restype = None
 _lib.mgo_graph_eval_attr.argtypes = [_u32p, _u32p, _f64p, _u64, _u64, _u32, _f64p, _f64p]
@@ -165,6 +168,21 @@ def brute_force_level(seg_index, n_seg, level):
     h = np.zeros((zl, yl, xl, n_seg), dtype=np.float64)
     _lib.mgo_brute_force_level(seg_index.reshape(-1), X, Y, Z, n_seg, level, h.reshape(-1))
     return h
+
+
+def direct_colour_level(seg_index, tf, level, k_begin=0, k_end=None):
+    """C_dir = sum_s H[s] TF[s] of EVERY voxel of the coarse z-slabs [k_begin, k_end) of ``level``, accumulated finest
+    voxel by finest voxel with the unrolled weights of Eq. 4 (O-3c; no histogram table, so it runs at full size):
+    fp64 [k_end - k_begin, Y_l, X_l, 4]."""
+    seg_index = _c(seg_index, np.uint32)
+    tf = _c(tf, np.float64)
+    Z, Y, X = seg_index.shape
+    xl, yl, zl = mip_dims((X, Y, Z))[level]
+    k_end = zl if k_end is None else int(k_end)
+    assert 0 <= k_begin <= k_end <= zl and tf.ndim == 2 and tf.shape[1] == 4
+    out = np.zeros((k_end - k_begin, yl, xl, 4), dtype=np.float64)
+    _lib.mgo_direct_colour_level(seg_index.reshape(-1), X, Y, Z, tf.reshape(-1), level, k_begin, k_end, out.reshape(-1))
+    return out
 
 
 def graph_eval(child_a, child_b, weight, n_leaves, tf):

@@ -9,7 +9,7 @@
  * load it.  No blocking, fusion or reordering beyond what each cited definition states.
  *
  * Pins (tests/test_oracle_*.py, -m "not gpu"): Table 2 voxel totals (O-1), brute force vs
- * recursion and the textbook box filter (O-2/O-3), Fig. 2 / Fig. 4 worked examples and closed-form
+ * recursion and the textbook box filter (O-2/O-3/O-3c), Fig. 2 / Fig. 4 worked examples and closed-form
  * chains (O-4), mu . TF == colour and row sums (O-5), known values for the output conversions;
  * hand-worked rays / scipy map_coordinates / Beer-Lambert closed forms (ray-marcher, R1-R6); Table 4's fetch
  * counts, brute-force tilings, np.bincount and the sum-to-volume identity (range queries); a hand-worked
@@ -177,6 +177,53 @@ void mgo_brute_force_level(const uint32_t *seg_index, uint64_t x0, uint64_t y0, 
                     row[(x >> l) * n_seg + s[x]] += wx[x] * wzy;
             }
     }
+    free(wx);
+    free(wy);
+    free(wz);
+}
+
+/* ---- O-3c: the COLOUR of every voxel of level l straight from the definition, for volumes whose dense histogram
+ * table would not fit: C_dir(i,j,k,l) = <H(i,j,k,l), TF> = sum_s H(i,j,k,l)[s] TF[s] (L66 with the histogram of Eq. 4,
+ * L78-L80).  With H unrolled as in O-3 -- finest voxel (x,y,z) contributes wx(x) wy(y) wz(z) to bin S(x,y,z) of its
+ * level-l ancestor -- the sum over bins becomes a sum over the ancestor's finest voxels,
+ *     C_dir(i,j,k,l) = sum_{(x,y,z): x>>l == i, y>>l == j, z>>l == k}  wx(x) wy(y) wz(z) TF[S(x,y,z)],
+ * which is what is accumulated here, one finest voxel after the other; no histogram is formed.  Only the coarse
+ * z-slabs k_begin <= k < k_end are computed (the caller bounds the memory): out is [k_end - k_begin][Y_l][X_l][4].
+ * Pins (tests/test_oracle_pins.py): direct_colour of the recursion's integer histograms (O-2) on a ragged volume,
+ * slab by slab; numpy's box mean of TF[S] on a power-of-two volume; exact fractions on the 5 x 1 x 1 border case. */
+void mgo_direct_colour_level(const uint32_t *seg_index, uint64_t x0, uint64_t y0, uint64_t z0,
+                             const double *tf, uint32_t l, uint64_t k_begin, uint64_t k_end, double *out)
+{
+    uint64_t xl = x0, yl = y0;
+    for (uint32_t m = 0; m < l; m++) {
+        xl = (xl + 1) / 2;
+        yl = (yl + 1) / 2;
+    }
+    double *wx = (double *)malloc(x0 * sizeof(double));
+    double *wy = (double *)malloc(y0 * sizeof(double));
+    double *wz = (double *)malloc(z0 * sizeof(double));
+    for (uint64_t x = 0; x < x0; x++) wx[x] = axis_weight(x, x0, l);
+    for (uint64_t y = 0; y < y0; y++) wy[y] = axis_weight(y, y0, l);
+    for (uint64_t z = 0; z < z0; z++) wz[z] = axis_weight(z, z0, l);
+    memset(out, 0, (size_t)((k_end - k_begin) * yl * xl) * 4 * sizeof(double));
+    /* the coarse rows (k, j) are independent: one thread per row, walking its own finest voxels in (z, y, x) order */
+#pragma omp parallel for collapse(2) schedule(dynamic, 4)
+    for (int64_t k = (int64_t)k_begin; k < (int64_t)k_end; k++)
+        for (int64_t j = 0; j < (int64_t)yl; j++) {
+            double *row = out + ((((uint64_t)k - k_begin) * yl + (uint64_t)j) * xl) * 4;
+            for (uint64_t z = (uint64_t)k << l; z < z0 && (z >> l) == (uint64_t)k; z++)
+                for (uint64_t y = (uint64_t)j << l; y < y0 && (y >> l) == (uint64_t)j; y++) {
+                    const uint32_t *s = seg_index + (z * y0 + y) * x0;
+                    double wzy = wz[z] * wy[y];
+                    for (uint64_t x = 0; x < x0; x++) {
+                        double w = wx[x] * wzy;
+                        const double *c = tf + 4 * (uint64_t)s[x];
+                        double *o = row + 4 * (x >> l);
+                        for (int ch = 0; ch < 4; ch++)
+                            o[ch] += w * c[ch];
+                    }
+                }
+        }
     free(wx);
     free(wy);
     free(wz);

@@ -126,6 +126,49 @@ def test_brute_force_level_is_the_per_voxel_brute_force_and_the_box_filter():
     assert oracle.brute_force_level(S, 5, 1)[0, 0].tolist() == [[.5, .5, 0, 0, 0], [0, 0, .5, .5, 0], [0, 0, 0, 0, 1]]
 
 
+def test_direct_colour_level_is_the_scalar_product_with_the_histogram():
+    """direct_colour_level (O-3c: the colour of every voxel of a level accumulated over its finest voxels, no histogram
+    table) against what fixes it: <H, TF> with the recursion's exact integer histograms (O-2, Eq. 4) on a ragged
+    7 x 9 x 13 volume, whole levels and z-slab by z-slab; numpy's box mean of TF[S] on a power-of-two volume; exact
+    fractions on the 5 x 1 x 1 border case (N = 1 parents, Q2); level 0 is TF[S] itself."""
+    S = _random_labels((7, 9, 13), 5, 14)
+    tf = np.random.default_rng(3).random((5, 4))
+    H = oracle.histogram_mipmap(S, 5)
+    for l in range(len(H)):
+        want = oracle.direct_colour(H[l], l, tf).reshape(H[l].shape[:3] + (4,))
+        got = oracle.direct_colour_level(S, tf, l)
+        assert got.shape == want.shape
+        np.testing.assert_allclose(got, want, rtol=0, atol=1e-13)     # (up to 819 terms in another order)
+        zl = want.shape[0]
+        for k0, k1 in [(0, 1), (zl - 1, zl), (zl // 2, zl), (1, 1)]:
+            if k0 <= k1 <= zl:
+                np.testing.assert_array_equal(oracle.direct_colour_level(S, tf, l, k0, k1), got[k0:k1])
+    assert np.array_equal(oracle.direct_colour_level(S, tf, 0), tf[S])
+    S = _random_labels((16, 16, 16), 6, 15)
+    tf = np.random.default_rng(4).random((6, 4))
+    for l in range(5):
+        b = 1 << l
+        box = tf[S].reshape(16 // b, b, 16 // b, b, 16 // b, b, 4).mean(axis=(1, 3, 5))
+        np.testing.assert_allclose(oracle.direct_colour_level(S, tf, l), box, rtol=0, atol=1e-15)
+    S = np.array([[[0, 1, 2, 3, 4]]], dtype=np.uint32)
+    tf = np.zeros((5, 4))
+    tf[:, 0] = [1, 2, 4, 8, 16]
+    tf[:, 3] = 1
+    assert oracle.direct_colour_level(S, tf, 1)[0, 0, :, 0].tolist() == [1.5, 6.0, 16.0]          # (1+2)/2, (4+8)/2, 16
+    assert oracle.direct_colour_level(S, tf, 2)[0, 0, :, 0].tolist() == [3.75, 16.0]              # (1.5+6)/2, 16
+    assert oracle.direct_colour_level(S, tf, 3)[0, 0, 0].tolist() == [9.875, 0, 0, 1.0]           # (3.75+16)/2; alpha stays 1
+    # a transposed axis or a dropped weight shows: anisotropic ragged volume, one voxel of another segment in a corner
+    #   x axis 5 -> 3 -> 2 -> 1: voxel 4 is an only child twice (1, 1), then one of two (1/2)        -> 1/2
+    #   y axis 2 -> 1 -> 1 -> 1: voxel 1 is one of two (1/2), then an only child twice                -> 1/2
+    #   z axis 3 -> 2 -> 1 -> 1: voxel 2 is an only child (1), one of two (1/2), an only child (1)    -> 1/2
+    S = np.zeros((3, 2, 5), dtype=np.uint32)
+    S[2, 1, 4] = 1
+    tf = np.array([[0, 0, 0, 0], [1, 0, 0, 0.]])
+    top = oracle.direct_colour_level(S, tf, 3)
+    assert top.shape == (1, 1, 1, 4) and top[0, 0, 0, 0] == 0.125
+    assert oracle.direct_colour_level(S, tf, 1)[1, 0, :, 0].tolist() == [0.0, 0.0, 0.5]   # level 1 is 2 x 1 x 3: only y halves there
+
+
 def test_level0_is_lossless_unit_vector():
     """L223: the finest level holds exactly one ID per voxel."""
     S = _random_labels((4, 5, 6), 7, 6)
