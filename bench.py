@@ -216,6 +216,8 @@ def workload_config(w, args, n_gpus: int) -> dict:
            "l2": "inputs larger than L2 (node-index stream %.2f GB per step, L2 126 MB); no explicit flush" % (4e-9 * w.n_voxels)}
     if "quant_bits" in s:
         cfg["quant_bits"] = s["quant_bits"]
+    cfg["tf_sequence"] = "%s, %d distinct updates cycled in order" % (w.cfg.get("tf_sequence", "random"),
+                                                                       max(1, min(args.steps + args.warmup, w.n_updates)))
     if args.scale != 1.0:
         cfg["scale"] = args.scale
     return cfg
@@ -307,7 +309,7 @@ def run_b200(args) -> dict:
     out_bytes = 4 if args.format == "rgba8" else 8
     nodes = torch.empty((n_nodes, 4), dtype=torch.float32, device="cuda")
     out = torch.empty(w.n_voxels_padded * out_bytes, dtype=torch.uint8, device="cuda")
-    n_tf = max(1, min(args.steps + args.warmup, 16))
+    n_tf = max(1, min(args.steps + args.warmup, w.n_updates))             # the config's own update sequence (100 TFs), in order
     tfs = [torch.from_numpy(w.tf(u)).cuda() for u in range(n_tf)]          # resident in HBM before the timed region
     stream = torch.cuda.current_stream()
     st = stream.cuda_stream
@@ -364,6 +366,37 @@ def run_b200(args) -> dict:
             evd[k][1].record(stream)
         torch.cuda.synchronize()
         derive = float(np.mean([e[0].elapsed_time(e[1]) for e in evd]))
+
+    # ---- SURVEY.md section 8(d)'s metric as the paper timed it: "GPU timings include the data upload of one float4 color per
+    # source" -- mg_propagate_host from PINNED host TFs (H2D of n_leaves float4 + propagation), alone
+    # and followed by the colourise of all levels; CUDA events on the launch stream, the config's TF sequence in order
+    upload = None
+    if rank == 0:
+        ku = min(K, 100)
+        tf_pin = [torch.from_numpy(w.tf(u)).pin_memory() for u in range(min(n_tf, ku))]
+        for k in range(3):
+            g.propagate_host(tf_pin[k % len(tf_pin)], nodes, st)
+        torch.cuda.synchronize()
+        evu = [[torch.cuda.Event(enable_timing=True) for _ in range(2)] for _ in range(ku)]
+        for k in range(ku):
+            evu[k][0].record(stream)
+            g.propagate_host(tf_pin[k % len(tf_pin)], nodes, st)
+            evu[k][1].record(stream)
+        torch.cuda.synchronize()
+        ph = np.array([e[0].elapsed_time(e[1]) for e in evu])
+        for k in range(ku):
+            evu[k][0].record(stream)
+            g.propagate_host(tf_pin[k % len(tf_pin)], nodes, st)
+            g.colorize(idx_part, n_part, nodes, out_part, fmt=fmt, stream=st, from_last_propagate=True)
+            evu[k][1].record(stream)
+        torch.cuda.synchronize()
+        uh = np.array([e[0].elapsed_time(e[1]) for e in evu])
+        upload = {"propagate_host_ms": float(ph.mean()), "propagate_host_ms_median": float(np.median(ph)),
+                  "update_incl_tf_upload_ms": float(uh.mean()), "update_incl_tf_upload_ms_median": float(np.median(uh)),
+                  "tf_upload_bytes": int(w.n_leaves * 16), "steps": ku,
+                  "what": "mg_propagate_host (pinned host TF -> H2D -> all levels): the quantity the paper times (L371-L373), and the "
+                          "same followed by mg_colorize of every mip level"}
+        del tf_pin
 
     # ---- NEXT-3 variant: the same update with the node IDs bit-packed at r(l) bits per voxel (Table 1)
     packed = None
@@ -542,8 +575,9 @@ def run_b200(args) -> dict:
                      nodes=nodes.cpu().numpy(), tf_update=(ke - 1) % len(tf_pinned), n_voxels_padded=w.n_voxels_padded)
         e2e = {"value": e2e_ms / ke, "unit": UNIT,
                "h2d_bytes_per_step": int(w.n_leaves * 16), "d2h_bytes_per_step": int(n_part * out_bytes), "steps": ke,
+               "d2h_gbs": n_part * out_bytes / (e2e_ms / ke * 1e-3) / 1e9,
                "what": "mg_tf_update_host: pinned-host TF -> H2D -> propagate -> colourise all levels -> D2H of the whole "
-                       "mipmap into pinned host memory (PCIe-bound)"}
+                       "mipmap into pinned host memory (PCIe-bound: d2h_gbs = the output bytes over the whole step time)"}
         del out_host
 
     if rank != 0:
@@ -611,6 +645,10 @@ def run_b200(args) -> dict:
     }
     if derive is not None:
         res["colorize_deriving_palette_ms"] = derive      # mg_colorize's default (no MG_PALETTE_FROM_LAST_PROPAGATE): + k_convert_palette
+    if upload is not None:
+        res["propagate_host_ms"] = upload["propagate_host_ms"]             # section 8(d): what the paper timed (L371-L373)
+        res["update_incl_tf_upload_ms"] = upload["update_incl_tf_upload_ms"]
+        res["tf_upload"] = upload
     if prop_roofline is not None:
         res["roofline_second_kernel"] = prop_roofline
     if packed is not None:

@@ -46,11 +46,23 @@ class Workload:
         self.packed_bytes = 0
         self.perm = None                          # uint32 [n_nodes]: library index of the caller's node (only after MG_RELABEL)
 
+    @property
+    def n_updates(self) -> int:
+        """Length of the config's TF-update sequence (BASELINE.json: 100 consecutive updates)."""
+        return int(self.cfg.get("n_updates", 100))
+
     def tf(self, update: int = 0) -> np.ndarray:
-        """fp32 [n_leaves, 4] transfer function number ``update`` of this config (synth recipe)."""
+        """fp32 [n_leaves, 4]: update number ``update`` of this config's TF sequence (synth recipe).  "random": an
+        independent TF per update; "single_segment" (config 4): update u is update u - 1 with ONE random segment re-drawn."""
         c = self.cfg
-        return synth.random_tf(self.n_leaves, c.get("seed", 0), update=update,
-                               alpha_zero_frac=c.get("alpha_zero_frac", 0.0))
+        seed = c.get("seed", 0)
+        if c.get("tf_sequence", "random") != "single_segment":
+            return synth.random_tf(self.n_leaves, seed, update=update, alpha_zero_frac=c.get("alpha_zero_frac", 0.0))
+        chain = self.__dict__.setdefault("_tf_chain", [synth.random_tf(self.n_leaves, seed, update=0,
+                                                                       alpha_zero_frac=c.get("alpha_zero_frac", 0.0))])
+        while len(chain) <= update:
+            chain.append(synth.single_segment_update(chain[-1], seed, len(chain)))
+        return chain[update].copy()
 
     def host_level(self, l: int) -> np.ndarray:
         """Node indices of mip level ``l`` on the host, flat uint32 (downloaded when the host never had them)."""

@@ -8,11 +8,14 @@ mg_load_graph -> ONE concatenated node-index mipmap, ONE mg_colorize call over a
     with S from the input generator (not from the builder) and the 4 x n_leaves codes from the oracle;
   * every other level: EVERY voxel against the oracle's lookup/conversion on the same graph (host-built node
     indices), and padding voxels against node 0;
-  * quantised-graph colour vs the DIRECT histogram (O-3 brute force on the generator's volume): EVERY voxel of
-    every level whose dense histogram table fits 2 GB (levels >= 5 or 6: where the mixtures have hundreds of
-    components and the quantisation error peaks, Table 2), >= 1000 mixed voxels of each finer level:
-    max-abs <= 2e-3 (north_star); max ||mu - H||_1 (I11) and the bound I12 on the same voxels.  The per-level
-    maxima go to $MG_PARITY_REPORT_DIR/direct_parity_cfg<N>.json when that is set (DESIGN.md section 9 quotes them).
+  * quantised-graph colour vs the DIRECT definition C_dir = sum_s H[s] TF[s] on the generator's volume: EVERY voxel of
+    EVERY level >= 1 (oracle.direct_colour_level, O-3c), max-abs <= 2e-3 (north_star), and every voxel whose index is a
+    leaf must have C_dir == TF[leaf] to 1e-12 (a mixed voxel taken for pure fails);
+  * the graph's symbolic mixtures mu against the histograms H (O-3 brute force): max ||mu - H||_1 (I11) and the bound
+    I12 on every voxel of every level whose dense histogram table fits 2 GB (levels >= 5 or 6: where the mixtures have
+    hundreds of components and the quantisation error peaks, Table 2) and on >= 1000 mixed voxels of each finer
+    level.  The per-level maxima go to $MG_PARITY_REPORT_DIR/direct_parity_cfg<N>.json when that is set (DESIGN.md
+    section 9 quotes them).
 """
 import json
 import os
@@ -96,6 +99,88 @@ def _sample_positions(n, k, seed, stream):
     return np.unique(np.concatenate([pos, edge]))
 
 
+def _check_mipmap_every_voxel(w, out, tf, ref_nodes, seg_index, sample_seed):
+    """The colourised RGBA8 mipmap `out` (all levels, padded layout) of one update, EVERY voxel: level 0 must be the code of
+    TF[S(v)] (I5, L223; S from the generator, the codes from the oracle), every other level the oracle's lookup +
+    conversion on the same graph with the node indices the host builder produced; padding voxels are node 0."""
+    out4 = out.view(-1, 4)
+    code_tf = torch.from_numpy(oracle.to_rgba8(tf.astype(np.float64)).view(np.uint32).reshape(-1).astype(np.int64)).cuda()
+    n0 = w.level_voxels[0]
+    flat = seg_index.reshape(-1)
+    out32 = out.view(torch.int32)
+    bad = 0
+    step = 1 << 27
+    for o in range(0, n0, step):
+        e = min(n0, o + step)
+        s = torch.from_numpy(flat[o:e].astype(np.int64)).cuda()
+        exp = code_tf[s]
+        got = out32[o:e].to(torch.int64) & 0xFFFFFFFF
+        bad += int((got != exp).sum().item())
+    assert bad == 0, f"{bad} level-0 voxels differ from code(TF[S(v)])"
+    for l, (s0, nv) in enumerate(zip(w.level_start, w.level_voxels)):
+        if l == 0:                                                       # additionally on samples through the oracle's lookup
+            pos = _sample_positions(nv, 200000, sample_seed, l)
+            got = out4[torch.from_numpy(pos + s0).cuda()].cpu().numpy()
+            assert _rgba8_close(got, oracle.lookup(seg_index.reshape(-1)[pos], ref_nodes)), "level 0"
+        else:
+            idx_l = w.host_idx[l].reshape(-1)
+            chunk = 1 << 23
+            for o in range(0, nv, chunk):
+                e = min(nv, o + chunk)
+                got = out4[s0 + o:s0 + e].cpu().numpy()
+                assert _rgba8_close(got, oracle.lookup(idx_l[o:e], ref_nodes)), f"level {l}, voxels {o}..{e}"
+        pad_end = w.level_start[l + 1] if l + 1 < len(w.level_start) else w.n_voxels_padded
+        if pad_end > s0 + nv:                                            # padding voxels: node 0
+            padv = out4[s0 + nv:pad_end].cpu().numpy()
+            assert _rgba8_close(padv, np.broadcast_to(ref_nodes[0], padv.shape).copy())
+
+
+def _check_update_sequence(mg, w, seg_index, cfg_id, n_updates=100):
+    """The config's OWN update sequence as BASELINE.json names it -- config 2: "100 consecutive random TF updates", config
+    4: "per-update TF changes one random segment" (the paper performs full updates only, L221, "whenever the user changes
+    the color transfer function", L373) -- enqueued back to back with no host synchronisation in between.  node_rgba is
+    snapshotted after every update (stream-ordered copies) and EVERY node of EVERY update is compared with the same-graph
+    oracle (leaves bit-exact, 1e-5); the colourised mipmap of the first, the middle and the last update is checked on
+    every voxel."""
+    g = w.graph
+    n_nodes = int(g.info.n_nodes)
+    assert w.n_updates >= n_updates
+    tfs = [w.tf(u) for u in range(n_updates)]
+    changed = [int((tfs[u] != tfs[u - 1]).any(axis=1).sum()) for u in range(1, n_updates)]
+    if w.cfg.get("tf_sequence") == "single_segment":
+        assert max(changed) == 1 and sum(changed) >= n_updates - 5          # one segment per update (a re-draw may repeat a value)
+    else:
+        assert min(changed) > 0.9 * w.n_leaves                              # independent TFs
+    st = torch.cuda.current_stream().cuda_stream
+    d_tfs = [torch.from_numpy(t).cuda() for t in tfs]
+    nodes = torch.full((n_nodes, 4), float("nan"), dtype=torch.float32, device="cuda")
+    snaps = torch.empty((n_updates, n_nodes, 4), dtype=torch.float32, device="cuda")
+    out = torch.full((w.n_voxels_padded * 4,), 0xAB, dtype=torch.uint8, device="cuda")
+    keep = {u: torch.empty_like(out) for u in (0, n_updates // 2, n_updates - 1)}
+    torch.cuda.synchronize()
+    for u in range(n_updates):
+        g.propagate(d_tfs[u], nodes, st)
+        g.colorize(w.d_idx, w.n_voxels_padded, nodes, out, fmt=mg.MG_RGBA8, stream=st, from_last_propagate=True)
+        snaps[u].copy_(nodes, non_blocking=True)
+        if u in keep:
+            keep[u].copy_(out, non_blocking=True)
+    torch.cuda.synchronize()
+    hg = w.host_graph
+    nl = hg["n_leaves"]
+    worst = 0.0
+    for u in range(n_updates):
+        ref = oracle.graph_eval(hg["child_a"], hg["child_b"], hg["weight"], nl, tfs[u].astype(np.float64))
+        got = snaps[u].cpu().numpy()
+        assert np.array_equal(got[:nl].view(np.uint32), tfs[u].view(np.uint32)), f"update {u}: leaves not bit-exact"
+        err = float(np.abs(got - ref).max())
+        assert err <= TOL, (u, err)
+        worst = max(worst, err)
+        if u in keep:
+            _check_mipmap_every_voxel(w, keep[u], tfs[u], ref, seg_index, 500 + u)
+    print(f"cfg {cfg_id}: {n_updates} consecutive updates ({w.cfg.get('tf_sequence', 'random')}), every node of every update: "
+          f"max |err| = {worst:.2e}; mipmaps of updates {sorted(keep)} checked on every voxel")
+
+
 @pytest.mark.parametrize("cfg_id", [3, 2, 4])
 def test_volume_config_full_size(libs, cfg_id):
     mg, workload = libs
@@ -111,46 +196,16 @@ def test_volume_config_full_size(libs, cfg_id):
         ref_nodes = _check_nodes(w, nodes, tf)
         out4 = out.view(-1, 4)
 
-        # ---- level 0, every voxel: out == code(TF[S(v)])  (I5; S from the generator)
         ids, seg_index = _leaf_index_chunked(w.seg)
         assert np.array_equal(ids, w.host_graph["leaf_segment_id"])
-        code_tf = torch.from_numpy(oracle.to_rgba8(tf.astype(np.float64)).view(np.uint32).reshape(-1).astype(np.int64)).cuda()
-        n0 = w.level_voxels[0]
-        flat = seg_index.reshape(-1)
-        out32 = out.view(torch.int32)
-        bad = 0
-        step = 1 << 27
-        for o in range(0, n0, step):
-            e = min(n0, o + step)
-            s = torch.from_numpy(flat[o:e].astype(np.int64)).cuda()
-            exp = code_tf[s]
-            got = out32[o:e].to(torch.int64) & 0xFFFFFFFF
-            bad += int((got != exp).sum().item())
-        assert bad == 0, f"{bad} level-0 voxels differ from code(TF[S(v)])"
-
-        # ---- every level >= 1, EVERY voxel (chunked): the oracle's lookup + conversion on the same graph, with the node
-        # indices the host builder produced; level 0 additionally on samples through the oracle's lookup (its every-voxel
-        # check is the TF-code comparison above); padding voxels against node 0
-        for l, (s0, nv) in enumerate(zip(w.level_start, w.level_voxels)):
-            if l == 0:
-                pos = _sample_positions(nv, 200000, 77 + cfg_id, l)
-                got = out4[torch.from_numpy(pos + s0).cuda()].cpu().numpy()
-                assert _rgba8_close(got, oracle.lookup(seg_index.reshape(-1)[pos], ref_nodes)), "level 0"
-            else:
-                idx_l = w.host_idx[l].reshape(-1)
-                chunk = 1 << 23
-                for o in range(0, nv, chunk):
-                    e = min(nv, o + chunk)
-                    got = out4[s0 + o:s0 + e].cpu().numpy()
-                    assert _rgba8_close(got, oracle.lookup(idx_l[o:e], ref_nodes)), f"level {l}, voxels {o}..{e}"
-            pad_end = w.level_start[l + 1] if l + 1 < len(w.level_start) else w.n_voxels_padded
-            if pad_end > s0 + nv:                                            # padding voxels: node 0
-                padv = out4[s0 + nv:pad_end].cpu().numpy()
-                assert _rgba8_close(padv, np.broadcast_to(ref_nodes[0], padv.shape).copy())
+        _check_mipmap_every_voxel(w, out, tf, ref_nodes, seg_index, 77 + cfg_id)
 
         # ---- quantised graph vs the DIRECT histogram (north_star's second tolerance; I11 / I12)
         _check_direct_histogram(w, cfg_id, tf, nodes.cpu().numpy().astype(np.float64), seg_index, ids.size)
         _check_render_full_size(mg, w, tf, seg_index)
+        if cfg_id in (2, 4):                                                 # the configs BASELINE.json names by their update sequence
+            del nodes, out
+            _check_update_sequence(mg, w, seg_index, cfg_id)
     finally:
         w.close()
 
@@ -193,10 +248,42 @@ def _check_direct_histogram(w, cfg_id, tf, nodes_host, seg_index, nl, dense_byte
         report["levels"].append({"level": l, "voxels": int(nv), "checked": int(vox.size), "every_voxel": bool(vox.size == nv),
                                  "max_abs_colour": float(err_c.max()), "max_l1_mixture": float(l1.max())})
         worst_c, worst_l1 = max(worst_c, float(err_c.max())), max(worst_l1, float(l1.max()))
+    # ---- EVERY voxel of EVERY level >= first_level against the direct definition C_dir = sum_s H[s] TF[s] (O-3c: accumulated
+    # from the generator's volume, coarse z-slab by z-slab; no histogram table).  A voxel the builder calls pure (its index
+    # is a leaf) must BE pure: C_dir equals TF[leaf] to rounding -- a mixed voxel mis-classified as pure fails here.
+    worst_all = 0.0
+    done = {r["level"]: r for r in report["levels"]}
+    for l in range(first_level, len(w.mip_dims)):
+        xl, yl, zl = w.mip_dims[l]
+        idx_l = w.host_idx[l].reshape(-1)
+        per_k = xl * yl
+        dk = max(1, (1 << 24) // per_k)
+        lvl_max, n_pure, pure_max = 0.0, 0, 0.0
+        for k0 in range(0, zl, dk):
+            k1 = min(zl, k0 + dk)
+            c_dir = oracle.direct_colour_level(seg_index, tf64, l, k0, k1).reshape(-1, 4)
+            node = idx_l[k0 * per_k:k1 * per_k].astype(np.int64)
+            lvl_max = max(lvl_max, float(np.abs(nodes_host[node] - c_dir).max()))
+            pure = node < nl
+            if pure.any():
+                n_pure += int(pure.sum())
+                pure_max = max(pure_max, float(np.abs(c_dir[pure] - tf64[node[pure]]).max()))
+        assert pure_max <= 1e-12, f"level {l}: a voxel indexed as a leaf is not pure (|C_dir - TF[leaf]| = {pure_max:.3e})"
+        assert lvl_max <= tol, f"level {l}: max |C_graph - C_dir| over all {idx_l.size} voxels = {lvl_max:.3e}"
+        r = done.get(l)
+        if r is None:
+            r = {"level": l, "voxels": int(idx_l.size), "checked": 0, "every_voxel": False, "max_abs_colour": 0.0, "max_l1_mixture": 0.0}
+            report["levels"].append(r)
+        r.update(colour_checked_on="all", max_abs_colour_all_voxels=lvl_max, pure_voxels=n_pure, max_abs_pure_vs_tf=pure_max)
+        worst_all = max(worst_all, lvl_max)
+    report["levels"].sort(key=lambda r: r["level"])
+    report["max_abs_colour_all_voxels"] = worst_all
+    worst_c = max(worst_c, worst_all)
     report["max_abs_colour"], report["max_l1_mixture"] = worst_c, worst_l1
     print(f"cfg {cfg_id} (b = {report['quant_bits']}, {report['n_nodes']} nodes, depth {report['depth']}): max |C_graph - C_dir| = "
           f"{worst_c:.3e}, max ||mu - H||_1 = {worst_l1:.3e}; per level: " +
-          ", ".join(f"l{r['level']}:{r['max_abs_colour']:.1e}/{r['max_l1_mixture']:.1e}({r['checked']})" for r in report["levels"]))
+          ", ".join(f"l{r['level']}:{r['max_abs_colour']:.1e}/{r['max_l1_mixture']:.1e}({r['checked']})" for r in report["levels"]) +
+          f"; colour on ALL voxels of every level: max {worst_all:.3e}")
     out_dir = os.environ.get("MG_PARITY_REPORT_DIR")
     if out_dir:
         os.makedirs(out_dir, exist_ok=True)

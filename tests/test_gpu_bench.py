@@ -38,6 +38,8 @@ def test_bench_line_has_the_contract_keys():
     assert abs(r["frac"] - r["achieved"] / r["peak"]) < 1e-9 and r["achieved"] > 0
     c = d["cpu_baseline"]
     assert c["kind"] == "oracle" and c["cores"] >= 1 and c["value"] > 0 and c["sample"]
+    assert d["propagate_host_ms"] > 0 and d["update_incl_tf_upload_ms"] > d["propagate_host_ms"]     # incl. the TF upload
+    assert d["tf_upload"]["tf_upload_bytes"] == 16 * d["config"]["leaves"] and "tf_sequence" in d["config"]
     e = d["e2e"]
     # (at this scale an update is tens of microseconds, so the two timings differ by their event overheads in either
     # direction: e2e must be a measurement of its own with its copies declared, not a value above the device-resident one)

@@ -29,6 +29,29 @@ def test_tf_configs():
     assert (t0 != t1).any(axis=1).sum() == 1
 
 
+def test_config_tf_sequences_are_the_ones_baseline_names():
+    """Config 2: 100 consecutive random TFs; config 4: update u is update u - 1 with one random segment re-drawn
+    (BASELINE.json configs[1], configs[3]); Workload.tf(u) is that sequence, whatever order it is asked in."""
+    from paper_2009_02702_b200.workload import Workload
+    for cid, n_leaves in ((2, 353), (4, 15918)):
+        w = Workload("t")
+        w.cfg = dict(synth.CONFIGS[cid])
+        w.n_leaves = n_leaves
+        assert w.n_updates == 100
+        last = w.tf(99)
+        tfs = [w.tf(u) for u in range(100)]
+        assert np.array_equal(tfs[99], last) and all(t.shape == (n_leaves, 4) and t.dtype == np.float32 for t in tfs)
+        changed = [int((tfs[u] != tfs[u - 1]).any(axis=1).sum()) for u in range(1, 100)]
+        if cid == 4:
+            assert max(changed) == 1 and sum(changed) >= 95
+            assert np.array_equal(tfs[7], synth.single_segment_update(tfs[6], 4, 7))
+            tfs[3][0, 0] = 9.0                                                 # callers get copies
+            assert w.tf(3)[0, 0] != 9.0
+        else:
+            assert min(changed) == n_leaves and len({t.tobytes() for t in tfs}) == 100
+            assert np.array_equal(tfs[5], synth.random_tf(353, 2, update=5))
+
+
 def test_config1_volume():
     c = synth.CONFIGS[1]
     S = synth.make_volume(c)
