@@ -17,7 +17,19 @@ import time
 
 import numpy as np
 
-from . import builder, mg, synth
+from . import builder, synth
+
+
+class _LazyMg:
+    """``mg`` (the ctypes binding of libmg.so) is loaded on first use: a workload assembled with ``load=False`` for the
+    reference arm of bench.py (generator + host builder + oracle) then never maps the CUDA library."""
+
+    def __getattr__(self, name):
+        from . import mg as _mg
+        return getattr(_mg, name)
+
+
+mg = _LazyMg()
 
 LEVEL_ALIGN = 64          # voxels
 

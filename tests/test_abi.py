@@ -48,3 +48,16 @@ def test_no_device_means_an_error_code_not_a_fallback():
     with pytest.raises(mg.MgError) as ei:
         mg.Graph(z, z, np.zeros(2, np.float32), 2, level_offsets=np.array([0, 2], np.uint64))
     assert ei.value.code in (mg.MG_ERR_CUDA, mg.MG_ERR_OOM)
+
+
+def test_reference_arm_workload_does_not_map_the_cuda_library():
+    """bench.py --impl reference assembles its inputs with the generator and the host builder only (load=False): the
+    binding of libmg.so is imported lazily, so that arm's process never maps the product's CUDA library."""
+    import subprocess
+    import sys
+    code = ("import sys; from paper_2009_02702_b200 import workload; w = workload.make(1, load=False, device_synth=False); "
+            "assert w.graph is None and w.host_graph['child_a'].size > 16; "
+            "assert 'paper_2009_02702_b200.mg' not in sys.modules; "
+            "assert 'libmg.so' not in open('/proc/self/maps').read(); print('ok')")
+    out = subprocess.run([sys.executable, "-c", code], cwd=ROOT, capture_output=True, text=True, timeout=600)
+    assert out.returncode == 0 and out.stdout.strip() == "ok", out.stderr[-2000:]
